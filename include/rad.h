@@ -1,0 +1,176 @@
+/* rad.h -- C ABI of librad.so: the explicit-plus-locally-implicit radiation stage of the
+ * finite-solid-angle GR transport of White et al., arXiv 2302.04283, for one NVIDIA B200 (sm_100a).
+ *
+ * Citations: P:L<n> = line n of the paper text; "R#" = a reading listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Plain C types only.  Every pointer is marked HOST or DEVICE.  DEVICE pointers must live on the
+ *    device given to rad_create.  The library owns only what it builds (angle tables, geometry tables,
+ *    scratch); the caller owns intensity, fluid, opacity and output buffers.
+ *  - No exceptions or aborts cross the ABI: every call returns a rad_status; rad_last_error() gives text.
+ *  - Work is enqueued on the caller's CUDA stream (a cudaStream_t passed as void*; NULL = default
+ *    stream).  No implicit synchronisation except where stated.
+ *  - There is no CPU fallback: if no CUDA device is usable, rad_create returns RAD_ECUDA.
+ *
+ * Arrays
+ *  - Grid: uniform Cartesian, n[0..2] interior cells along x,y,z, ng = 2 ghost cells per side
+ *    (PLM needs two).  NI = n[0]+2ng etc.  Cell (k,j,i) has flat index c = (k*NJ + j)*NI + i.
+ *  - Intensity I[c][n]: angle index n innermost (contiguous), N = number of angles.  FP64.
+ *  - Per-cell scalars are SoA: field[f][c].
+ */
+#ifndef RAD_H
+#define RAD_H
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rad_ctx rad_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    RAD_OK = 0,
+    RAD_EINVAL = 1,       /* bad argument (NULL, non-finite, bad shape, aliasing) */
+    RAD_ENOMEM = 2,       /* host or device allocation failed */
+    RAD_ECUDA = 3,        /* CUDA runtime error (text in rad_last_error) */
+    RAD_EUNSUPPORTED = 4, /* valid request the library does not implement */
+    RAD_ESTATE = 5        /* call not valid in this state */
+} rad_status;
+
+/* ---- geometry record layouts (doubles), also the input format of metric kind 2 ------------------
+ * Cell centre record, RAD_NCELL doubles:
+ *   [0]      n^0 = e^0_0hat = 1/alpha   (Eq.5a, Eq.11; the same for every angle because e^0_ahat = 0, R2)
+ *   [1..4]   E_alphahat = g_{0 mu} e^mu_alphahat, alphahat = 0..3  (E_0hat = -alpha);  n_0 = E_0 + E_a n^a
+ *   [5..34]  S[c][k], c = 1..3, k over (00,01,02,03,11,12,13,22,23,33):
+ *            S = omega^c_{ab} + omega^c_{ba} (a<b), omega^c_{aa} (a=b); Ricci rotation coefficients Eq.17
+ *   [35..37] beta^i (Eq.5c)
+ *   [38..43] triad e^i_ahat, upper triangular (R2): (x1,x2,x3,y2,y3,z3)
+ *   [44..49] co-triad theta^ahat_i = e^ahat_i, upper triangular: (1x,1y,1z,2y,2z,3z); n_i = theta^a_i n^a
+ *   [50]     1.0 if the cell is excised, else 0.0;  [51] unused
+ * Face centre record, RAD_NFACE doubles, three per cell (the LOWER x, y, z face of the cell), R6:
+ *   [0..3]   e^a_alphahat for the face's own axis a (alphahat = 0..3);  n^a = e^a_0 + e^a_b n^b
+ *   [4..7]   E_alphahat at the face centre
+ */
+#define RAD_NCELL 52
+#define RAD_NFACE 8
+#define RAD_MAXNBR 6
+
+typedef struct {
+    int kind;        /* 0 Minkowski, 1 Cartesian Kerr-Schild, 2 tabulated */
+    double M, a;     /* kind 1: mass and spin */
+    double excise_r; /* kind 1: cells whose centre has Kerr-Schild radius r < excise_r are excised
+                        (I_out = 0, T and fluid increments untouched); 0 = none */
+    const double *cell_tab; /* kind 2, DEVICE, [ncells_total][RAD_NCELL]; copied at create */
+    const double *face_tab; /* kind 2, DEVICE, [ncells_total][3][RAD_NFACE]; copied at create */
+} rad_metric;
+
+typedef struct {
+    int n[3], ng;           /* interior cells per axis; ng must be 2 */
+    double x0[3], dx[3];    /* lower corner of the interior and cell sizes */
+    int bc_lo[3], bc_hi[3]; /* 0 caller-filled, 1 periodic, 2 outflow (copy of nearest interior cell) */
+} rad_grid;
+
+typedef struct {
+    int kind; /* 0 latitude-longitude (nzeta x npsi), 1 geodesic (level nlev) */
+    int nzeta, npsi, nlev;
+} rad_angles;
+
+typedef struct { /* fluid-frame absorptivities, DEVICE, each [ncells_total], NOT owned;
+                    contents may change between stages */
+    const double *alpha_a_planck, *alpha_a_energy, *alpha_s;
+} rad_opac;
+
+typedef struct {
+    double gamma_gas;         /* adiabatic index Gamma (Eq.48); k_B/(mu m_p) = 1 */
+    double a_rad;             /* radiation constant (Eq.34) */
+    double n0_crit;           /* Ihat is zeroed where |n_0| < n0_crit; <= 0 disables */
+    int recon_space;          /* 0 donor cell, 1 PLM van Leer */
+    int recon_angle;          /* 0 donor cell; others RAD_EUNSUPPORTED */
+    int renorm_fluid_weights; /* R12: 1 = rescale fluid-frame solid angles to sum to 4 pi */
+    int couple;               /* 0 = transport only, 1 = with implicit coupling (section 2.5) */
+    double tau_factor;        /* constant of Eq.26; only 0 (free-streaming flux, Eq.24) is implemented */
+} rad_params;
+
+/* Build a context: angle tables on the host (section 2.6), geometry tables on the device (section 2.1-2.2,
+ * one kernel launch; synchronises the device once).  `device` is the CUDA ordinal.
+ * Errors: RAD_EINVAL (NULL, ng != 2, n < 1, non-finite or non-positive dx, bad enum), RAD_EUNSUPPORTED
+ * (recon_angle != 0, tau_factor != 0), RAD_ENOMEM, RAD_ECUDA.  On error *out is NULL. */
+rad_status rad_create(const rad_metric *, const rad_grid *, const rad_angles *, const rad_opac *,
+                      const rad_params *, int device, rad_ctx **out);
+
+/* One radiation stage (P:L69-81 tasks 1,3,4,7,8; Eq.22,24,25, Eq.31-50):
+ *   ghost fill of I_in per bc (writes I_in's ghost cells; no-op for caller-filled)
+ *   C_new = gam0 C0 + gam1 C - beta_dt (spatial + angular flux divergence),  C = n^0 n_0 I;  I_new = C_new / (n^0 n_0)
+ *   coupling over beta_dt (if params.couple): I_new -> I_+, gas temperature T_+, fluid increment
+ *   mask |n_0| < n0_crit
+ * I_in, I_out, I0: DEVICE [ncells_total][N]; I_out must not alias I_in or I0 (RAD_EINVAL); only the
+ *   interior of I_out is written.  I0 may be NULL (then the gam0 term is absent).
+ * fluid: DEVICE SoA [5][ncells_total] = rho, T, u^1', u^2', u^3' (normal-frame velocity).
+ * T_out: DEVICE [ncells_total] or NULL.  dT0: DEVICE [4][ncells_total] or NULL: increment of the
+ *   fluid's T^0_alpha = -(change of R^0_alpha in the coupling).  Interior cells only.
+ * n_noroot: HOST or NULL.  If given, the call synchronises the stream and stores the number of cells
+ *   whose quartic (Eq.49) had no positive root (those cells are left uncoupled, R13).
+ * Forward Euler is (gam0, gam1, beta_dt) = (0, 1, dt). */
+rad_status rad_stage(rad_ctx *, double *I_in, double *I_out, const double *I0, const double *fluid,
+                     double gam0, double gam1, double beta_dt, double *T_out, double *dT0,
+                     long long *n_noroot, void *cuda_stream);
+
+/* Same stage with HOST buffers (same shapes): copies I_in, fluid and the three opacity arrays
+ * host->device into library-owned scratch, runs rad_stage, copies I_out, T_out, dT0 back, and
+ * synchronises.  opac_host: HOST SoA [3][ncells_total] = alpha_a_planck, alpha_a_energy, alpha_s.
+ * I0 is not supported here (forward-Euler style stages only).  Pinned host memory makes the copies faster
+ * but is not required. */
+rad_status rad_stage_host(rad_ctx *, const double *I_in_host, double *I_out_host, const double *fluid_host,
+                          const double *opac_host, double gam0, double gam1, double beta_dt,
+                          double *T_out_host, double *dT0_host, long long *n_noroot);
+
+/* The two halves of a stage, separately (used by tests and profiling):
+ * rad_transport = ghost fill + flux-divergence kernel; rad_couple = coupling + mask in place on I. */
+rad_status rad_fill_ghosts(rad_ctx *, double *I, void *cuda_stream);
+rad_status rad_transport(rad_ctx *, double *I_in, double *I_out, const double *I0, double gam0, double gam1,
+                         double beta_dt, void *cuda_stream);
+rad_status rad_couple(rad_ctx *, double *I, const double *fluid, double dt, double *T_out, double *dT0,
+                      long long *n_noroot, void *cuda_stream);
+
+/* Angular moments of I (Eq.45, Eq.38) for interior cells, DEVICE out SoA [ncomp][ncells_total]:
+ * frame 0: coordinate R^{ab} (10: 00,01,02,03,11,12,13,22,23,33); 1: mixed R^0_a (4);
+ * frame 2: tetrad R^{ahat bhat} (10); 3: fluid frame Ebar, F^abar (4; needs fluid, Eq.13-14). */
+rad_status rad_moments(rad_ctx *, const double *I, int frame, const double *fluid, double *out, void *cuda_stream);
+
+/* Tables for parity checks.  Copies `nbytes` (must equal the table's size) to HOST memory; synchronises. */
+typedef enum {
+    RAD_TAB_NANG = 0,       /* int[1] */
+    RAD_TAB_NEDGE = 1,      /* int[1] */
+    RAD_TAB_NHAT = 2,       /* double[N][3] */
+    RAD_TAB_DOMEGA = 3,     /* double[N] */
+    RAD_TAB_NNBR = 4,       /* int[N] */
+    RAD_TAB_NBR = 5,        /* int[N][6], -1 = none; geodesic: counter-clockwise from outside starting at the
+                               smallest index (R3); lat-lon: zeta-, zeta+, psi-, psi+ */
+    RAD_TAB_NBR_EDGE = 6,   /* int[N][6] unique edge id */
+    RAD_TAB_EDGE_LO = 7,    /* int[E]  lower angle index of each unique edge */
+    RAD_TAB_EDGE_HI = 8,    /* int[E] */
+    RAD_TAB_EDGE_LEN = 9,   /* double[E] Delta lambda_e (Eq.20f) */
+    RAD_TAB_EDGE_MID = 10,  /* double[E][3] unit vector to the edge midpoint */
+    RAD_TAB_EDGE_NRM = 11,  /* double[E][3] in-sphere edge normal, pointing lo -> hi */
+    RAD_TAB_CELL = 12,      /* double[ncells_total][RAD_NCELL] */
+    RAD_TAB_FACE = 13,      /* double[ncells_total][3][RAD_NFACE] */
+    RAD_TAB_FACE_SIGN = 14, /* signed char[ncells_total][3][N]: sgn n^a at each cell's lower faces (upwind index, Eq.24) */
+    RAD_TAB_EDGE_SIGN = 15, /* signed char[ncells_total][E]: sgn c_e (upwind index, Eq.25) */
+    RAD_TAB_MAXSPEED = 16   /* double[3]: max over faces and angles of |n^a / n^0| per axis (for the CFL step, R9) */
+} rad_table;
+rad_status rad_get_table(rad_ctx *, int which, void *host_out, size_t nbytes);
+
+/* number of cells including ghosts, = NI*NJ*NK */
+long long rad_ncells_total(const rad_ctx *);
+/* kernels launched by this context so far (bench.py's gpu_launches) */
+long long rad_launch_count(const rad_ctx *);
+
+/* Text of the last error on this context (or of the last failed rad_create if ctx is NULL).  Never NULL. */
+const char *rad_last_error(const rad_ctx *);
+
+void rad_destroy(rad_ctx *);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,314 @@
+// api.cu -- the C ABI of librad.so (include/rad.h): argument checking, context ownership, launches.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "rad_internal.h"
+
+struct rad_ctx {
+    int device = 0;
+    rad_metric metric{};
+    rad_grid grid{};
+    rad_angles angles{};
+    rad_opac opac{};
+    rad_params params{};
+    rad::AngleTables host;
+    rad::DeviceTables dev{};
+    rad::Params kp{};
+    std::vector<void *> owned;  // device allocations to free
+    double *scratch_I[2] = {nullptr, nullptr};  // rad_stage_host
+    double *scratch_small = nullptr;            // fluid[5] + opac[3] + T[1] + dT0[4] per cell
+    unsigned long long *d_noroot = nullptr;
+    long long launches = 0;
+    std::string err;
+};
+
+namespace {
+std::string g_create_err;
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok;
+    explicit DeviceGuard(int dev) { ok = cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+rad_status fail(rad_ctx *c, rad_status st, const std::string &msg) {
+    if (c) c->err = msg; else g_create_err = msg;
+    return st;
+}
+rad_status cuda_fail(rad_ctx *c, const char *where) {
+    cudaError_t e = cudaGetLastError();
+    return fail(c, RAD_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+template <class T>
+bool upload(rad_ctx *c, const std::vector<T> &h, const T **dptr) {
+    void *p = nullptr;
+    const size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(T);
+    if (cudaMalloc(&p, bytes) != cudaSuccess) return false;
+    c->owned.push_back(p);
+    if (!h.empty() && cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return false;
+    *dptr = static_cast<const T *>(p);
+    return true;
+}
+
+bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+}  // namespace
+
+extern "C" {
+
+rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *a, const rad_opac *o, const rad_params *p,
+                      int device, rad_ctx **out) {
+    if (out) *out = nullptr;
+    if (!m || !g || !a || !p || !out) return fail(nullptr, RAD_EINVAL, "rad_create: NULL argument");
+    if (g->ng != 2) return fail(nullptr, RAD_EINVAL, "rad_create: ng must be 2");
+    for (int d = 0; d < 3; d++) {
+        if (g->n[d] < 1) return fail(nullptr, RAD_EINVAL, "rad_create: n[d] must be >= 1");
+        if (!finite_pos(g->dx[d]) || !std::isfinite(g->x0[d])) return fail(nullptr, RAD_EINVAL, "rad_create: bad x0/dx");
+        if (g->bc_lo[d] < 0 || g->bc_lo[d] > 2 || g->bc_hi[d] < 0 || g->bc_hi[d] > 2) return fail(nullptr, RAD_EINVAL, "rad_create: bad boundary code");
+    }
+    if (m->kind < 0 || m->kind > 2) return fail(nullptr, RAD_EINVAL, "rad_create: bad metric kind");
+    if (m->kind == 1 && (!finite_pos(m->M) || !std::isfinite(m->a) || std::fabs(m->a) > m->M)) return fail(nullptr, RAD_EINVAL, "rad_create: bad M or a");
+    if (m->kind == 2 && (!m->cell_tab || !m->face_tab)) return fail(nullptr, RAD_EINVAL, "rad_create: tabulated metric needs cell_tab and face_tab");
+    if (!(p->gamma_gas > 1.0) || !std::isfinite(p->gamma_gas) || !std::isfinite(p->a_rad) || p->a_rad < 0.0 || !std::isfinite(p->n0_crit))
+        return fail(nullptr, RAD_EINVAL, "rad_create: bad gamma_gas / a_rad / n0_crit");
+    if (p->recon_space < 0 || p->recon_space > 1) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: recon_space must be 0 (DC) or 1 (PLM)");
+    if (p->recon_angle != 0) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: only donor-cell angular reconstruction is implemented");
+    if (p->tau_factor != 0.0) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: only tau_factor = 0 (Eq.24) is implemented");
+    if (p->couple && (!o || !o->alpha_a_planck || !o->alpha_a_energy || !o->alpha_s)) return fail(nullptr, RAD_EINVAL, "rad_create: coupling needs opacities");
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return fail(nullptr, RAD_ECUDA, "rad_create: no usable CUDA device (there is no CPU fallback)");
+    }
+    DeviceGuard guard(device);
+    if (!guard.ok) return cuda_fail(nullptr, "rad_create: cudaSetDevice");
+
+    rad_ctx *c = new (std::nothrow) rad_ctx;
+    if (!c) return fail(nullptr, RAD_ENOMEM, "rad_create: out of host memory");
+    c->device = device; c->metric = *m; c->grid = *g; c->angles = *a; c->params = *p;
+    if (o) c->opac = *o;
+    std::string err;
+    bool ok = (a->kind == 0) ? rad::build_latlon(a->nzeta, a->npsi, c->host, err)
+            : (a->kind == 1) ? rad::build_geodesic(a->nlev, c->host, err) : (err = "bad angle grid kind", false);
+    if (!ok) { delete c; return fail(nullptr, RAD_EINVAL, "rad_create: " + err); }
+
+    rad::DeviceTables &t = c->dev;
+    const rad::AngleTables &h = c->host;
+    t.N = h.N; t.E = h.E; t.ng = g->ng;
+    for (int d = 0; d < 3; d++) { t.n[d] = g->n[d]; t.inv_dx[d] = 1.0 / g->dx[d]; }
+    t.NI = g->n[0] + 2 * g->ng; t.NJ = g->n[1] + 2 * g->ng; t.NK = g->n[2] + 2 * g->ng;
+    t.ncell = (long long)t.NI * t.NJ * t.NK;
+    // derived angle tables: pinned products T[e][c][k] = N^c * (n^alpha n^beta), and per-angle signed edge weights
+    std::vector<double> edge_T((size_t)h.E * 30), nbr_w((size_t)h.N * RAD_MAXNBR, 0.0);
+    for (int e = 0; e < h.E; e++) {
+        const double n4[4] = {1.0, h.edge_mid[3 * e], h.edge_mid[3 * e + 1], h.edge_mid[3 * e + 2]};
+        double q[10];
+        int w = 0;
+        for (int al = 0; al < 4; al++) for (int be = al; be < 4; be++) q[w++] = n4[al] * n4[be];
+        for (int ch = 0; ch < 3; ch++) for (int k = 0; k < 10; k++) edge_T[(size_t)e * 30 + ch * 10 + k] = h.edge_nrm[3 * e + ch] * q[k];
+    }
+    for (int n = 0; n < h.N; n++)
+        for (int s = 0; s < RAD_MAXNBR; s++) {
+            const int e = h.nbr_edge[n * RAD_MAXNBR + s];
+            if (e >= 0) nbr_w[n * RAD_MAXNBR + s] = (h.edge_lo[e] == n ? 1.0 : -1.0) / h.domega[n];
+        }
+    const double *d_edge_nrm_unused = nullptr;
+    (void)d_edge_nrm_unused;
+    ok = upload(c, h.nhat, &t.nhat) && upload(c, h.domega, &t.domega) && upload(c, h.nnbr, &t.nnbr) && upload(c, h.nbr_edge, &t.nbr_edge) &&
+         upload(c, h.edge_lo, &t.edge_lo) && upload(c, h.edge_hi, &t.edge_hi) && upload(c, h.edge_len, &t.edge_len) &&
+         upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
+    double *cell = nullptr, *face = nullptr;
+    if (ok) ok = cudaMalloc((void **)&cell, sizeof(double) * t.ncell * RAD_NCELL) == cudaSuccess;
+    if (ok) c->owned.push_back(cell);
+    if (ok) ok = cudaMalloc((void **)&face, sizeof(double) * t.ncell * 3 * RAD_NFACE) == cudaSuccess;
+    if (ok) c->owned.push_back(face);
+    if (ok) ok = cudaMalloc((void **)&c->d_noroot, sizeof(unsigned long long)) == cudaSuccess;
+    if (ok) c->owned.push_back(c->d_noroot);
+    if (!ok) {
+        cudaError_t e = cudaGetLastError();
+        std::string msg = std::string("rad_create: device allocation/upload failed: ") + cudaGetErrorString(e);
+        rad_destroy(c);
+        return fail(nullptr, e == cudaErrorMemoryAllocation ? RAD_ENOMEM : RAD_ECUDA, msg);
+    }
+    t.cell = cell; t.face = face;
+    if (m->kind == 2) {
+        ok = cudaMemcpy(cell, m->cell_tab, sizeof(double) * t.ncell * RAD_NCELL, cudaMemcpyDeviceToDevice) == cudaSuccess &&
+             cudaMemcpy(face, m->face_tab, sizeof(double) * t.ncell * 3 * RAD_NFACE, cudaMemcpyDeviceToDevice) == cudaSuccess;
+    } else {
+        int nl = rad::launch_geometry(*m, *g, cell, face, t.ncell, 0);
+        ok = nl > 0 && cudaDeviceSynchronize() == cudaSuccess;
+        if (ok) c->launches += nl;
+    }
+    if (!ok) {
+        std::string msg = std::string("rad_create: geometry: ") + cudaGetErrorString(cudaGetLastError());
+        rad_destroy(c);
+        return fail(nullptr, RAD_ECUDA, msg);
+    }
+    c->metric.cell_tab = nullptr; c->metric.face_tab = nullptr;
+    c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit;
+    c->kp.recon_space = p->recon_space; c->kp.renorm = p->renorm_fluid_weights; c->kp.couple = p->couple;
+    *out = c;
+    return RAD_OK;
+}
+
+void rad_destroy(rad_ctx *c) {
+    if (!c) return;
+    DeviceGuard guard(c->device);
+    for (void *p : c->owned) cudaFree(p);
+    for (int q = 0; q < 2; q++) if (c->scratch_I[q]) cudaFree(c->scratch_I[q]);
+    if (c->scratch_small) cudaFree(c->scratch_small);
+    delete c;
+}
+
+const char *rad_last_error(const rad_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+long long rad_ncells_total(const rad_ctx *c) { return c ? c->dev.ncell : 0; }
+long long rad_launch_count(const rad_ctx *c) { return c ? c->launches : 0; }
+
+rad_status rad_fill_ghosts(rad_ctx *c, double *I, void *stream) {
+    if (!c || !I) return fail(c, RAD_EINVAL, "rad_fill_ghosts: NULL argument");
+    DeviceGuard guard(c->device);
+    int nl = rad::launch_fill_ghosts(c->dev, c->grid.bc_lo, c->grid.bc_hi, I, (cudaStream_t)stream);
+    if (nl < 0) return cuda_fail(c, "rad_fill_ghosts");
+    c->launches += nl;
+    return RAD_OK;
+}
+
+rad_status rad_transport(rad_ctx *c, double *I_in, double *I_out, const double *I0, double gam0, double gam1, double beta_dt, void *stream) {
+    if (!c || !I_in || !I_out) return fail(c, RAD_EINVAL, "rad_transport: NULL argument");
+    if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_transport: I_out must not alias I_in or I0 (the stencil reads old values)");
+    if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_transport: non-finite weights");
+    DeviceGuard guard(c->device);
+    rad_status st = rad_fill_ghosts(c, I_in, stream);
+    if (st != RAD_OK) return st;
+    int nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, (cudaStream_t)stream);
+    if (nl < 0) return cuda_fail(c, "rad_transport");
+    c->launches += nl;
+    return RAD_OK;
+}
+
+rad_status rad_couple(rad_ctx *c, double *I, const double *fluid, double dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
+    if (!c || !I || !fluid) return fail(c, RAD_EINVAL, "rad_couple: NULL argument");
+    if (!std::isfinite(dt)) return fail(c, RAD_EINVAL, "rad_couple: non-finite dt");
+    if (c->kp.couple && (!c->opac.alpha_a_planck || !c->opac.alpha_a_energy || !c->opac.alpha_s)) return fail(c, RAD_ESTATE, "rad_couple: context has no opacities");
+    DeviceGuard guard(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_couple: memset");
+    int nl = rad::launch_coupling(c->dev, c->kp, I, fluid, c->opac.alpha_a_planck, c->opac.alpha_a_energy, c->opac.alpha_s, dt, T_out, dT0,
+                                  n_noroot ? c->d_noroot : nullptr, s);
+    if (nl < 0) return cuda_fail(c, "rad_couple");
+    c->launches += nl;
+    if (n_noroot) {
+        unsigned long long v = 0;
+        if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+            return cuda_fail(c, "rad_couple: readback");
+        *n_noroot = (long long)v;
+    }
+    return RAD_OK;
+}
+
+rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
+                     double beta_dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
+    if (!c || !fluid) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
+    rad_status st = rad_transport(c, I_in, I_out, I0, gam0, gam1, beta_dt, stream);
+    if (st != RAD_OK) return st;
+    return rad_couple(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot, stream);
+}
+
+rad_status rad_stage_host(rad_ctx *c, const double *I_in_host, double *I_out_host, const double *fluid_host, const double *opac_host,
+                          double gam0, double gam1, double beta_dt, double *T_out_host, double *dT0_host, long long *n_noroot) {
+    if (!c || !I_in_host || !I_out_host || !fluid_host) return fail(c, RAD_EINVAL, "rad_stage_host: NULL argument");
+    if (c->kp.couple && !opac_host) return fail(c, RAD_EINVAL, "rad_stage_host: coupling needs opac_host");
+    DeviceGuard guard(c->device);
+    const long long nc = c->dev.ncell;
+    const size_t ibytes = sizeof(double) * nc * c->dev.N, cb = sizeof(double) * nc;
+    for (int q = 0; q < 2; q++)
+        if (!c->scratch_I[q] && cudaMalloc((void **)&c->scratch_I[q], ibytes) != cudaSuccess) return fail(c, RAD_ENOMEM, "rad_stage_host: device scratch");
+    if (!c->scratch_small && cudaMalloc((void **)&c->scratch_small, 13 * cb) != cudaSuccess) return fail(c, RAD_ENOMEM, "rad_stage_host: device scratch");
+    double *dfl = c->scratch_small, *dop = dfl + 5 * nc, *dT = dop + 3 * nc, *ddT0 = dT + nc;
+    cudaStream_t s = 0;
+    bool ok = cudaMemcpyAsync(c->scratch_I[0], I_in_host, ibytes, cudaMemcpyHostToDevice, s) == cudaSuccess &&
+              cudaMemcpyAsync(dfl, fluid_host, 5 * cb, cudaMemcpyHostToDevice, s) == cudaSuccess;
+    if (ok && opac_host) ok = cudaMemcpyAsync(dop, opac_host, 3 * cb, cudaMemcpyHostToDevice, s) == cudaSuccess;
+    if (!ok) return cuda_fail(c, "rad_stage_host: H2D");
+    // interior-only writes: start I_out from I_in so that ghost cells of the returned array are defined
+    if (cudaMemcpyAsync(c->scratch_I[1], c->scratch_I[0], ibytes, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return cuda_fail(c, "rad_stage_host: D2D");
+    const rad_opac saved = c->opac;
+    c->opac.alpha_a_planck = dop; c->opac.alpha_a_energy = dop + nc; c->opac.alpha_s = dop + 2 * nc;
+    rad_status st = rad_stage(c, c->scratch_I[0], c->scratch_I[1], nullptr, dfl, gam0, gam1, beta_dt, dT, ddT0, n_noroot, s);
+    c->opac = saved;
+    if (st != RAD_OK) return st;
+    ok = cudaMemcpyAsync(I_out_host, c->scratch_I[1], ibytes, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (ok && T_out_host) ok = cudaMemcpyAsync(T_out_host, dT, cb, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (ok && dT0_host) ok = cudaMemcpyAsync(dT0_host, ddT0, 4 * cb, cudaMemcpyDeviceToHost, s) == cudaSuccess;
+    if (!ok || cudaStreamSynchronize(s) != cudaSuccess) return cuda_fail(c, "rad_stage_host: D2H");
+    return RAD_OK;
+}
+
+rad_status rad_moments(rad_ctx *c, const double *I, int frame, const double *fluid, double *out, void *stream) {
+    if (!c || !I || !out) return fail(c, RAD_EINVAL, "rad_moments: NULL argument");
+    if (frame < 0 || frame > 3) return fail(c, RAD_EINVAL, "rad_moments: frame must be 0..3");
+    if (frame == 3 && !fluid) return fail(c, RAD_EINVAL, "rad_moments: fluid frame needs fluid");
+    DeviceGuard guard(c->device);
+    int nl = rad::launch_moments(c->dev, I, frame, fluid, out, (cudaStream_t)stream);
+    if (nl < 0) return cuda_fail(c, "rad_moments");
+    c->launches += nl;
+    return RAD_OK;
+}
+
+rad_status rad_get_table(rad_ctx *c, int which, void *host_out, size_t nbytes) {
+    if (!c || !host_out) return fail(c, RAD_EINVAL, "rad_get_table: NULL argument");
+    DeviceGuard guard(c->device);
+    const rad::AngleTables &h = c->host;
+    const rad::DeviceTables &t = c->dev;
+    const void *src = nullptr;
+    size_t need = 0;
+    int nang = h.N, nedge = h.E;
+    switch (which) {
+        case RAD_TAB_NANG: src = &nang; need = sizeof(int); break;
+        case RAD_TAB_NEDGE: src = &nedge; need = sizeof(int); break;
+        case RAD_TAB_NHAT: src = h.nhat.data(); need = sizeof(double) * 3 * h.N; break;
+        case RAD_TAB_DOMEGA: src = h.domega.data(); need = sizeof(double) * h.N; break;
+        case RAD_TAB_NNBR: src = h.nnbr.data(); need = sizeof(int) * h.N; break;
+        case RAD_TAB_NBR: src = h.nbr.data(); need = sizeof(int) * RAD_MAXNBR * h.N; break;
+        case RAD_TAB_NBR_EDGE: src = h.nbr_edge.data(); need = sizeof(int) * RAD_MAXNBR * h.N; break;
+        case RAD_TAB_EDGE_LO: src = h.edge_lo.data(); need = sizeof(int) * h.E; break;
+        case RAD_TAB_EDGE_HI: src = h.edge_hi.data(); need = sizeof(int) * h.E; break;
+        case RAD_TAB_EDGE_LEN: src = h.edge_len.data(); need = sizeof(double) * h.E; break;
+        case RAD_TAB_EDGE_MID: src = h.edge_mid.data(); need = sizeof(double) * 3 * h.E; break;
+        case RAD_TAB_EDGE_NRM: src = h.edge_nrm.data(); need = sizeof(double) * 3 * h.E; break;
+        case RAD_TAB_CELL: need = sizeof(double) * t.ncell * RAD_NCELL; break;
+        case RAD_TAB_FACE: need = sizeof(double) * t.ncell * 3 * RAD_NFACE; break;
+        case RAD_TAB_FACE_SIGN: need = (size_t)t.ncell * 3 * t.N; break;
+        case RAD_TAB_EDGE_SIGN: need = (size_t)t.ncell * t.E; break;
+        case RAD_TAB_MAXSPEED: need = 3 * sizeof(double); break;
+        default: return fail(c, RAD_EINVAL, "rad_get_table: unknown table");
+    }
+    if (nbytes != need) {
+        char buf[128];
+        snprintf(buf, sizeof buf, "rad_get_table: table %d has %zu bytes, caller gave %zu", which, need, nbytes);
+        return fail(c, RAD_EINVAL, buf);
+    }
+    if (src) { memcpy(host_out, src, need); return RAD_OK; }
+    if (which == RAD_TAB_CELL || which == RAD_TAB_FACE) {
+        if (cudaMemcpy(host_out, which == RAD_TAB_CELL ? t.cell : t.face, need, cudaMemcpyDeviceToHost) != cudaSuccess) return cuda_fail(c, "rad_get_table");
+        return RAD_OK;
+    }
+    void *tmp = nullptr;
+    if (cudaMalloc(&tmp, need) != cudaSuccess) { cudaGetLastError(); return fail(c, RAD_ENOMEM, "rad_get_table: device scratch"); }
+    int nl = 0;
+    if (which == RAD_TAB_FACE_SIGN) nl = rad::launch_sign_tables(t, (signed char *)tmp, nullptr, 0);
+    else if (which == RAD_TAB_EDGE_SIGN) nl = rad::launch_sign_tables(t, nullptr, (signed char *)tmp, 0);
+    else nl = rad::launch_maxspeed(t, (double *)tmp, 0);
+    bool ok = nl >= 0 && cudaMemcpy(host_out, tmp, need, cudaMemcpyDeviceToHost) == cudaSuccess;
+    cudaFree(tmp);
+    if (!ok) return cuda_fail(c, "rad_get_table");
+    c->launches += nl;
+    return RAD_OK;
+}
+
+}  // extern "C"

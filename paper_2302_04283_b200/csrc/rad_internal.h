@@ -1,0 +1,69 @@
+// rad_internal.h -- shared declarations of librad.so's translation units (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "rad.h"
+
+namespace rad {
+
+// Angle grid tables, built on the host (section 2.6 of the paper).
+struct AngleTables {
+    int N = 0, E = 0;
+    std::vector<double> nhat;      // [N][3]
+    std::vector<double> domega;    // [N]
+    std::vector<int> nnbr;         // [N]
+    std::vector<int> nbr;          // [N][6]
+    std::vector<int> nbr_edge;     // [N][6]
+    std::vector<int> edge_lo, edge_hi;  // [E]
+    std::vector<double> edge_len;  // [E]
+    std::vector<double> edge_mid;  // [E][3]
+    std::vector<double> edge_nrm;  // [E][3]
+};
+bool build_latlon(int nzeta, int npsi, AngleTables &out, std::string &err);
+bool build_geodesic(int nlev, AngleTables &out, std::string &err);
+
+// Everything the kernels read besides the caller's arrays (device pointers).
+struct DeviceTables {
+    int N, E;
+    int n[3], ng, NI, NJ, NK;
+    long long ncell;
+    double inv_dx[3];
+    // angle tables
+    const double *nhat;      // [N][3]
+    const double *domega;    // [N]
+    const int *nnbr;         // [N]
+    const int *nbr_edge;     // [N][6]
+    const int *edge_lo, *edge_hi;  // [E]
+    const double *edge_len;  // [E]
+    const double *edge_mid;  // [E][3]
+    const double *edge_T;    // [E][30]  pinned products N^c * (n^a n^b)
+    // per angle: signed weights of its edges, sgn * dlambda_e / dOmega_n, [N][6] (0 where no edge)
+    const double *nbr_w;
+    // geometry
+    const double *cell;  // [ncell][RAD_NCELL]
+    const double *face;  // [ncell][3][RAD_NFACE]
+};
+
+struct Params {
+    double gamma_gas, a_rad, n0_crit;
+    int recon_space, renorm, couple;
+};
+
+// kernel launchers (each returns the number of kernels it launched, or -1 after setting a CUDA error)
+int launch_geometry(const rad_metric &m, const rad_grid &g, double *cell, double *face, long long ncell,
+                    cudaStream_t s);
+int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_hi[3], double *I, cudaStream_t s);
+int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, const double *I0, double gam0,
+                   double gam1, double beta_dt, double *I_out, cudaStream_t s);
+int launch_coupling(const DeviceTables &t, const Params &p, double *I, const double *fluid, const double *aP,
+                    const double *aE, const double *aS, double dt, double *T_out, double *dT0,
+                    unsigned long long *noroot, cudaStream_t s);
+int launch_moments(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out,
+                   cudaStream_t s);
+int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed char *edge_sign, cudaStream_t s);
+int launch_maxspeed(const DeviceTables &t, double *out3, cudaStream_t s);
+
+}  // namespace rad

@@ -1,0 +1,190 @@
+// transport.cu -- subsystems 2 and 4: fused spatial+angular flux-divergence kernel and ghost fill.
+//
+// Paper: section 2.3-2.4.  Eq.24 spatial upwind flux, Eq.25 angular upwind flux, Eq.22 update
+// of C = n^0 n_0 I, then I* = C*/(n^0 n_0).  Intensities are I[cell][angle], angle innermost.
+#include <math.h>
+
+#include "rad_internal.h"
+
+namespace rad {
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// ghost fill: one launch per axis, in x, y, z order so that edges and corners are filled
+// ------------------------------------------------------------------------------------------------
+__global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int NK, int ng, int axis, int nint, int bc_lo, int bc_hi) {
+    // one CTA per ghost cell of this axis' two slabs; threads over angles
+    const int dims[3] = {NI, NJ, NK};
+    int d[3];
+    // enumerate ghost cells: along `axis` 2*ng layers, full extent in the other two
+    int ext[3] = {NI, NJ, NK};
+    ext[axis] = 2 * ng;
+    long long b = blockIdx.x;
+    d[0] = (int)(b % ext[0]); b /= ext[0];
+    d[1] = (int)(b % ext[1]); b /= ext[1];
+    d[2] = (int)b;
+    int q = d[axis];
+    const bool low = q < ng;
+    if (!low) q = dims[axis] - 2 * ng + q;  // upper slab
+    d[axis] = q;
+    const int bc = low ? bc_lo : bc_hi;
+    if (bc == 0) return;
+    int src = q;
+    if (bc == 1) src = ng + (((q - ng) % nint) + nint) % nint;
+    else src = low ? ng : ng + nint - 1;
+    int s[3] = {d[0], d[1], d[2]};
+    s[axis] = src;
+    const long long cd = ((long long)d[2] * NJ + d[1]) * NI + d[0], cs = ((long long)s[2] * NJ + s[1]) * NI + s[0];
+    const double2 *ps = reinterpret_cast<const double2 *>(I + cs * N);
+    double2 *pd = reinterpret_cast<double2 *>(I + cd * N);
+    if ((N & 1) == 0) {
+        for (int n = threadIdx.x; n < N / 2; n += blockDim.x) pd[n] = ps[n];
+    } else {
+        for (int n = threadIdx.x; n < N; n += blockDim.x) I[cd * N + n] = I[cs * N + n];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// fused flux divergence, version 1: one CTA per run of CX cells along x
+// ------------------------------------------------------------------------------------------------
+constexpr int CX = 8;
+
+__device__ __forceinline__ double chain4(const double *r, double n1, double n2, double n3) {
+    // pinned order (decides upwind signs): fma(r3,n3, fma(r2,n2, fma(r1,n1, r0)))
+    return fma(r[3], n3, fma(r[2], n2, fma(r[1], n1, r[0])));
+}
+
+__device__ __forceinline__ double vl_slope(double qm, double q0, double qp) {
+    // van Leer harmonic-mean limiter (R7)
+    const double dl = q0 - qm, dr = qp - q0, pr = dl * dr;
+    return pr > 0.0 ? 2.0 * pr / (dl + dr) : 0.0;
+}
+
+// flux through the face whose record is `f`, between cells L (lower) and R (upper) along a stride `st`
+template <bool PLM>
+__device__ __forceinline__ double face_flux(const double *f, double n1, double n2, double n3, const double *__restrict__ pR, long long st) {
+    const double na = chain4(f, n1, n2, n3), n0 = chain4(f + 4, n1, n2, n3);
+    double up;
+    if (na > 0.0) {
+        const double qL = pR[-st];
+        up = qL;
+        if (PLM) up = qL + 0.5 * vl_slope(pR[-2 * st], qL, pR[0]);
+    } else if (na < 0.0) {
+        const double qR = pR[0];
+        up = qR;
+        if (PLM) up = qR - 0.5 * vl_slope(pR[-st], qR, pR[st]);
+    } else {
+        return 0.0;
+    }
+    return na * n0 * up;
+}
+
+template <bool PLM>
+__global__ void __launch_bounds__(256) k_fluxdiv_v1(DeviceTables t, const double *__restrict__ I_in, const double *__restrict__ I0,
+                                                   double gam0, double gam1, double beta_dt, double *__restrict__ I_out) {
+    extern __shared__ double smem[];
+    const int N = t.N, E = t.E;
+    double *sCell = smem;                 // [CX][36]: n^0, E[4], S[30], excised
+    double *sFx = sCell + CX * 36;        // [CX+1][8]  lower x-face of cells i0..i0+CX
+    double *sFy = sFx + (CX + 1) * 8;     // [2][CX][8] lower y-face of (j) and (j+1)
+    double *sFz = sFy + 2 * CX * 8;       // [2][CX][8]
+    double *sFe = sFz + 2 * CX * 8;       // [CX][E]   dlambda_e * c_e * n_0e * I_up
+
+    const int nxb = (t.n[0] + CX - 1) / CX;
+    long long b = blockIdx.x;
+    const int ib = (int)(b % nxb); b /= nxb;
+    const int j = (int)(b % t.n[1]) + t.ng;
+    const int k = (int)(b / t.n[1]) + t.ng;
+    const int i0 = ib * CX + t.ng;
+    const int ncx = min(CX, t.n[0] + t.ng - i0);
+    const long long sy = t.NI, sz = (long long)t.NI * t.NJ;
+    const long long c0 = ((long long)k * t.NJ + j) * t.NI + i0;
+
+    for (int q = threadIdx.x; q < ncx * 36; q += blockDim.x) {
+        const int cl = q / 36, w = q % 36;
+        sCell[q] = (w < 35) ? t.cell[(c0 + cl) * RAD_NCELL + w] : t.cell[(c0 + cl) * RAD_NCELL + 50];
+    }
+    for (int q = threadIdx.x; q < (ncx + 1) * 8; q += blockDim.x) sFx[q] = t.face[((c0 + q / 8) * 3 + 0) * RAD_NFACE + q % 8];
+    for (int q = threadIdx.x; q < 2 * ncx * 8; q += blockDim.x) {
+        const int up = q / (ncx * 8), r = q % (ncx * 8);
+        sFy[up * CX * 8 + r] = t.face[((c0 + r / 8 + up * sy) * 3 + 1) * RAD_NFACE + r % 8];
+        sFz[up * CX * 8 + r] = t.face[((c0 + r / 8 + up * sz) * 3 + 2) * RAD_NFACE + r % 8];
+    }
+    __syncthreads();
+
+    // phase A: angular fluxes, once per unique edge (Eq.25, donor cell in angle)
+    for (int q = threadIdx.x; q < ncx * E; q += blockDim.x) {
+        const int cl = q / E, e = q % E;
+        const double *S = sCell + cl * 36 + 5;
+        const double *T = t.edge_T + (long long)e * 30;
+        double acc = 0.0;
+#pragma unroll
+        for (int w = 0; w < 30; w++) acc = fma(S[w], __ldg(T + w), acc);  // pinned 30-term chain
+        const double ce = -acc;
+        const double n0e = chain4(sCell + cl * 36 + 1, __ldg(t.edge_mid + 3 * e), __ldg(t.edge_mid + 3 * e + 1), __ldg(t.edge_mid + 3 * e + 2));
+        const int a_up = ce > 0.0 ? __ldg(t.edge_lo + e) : __ldg(t.edge_hi + e);
+        const double Iup = I_in[(c0 + cl) * N + a_up];
+        sFe[cl * E + e] = (ce == 0.0) ? 0.0 : __ldg(t.edge_len + e) * (ce * n0e * Iup);
+    }
+    __syncthreads();
+
+    // phase B: spatial fluxes and the update, per (cell, angle)
+    for (int q = threadIdx.x; q < ncx * N; q += blockDim.x) {
+        const int cl = q / N, n = q % N;
+        const long long c = c0 + cl;
+        const double *cg = sCell + cl * 36;
+        double *out = I_out + c * N + n;
+        if (cg[35] != 0.0) { *out = 0.0; continue; }
+        const double n1 = __ldg(t.nhat + 3 * n), n2 = __ldg(t.nhat + 3 * n + 1), n3 = __ldg(t.nhat + 3 * n + 2);
+        const double *p = I_in + c * N + n;
+        const long long sx = N;
+        double div = 0.0;
+        div += (face_flux<PLM>(sFx + (cl + 1) * 8, n1, n2, n3, p + sx, sx) - face_flux<PLM>(sFx + cl * 8, n1, n2, n3, p, sx)) * t.inv_dx[0];
+        div += (face_flux<PLM>(sFy + CX * 8 + cl * 8, n1, n2, n3, p + sy * N, sy * N) - face_flux<PLM>(sFy + cl * 8, n1, n2, n3, p, sy * N)) * t.inv_dx[1];
+        div += (face_flux<PLM>(sFz + CX * 8 + cl * 8, n1, n2, n3, p + sz * N, sz * N) - face_flux<PLM>(sFz + cl * 8, n1, n2, n3, p, sz * N)) * t.inv_dx[2];
+        double adiv = 0.0;
+#pragma unroll
+        for (int s = 0; s < RAD_MAXNBR; s++) {
+            const int e = __ldg(t.nbr_edge + n * RAD_MAXNBR + s);
+            if (e >= 0) adiv = fma(__ldg(t.nbr_w + n * RAD_MAXNBR + s), sFe[cl * E + e], adiv);
+        }
+        div += adiv;
+        const double w = cg[0] * chain4(cg + 1, n1, n2, n3);  // n^0 n_0
+        double C = gam1 * (w * p[0]);
+        if (I0 != nullptr) C = fma(gam0, w * I0[c * N + n], C);
+        *out = (C - beta_dt * div) / w;
+    }
+}
+
+}  // namespace
+
+int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_hi[3], double *I, cudaStream_t s) {
+    int launches = 0;
+    for (int ax = 0; ax < 3; ax++) {
+        if (bc_lo[ax] == 0 && bc_hi[ax] == 0) continue;
+        long long ext[3] = {t.NI, t.NJ, t.NK};
+        ext[ax] = 2 * t.ng;
+        const long long blocks = ext[0] * ext[1] * ext[2];
+        k_fill_ghosts<<<(unsigned)blocks, 64, 0, s>>>(I, t.N, t.NI, t.NJ, t.NK, t.ng, ax, t.n[ax], bc_lo[ax], bc_hi[ax]);
+        if (cudaGetLastError() != cudaSuccess) return -1;
+        launches++;
+    }
+    return launches;
+}
+
+int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, const double *I0, double gam0, double gam1,
+                   double beta_dt, double *I_out, cudaStream_t s) {
+    const int nxb = (t.n[0] + CX - 1) / CX;
+    const long long blocks = (long long)nxb * t.n[1] * t.n[2];
+    const size_t smem = sizeof(double) * (CX * 36 + (CX + 1) * 8 + 4 * CX * 8 + (size_t)CX * t.E);
+    if (p.recon_space == 1) {
+        cudaFuncSetAttribute(k_fluxdiv_v1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        k_fluxdiv_v1<true><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out);
+    } else {
+        cudaFuncSetAttribute(k_fluxdiv_v1<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        k_fluxdiv_v1<false><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out);
+    }
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace rad

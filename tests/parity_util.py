@@ -1,0 +1,59 @@
+"""Shared helpers of the GPU parity tests: build the same problem on both sides, convert the oracle's
+geometry records to the library's tabulated-metric layout (rad.h), compare."""
+import numpy as np
+
+from paper_2302_04283_b200 import workloads as W
+
+TOL_I, TOL_FLUID = 1e-11, 1e-10   # north_star: max relative error per intensity / on fluid energy after one stage
+
+
+def oracle_tables_to_rad(cell, face, excised):
+    """oracle cell record (alpha, e[4][4], L[4][4], S[30], beta[3], gamma[6]) -> rad.h RAD_NCELL layout"""
+    nc = cell.shape[0]
+    e = cell[:, 1:17].reshape(nc, 4, 4); L = cell[:, 17:33].reshape(nc, 4, 4)
+    out = np.zeros((nc, 52))
+    out[:, 0] = e[:, 0, 0]
+    out[:, 1:5] = L[:, 0, :]
+    out[:, 5:35] = cell[:, 33:63]
+    out[:, 35:38] = cell[:, 63:66]
+    out[:, 38:44] = np.stack([e[:, 1, 1], e[:, 1, 2], e[:, 1, 3], e[:, 2, 2], e[:, 2, 3], e[:, 3, 3]], 1)
+    out[:, 44:50] = np.stack([L[:, 1, 1], L[:, 2, 1], L[:, 3, 1], L[:, 2, 2], L[:, 3, 2], L[:, 3, 3]], 1)
+    out[:, 50] = excised
+    return out, face.copy()
+
+
+def make_oracle(oracle, cfg, n=None, **kw):
+    c = W.CONFIGS[cfg]
+    A = oracle.Angles(*c["angles"])
+    nn, ng, x0, dx = W.grid(cfg, n)
+    args = dict(metric_kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg), bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3,
+                gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=1, renorm=1, couple=1)
+    args.update(kw)
+    return A, oracle.Problem(A, nn, x0, dx, **args)
+
+
+def make_rad(B, cfg, opac, n=None, tabulated=None, device=0, **kw):
+    """rad_create for config cfg; opac = CUDA tensor [3, ncell]; tabulated = (cell_tab, face_tab) CUDA tensors or None"""
+    c = W.CONFIGS[cfg]
+    nn, ng, x0, dx = W.grid(cfg, n)
+    metric = dict(kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg))
+    if tabulated is not None:
+        metric = dict(kind=2, cell_tab=tabulated[0], face_tab=tabulated[1])
+    grid = dict(n=nn, x0=x0, dx=dx, bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3)
+    params = dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=1, renorm_fluid_weights=1, couple=1)
+    params.update(kw)
+    op = None if opac is None else (opac[0], opac[1], opac[2])
+    return B.rad_create(metric, grid, c["angles"], op, params, device)
+
+
+def rel_err_I(got, ref):
+    """max over interior (cell, angle) of |dI| / max(|I_ref|, 1e-12 * mean_n |I_ref| of the cell)"""
+    den = np.maximum(np.abs(ref), 1e-12 * np.abs(ref).mean(-1, keepdims=True))
+    den = np.where(den == 0, 1.0, den)
+    return float((np.abs(got - ref) / den).max())
+
+
+def rel_err(got, ref, floor):
+    den = np.maximum(np.abs(ref), floor)
+    den = np.where(den == 0, 1.0, den)
+    return float((np.abs(got - ref) / den).max())

@@ -1,0 +1,293 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Bars (north_star): intensities <= 1e-11 relative, fluid energy / four-momentum <= 1e-10,
+integer tables (angle neighbours, upwind signs) bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2302_04283_b200 import workloads as W
+from parity_util import TOL_FLUID, TOL_I, make_oracle, make_rad, oracle_tables_to_rad, rel_err, rel_err_I
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2302_04283_b200 import binding, build
+    build.build()
+    binding.lib()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return binding
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a)).cuda()
+
+
+# ------------------------------------------------------------------------------------------------ tables
+@pytest.mark.parametrize("angles", [("latlon", 5, 16), ("latlon", 1, 4), ("latlon", 2, 1), ("geodesic", 1), ("geodesic", 3), ("geodesic", 4), ("geodesic", 7)])
+def test_angle_tables_bit_exact(oracle, B, angles):
+    A = oracle.Angles(*angles)
+    h = B.rad_create(dict(kind=0), dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1)), angles, None, dict(couple=0))
+    try:
+        assert B.rad_get_table(h, B.TAB_NANG) == A.N and B.rad_get_table(h, B.TAB_NEDGE) == A.E
+        for tab, ref in ((B.TAB_NNBR, A.nnbr), (B.TAB_NBR, A.nbr), (B.TAB_NBR_EDGE, A.nbr_edge), (B.TAB_EDGE_LO, A.edge_lo), (B.TAB_EDGE_HI, A.edge_hi)):
+            assert np.array_equal(B.rad_get_table(h, tab), ref)
+        assert np.array_equal(B.rad_get_table(h, B.TAB_NHAT), A.nhat)     # same operation order => same bits
+        for tab, ref in ((B.TAB_DOMEGA, A.domega), (B.TAB_EDGE_LEN, A.edge_len), (B.TAB_EDGE_MID, A.edge_mid), (B.TAB_EDGE_NRM, A.edge_nrm)):
+            assert np.abs(B.rad_get_table(h, tab) - ref).max() < 1e-15
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("cfg,n", [("C1", 6), ("C2", 10), ("C3", 9), ("C4", 8), ("C5", 10)])
+def test_geometry_tables(oracle, B, cfg, n):
+    """level 1: geometry built by the CUDA kernel vs the oracle's, <= 1e-13; upwind sign mismatches counted (expected 0)"""
+    A, P = make_oracle(oracle, cfg, n)
+    cell, face, ex = P.geometry()
+    rc, rf = oracle_tables_to_rad(cell, face, ex)
+    h = make_rad(B, cfg, None, n, couple=0)
+    try:
+        gc, gf = B.rad_get_table(h, B.TAB_CELL), B.rad_get_table(h, B.TAB_FACE)
+        assert np.abs(gc - rc).max() < 1e-13, np.abs(gc - rc).max(0)
+        assert np.abs(gf - rf).max() < 1e-13
+        fs, es = P.upwind_tables()
+        assert (B.rad_get_table(h, B.TAB_FACE_SIGN) != fs).sum() == 0
+        assert (B.rad_get_table(h, B.TAB_EDGE_SIGN) != es).sum() == 0
+        vmax, vax = P.max_speed()
+        assert np.abs(B.rad_get_table(h, B.TAB_MAXSPEED) - np.array(vax)).max() < 1e-13
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("cfg,n", [("C2", 10), ("C3", 9)])
+def test_upwind_tables_bit_exact_on_shared_geometry(oracle, B, cfg, n):
+    """level 2: fed the oracle's geometry tables, the upwind index tables are identical bit for bit"""
+    A, P = make_oracle(oracle, cfg, n)
+    cell, face, ex = P.geometry()
+    rc, rf = oracle_tables_to_rad(cell, face, ex)
+    h = make_rad(B, cfg, None, n, tabulated=(dev(rc), dev(rf)), couple=0)
+    try:
+        fs, es = P.upwind_tables()
+        assert np.array_equal(B.rad_get_table(h, B.TAB_FACE_SIGN), fs)
+        assert np.array_equal(B.rad_get_table(h, B.TAB_EDGE_SIGN), es)
+        assert (es != 0).any() and (fs != 0).all()
+    finally:
+        B.rad_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ the stage
+def run_both(oracle, B, cfg, n, level, I0w=None, **kw):
+    okw = {{"renorm_fluid_weights": "renorm"}.get(k, k): v for k, v in kw.items()}
+    A, P = make_oracle(oracle, cfg, n, **okw)
+    inp = W.make_inputs(cfg, A.nhat, n=n)
+    I = inp["I"].numpy().reshape(-1, A.N).copy()
+    fluid = inp["fluid"].numpy().reshape(5, -1).copy(); opac = inp["opac"].numpy().reshape(3, -1).copy()
+    vmax, _ = P.max_speed()
+    nn, ng, x0, dx = W.grid(cfg, n)
+    dt = W.CFL * min(dx) / vmax
+    I0 = None
+    gam0, gam1, bdt = 0.0, 1.0, dt
+    if I0w is not None:
+        I0 = I * (1.0 + 0.05 * np.sin(np.arange(I.size).reshape(I.shape)))
+        gam0, gam1, bdt = I0w
+        bdt *= dt
+    d_opac = dev(opac)
+    tab = None
+    if level == 2:
+        rc, rf = oracle_tables_to_rad(*P.geometry())
+        tab = (dev(rc), dev(rf))
+    h = make_rad(B, cfg, d_opac, n, tabulated=tab, **kw)
+    try:
+        dI = dev(I); dO = torch.full_like(dI, -7.0); dfl = dev(fluid)
+        dT = torch.zeros(P.ncell, dtype=torch.float64, device="cuda"); ddT0 = torch.zeros(4, P.ncell, dtype=torch.float64, device="cuda")
+        nf_g = B.rad_stage(h, dI, dO, None if I0 is None else dev(I0), dfl, gam0, gam1, bdt, dT, ddT0, count_noroot=True)
+        torch.cuda.synchronize()
+        Iin_after = dI.cpu().numpy()
+        out_g, T_g, dT0_g = dO.cpu().numpy(), dT.cpu().numpy(), ddT0.cpu().numpy()
+    finally:
+        B.rad_destroy(h)
+    Iorc = I.copy()
+    out_o, T_o, dT0_o, nf_o = P.stage(Iorc, fluid, opac, bdt, I0=I0, gam0=gam0, gam1=gam1)
+    # ghost fill of I_in agrees bit for bit; ghosts of I_out are not touched
+    assert np.array_equal(Iin_after, Iorc)
+    full = out_g.reshape(P.shape + (A.N,)).copy()
+    P.interior(full)[...] = -7.0
+    assert (full == -7.0).all()
+    R0 = P.moments(out_o, 1)
+    res = dict(I=rel_err_I(P.interior(out_g), P.interior(out_o)), T=rel_err(P.interior(T_g), P.interior(T_o), 0.0),
+               dT0=max(rel_err(P.interior(dT0_g[m]), P.interior(dT0_o[m]), 1e-12 * np.abs(P.interior(R0[m])).max() + 1e-300) for m in range(4)),
+               nf=(nf_g, nf_o), Tchange=float(np.abs(P.interior(T_o) / P.interior(fluid[1]) - 1).max()))
+    return res
+
+
+@pytest.mark.parametrize("level", [1, 2])
+@pytest.mark.parametrize("cfg,n", [("C1", 16), ("C2", 21), ("C3", 19), ("C4", 13), ("C5", 18)])
+def test_stage_parity(oracle, B, cfg, n, level):
+    r = run_both(oracle, B, cfg, n, level)
+    assert r["nf"][0] == r["nf"][1] == 0
+    assert r["I"] <= TOL_I, r
+    assert r["T"] <= TOL_FLUID and r["dT0"] <= TOL_FLUID, r
+    assert r["Tchange"] > 1e-6  # the coupling did something
+
+
+@pytest.mark.parametrize("kw", [dict(recon_space=0), dict(couple=0), dict(renorm_fluid_weights=0), dict(n0_crit=0.0)])
+def test_stage_parity_options(oracle, B, kw):
+    r = run_both(oracle, B, "C2", 11, 1, **kw)
+    assert r["I"] <= TOL_I and r["T"] <= TOL_FLUID and r["dT0"] <= TOL_FLUID, r
+
+
+def test_stage_parity_rk_weights(oracle, B):
+    """R8: second Heun stage, C* = (C0 + C)/2 - (dt/2) div"""
+    r = run_both(oracle, B, "C2", 9, 1, I0w=(0.5, 0.5, 0.5))
+    assert r["I"] <= TOL_I and r["T"] <= TOL_FLUID and r["dT0"] <= TOL_FLUID, r
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+def small_problem(oracle, B, n, angles, kind=1, a=0.9, bc=(0, 0, 0, 0, 0, 0), x0=(3.0, 2.0, 1.0), dx=(0.3, 0.25, 0.2), excise_r=0.0, **params):
+    A = oracle.Angles(*angles)
+    bl, bh = bc[:3], bc[3:]
+    okw = dict(recon_space=params.get("recon_space", 1), renorm=params.get("renorm_fluid_weights", 1), couple=params.get("couple", 1),
+               n0_crit=params.get("n0_crit", 0.1))
+    P = oracle.Problem(A, n, x0, dx, metric_kind=kind, M=1.0, a=a, excise_r=excise_r, bc_lo=bl, bc_hi=bh, **okw)
+    rng = np.random.default_rng(42)
+    nc = P.ncell
+    I = np.exp(rng.normal(size=(nc, A.N)))
+    fluid = np.stack([rng.uniform(0.5, 2, nc), rng.uniform(0.3, 1.5, nc)] + [rng.uniform(-0.4, 0.4, nc) for _ in range(3)])
+    opac = np.stack([rng.uniform(0.1, 30, nc)] * 2 + [rng.uniform(0.1, 30, nc)])
+    d_opac = dev(opac)
+    h = B.rad_create(dict(kind=kind, M=1.0, a=a, excise_r=excise_r), dict(n=n, x0=x0, dx=dx, bc_lo=bl, bc_hi=bh), angles,
+                     (d_opac[0], d_opac[1], d_opac[2]), dict(params))
+    return A, P, h, I, fluid, opac, d_opac
+
+
+def compare_stage(B, A, P, h, I, fluid, opac, dt):
+    dI = dev(I); dO = torch.zeros_like(dI); dfl = dev(fluid)
+    dT = torch.zeros(P.ncell, dtype=torch.float64, device="cuda"); ddT0 = torch.zeros(4, P.ncell, dtype=torch.float64, device="cuda")
+    nf = B.rad_stage(h, dI, dO, None, dfl, 0.0, 1.0, dt, dT, ddT0, count_noroot=True)
+    Io = I.copy()
+    out_o, T_o, dT0_o, nf_o = P.stage(Io, fluid, opac, dt)
+    assert nf == nf_o
+    assert np.array_equal(dI.cpu().numpy(), Io)
+    eI = rel_err_I(P.interior(dO.cpu().numpy()), P.interior(out_o))
+    eT = rel_err(P.interior(dT.cpu().numpy()), P.interior(T_o), 0.0)
+    assert eI <= TOL_I and eT <= TOL_FLUID, (eI, eT)
+    return dO.cpu().numpy(), out_o
+
+
+@pytest.mark.parametrize("n", [(1, 1, 1), (3, 5, 9), (17, 2, 3), (8, 8, 8)])
+@pytest.mark.parametrize("bc", [(0, 0, 0, 0, 0, 0), (1, 1, 1, 1, 1, 1), (2, 1, 0, 2, 1, 2)])
+def test_ragged_grids_and_boundaries(oracle, B, n, bc):
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, ("geodesic", 2), bc=bc)
+    try:
+        compare_stage(B, A, P, h, I, fluid, opac, 0.05)
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("angles", [("latlon", 1, 4), ("latlon", 3, 1), ("latlon", 4, 8), ("geodesic", 1), ("geodesic", 5)])
+def test_angle_grids(oracle, B, angles):
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (5, 4, 3), angles)
+    try:
+        compare_stage(B, A, P, h, I, fluid, opac, 0.05)
+    finally:
+        B.rad_destroy(h)
+
+
+def test_ergosphere_mask_and_excision(oracle, B):
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (8, 8, 4), ("geodesic", 3), x0=(-2.0, -2.0, -0.2), dx=(0.5, 0.5, 0.1), excise_r=1.5)
+    try:
+        got, ref = compare_stage(B, A, P, h, I, fluid, opac, 0.01)
+        gi, ri = P.interior(got), P.interior(ref)
+        assert np.array_equal(gi == 0.0, ri == 0.0)          # same cells/angles masked or excised
+        ex = P.interior(P.geometry()[2].astype(bool))
+        assert ex.any() and (ri[ex] == 0).all() and (ri[~ex] == 0).any() and (ri[~ex] != 0).any()
+    finally:
+        B.rad_destroy(h)
+
+
+def test_no_root_is_counted(oracle, B):
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (4, 3, 2), ("latlon", 2, 4), kind=0, a=0.0)
+    try:
+        fluid[1, ::2] = -3.0   # unphysical negative gas temperature in every other cell => no positive root there
+        I[:] = 0.0
+        dI = dev(I); dO = torch.zeros_like(dI); dfl = dev(fluid); dT = torch.zeros(P.ncell, dtype=torch.float64, device="cuda")
+        nf = B.rad_stage(h, dI, dO, None, dfl, 0.0, 1.0, 0.1, dT, None, count_noroot=True)
+        out_o, T_o, _, nf_o = P.stage(I.copy(), fluid, opac, 0.1)
+        assert nf == nf_o and nf > 0
+        assert np.array_equal(P.interior(dT.cpu().numpy())[P.interior(fluid[1]) < 0], P.interior(fluid[1])[P.interior(fluid[1]) < 0])
+    finally:
+        B.rad_destroy(h)
+
+
+def test_error_codes(oracle, B):
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (2, 2, 2), ("latlon", 2, 4))
+    try:
+        dI = dev(I); dfl = dev(fluid)
+        with pytest.raises(B.RadError) as e:
+            B.rad_stage(h, dI, dI, None, dfl, 0.0, 1.0, 0.1)
+        assert e.value.status == 1 and "alias" in str(e.value)
+        with pytest.raises(B.RadError) as e:
+            B.rad_stage(h, dI, torch.zeros_like(dI), None, dfl, 0.0, 1.0, float("nan"))
+        assert e.value.status == 1
+        with pytest.raises(B.RadError):
+            B.rad_moments(h, dI, 7, None, torch.zeros(10, P.ncell, dtype=torch.float64, device="cuda"))
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("frame", [0, 1, 2, 3])
+def test_moments_parity(oracle, B, frame):
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (5, 4, 3), ("geodesic", 3))
+    try:
+        ncomp = 10 if frame in (0, 2) else 4
+        out = torch.zeros(ncomp, P.ncell, dtype=torch.float64, device="cuda")
+        B.rad_moments(h, dev(I), frame, dev(fluid), out)
+        ref = P.moments(I, frame, fluid)
+        for q in range(ncomp):
+            assert rel_err(P.interior(out[q].cpu().numpy()), P.interior(ref[q]), 1e-13 * np.abs(ref).max()) < 1e-12
+    finally:
+        B.rad_destroy(h)
+
+
+def test_stage_host_equals_stage(oracle, B):
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (6, 5, 4), ("geodesic", 2), bc=(1, 1, 1, 1, 1, 1))
+    try:
+        out_h = np.zeros_like(I); T_h = np.zeros(P.ncell); dT0_h = np.zeros((4, P.ncell))
+        nf = B.rad_stage_host(h, I, out_h, fluid, opac, 0.0, 1.0, 0.05, T_h, dT0_h, count_noroot=True)
+        out_o, T_o, dT0_o, nf_o = P.stage(I.copy(), fluid, opac, 0.05)
+        assert nf == nf_o
+        assert rel_err_I(P.interior(out_h), P.interior(out_o)) <= TOL_I
+        assert rel_err(P.interior(T_h), P.interior(T_o), 0.0) <= TOL_FLUID
+    finally:
+        B.rad_destroy(h)
+
+
+def test_invariants_on_gpu(oracle, B):
+    """properties that hold at any size, checked on the CUDA path itself: isotropic fixed point in Minkowski (bit for bit)
+    and conservation of sum n^0 n_0 I dOmega with sources off in Kerr-Schild"""
+    n = (24, 20, 16)
+    h = B.rad_create(dict(kind=0), dict(n=n, x0=(0, 0, 0), dx=(0.1, 0.1, 0.1), bc_lo=(1, 1, 1), bc_hi=(1, 1, 1)), ("geodesic", 3), None, dict(couple=0))
+    try:
+        nc = B.rad_ncells_total(h)
+        I = torch.full((nc, 92), 0.731, dtype=torch.float64, device="cuda"); O = torch.zeros_like(I)
+        B.rad_transport(h, I, O, None, 0.0, 1.0, 0.03)
+        Oi = O.reshape(n[2] + 4, n[1] + 4, n[0] + 4, 92)[2:-2, 2:-2, 2:-2]
+        assert (Oi == 0.731).all()
+    finally:
+        B.rad_destroy(h)
+    h = B.rad_create(dict(kind=1, M=1.0, a=0.9), dict(n=n, x0=(3, 2, 1), dx=(0.2, 0.2, 0.2)), ("geodesic", 3), None, dict(couple=0, n0_crit=0.0))
+    try:
+        shp = (n[2] + 4, n[1] + 4, n[0] + 4, 92)
+        I = torch.zeros(shp, dtype=torch.float64, device="cuda")
+        g = torch.Generator(device="cuda").manual_seed(1)
+        I[6:-6, 6:-6, 6:-6] = torch.exp(torch.randn((n[2] - 8, n[1] - 8, n[0] - 8, 92), generator=g, device="cuda", dtype=torch.float64))
+        O = torch.zeros_like(I)
+        vmax = B.rad_get_table(h, B.TAB_MAXSPEED).max()
+        B.rad_transport(h, I, O, None, 0.0, 1.0, 0.3 * 0.2 / vmax)
+        R0 = torch.zeros(4, nc, dtype=torch.float64, device="cuda"); R1 = torch.zeros_like(R0)
+        B.rad_moments(h, I, 1, None, R0); B.rad_moments(h, O, 1, None, R1)
+        e0, e1 = R0[0].sum().item(), R1[0].sum().item()   # R^0_0 = sum n^0 n_0 I dOmega per cell
+        assert abs(e1 - e0) < 1e-12 * abs(e0) and e0 != 0
+    finally:
+        B.rad_destroy(h)
