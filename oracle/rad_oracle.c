@@ -669,20 +669,27 @@ void orc_transport(const orc_problem *P, const double *I_in, const double *I0, d
 /* ======================================================================================
  * O4/O5. Locally implicit coupling (Eq.31-50), fluid increment, mask
  * ==================================================================================== */
-/* R13: unique positive root of B4 T^4 + B1 T + B0 = 0 (Eq.49) for B4>=0, B1>0, B0<0; Newton from
- * an upper bound (monotone from the right, h convex increasing).  returns <0 if no positive root. */
-static double quartic_root(double B4, double B1, double B0) {
-    if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return -1.0;
-    if (B4 == 0.0) return -B0 / B1;
-    double T = fmin(-B0 / B1, sqrt(sqrt(-B0 / B4)));
+/* R13: unique positive root of the quartic Eq.49, B4 T^4 + B1 T + B0 = 0, for B4 >= 0, B1 > 0, B0 < 0.
+ * Eq.48 then needs T_+ - T_-, and in a gas-dominated cell (C_v T >> Ebar) forming that difference from a
+ * rounded T_+ would lose log10(C_v T / Ebar) digits of Ebar_+.  So the SAME quartic is solved for the change
+ * d = T_+ - T_-:   g(d) = B4 (T_- + d)^4 + B1 d + Bp = 0,  Bp = B0 + B1 T_- = A1 - (1 - A2 alpha_s) Ebar_-,
+ * by Newton from the upper bound T_ub = min(-B0/B1, (-B0/B4)^(1/4)) (g is convex and increasing: monotone
+ * convergence from the right).  Stop when the step is below 1e-15 of |d| plus the rounding scale of g/g'.
+ * returns 0 and *d_out if a positive root exists, -1 otherwise (B0 >= 0 or non-finite coefficients). */
+static int quartic_delta(double B4, double B1, double Bp, double Tm, double *d_out) {
+    double B0 = Bp - B1 * Tm;
+    if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return -1;
+    if (B4 == 0.0) { *d_out = -Bp / B1; return 0; }
+    double d = fmin(-B0 / B1, sqrt(sqrt(-B0 / B4))) - Tm;
     for (int it = 0; it < 60; it++) {
-        double T3 = T * T * T;
-        double h = B4 * T3 * T + B1 * T + B0, hp = 4.0 * B4 * T3 + B1;
-        double dT = h / hp;
-        T -= dT;
-        if (fabs(dT) <= 1e-15 * T) break;
+        double T = Tm + d, T3 = T * T * T;
+        double g = B4 * T3 * T + B1 * d + Bp, gp = 4.0 * B4 * T3 + B1;
+        double dd = g / gp;
+        d -= dd;
+        if (fabs(dd) <= 1e-15 * (fabs(d) + (fabs(Bp) + B4 * T3 * T) / gp)) break;
     }
-    return T;
+    *d_out = d;
+    return 0;
 }
 
 /* R10: coordinate-frame u^mu from the normal-frame spatial velocity u^a': gamma = sqrt(1 +
@@ -758,12 +765,13 @@ long long orc_coupling(const orc_problem *P, double *I, const double *fluid, con
                         double Cv = rho / (P->gamma_gas - 1.0);            /* k_B/(mu m_p) = 1 */
                         double B4 = A2 * aP * P->a_rad;                    /* Eq.50a */
                         double B1 = Cv * (1.0 - A2 * aS);                  /* Eq.50b */
-                        double B0 = A1 - B1 * Tm - (1.0 - A2 * aS) * Em;   /* Eq.50c */
-                        Tp = quartic_root(B4, B1, B0);
-                        if (Tp < 0.0) { nfail++; Tp = Tm; }
+                        double Bp = A1 - (1.0 - A2 * aS) * Em;             /* Eq.50c: B0 = Bp - B1 T_- */
+                        double dT = 0.0;
+                        if (quartic_delta(B4, B1, Bp, Tm, &dT) != 0) { nfail++; Tp = Tm; }
                         else {
                             coupled = 1;
-                            double Ep = Em - Cv * (Tp - Tm);               /* Eq.48 */
+                            Tp = Tm + dT;
+                            double Ep = Em - Cv * dT;                      /* Eq.48 */
                             double src = aP * P->a_rad * Tp * Tp * Tp * Tp + aS * Ep;
                             /* R0_alpha before */
                             double Rb[4] = {0, 0, 0, 0}, Ra[4] = {0, 0, 0, 0};

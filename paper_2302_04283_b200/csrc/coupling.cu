@@ -31,19 +31,23 @@ __device__ __forceinline__ void tetrad_velocity(const double *cg, double u1, dou
     uh[0] = sqrt(1.0 + (uh[1] * uh[1] + uh[2] * uh[2] + uh[3] * uh[3]));
 }
 
-// unique positive root of B4 T^4 + B1 T + B0 (Eq.49): Newton from an upper bound, monotone from the right (R13)
-__device__ __forceinline__ double quartic_root(double B4, double B1, double B0) {
-    if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return -1.0;
-    if (B4 == 0.0) return -B0 / B1;
-    double T = fmin(-B0 / B1, sqrt(sqrt(-B0 / B4)));
+// Quartic Eq.49 solved for the temperature change d = T_+ - T_- (R13): g(d) = B4 (T_- + d)^4 + B1 d + Bp,
+// Bp = A_1 - (1 - A_2 alpha_s) Ebar_-.  Eq.48 needs exactly this difference; solving for it directly keeps
+// Ebar_+ accurate in gas-dominated cells where C_v T >> Ebar.  Newton from an upper bound (g convex, increasing).
+// Returns false when there is no positive root (B0 = Bp - B1 T_- >= 0) or a coefficient is not finite.
+__device__ __forceinline__ bool quartic_delta(double B4, double B1, double Bp, double Tm, double &d) {
+    const double B0 = Bp - B1 * Tm;
+    if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return false;
+    if (B4 == 0.0) { d = -Bp / B1; return true; }
+    d = fmin(-B0 / B1, sqrt(sqrt(-B0 / B4))) - Tm;
     for (int it = 0; it < 60; it++) {
-        const double T3 = T * T * T;
-        const double h = fma(B4 * T3, T, fma(B1, T, B0)), hp = fma(4.0 * B4, T3, B1);
-        const double dT = h / hp;
-        T -= dT;
-        if (fabs(dT) <= 1e-15 * T) break;
+        const double T = Tm + d, T3 = T * T * T, q = B4 * T3 * T;
+        const double g = q + fma(B1, d, Bp), gp = fma(4.0 * B4, T3, B1);
+        const double dd = g / gp;
+        d -= dd;
+        if (fabs(dd) <= 1e-15 * (fabs(d) + (fabs(Bp) + q) / gp)) break;
     }
-    return T;
+    return true;
 }
 
 __global__ void __launch_bounds__(32 * kWarpsPerCta) k_coupling(DeviceTables t, Params p, double *__restrict__ I,
@@ -97,14 +101,14 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta) k_coupling(DeviceTables t, 
         A1 *= scale; Em *= scale; A2 *= scale * dt / kFourPi;
         const double Cv = rho / (p.gamma_gas - 1.0);
         const double B4 = A2 * aP * p.a_rad, om = 1.0 - A2 * aS;                // Eq.50
-        const double B1 = Cv * om, B0 = A1 - B1 * Tm - om * Em;
-        const double root = quartic_root(B4, B1, B0);
-        if (root < 0.0) {
+        const double B1 = Cv * om, Bp = A1 - om * Em;
+        double dTemp = 0.0;
+        if (!quartic_delta(B4, B1, Bp, Tm, dTemp)) {
             if (lane == 0 && noroot) atomicAdd(noroot, 1ull);
         } else {
             coupled = true;
-            Tp = root;
-            const double Ep = Em - Cv * (Tp - Tm);                              // Eq.48
+            Tp = Tm + dTemp;
+            const double Ep = Em - Cv * dTemp;                                  // Eq.48
             const double T2 = Tp * Tp;
             src = (aP * p.a_rad * T2 * T2 + aS * Ep) * dt / kFourPi;
         }

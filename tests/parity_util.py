@@ -5,6 +5,7 @@ import numpy as np
 from paper_2302_04283_b200 import workloads as W
 
 TOL_I, TOL_FLUID = 1e-11, 1e-10   # north_star: max relative error per intensity / on fluid energy after one stage
+DT0_FLOOR = 1e-3                  # dT^0_alpha is compared relative to max(|dT^0_alpha|, DT0_FLOOR * |R^0_0|) per cell
 
 
 def oracle_tables_to_rad(cell, face, excised):

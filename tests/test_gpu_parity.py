@@ -6,7 +6,7 @@ import pytest
 import torch
 
 from paper_2302_04283_b200 import workloads as W
-from parity_util import TOL_FLUID, TOL_I, make_oracle, make_rad, oracle_tables_to_rad, rel_err, rel_err_I
+from parity_util import DT0_FLOOR, TOL_FLUID, TOL_I, make_oracle, make_rad, oracle_tables_to_rad, rel_err, rel_err_I
 
 pytestmark = pytest.mark.gpu
 
@@ -114,9 +114,12 @@ def run_both(oracle, B, cfg, n, level, I0w=None, **kw):
     full = out_g.reshape(P.shape + (A.N,)).copy()
     P.interior(full)[...] = -7.0
     assert (full == -7.0).all()
-    R0 = P.moments(out_o, 1)
+    # The oracle forms dT^0_alpha literally as the difference of two N-term sums R^0_alpha[after] - R^0_alpha[before]
+    # (P:L472), whose own rounding noise is ~N 2^-53 |R^0_0|; the relative bar therefore has the floor DT0_FLOOR |R^0_0|
+    # per cell ("tolerances").
+    R0 = np.abs(P.interior(P.moments(out_o, 1)[0]))
     res = dict(I=rel_err_I(P.interior(out_g), P.interior(out_o)), T=rel_err(P.interior(T_g), P.interior(T_o), 0.0),
-               dT0=max(rel_err(P.interior(dT0_g[m]), P.interior(dT0_o[m]), 1e-12 * np.abs(P.interior(R0[m])).max() + 1e-300) for m in range(4)),
+               dT0=max(rel_err(P.interior(dT0_g[m]), P.interior(dT0_o[m]), DT0_FLOOR * R0 + 1e-300) for m in range(4)),
                nf=(nf_g, nf_o), Tchange=float(np.abs(P.interior(T_o) / P.interior(fluid[1]) - 1).max()))
     return res
 
@@ -128,7 +131,7 @@ def test_stage_parity(oracle, B, cfg, n, level):
     assert r["nf"][0] == r["nf"][1] == 0
     assert r["I"] <= TOL_I, r
     assert r["T"] <= TOL_FLUID and r["dT0"] <= TOL_FLUID, r
-    assert r["Tchange"] > 1e-6  # the coupling did something
+    assert r["Tchange"] > 1e-8  # the coupling did something (C2, C5 are gas-dominated: ~5e-7)
 
 
 @pytest.mark.parametrize("kw", [dict(recon_space=0), dict(couple=0), dict(renorm_fluid_weights=0), dict(n0_crit=0.0)])
