@@ -89,6 +89,12 @@ typedef struct {
     int renorm_fluid_weights; /* R12: 1 = rescale fluid-frame solid angles to sum to 4 pi */
     int couple;               /* 0 = transport only, 1 = with implicit coupling (section 2.5) */
     double tau_factor;        /* constant of Eq.26; only 0 (free-streaming flux, Eq.24) is implemented */
+    int recompute_edge_coeffs; /* stored-versus-recomputed angular geometry:
+                                  0 = the angular-edge coefficients dlambda_e c_e n_0e (Eq.16-17, Eq.25) are built once
+                                      in rad_create and stored, 3 N doubles per interior cell (adds 24 B per
+                                      intensity update of HBM traffic, removes ~100 FP64 operations per update);
+                                  1 = not stored: every stage recomputes them from the Ricci rotation coefficients
+                                      (no extra memory; the stage then runs as two kernels and is FP64-bound). */
 } rad_params;
 
 /* Build a context: angle tables on the host (section 2.6), geometry tables on the device (section 2.1-2.2,

@@ -15,6 +15,8 @@ struct rad_ctx {
     rad_opac opac{};
     rad_params params{};
     rad::AngleTables host;
+    rad::EdgeOwnership own;
+    double *ke = nullptr;  // stored edge coefficients (owned)
     rad::DeviceTables dev{};
     rad::Params kp{};
     std::vector<void *> owned;  // device allocations to free
@@ -92,6 +94,8 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     if (!c) return fail(nullptr, RAD_ENOMEM, "rad_create: out of host memory");
     c->device = device; c->metric = *m; c->grid = *g; c->angles = *a; c->params = *p;
     if (o) c->opac = *o;
+    c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit;
+    c->kp.recon_space = p->recon_space; c->kp.renorm = p->renorm_fluid_weights; c->kp.couple = p->couple;
     std::string err;
     bool ok = (a->kind == 0) ? rad::build_latlon(a->nzeta, a->npsi, c->host, err)
             : (a->kind == 1) ? rad::build_geodesic(a->nlev, c->host, err) : (err = "bad angle grid kind", false);
@@ -122,6 +126,24 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     ok = upload(c, h.nhat, &t.nhat) && upload(c, h.domega, &t.domega) && upload(c, h.nnbr, &t.nnbr) && upload(c, h.nbr_edge, &t.nbr_edge) &&
          upload(c, h.edge_lo, &t.edge_lo) && upload(c, h.edge_hi, &t.edge_hi) && upload(c, h.edge_len, &t.edge_len) &&
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
+    // fused stage kernel: balanced edge ownership, per-angle records, 1/dOmega
+    t.fused_ok = 0; t.ang_rec = nullptr; t.winv = nullptr; t.own_edge = nullptr; t.ke = nullptr;
+    if (ok && h.N <= 192) {
+        std::string oerr;
+        if (rad::build_edge_ownership(h, c->own, oerr)) {
+            std::vector<short> rec((size_t)h.N * 8, 0);
+            std::vector<double> winv(h.N);
+            for (int n = 0; n < h.N; n++) {
+                for (int q = 0; q < 3; q++) {
+                    rec[(size_t)n * 8 + q] = (short)c->own.own_partner[(size_t)n * 3 + q];
+                    rec[(size_t)n * 8 + 3 + q] = (short)c->own.pull_pos[(size_t)n * 3 + q];
+                }
+                winv[n] = 1.0 / h.domega[n];
+            }
+            ok = upload(c, rec, &t.ang_rec) && upload(c, winv, &t.winv) && upload(c, c->own.own_edge, &t.own_edge);
+            t.fused_ok = ok ? 1 : 0;
+        }
+    }
     double *cell = nullptr, *face = nullptr;
     if (ok) ok = cudaMalloc((void **)&cell, sizeof(double) * t.ncell * RAD_NCELL) == cudaSuccess;
     if (ok) c->owned.push_back(cell);
@@ -150,8 +172,23 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
         return fail(nullptr, RAD_ECUDA, msg);
     }
     c->metric.cell_tab = nullptr; c->metric.face_tab = nullptr;
-    c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit;
-    c->kp.recon_space = p->recon_space; c->kp.renorm = p->renorm_fluid_weights; c->kp.couple = p->couple;
+    // stored edge coefficients q_e per (interior cell, owned edge): 3 N doubles per cell
+    if (t.fused_ok && !p->recompute_edge_coeffs) {
+        const size_t bytes = sizeof(double) * (size_t)g->n[0] * g->n[1] * g->n[2] * 3 * h.N;
+        if (cudaMalloc((void **)&c->ke, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            rad_destroy(c);
+            return fail(nullptr, RAD_ENOMEM, "rad_create: no device memory for the stored edge coefficients (set recompute_edge_coeffs = 1)");
+        }
+        int nl = rad::launch_build_ke(t, c->ke, 0);
+        if (nl < 0 || cudaDeviceSynchronize() != cudaSuccess) {
+            std::string msg = std::string("rad_create: edge coefficients: ") + cudaGetErrorString(cudaGetLastError());
+            rad_destroy(c);
+            return fail(nullptr, RAD_ECUDA, msg);
+        }
+        c->launches += nl;
+        t.ke = c->ke;
+    }
     *out = c;
     return RAD_OK;
 }
@@ -162,6 +199,7 @@ void rad_destroy(rad_ctx *c) {
     for (void *p : c->owned) cudaFree(p);
     for (int q = 0; q < 2; q++) if (c->scratch_I[q]) cudaFree(c->scratch_I[q]);
     if (c->scratch_small) cudaFree(c->scratch_small);
+    if (c->ke) cudaFree(c->ke);
     delete c;
 }
 
@@ -185,7 +223,10 @@ rad_status rad_transport(rad_ctx *c, double *I_in, double *I_out, const double *
     DeviceGuard guard(c->device);
     rad_status st = rad_fill_ghosts(c, I_in, stream);
     if (st != RAD_OK) return st;
-    int nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, (cudaStream_t)stream);
+    rad::StageArgs a{};
+    a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
+    int nl = rad::launch_stage_fused(c->dev, c->kp, a, false, (cudaStream_t)stream);
+    if (nl == 0) nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, (cudaStream_t)stream);
     if (nl < 0) return cuda_fail(c, "rad_transport");
     c->launches += nl;
     return RAD_OK;
@@ -214,6 +255,35 @@ rad_status rad_couple(rad_ctx *c, double *I, const double *fluid, double dt, dou
 rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
                      double beta_dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
     if (!c || !fluid) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
+    if (c->dev.fused_ok && c->dev.ke && c->dev.N <= 192) {
+        // one launch: flux divergence + coupling + mask (stage.cu)
+        if (!I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
+        if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_stage: I_out must not alias I_in or I0 (the stencil reads old values)");
+        if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_stage: non-finite weights");
+        if (c->kp.couple && (!c->opac.alpha_a_planck || !c->opac.alpha_a_energy || !c->opac.alpha_s)) return fail(c, RAD_ESTATE, "rad_stage: context has no opacities");
+        DeviceGuard guard(c->device);
+        cudaStream_t s = (cudaStream_t)stream;
+        rad_status st = rad_fill_ghosts(c, I_in, stream);
+        if (st != RAD_OK) return st;
+        if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
+        rad::StageArgs a{};
+        a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
+        a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
+        a.T_out = T_out; a.dT0 = dT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
+        int nl = rad::launch_stage_fused(c->dev, c->kp, a, true, s);
+        if (nl < 0) return cuda_fail(c, "rad_stage");
+        if (nl > 0) {
+            c->launches += nl;
+            if (n_noroot) {
+                unsigned long long v = 0;
+                if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+                    return cuda_fail(c, "rad_stage: readback");
+                *n_noroot = (long long)v;
+            }
+            return RAD_OK;
+        }
+        // not served: fall through to the two-kernel path (ghosts are already filled; filling twice is harmless)
+    }
     rad_status st = rad_transport(c, I_in, I_out, I0, gam0, gam1, beta_dt, stream);
     if (st != RAD_OK) return st;
     return rad_couple(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot, stream);

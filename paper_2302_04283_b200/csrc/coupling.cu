@@ -6,50 +6,78 @@
 // Eq.49 for T_+ is solved redundantly by every lane in registers; a second sweep applies Eq.40, transforms
 // back to the tetrad frame, masks |n_0| < n_0^crit and accumulates the fluid increment
 // dT^0_alpha = -sum_n n^0 n_alpha (I_+ - I*) dOmega_n with a second shuffle tree.
-#include <math.h>
-
-#include "rad_internal.h"
+#include "stage_math.cuh"
 
 namespace rad {
 namespace {
 
-constexpr double kFourPi = 12.566370614359172954;
 constexpr int kWarpsPerCta = 8;
 
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+// legacy signature of tetrad_velocity on a cell record
+__device__ __forceinline__ void tetrad_velocity_rec(const double *cg, double u1, double u2, double u3, double uh[4]) {
+    const double th[6] = {cg[44], cg[45], cg[46], cg[47], cg[48], cg[49]};
+    rad::tetrad_velocity(th, u1, u2, u3, uh);
 }
 
-// tetrad-frame four-velocity from the normal-frame spatial velocity u^a':
-// u^ahat = theta^ahat_j u^j' (the co-triad is the spatial inverse tetrad), u^0hat = sqrt(1 + |u^ahat|^2)
-__device__ __forceinline__ void tetrad_velocity(const double *cg, double u1, double u2, double u3, double uh[4]) {
-    uh[1] = cg[44] * u1 + cg[45] * u2 + cg[46] * u3;
-    uh[2] = cg[47] * u2 + cg[48] * u3;
-    uh[3] = cg[49] * u3;
-    uh[0] = sqrt(1.0 + (uh[1] * uh[1] + uh[2] * uh[2] + uh[3] * uh[3]));
-}
-
-// Quartic Eq.49 solved for the temperature change d = T_+ - T_- (R13): g(d) = B4 (T_- + d)^4 + B1 d + Bp,
-// Bp = A_1 - (1 - A_2 alpha_s) Ebar_-.  Eq.48 needs exactly this difference; solving for it directly keeps
-// Ebar_+ accurate in gas-dominated cells where C_v T >> Ebar.  Newton from an upper bound (g convex, increasing).
-// Returns false when there is no positive root (B0 = Bp - B1 T_- >= 0) or a coefficient is not finite.
-__device__ __forceinline__ bool quartic_delta(double B4, double B1, double Bp, double Tm, double &d) {
-    const double B0 = Bp - B1 * Tm;
-    if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return false;
-    if (B4 == 0.0) { d = -Bp / B1; return true; }
-    d = fmin(-B0 / B1, sqrt(sqrt(-B0 / B4))) - Tm;
-    for (int it = 0; it < 60; it++) {
-        const double T = Tm + d, T3 = T * T * T, q = B4 * T3 * T;
-        const double g = q + fma(B1, d, Bp), gp = fma(4.0 * B4, T3, B1);
-        const double dd = g / gp;
-        d -= dd;
-        if (fabs(dd) <= 1e-15 * (fabs(d) + (fabs(Bp) + q) / gp)) break;
+// ------------------------------------------------------------------------------------------------
+// coupling, one warp per cell, angles in registers (the same couple_cell the fused stage kernel uses)
+// ------------------------------------------------------------------------------------------------
+template <int NITER>
+__global__ void __launch_bounds__(32 * kWarpsPerCta) k_coupling_w(DeviceTables t, Params p, double *__restrict__ I,
+                                                                  const double *__restrict__ fluid, const double *__restrict__ aP_,
+                                                                  const double *__restrict__ aE_, const double *__restrict__ aS_,
+                                                                  double dt, double *__restrict__ T_out, double *__restrict__ dT0,
+                                                                  unsigned long long *__restrict__ noroot_count) {
+    const int lane = threadIdx.x & 31;
+    const long long wid = (long long)blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5);
+    const long long nint = (long long)t.n[0] * t.n[1] * t.n[2];
+    if (wid >= nint) return;
+    const int i = (int)(wid % t.n[0]) + t.ng, j = (int)((wid / t.n[0]) % t.n[1]) + t.ng, k = (int)(wid / ((long long)t.n[0] * t.n[1])) + t.ng;
+    const long long c = ((long long)k * t.NJ + j) * t.NI + i;
+    const int N = t.N;
+    const double *cg = t.cell + c * RAD_NCELL;
+    double *Ic = I + c * N;
+    const double Tm = fluid[1 * t.ncell + c];
+    if (cg[50] != 0.0) {  // excised
+        if (lane == 0) {
+            if (T_out) T_out[c] = Tm;
+            if (dT0) for (int m = 0; m < 4; m++) dT0[m * t.ncell + c] = 0.0;
+        }
+        return;
     }
-    return true;
+    double n1[NITER], n2[NITER], n3[NITER], dom[NITER], Is[NITER], Iold[NITER];
+#pragma unroll
+    for (int it = 0; it < NITER; it++) {
+        const int n = min(it * 32 + lane, N - 1);  // lanes past the last angle redo angle N-1 and do not store
+        n1[it] = __ldg(t.nhat + 3 * n); n2[it] = __ldg(t.nhat + 3 * n + 1); n3[it] = __ldg(t.nhat + 3 * n + 2); dom[it] = __ldg(t.domega + n); Is[it] = Ic[n];
+        Iold[it] = Is[it];
+    }
+    CoupleCell cc;
+    cc.nup0 = cg[0];
+    for (int q = 0; q < 4; q++) cc.E[q] = cg[1 + q];
+    for (int q = 0; q < 6; q++) cc.th[q] = cg[44 + q];
+    cc.Tm = Tm;
+    cc.rho = cc.u1 = cc.u2 = cc.u3 = cc.aP = cc.aEa = cc.aS = 0.0;
+    if (p.couple) {
+        cc.rho = fluid[c]; cc.u1 = fluid[2 * t.ncell + c]; cc.u2 = fluid[3 * t.ncell + c]; cc.u3 = fluid[4 * t.ncell + c];
+        cc.aP = aP_[c]; cc.aEa = aE_[c]; cc.aS = aS_[c];
+    }
+    double Tp, dR[4];
+    bool noroot;
+    couple_cell<NITER>(p, cc, dt, lane, N, n1, n2, n3, dom, Is, Tp, dR, noroot);
+    if (noroot && lane == 0 && noroot_count) atomicAdd(noroot_count, 1ull);
+#pragma unroll
+    for (int it = 0; it < NITER; it++) {
+        const int n = it * 32 + lane;
+        if (n < N && Is[it] != Iold[it]) Ic[n] = Is[it];
+    }
+    if (lane == 0) {
+        if (T_out) T_out[c] = Tp;
+        if (dT0) for (int m = 0; m < 4; m++) dT0[m * t.ncell + c] = -dR[m];
+    }
 }
 
+// generic fallback for angle grids with more than 192 angles: lanes stride over the angles, two sweeps over memory
 __global__ void __launch_bounds__(32 * kWarpsPerCta) k_coupling(DeviceTables t, Params p, double *__restrict__ I,
                                                                 const double *__restrict__ fluid, const double *__restrict__ aP_,
                                                                 const double *__restrict__ aE_, const double *__restrict__ aS_,
@@ -79,7 +107,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta) k_coupling(DeviceTables t, 
     double uh[4] = {1.0, 0.0, 0.0, 0.0}, aE = 0.0, src = 0.0;
     if (p.couple) {
         const double rho = fluid[c];
-        tetrad_velocity(cg, fluid[2 * t.ncell + c], fluid[3 * t.ncell + c], fluid[4 * t.ncell + c], uh);
+        tetrad_velocity_rec(cg, fluid[2 * t.ncell + c], fluid[3 * t.ncell + c], fluid[4 * t.ncell + c], uh);
         const double aP = aP_[c], aS = aS_[c];
         aE = aE_[c] + aS;  // Eq.33b
         // sweep 1: fluid-frame quantities and the four reductions
@@ -161,7 +189,7 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta) k_moments(DeviceTables t, c
 #pragma unroll
     for (int q = 0; q < 10; q++) acc[q] = 0.0;
     double uh[4] = {1.0, 0.0, 0.0, 0.0};
-    if (frame == 3) tetrad_velocity(cg, fluid[2 * t.ncell + c], fluid[3 * t.ncell + c], fluid[4 * t.ncell + c], uh);
+    if (frame == 3) tetrad_velocity_rec(cg, fluid[2 * t.ncell + c], fluid[3 * t.ncell + c], fluid[4 * t.ncell + c], uh);
     const double nup0 = cg[0];
     for (int n = lane; n < N; n += 32) {
         const double n1 = __ldg(t.nhat + 3 * n), n2 = __ldg(t.nhat + 3 * n + 1), n3 = __ldg(t.nhat + 3 * n + 2);
@@ -210,7 +238,17 @@ int launch_coupling(const DeviceTables &t, const Params &p, double *I, const dou
                     const double *aS, double dt, double *T_out, double *dT0, unsigned long long *noroot, cudaStream_t s) {
     const long long nint = (long long)t.n[0] * t.n[1] * t.n[2];
     const long long blocks = (nint + kWarpsPerCta - 1) / kWarpsPerCta;
-    k_coupling<<<(unsigned)blocks, 32 * kWarpsPerCta, 0, s>>>(t, p, I, fluid, aP, aE, aS, dt, T_out, dT0, noroot);
+#define RAD_CPL(NIT) k_coupling_w<NIT><<<(unsigned)blocks, 32 * kWarpsPerCta, 0, s>>>(t, p, I, fluid, aP, aE, aS, dt, T_out, dT0, noroot)
+    switch ((t.N + 31) / 32) {
+        case 1: RAD_CPL(1); break;
+        case 2: RAD_CPL(2); break;
+        case 3: RAD_CPL(3); break;
+        case 4: RAD_CPL(4); break;
+        case 5: RAD_CPL(5); break;
+        case 6: RAD_CPL(6); break;
+        default: k_coupling<<<(unsigned)blocks, 32 * kWarpsPerCta, 0, s>>>(t, p, I, fluid, aP, aE, aS, dt, T_out, dT0, noroot);
+    }
+#undef RAD_CPL
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

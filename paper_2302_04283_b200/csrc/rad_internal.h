@@ -22,6 +22,16 @@ struct AngleTables {
     std::vector<double> edge_mid;  // [E][3]
     std::vector<double> edge_nrm;  // [E][3]
 };
+// Balanced ownership of the unique angular edges (edges.cpp): every angle owns <= kMaxOwn of its edges and
+// receives the flux of <= kMaxOwn others.
+constexpr int kMaxOwn = 3;
+struct EdgeOwnership {
+    std::vector<int> own_edge;     // [N][3] unique edge id owned in slot j, or -1
+    std::vector<int> own_partner;  // [N][3] angle at the far end of that edge, or -1
+    std::vector<int> pull_pos;     // [N][3] position j*N + owner of a flux this angle receives, or -1
+};
+bool build_edge_ownership(const AngleTables &a, EdgeOwnership &out, std::string &err);
+
 bool build_latlon(int nzeta, int npsi, AngleTables &out, std::string &err);
 bool build_geodesic(int nlev, AngleTables &out, std::string &err);
 
@@ -45,6 +55,23 @@ struct DeviceTables {
     // geometry
     const double *cell;  // [ncell][RAD_NCELL]
     const double *face;  // [ncell][3][RAD_NFACE]
+    // fused stage kernel (stage.cu): per-angle record {own_partner[3], pull_pos[3], 0, 0} as 8 x int16 (16 B),
+    // 1/dOmega, the owned edge ids, and the stored edge coefficients
+    const short *ang_rec;    // [N][8]
+    const double *winv;      // [N]
+    const int *own_edge;     // [N][3]
+    const double *ke;        // [n2][n1][n0][3][N] interior cells only, or nullptr (not stored)
+    int fused_ok;            // 1 if the fused kernel can serve this angle grid
+};
+
+// arguments of one stage (device pointers are the caller's)
+struct StageArgs {
+    const double *I_in, *I0;
+    double *I_out;
+    double gam0, gam1, beta_dt;
+    const double *fluid, *aP, *aE, *aS;  // coupling only
+    double *T_out, *dT0;
+    unsigned long long *noroot;
 };
 
 struct Params {
@@ -63,6 +90,10 @@ int launch_coupling(const DeviceTables &t, const Params &p, double *I, const dou
                     unsigned long long *noroot, cudaStream_t s);
 int launch_moments(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out,
                    cudaStream_t s);
+// fused stage kernel: flux divergence (+ coupling and mask when couple != 0) in one launch; returns 0 if this
+// configuration is not served (caller falls back to launch_fluxdiv + launch_coupling)
+int launch_stage_fused(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
+int launch_build_ke(const DeviceTables &t, double *ke, cudaStream_t s);
 int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed char *edge_sign, cudaStream_t s);
 int launch_maxspeed(const DeviceTables &t, double *out3, cudaStream_t s);
 
