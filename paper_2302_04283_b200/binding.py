@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "librad.so")
+_SO = os.environ.get("RAD_LIBRAD_PATH") or os.path.join(_HERE, "librad.so")  # override: an experimental build of the same ABI
 NCELL, NFACE, MAXNBR = 52, 8, 6
 
 (TAB_NANG, TAB_NEDGE, TAB_NHAT, TAB_DOMEGA, TAB_NNBR, TAB_NBR, TAB_NBR_EDGE, TAB_EDGE_LO, TAB_EDGE_HI, TAB_EDGE_LEN,

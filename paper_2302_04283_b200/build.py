@@ -23,7 +23,11 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
 
 
-def build(force=False, verbose=False):
+def build(force=False, verbose=False, out=None, extra=()):
+    """out/extra: an experimental build (other -D flags) written somewhere else; the default build is librad.so"""
+    if out is not None:
+        subprocess.check_call([NVCC] + FLAGS + list(extra) + ["-shared", "-o", out] + sources())
+        return out
     deps = sources() + glob.glob(os.path.join(CSRC, "*.h")) + [os.path.join(ROOT, "include", "rad.h"), os.path.abspath(__file__)]
     if not force and os.path.exists(SO) and os.path.getmtime(SO) >= max(os.path.getmtime(d) for d in deps):
         return SO

@@ -11,7 +11,7 @@
 namespace rad {
 namespace {
 
-constexpr int kWarpsPerCta = 8;
+constexpr int kWarpsPerCta = 12;
 
 // legacy signature of tetrad_velocity on a cell record
 __device__ __forceinline__ void tetrad_velocity_rec(const double *cg, double u1, double u2, double u3, double uh[4]) {

@@ -6,24 +6,38 @@
 //   * one WARP per cell; a lane holds the angles n = it*32 + lane, it < NITER, whose directions stay in
 //     registers for the whole kernel.  Intensities are I[cell][angle], angle innermost, so every load and
 //     store of a warp is a run of consecutive doubles.
-//   * a CTA is a TY x TZ bundle of such warps (neighbouring pencils in y and z) that marches along x in lock
-//     step, one cell per step.  The flux through the upper x face is carried in registers to the next step;
-//     the fluxes through the lower y and z faces are published in shared memory for the warps of the
-//     neighbouring pencils (one __syncthreads per step, double-buffered), so every face flux is computed once
-//     except on the rim of the bundle.
-//   * geometry per face and per cell (8 + 8 + 8 + 5 doubles) is warp-uniform and read once per cell.
+//   * a warp marches along x through a run of KX cells of one pencil; the flux through the upper x face is
+//     carried in registers to the next step.  Warps are independent (no block barrier): while one waits for
+//     memory the others compute.  The y and z face fluxes are computed by both cells that share the face,
+//     with bitwise identical results (same inputs, same non-contracted products), so the scheme stays
+//     conservative to rounding.  The warps of a CTA take neighbouring pencils, so the rows one warp loads as
+//     its y/z neighbours are the rows its neighbours load as their own: L1 serves the overlap.
+//   * geometry per face and per cell (5 x 8 + 5 doubles) is warp-uniform and read once per cell.
 //   * angular fluxes: every unique edge is owned by one of its two angles (edges.cpp).  The owner reads the
 //     stored edge coefficient q_e = +-dlambda_e c_e n_0e (one coalesced load; its lowest mantissa bit says which
 //     end is upwind), multiplies by the upwind intensity taken from the cell's row in shared memory, and
-//     publishes the flux for the partner angle.
+//     publishes the flux for the partner angle (warp-private shared memory, __syncwarp only).
 //   * the warp then holds all N post-transport intensities of its cell in registers, so the coupling's angle
 //     reductions are warp shuffles and the intermediate I* never goes to memory.
 #include "stage_math.cuh"
 
+#ifndef RAD_PREFETCH
+#define RAD_PREFETCH 1
+#endif
+#if RAD_PREFETCH == 2
+#define RAD_PF(p) prefetch_l2(p)
+#else
+#define RAD_PF(p) prefetch_l1(p)
+#endif
+
 namespace rad {
 namespace {
 
-constexpr int TY = 4, TZ = 3, NW = TY * TZ;
+#ifndef RAD_TY
+#define RAD_TY 4
+#define RAD_TZ 3
+#endif
+constexpr int TY = RAD_TY, TZ = RAD_TZ, NW = TY * TZ;
 
 __device__ __forceinline__ double2 ldg2(const double *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
 
@@ -35,243 +49,244 @@ __device__ __forceinline__ FaceRec load_face(const double *f) {
     return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
 }
 
+__device__ __forceinline__ FaceRec load_face_s(const double *f) {  // shared memory, warp-uniform address
+    const double2 a = *reinterpret_cast<const double2 *>(f), b = *reinterpret_cast<const double2 *>(f + 2),
+                  c = *reinterpret_cast<const double2 *>(f + 4), d = *reinterpret_cast<const double2 *>(f + 6);
+    return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
+}
+
 // Upwind flux n^a n_0 I (Eq.24) through the face between cells L and R; qLL, qL, qR, qRR are the
-// intensities of the four cells around it.  PLM: van Leer limited slope of the upwind cell (R7), written as
-// q +- dl dr / (dl + dr).  Branch free; the two products are never contracted, so the two cells that share a
-// face get the same bits from every call site.
+// intensities of the four cells around it.  PLM: van Leer limited slope of the upwind cell (R7): with
+// (far, mid, oth) = (LL, L, R) for n^a > 0 and (RR, R, L) otherwise, the face value is mid + dl dr / (dl + dr),
+// dl = mid - far, dr = oth - mid (the harmonic mean is odd under reversal, so one formula serves both signs).
+// Branch free; the two products are never contracted, so the two cells that share a face get the same bits.
 template <bool PLM>
 __device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double n2, double n3, double qLL, double qL, double qR,
                                             double qRR) {
     const double na = chain4(f.e0, f.e1, f.e2, f.e3, n1, n2, n3);
     const double n0 = chain4(f.E0, f.E1, f.E2, f.E3, n1, n2, n3);
     const bool pos = na > 0.0;
-    double up;
+    double up = pos ? qL : qR;
     if (PLM) {
-        const double a = pos ? qLL : qL, b = pos ? qL : qR, c = pos ? qR : qRR;
-        const double dl = b - a, dr = c - b, pr = dl * dr;
-        double h = pr * fast_rcp(dl + dr);
-        h = pr > 0.0 ? h : 0.0;
-        up = pos ? b + h : b - h;
-    } else {
-        up = pos ? qL : qR;
+        const double far = pos ? qLL : qRR, oth = pos ? qR : qL;
+        const double dl = up - far, dr = oth - up, pr = dl * dr;
+        const double h = pr * fast_rcp(dl + dr);
+        up += pr > 0.0 ? h : 0.0;
     }
-    const double F = __dmul_rn(__dmul_rn(na, n0), up);
-    return na == 0.0 ? 0.0 : F;
+    return __dmul_rn(__dmul_rn(na, n0), up);  // n^a = 0 gives 0 for finite intensities
 }
+
+// v[it] = row[angle of (lane, it)]; lanes past the last angle re-read angle N-1 (last_off)
+template <int NITER>
+__device__ __forceinline__ void load_row(const double *__restrict__ row, int lane, int last_off, double (&v)[NITER]) {
+#pragma unroll
+    for (int it = 0; it < NITER - 1; it++) v[it] = __ldg(row + lane + it * 32);
+    v[NITER - 1] = __ldg(row + last_off);
+}
+
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 template <int NITER, bool PLM, bool COUPLE>
 __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, const Params p, const StageArgs a, const int KX) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = t.N, Np = (N + 1) & ~1;
+    const int N = t.N, Np = (N + 2) & ~1;  // even, > N: slot N of a row is scratch
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int wy = w % TY, wz = w / TY;
     double *sm = reinterpret_cast<double *>(smem_raw);
-    double *sI = sm + (size_t)w * 4 * Np;             // [Np]    this warp's cell, all angles
-    double *sG = sI + Np;                             // [3*Np]  fluxes of owned edges, position j*N + n
-    double *sF = sm + (size_t)NW * 4 * Np;            // [2 buf][2 axis][NW][Np] lower y / z face fluxes
-    double *sWinv = sF + (size_t)4 * NW * Np;         // [Np] 1/dOmega
-    double *sDom = sWinv + Np;                        // [Np] dOmega
-    int4 *sRec = reinterpret_cast<int4 *>(sDom + Np); // [N]  {own_partner[3], pull_pos[3]} as int16
+    double *sI = sm + (size_t)w * 4 * Np;                    // [Np]    this warp's cell, all angles
+    double *sG = sI + Np;                                    // [3*N+1] fluxes of owned edges, position j*N + n; [3N] = 0
+    double *sU = sm + (size_t)NW * 4 * Np + (size_t)w * 64;  // [64] this cell's warp-uniform records (see below)
+    double *sWinv = sm + (size_t)NW * (4 * Np + 64);         // [Np] 1/dOmega
+    double *sDom = sWinv + Np;                               // [Np] dOmega
+    uint4 *sRec = reinterpret_cast<uint4 *>(sDom + Np);      // [N]  {own_partner[3], pull_pos[3]} as uint16
     for (int q = threadIdx.x; q < N; q += blockDim.x) {
         sWinv[q] = t.winv[q];
         sDom[q] = t.domega[q];
-        sRec[q] = reinterpret_cast<const int4 *>(t.ang_rec)[q];
+        sRec[q] = reinterpret_cast<const uint4 *>(t.ang_rec)[q];
     }
+    if (lane == 0) sG[3 * N] = 0.0;
     __syncthreads();
 
     const int ng = t.ng;
     const int j = blockIdx.y * TY + wy + ng, k = blockIdx.z * TZ + wz + ng;
-    const bool active = (j < t.n[1] + ng) && (k < t.n[2] + ng);
+    if (j >= t.n[1] + ng || k >= t.n[2] + ng) return;  // no block barrier below
     const int i_begin = blockIdx.x * KX + ng, i_end = min(i_begin + KX, t.n[0] + ng);
-    const bool top_y = (wy == TY - 1) || (j == t.n[1] + ng - 1);  // nobody in this CTA publishes my upper y flux
-    const bool top_z = (wz == TZ - 1) || (k == t.n[2] + ng - 1);
     const long long sy = (long long)t.NI * N, sz = (long long)t.NI * t.NJ * N;  // strides in doubles
     const double idx0 = t.inv_dx[0], idx1 = t.inv_dx[1], idx2 = t.inv_dx[2];
+    const int last_off = min((NITER - 1) * 32 + lane, N - 1);
+    const bool last_valid = (NITER - 1) * 32 + lane < N;
 
     double n1[NITER], n2[NITER], n3[NITER], carry[NITER];
 #pragma unroll
     for (int it = 0; it < NITER; it++) {
-        const int nc = min(it * 32 + lane, N - 1);
-        carry[it] = 0.0;
+        const int nc = it < NITER - 1 ? it * 32 + lane : last_off;
         n1[it] = t.nhat[3 * nc]; n2[it] = t.nhat[3 * nc + 1]; n3[it] = t.nhat[3 * nc + 2];
     }
-    if (active && i_begin < i_end) {  // flux through the lower x face of the first cell of this run
+    {   // flux through the lower x face of the first cell of this run
         const long long c = ((long long)k * t.NJ + j) * t.NI + i_begin;
         const FaceRec f = load_face(t.face + (c * 3 + 0) * RAD_NFACE);
         const double *Ic = a.I_in + c * N;
+        double qLL[NITER], qL[NITER], qR[NITER], qRR[NITER];
+        load_row<NITER>(Ic - N, lane, last_off, qL); load_row<NITER>(Ic, lane, last_off, qR);
+        if (PLM) { load_row<NITER>(Ic - 2 * N, lane, last_off, qLL); load_row<NITER>(Ic + N, lane, last_off, qRR); }
 #pragma unroll
-        for (int it = 0; it < NITER; it++) {
-            const int nc = min(it * 32 + lane, N - 1);
-            const double qLL = PLM ? __ldg(Ic - 2 * N + nc) : 0.0, qL = __ldg(Ic - N + nc), qR = __ldg(Ic + nc), qRR = PLM ? __ldg(Ic + N + nc) : 0.0;
-            carry[it] = face_flux<PLM>(f, n1[it], n2[it], n3[it], qLL, qL, qR, qRR);
-        }
+        for (int it = 0; it < NITER; it++) carry[it] = face_flux<PLM>(f, n1[it], n2[it], n3[it], PLM ? qLL[it] : 0.0, qL[it], qR[it], PLM ? qRR[it] : 0.0);
+    }
+
+    // Warp-uniform records of a cell, gathered two per lane in one round trip and broadcast through shared memory:
+    //   sU[0..7] x face above, [8..15] y face below, [16..23] y face above, [24..31] z face below, [32..39] z face above,
+    //   [40..44] cell n^0, E_0..E_3, [45] excised flag, [46..51] co-triad, [52..56] rho, T, u1', u2', u3', [57..59] alpha_P, alpha_E, alpha_s
+    const double *ptrA, *ptrB;
+    int strideB = RAD_NCELL;
+    {
+        const long long c = ((long long)k * t.NJ + j) * t.NI + i_begin, cz = (long long)t.NI * t.NJ;
+        const int g = lane >> 3, r = lane & 7;
+        ptrA = t.face + ((g == 0 ? c + 1 : (g == 2 ? c + t.NI : c)) * 3 + (g == 0 ? 0 : (g == 3 ? 2 : 1))) * RAD_NFACE + r;
+        ptrB = t.cell + c * RAD_NCELL;  // lanes 28..31: unused
+        if (lane < 8) { ptrB = t.face + ((c + cz) * 3 + 2) * RAD_NFACE + lane; strideB = 3 * RAD_NFACE; }
+        else if (lane < 13) ptrB += lane - 8;
+        else if (lane == 13) ptrB += 50;
+        else if (lane < 20) ptrB += 44 + (lane - 14);
+        else if (COUPLE && p.couple && lane < 28) {
+            ptrB = lane < 25 ? a.fluid + (long long)(lane - 20) * t.ncell + c : (lane == 25 ? a.aP : (lane == 26 ? a.aE : a.aS)) + c;
+            strideB = 1;
+        } else if (COUPLE && lane == 21) { ptrB = a.fluid + t.ncell + c; strideB = 1; }  // T_- is reported even when not coupling
     }
 
     for (int i = i_begin; i < i_end; i++) {
-        const int buf = (i - i_begin) & 1;
-        double *sFy = sF + (size_t)(buf * 2 + 0) * NW * Np, *sFz = sF + (size_t)(buf * 2 + 1) * NW * Np;
         const long long c = ((long long)k * t.NJ + j) * t.NI + i;
-        double div[NITER];
-        // Lanes past the last angle (n >= N) redo angle N-1 (index nc) and simply do not store: the code below
-        // is straight-line, so the loads of all NITER angles of a phase are in flight together.
-        if (active) {
-            const double *Ic = a.I_in + c * N;
-            const long long cint = ((long long)(k - ng) * t.n[1] + (j - ng)) * t.n[0] + (i - ng);
-            // ---- angular fluxes (Eq.25, donor cell in angle)
-            double Iown[NITER];
-#pragma unroll
-            for (int it = 0; it < NITER; it++) Iown[it] = __ldg(Ic + min(it * 32 + lane, N - 1));
-#pragma unroll
-            for (int it = 0; it < NITER; it++)
-                if (it * 32 + lane < N) sI[it * 32 + lane] = Iown[it];
-            __syncwarp();
+        const double *Ic = a.I_in + c * N;
+        const long long cint = ((long long)(k - ng) * t.n[1] + (j - ng)) * t.n[0] + (i - ng);
+        double div[NITER], Iown[NITER];
+#if RAD_PREFETCH
+        if (i + 1 < i_end) {  // pull the next step's rows towards the SM while this step computes
+            const double *In = Ic + N;
+            const int lines = (N * 8 + 127) / 128 + 1;
+            if (lane < lines) {
+                const long long lo = lane * 16;
+                RAD_PF(In + 2 * N + lo);
+                RAD_PF(In - sy + lo); RAD_PF(In + sy + lo); RAD_PF(In - sz + lo); RAD_PF(In + sz + lo);
+                if (PLM) { RAD_PF(In - 2 * sy + lo); RAD_PF(In + 2 * sy + lo); RAD_PF(In - 2 * sz + lo); RAD_PF(In + 2 * sz + lo); }
+            }
+            const double *kn = t.ke + (cint + 1) * 3 * N;
+            if (lane * 16 < 3 * N) RAD_PF(kn + lane * 16);
+        }
+#endif
+        // ---- angular fluxes (Eq.25, donor cell in angle)
+        {
             const double *kec = t.ke + cint * 3 * N;
-            double q[NITER][3];
+            double q0[NITER], q1[NITER], q2[NITER];
+            const double uA = __ldg(ptrA), uB = __ldg(ptrB);
+            ptrA += 3 * RAD_NFACE; ptrB += strideB;
+            load_row<NITER>(Ic, lane, last_off, Iown);
+            load_row<NITER>(kec, lane, last_off, q0); load_row<NITER>(kec + N, lane, last_off, q1); load_row<NITER>(kec + 2 * N, lane, last_off, q2);
+            __syncwarp();  // the previous step's readers of sI / sG / sU are done
+            sU[lane] = uA; sU[32 + lane] = uB;
 #pragma unroll
             for (int it = 0; it < NITER; it++)
-#pragma unroll
-                for (int jj = 0; jj < 3; jj++) q[it][jj] = __ldg(kec + jj * N + min(it * 32 + lane, N - 1));
+                if (it < NITER - 1 || last_valid) sI[it * 32 + lane] = Iown[it];
+            __syncwarp();
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const int n = it * 32 + lane, nc = min(n, N - 1);
-                const int4 rec = sRec[nc];
-                const int pj[3] = {(short)(rec.x & 0xffff), (short)(rec.x >> 16), (short)(rec.y & 0xffff)};
+                const int n = it < NITER - 1 ? it * 32 + lane : last_off;
+                const uint4 rec = sRec[n];
+                const unsigned pj[3] = {rec.x & 0xffffu, rec.x >> 16, rec.y & 0xffffu};
+                const double qq[3] = {q0[it], q1[it], q2[it]};
                 double asum = 0.0;
 #pragma unroll
-                for (int jj = 0; jj < 3; jj++) {
-                    const bool owner_up = (__double2loint(q[it][jj]) & 1) != 0;
-                    const double G = q[it][jj] * (owner_up ? Iown[it] : sI[max(pj[jj], 0)]);  // q = 0 in unused slots
+                for (int jj = 0; jj < 3; jj++) {  // unused slots have q = 0
+                    const bool owner_up = (__double2loint(qq[jj]) & 1) != 0;
+                    const double G = qq[jj] * sI[owner_up ? (unsigned)n : pj[jj]];
                     asum += G;
-                    if (n < N && pj[jj] >= 0) sG[jj * N + n] = G;
+                    if (it < NITER - 1 || last_valid) sG[jj * N + n] = G;
                 }
                 div[it] = asum;
             }
             __syncwarp();
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const int nc = min(it * 32 + lane, N - 1);
-                const int4 rec = sRec[nc];
-                const int pp[3] = {(short)(rec.y >> 16), (short)(rec.z & 0xffff), (short)(rec.z >> 16)};
-                double asum = div[it];
-#pragma unroll
-                for (int s = 0; s < 3; s++) {
-                    const double G = sG[max(pp[s], 0)];
-                    asum -= pp[s] >= 0 ? G : 0.0;
-                }
-                div[it] = asum * sWinv[nc];
-            }
-            // ---- x: flux through the upper face (the lower x face of cell i+1); the lower one is carried
-            {
-                const FaceRec f = load_face(t.face + ((c + 1) * 3 + 0) * RAD_NFACE);
-#pragma unroll
-                for (int it = 0; it < NITER; it++) {
-                    const int nc = min(it * 32 + lane, N - 1);
-                    const double qLL = PLM ? __ldg(Ic - N + nc) : 0.0, qL = Iown[it], qR = __ldg(Ic + N + nc), qRR = PLM ? __ldg(Ic + 2 * N + nc) : 0.0;
-                    const double F = face_flux<PLM>(f, n1[it], n2[it], n3[it], qLL, qL, qR, qRR);
-                    div[it] = fma(F - carry[it], idx0, div[it]);
-                    carry[it] = F;
-                }
-            }
-            // ---- y: flux through the lower face, published for the warp below; the rim computes its upper face too
-            {
-                const FaceRec f = load_face(t.face + (c * 3 + 1) * RAD_NFACE);
-#pragma unroll
-                for (int it = 0; it < NITER; it++) {
-                    const int n = it * 32 + lane, nc = min(n, N - 1);
-                    const double qLL = PLM ? __ldg(Ic - 2 * sy + nc) : 0.0, qL = __ldg(Ic - sy + nc), qR = Iown[it], qRR = PLM ? __ldg(Ic + sy + nc) : 0.0;
-                    const double F = face_flux<PLM>(f, n1[it], n2[it], n3[it], qLL, qL, qR, qRR);
-                    div[it] = fma(-F, idx1, div[it]);
-                    if (n < N) sFy[w * Np + n] = F;
-                }
-                if (top_y) {
-                    const FaceRec fu = load_face(t.face + ((c + t.NI) * 3 + 1) * RAD_NFACE);
-#pragma unroll
-                    for (int it = 0; it < NITER; it++) {
-                        const int nc = min(it * 32 + lane, N - 1);
-                        const double qLL = PLM ? __ldg(Ic - sy + nc) : 0.0, qL = Iown[it], qR = __ldg(Ic + sy + nc), qRR = PLM ? __ldg(Ic + 2 * sy + nc) : 0.0;
-                        div[it] = fma(face_flux<PLM>(fu, n1[it], n2[it], n3[it], qLL, qL, qR, qRR), idx1, div[it]);
-                    }
-                }
-            }
-            // ---- z
-            {
-                const FaceRec f = load_face(t.face + (c * 3 + 2) * RAD_NFACE);
-#pragma unroll
-                for (int it = 0; it < NITER; it++) {
-                    const int n = it * 32 + lane, nc = min(n, N - 1);
-                    const double qLL = PLM ? __ldg(Ic - 2 * sz + nc) : 0.0, qL = __ldg(Ic - sz + nc), qR = Iown[it], qRR = PLM ? __ldg(Ic + sz + nc) : 0.0;
-                    const double F = face_flux<PLM>(f, n1[it], n2[it], n3[it], qLL, qL, qR, qRR);
-                    div[it] = fma(-F, idx2, div[it]);
-                    if (n < N) sFz[w * Np + n] = F;
-                }
-                if (top_z) {
-                    const FaceRec fu = load_face(t.face + ((c + (long long)t.NI * t.NJ) * 3 + 2) * RAD_NFACE);
-#pragma unroll
-                    for (int it = 0; it < NITER; it++) {
-                        const int nc = min(it * 32 + lane, N - 1);
-                        const double qLL = PLM ? __ldg(Ic - sz + nc) : 0.0, qL = Iown[it], qR = __ldg(Ic + sz + nc), qRR = PLM ? __ldg(Ic + 2 * sz + nc) : 0.0;
-                        div[it] = fma(face_flux<PLM>(fu, n1[it], n2[it], n3[it], qLL, qL, qR, qRR), idx2, div[it]);
-                    }
-                }
+                const int n = it < NITER - 1 ? it * 32 + lane : last_off;
+                const uint4 rec = sRec[n];
+                const double asum = div[it] - ((sG[rec.y >> 16] + sG[rec.z & 0xffffu]) + sG[rec.z >> 16]);  // unused -> sG[3N] = 0
+                div[it] = asum * sWinv[n];
             }
         }
-        __syncthreads();
-        if (active) {
-            // ---- flux-divergence update of C = n^0 n_0 I (Eq.22, stage form R8) and cons -> prim
-            const double *cg = t.cell + c * RAD_NCELL;
-            const double2 c01 = ldg2(cg), c23 = ldg2(cg + 2), c45 = ldg2(cg + 4);
-            const double nup0 = c01.x, E0 = c01.y, E1 = c23.x, E2 = c23.y, E3 = c45.x;
-            const bool excised = __ldg(cg + 50) != 0.0;
-            double Is[NITER];
+        // ---- x: flux through the upper face (the lower x face of cell i+1); the lower one is carried
+        {
+            const FaceRec f = load_face_s(sU);
+            double qLL[NITER], qR[NITER], qRR[NITER];
+            load_row<NITER>(Ic + N, lane, last_off, qR);
+            if (PLM) { load_row<NITER>(Ic - N, lane, last_off, qLL); load_row<NITER>(Ic + 2 * N, lane, last_off, qRR); }
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const int nc = min(it * 32 + lane, N - 1);
-                double d = div[it];
-                if (!top_y) d = fma(sFy[(w + 1) * Np + nc], idx1, d);
-                if (!top_z) d = fma(sFz[(w + TY) * Np + nc], idx2, d);
+                const double F = face_flux<PLM>(f, n1[it], n2[it], n3[it], PLM ? qLL[it] : 0.0, Iown[it], qR[it], PLM ? qRR[it] : 0.0);
+                div[it] = fma(F - carry[it], idx0, div[it]);
+                carry[it] = F;
+            }
+        }
+        // ---- y and z: both faces (rows -2, -1, +1, +2 serve the two of them)
+#pragma unroll
+        for (int ax = 1; ax <= 2; ax++) {
+            const long long st = ax == 1 ? sy : sz;
+            const double idx = ax == 1 ? idx1 : idx2;
+            const FaceRec flo = load_face_s(sU + (ax == 1 ? 8 : 24)), fhi = load_face_s(sU + (ax == 1 ? 16 : 32));
+            double m2[NITER], m1[NITER], p1[NITER], p2[NITER];
+            load_row<NITER>(Ic - st, lane, last_off, m1); load_row<NITER>(Ic + st, lane, last_off, p1);
+            if (PLM) { load_row<NITER>(Ic - 2 * st, lane, last_off, m2); load_row<NITER>(Ic + 2 * st, lane, last_off, p2); }
+#pragma unroll
+            for (int it = 0; it < NITER; it++) {
+                const double Flo = face_flux<PLM>(flo, n1[it], n2[it], n3[it], PLM ? m2[it] : 0.0, m1[it], Iown[it], p1[it]);
+                const double Fhi = face_flux<PLM>(fhi, n1[it], n2[it], n3[it], m1[it], Iown[it], p1[it], PLM ? p2[it] : 0.0);
+                div[it] = fma(Fhi - Flo, idx, div[it]);
+            }
+        }
+        // ---- flux-divergence update of C = n^0 n_0 I (Eq.22, stage form R8) and cons -> prim
+        const double2 c01 = *reinterpret_cast<const double2 *>(sU + 40), c23 = *reinterpret_cast<const double2 *>(sU + 42),
+                      c45 = *reinterpret_cast<const double2 *>(sU + 44);
+        const double nup0 = c01.x, E0 = c01.y, E1 = c23.x, E2 = c23.y, E3 = c45.x;
+        const bool excised = c45.y != 0.0;
+        double Is[NITER];
+        {
+            double I0v[NITER];
+            if (a.I0 != nullptr) load_row<NITER>(a.I0 + c * N, lane, last_off, I0v);
+#pragma unroll
+            for (int it = 0; it < NITER; it++) {
                 const double wgt = nup0 * chain4(E0, E1, E2, E3, n1[it], n2[it], n3[it]);  // n^0 n_0
-                double v = a.gam1 * sI[nc];
-                if (a.I0 != nullptr) v = fma(a.gam0, __ldg(a.I0 + c * N + nc), v);
-                v = fma(-a.beta_dt * d, fast_rcp(wgt), v);
+                double v = a.gam1 * Iown[it];
+                if (a.I0 != nullptr) v = fma(a.gam0, I0v[it], v);
+                v = fma(-a.beta_dt * div[it], fast_rcp(wgt), v);
                 Is[it] = excised ? 0.0 : v;
             }
-            if (COUPLE) {
-                const double Tm = __ldg(a.fluid + 1 * t.ncell + c);
-                double Tp = Tm, dR[4] = {0.0, 0.0, 0.0, 0.0};
-                if (!excised) {
-                    CoupleCell cc;
-                    cc.nup0 = nup0; cc.E[0] = E0; cc.E[1] = E1; cc.E[2] = E2; cc.E[3] = E3;
-                    const double2 t0 = ldg2(cg + 44), t1 = ldg2(cg + 46), t2 = ldg2(cg + 48);
-                    cc.th[0] = t0.x; cc.th[1] = t0.y; cc.th[2] = t1.x; cc.th[3] = t1.y; cc.th[4] = t2.x; cc.th[5] = t2.y;
-                    cc.Tm = Tm;
-                    cc.rho = cc.u1 = cc.u2 = cc.u3 = cc.aP = cc.aEa = cc.aS = 0.0;
-                    if (p.couple) {
-                        cc.rho = __ldg(a.fluid + c);
-                        cc.u1 = __ldg(a.fluid + 2 * t.ncell + c); cc.u2 = __ldg(a.fluid + 3 * t.ncell + c); cc.u3 = __ldg(a.fluid + 4 * t.ncell + c);
-                        cc.aP = __ldg(a.aP + c); cc.aEa = __ldg(a.aE + c); cc.aS = __ldg(a.aS + c);
-                    }
-                    double dom[NITER];
+        }
+        if (COUPLE) {
+            CoupleCell cc;
+            cc.nup0 = nup0; cc.E[0] = E0; cc.E[1] = E1; cc.E[2] = E2; cc.E[3] = E3;
+            const double2 t0 = *reinterpret_cast<const double2 *>(sU + 46), t1 = *reinterpret_cast<const double2 *>(sU + 48),
+                          t2 = *reinterpret_cast<const double2 *>(sU + 50), f0 = *reinterpret_cast<const double2 *>(sU + 52),
+                          f1 = *reinterpret_cast<const double2 *>(sU + 54), f2 = *reinterpret_cast<const double2 *>(sU + 56),
+                          f3 = *reinterpret_cast<const double2 *>(sU + 58);
+            cc.th[0] = t0.x; cc.th[1] = t0.y; cc.th[2] = t1.x; cc.th[3] = t1.y; cc.th[4] = t2.x; cc.th[5] = t2.y;
+            cc.rho = f0.x; cc.Tm = f0.y; cc.u1 = f1.x; cc.u2 = f1.y; cc.u3 = f2.x; cc.aP = f2.y; cc.aEa = f3.x; cc.aS = f3.y;
+            double dom[NITER];
 #pragma unroll
-                    for (int it = 0; it < NITER; it++) dom[it] = sDom[min(it * 32 + lane, N - 1)];
-                    bool noroot;
-                    couple_cell<NITER>(p, cc, a.beta_dt, lane, N, n1, n2, n3, dom, Is, Tp, dR, noroot);
-                    if (noroot && lane == 0 && a.noroot) atomicAdd(a.noroot, 1ull);
+            for (int it = 0; it < NITER; it++) dom[it] = sDom[it < NITER - 1 ? it * 32 + lane : last_off];
+            double Tp, dR[4];
+            bool noroot;
+            couple_cell<NITER>(p, cc, a.beta_dt, lane, N, n1, n2, n3, dom, Is, Tp, dR, noroot, !excised);
+            if (lane == 0) {
+                if (noroot && a.noroot) atomicAdd(a.noroot, 1ull);
+                if (a.T_out) a.T_out[c] = Tp;
+                if (a.dT0) {
+#pragma unroll
+                    for (int m = 0; m < 4; m++) a.dT0[m * t.ncell + c] = -dR[m];
                 }
-                if (lane == 0) {
-                    if (a.T_out) a.T_out[c] = Tp;
-                    if (a.dT0) {
-#pragma unroll
-                        for (int m = 0; m < 4; m++) a.dT0[m * t.ncell + c] = -dR[m];
-                    }
-                }
-            }
-            double *out = a.I_out + c * N;
-#pragma unroll
-            for (int it = 0; it < NITER; it++) {
-                const int n = it * 32 + lane;
-                if (n < N) out[n] = Is[it];
             }
         }
+        double *out = a.I_out + c * N;
+#pragma unroll
+        for (int it = 0; it < NITER; it++)
+            if (it < NITER - 1 || last_valid) out[it * 32 + lane] = Is[it];
     }
 }
 
@@ -313,8 +328,8 @@ __global__ void __launch_bounds__(256) k_build_ke(const DeviceTables t, double *
 }
 
 size_t stage_smem_bytes(int N) {
-    const int Np = (N + 1) & ~1;
-    return sizeof(double) * ((size_t)NW * 4 * Np + (size_t)4 * NW * Np + 2 * (size_t)Np) + sizeof(int4) * (size_t)N;
+    const int Np = (N + 2) & ~1;
+    return sizeof(double) * ((size_t)NW * (4 * Np + 64) + 2 * (size_t)Np) + sizeof(uint4) * (size_t)N;
 }
 
 template <int NITER>

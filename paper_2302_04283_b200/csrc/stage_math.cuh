@@ -49,14 +49,16 @@ __device__ __forceinline__ void tetrad_velocity(const double th[6], double u1, d
 __device__ __forceinline__ bool quartic_delta(double B4, double B1, double Bp, double Tm, double &d) {
     const double B0 = Bp - B1 * Tm;
     if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return false;
-    if (B4 == 0.0) { d = -Bp / B1; return true; }
-    d = fmin(-B0 / B1, sqrt(sqrt(-B0 / B4))) - Tm;
+    const double rB1 = 1.0 / B1;
+    if (B4 == 0.0) { d = -Bp * rB1; return true; }
+    d = fmin(-B0 * rB1, sqrt(sqrt(-B0 / B4))) - Tm;
     for (int it = 0; it < 60; it++) {
         const double T = Tm + d, T3 = T * T * T, q = B4 * T3 * T;
         const double g = q + fma(B1, d, Bp), gp = fma(4.0 * B4, T3, B1);
-        const double dd = g / gp;
+        const double rgp = fast_rcp(gp);  // gp >= B1 > 0, finite
+        const double dd = g * rgp;
         d -= dd;
-        if (fabs(dd) <= 1e-15 * (fabs(d) + (fabs(Bp) + q) / gp)) break;
+        if (fabs(dd) <= 1e-15 * (fabs(d) + (fabs(Bp) + q) * rgp)) break;
     }
     return true;
 }
@@ -77,36 +79,43 @@ template <int NITER>
 __device__ __forceinline__ void couple_cell(const Params &p, const CoupleCell &cc, double dt, int lane, int N,
                                             const double (&n1)[NITER], const double (&n2)[NITER], const double (&n3)[NITER],
                                             const double (&dom)[NITER], double (&Is)[NITER], double &Tp, double (&dR)[4],
-                                            bool &noroot) {
+                                            bool &noroot, bool enable = true) {
+    // `enable` (warp-uniform) = this cell takes part (false for excised cells: nothing changes).  All shuffles below run in warp-uniform control flow: cells that are not coupled (params.couple == 0) still
+    // take the same path with src = 0, g1 = 1 so that Is is unchanged.
+    double uh[4] = {1.0, 0.0, 0.0, 0.0};
+    if (p.couple && enable) tetrad_velocity(cc.th, cc.u1, cc.u2, cc.u3, uh);
+    const double aE = cc.aEa + cc.aS;  // Eq.33b
+    // sweep 1: fluid-frame quantities and the four reductions.  With g1 = n^0/(n^0 + n^0bar alpha_E dt) and
+    // g2 = n^0bar/(n^0 + n^0bar alpha_E dt):  A_1 = sum g1 Ibar dOmega_bar, A_2 = dt/4pi sum g2 dOmega_bar (Eq.42),
+    // and Eq.40 back in the tetrad frame is  Ihat_+ = g1 Ihat_- + g2 (n^0bar)^-4 dt/4pi (alpha_P a T^4 + alpha_s Ebar_+).
+    double g1[NITER], g2r4[NITER];
+    double W = 0.0, A1 = 0.0, A2 = 0.0, Em = 0.0;
+#pragma unroll
+    for (int it = 0; it < NITER; it++) {
+        const double nb = uh[0] - (uh[1] * n1[it] + uh[2] * n2[it] + uh[3] * n3[it]);  // n^0bar = -u_alpha n^alpha
+        const double nb2 = nb * nb;
+        const double r2 = fast_rcp(nb2);
+        const double dOm = (it * 32 + lane < N) ? dom[it] * r2 : 0.0;                  // dOmega_bar (R11); 0 for idle lanes
+        const double Ib = nb2 * nb2 * Is[it];                                          // Ibar_- = (n^0bar)^4 Ihat (R11)
+        const double rd = fast_rcp(fma(nb * aE, dt, cc.nup0));                         // 1/(n^0 + n^0bar alpha_E dt)
+        g1[it] = cc.nup0 * rd;
+        const double g2 = nb * rd;
+        g2r4[it] = g2 * (r2 * r2);
+        W += dOm;
+        A1 = fma(g1[it] * Ib, dOm, A1);                                                // Eq.42a
+        A2 = fma(g2, dOm, A2);                                                         // Eq.42b
+        Em = fma(Ib, dOm, Em);                                                         // Eq.38
+    }
+    W = warp_sum(W); A1 = warp_sum(A1); A2 = warp_sum(A2); Em = warp_sum(Em);
     Tp = cc.Tm;
     noroot = false;
-    dR[0] = dR[1] = dR[2] = dR[3] = 0.0;
     bool coupled = false;
-    double uh[4] = {1.0, 0.0, 0.0, 0.0}, src = 0.0;
-    const double aE = cc.aEa + cc.aS;  // Eq.33b
-    double rd[NITER], r2[NITER];
-    if (p.couple) {
-        tetrad_velocity(cc.th, cc.u1, cc.u2, cc.u3, uh);
-        // sweep 1: fluid-frame quantities and the four reductions
-        double W = 0.0, A1 = 0.0, A2 = 0.0, Em = 0.0;
-#pragma unroll
-        for (int it = 0; it < NITER; it++) {
-            const double nb = uh[0] - (uh[1] * n1[it] + uh[2] * n2[it] + uh[3] * n3[it]);  // n^0bar = -u_alpha n^alpha
-            const double nb2 = nb * nb;
-            r2[it] = fast_rcp(nb2);
-            const double dOm = (it * 32 + lane < N) ? dom[it] * r2[it] : 0.0;                // dOmega_bar (R11); 0 for idle lanes
-            const double Ib = nb2 * nb2 * Is[it];                                            // Ibar_- = (n^0bar)^4 Ihat (R11)
-            rd[it] = fast_rcp(fma(nb * aE, dt, cc.nup0));                                    // 1/(n^0 + n^0bar alpha_E dt)
-            W += dOm;
-            A1 = fma(cc.nup0 * rd[it] * Ib, dOm, A1);                                        // Eq.42a
-            A2 = fma(nb * rd[it], dOm, A2);                                                  // Eq.42b
-            Em = fma(Ib, dOm, Em);                                                           // Eq.38
-        }
-        W = warp_sum(W); A1 = warp_sum(A1); A2 = warp_sum(A2); Em = warp_sum(Em);
-        const double scale = p.renorm ? kFourPi / W : 1.0;                                       // R12
+    double src = 0.0;
+    if (p.couple && enable) {
+        const double scale = p.renorm ? kFourPi / W : 1.0;                             // R12
         A1 *= scale; Em *= scale; A2 *= scale * dt / kFourPi;
         const double Cv = cc.rho / (p.gamma_gas - 1.0);
-        const double B4 = A2 * cc.aP * p.a_rad, om = 1.0 - A2 * cc.aS;                           // Eq.50
+        const double B4 = A2 * cc.aP * p.a_rad, om = 1.0 - A2 * cc.aS;                 // Eq.50
         const double B1 = Cv * om, Bp = A1 - om * Em;
         double dTemp = 0.0;
         if (!quartic_delta(B4, B1, Bp, cc.Tm, dTemp)) {
@@ -114,38 +123,31 @@ __device__ __forceinline__ void couple_cell(const Params &p, const CoupleCell &c
         } else {
             coupled = true;
             Tp = cc.Tm + dTemp;
-            const double Ep = Em - Cv * dTemp;                                                   // Eq.48
+            const double Ep = Em - Cv * dTemp;                                         // Eq.48
             const double T2 = Tp * Tp;
             src = (cc.aP * p.a_rad * T2 * T2 + cc.aS * Ep) * dt / kFourPi;
         }
     }
-    // sweep 2: Eq.40, back to the tetrad frame, fluid increment through the tetrad-frame first moments, mask
+    // sweep 2: Eq.40, fluid increment through the tetrad-frame first moments of the change, mask
     double M0 = 0.0, M1 = 0.0, M2 = 0.0, M3 = 0.0;
 #pragma unroll
     for (int it = 0; it < NITER; it++) {
         const double Iold = Is[it];
-        double Inew = Iold;
-        if (coupled) {
-            const double nb = uh[0] - (uh[1] * n1[it] + uh[2] * n2[it] + uh[3] * n3[it]);
-            const double nb2 = nb * nb, nb4 = nb2 * nb2;
-            Inew = fma(cc.nup0 * nb4, Iold, nb * src) * rd[it] * (r2[it] * r2[it]);          // Eq.40, Ihat = Ibar/(n^0bar)^4
-            const double wI = (it * 32 + lane < N) ? dom[it] * (Inew - Iold) : 0.0;
-            M0 += wI; M1 = fma(wI, n1[it], M1); M2 = fma(wI, n2[it], M2); M3 = fma(wI, n3[it], M3);
-        }
-        if (p.n0_crit > 0.0) {
+        double Inew = coupled ? fma(src, g2r4[it], g1[it] * Iold) : Iold;
+        const double wI = (it * 32 + lane < N) ? dom[it] * (Inew - Iold) : 0.0;
+        M0 += wI; M1 = fma(wI, n1[it], M1); M2 = fma(wI, n2[it], M2); M3 = fma(wI, n3[it], M3);
+        if (p.n0_crit > 0.0 && enable) {
             const double n0 = chain4(cc.E[0], cc.E[1], cc.E[2], cc.E[3], n1[it], n2[it], n3[it]);  // cell-centre n_0
             if (fabs(n0) < p.n0_crit) Inew = 0.0;
         }
         Is[it] = Inew;
     }
-    if (coupled) {
-        M0 = warp_sum(M0); M1 = warp_sum(M1); M2 = warp_sum(M2); M3 = warp_sum(M3);
-        // R^0_alpha = sum n^0 n_alpha I dOmega; n_0 = E_ahat n^ahat, n_i = theta^a_i n^a
-        dR[0] = cc.nup0 * (cc.E[0] * M0 + cc.E[1] * M1 + cc.E[2] * M2 + cc.E[3] * M3);
-        dR[1] = cc.nup0 * (cc.th[0] * M1);
-        dR[2] = cc.nup0 * (cc.th[1] * M1 + cc.th[3] * M2);
-        dR[3] = cc.nup0 * (cc.th[2] * M1 + cc.th[4] * M2 + cc.th[5] * M3);
-    }
+    M0 = warp_sum(M0); M1 = warp_sum(M1); M2 = warp_sum(M2); M3 = warp_sum(M3);
+    // R^0_alpha = sum n^0 n_alpha I dOmega; n_0 = E_ahat n^ahat, n_i = theta^a_i n^a
+    dR[0] = cc.nup0 * (cc.E[0] * M0 + cc.E[1] * M1 + cc.E[2] * M2 + cc.E[3] * M3);
+    dR[1] = cc.nup0 * (cc.th[0] * M1);
+    dR[2] = cc.nup0 * (cc.th[1] * M1 + cc.th[3] * M2);
+    dR[3] = cc.nup0 * (cc.th[2] * M1 + cc.th[4] * M2 + cc.th[5] * M3);
 }
 
 }  // namespace rad
