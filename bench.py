@@ -9,7 +9,7 @@ before the timed region; the intensity arrays (2 x 2.98 GB) exceed L2 (126 MB), 
 
 One JSON line on stdout (rank 0).  `value` is device-timed (CUDA events on the launching stream, max over ranks);
 `e2e` is the same stage through rad_stage_host with pinned HOST buffers, copies inside the timed region;
-`roofline` is for the fused flux-divergence kernel, timed alone with CUDA events; `cpu_baseline` is the oracle
+`roofline` is for the fused stage kernel (the only kernel of a step), from the CUDA-event time of the timed region; `cpu_baseline` is the oracle
 timed on the host cores on a bounded sub-block of the same workload.  With --gpus N > 1 (torchrun) every rank
 runs an independent replica of the block ("replicas only": the path has no collective), scaling = weak.
 """
@@ -30,9 +30,20 @@ UNIT = "updates/s"
 
 
 def algorithmic_bytes_per_update(N):
-    """flux-divergence kernel, recompute-geometry design: read I (8) + write I* (8) +
-    per cell the 35 doubles of the cell record it reads and 3 face records of 8 doubles (59 doubles = 472 B)"""
-    return 16.0 + 472.0 / N
+    """fused stage kernel, DESIGN.md 'rooflines' (single-pass stage): read I (8) + write I_+ (8) + per-cell
+    side data of both halves of the stage (536 B geometry + 104 B fluid, opacity and fluid outputs) spread over N angles"""
+    return 16.0 + 640.0 / N
+
+
+def design_bytes_per_update(N):
+    """what the kernel as built must move: the above without the 30 Ricci coefficients per cell (240 B) that the stored
+    design does not read, plus the stored angular-edge coefficients, 3 doubles per update"""
+    return 16.0 + 24.0 + 400.0 / N
+
+
+# FP64-pipe instruction slots per update of the stage kernel as designed (DESIGN.md 'rooflines', table 'FP64 budget'),
+# counted per lane; one slot = one DFMA-equivalent issue = 2 flop of the measured DFMA peak
+FP64_SLOTS_PER_UPDATE = {True: 160.0, False: 113.0}  # with / without coupling
 
 
 class ClockSampler:
@@ -69,6 +80,23 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def max_over_ranks(value, world, device=None):
+    """max of a per-rank scalar over all ranks (the contract's 'max over ranks' timing); `device` = where the backend's
+    tensors live ("cuda" for nccl, None/"cpu" for gloo)"""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([float(value)], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def whole_job_value(updates_per_rank, world, ms):
+    """whole-job throughput of N independent replicas ('replicas only', weak scaling): all ranks' updates / max time"""
+    return world * updates_per_rank / (ms * 1e-3)
+
+
 def measured_peak():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -77,24 +105,29 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def oracle_sample(cfg, nsub):
-    """time the oracle, as it stands, on the nsub^3 cells at the low corner of the workload's block (same spacing,
-    own ghosts, same input recipe); returns updates/s, seconds"""
-    from oracle import rad_oracle as O
-    from paper_2302_04283_b200 import workloads as W
-    c = W.CONFIGS[cfg]
-    A = O.Angles(*c["angles"])
-    nn, ng, x0, dx = W.grid(cfg, sub=nsub)
-    P = O.Problem(A, nn, x0, dx, metric_kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg),
-                  bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3)
-    inp = W.make_inputs(cfg, A.nhat, sub=nsub)
-    I = inp["I"].numpy().reshape(-1, A.N).copy()
-    fluid = inp["fluid"].numpy().reshape(5, -1).copy(); opac = inp["opac"].numpy().reshape(3, -1).copy()
-    dt = W.CFL * min(dx) / P.max_speed()[0]
-    t0 = time.perf_counter()
-    P.stage(I, fluid, opac, dt)
-    t1 = time.perf_counter()
-    return nsub ** 3 * A.N / (t1 - t0), t1 - t0
+class OracleSample:
+    """the oracle, as it stands, on the nsub^3 cells at the low corner of the workload's block (same spacing, own ghosts,
+    same input recipe); built once, each run() is one full stage on the same inputs"""
+
+    def __init__(self, cfg, nsub):
+        from oracle import rad_oracle as O
+        from paper_2302_04283_b200 import workloads as W
+        c = W.CONFIGS[cfg]
+        A = O.Angles(*c["angles"])
+        nn, ng, x0, dx = W.grid(cfg, sub=nsub)
+        self.P = O.Problem(A, nn, x0, dx, metric_kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg),
+                           bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3)
+        inp = W.make_inputs(cfg, A.nhat, sub=nsub)
+        self.I = inp["I"].numpy().reshape(-1, A.N).copy()
+        self.fluid = inp["fluid"].numpy().reshape(5, -1).copy(); self.opac = inp["opac"].numpy().reshape(3, -1).copy()
+        self.dt = W.CFL * min(dx) / self.P.max_speed()[0]
+        self.updates = nsub ** 3 * A.N
+
+    def run(self):
+        """seconds of one stage"""
+        t0 = time.perf_counter()
+        self.P.stage(self.I, self.fluid, self.opac, self.dt)
+        return time.perf_counter() - t0
 
 
 def run_reference(args):
@@ -104,17 +137,15 @@ def run_reference(args):
         return
     from paper_2302_04283_b200 import workloads as W
     cfg = args.config
-    nsub = args.ref_n
+    nsub = args.ref_n or 64
     N = W.n_angles(cfg)
     cores = os.cpu_count()
+    smp = OracleSample(cfg, nsub)
     for _ in range(args.warmup):
-        oracle_sample(cfg, min(nsub, 8))
-    times = []
-    for _ in range(args.steps):
-        ups, sec = oracle_sample(cfg, nsub)
-        times.append(sec)
+        smp.run()
+    times = [smp.run() for _ in range(args.steps)]
     ms = 1e3 * sum(times) / len(times)
-    val = nsub ** 3 * N / (ms * 1e-3)
+    val = smp.updates / (ms * 1e-3)
     sample = f"{nsub}^3-cell sub-block (low corner, own ghosts) of {cfg}, {N} angles, one full stage per step"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -132,7 +163,7 @@ def main():
     ap.add_argument("--config", default="C3")
     ap.add_argument("--n", type=int, default=None, help="override cells per axis (same box)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-n", type=int, default=32, help="sub-block size of the oracle sample")
+    ap.add_argument("--ref-n", type=int, default=None, help="sub-block size of the oracle sample (default: 64 for --impl reference, 96 for the cpu_baseline leg)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -210,13 +241,10 @@ def main():
     t1 = time.time()
     launches = B.rad_launch_count(h) - l0
     ms = ev0.elapsed_time(ev1) / args.steps
-    if world > 1:
-        tt = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+    ms = max_over_ranks(ms, world, "cuda")
     clocks = sampler.summary(t0, t1) if sampler else None
 
-    # the two kernels separately (same launch configuration), CUDA events on the launching stream
+    # the stage kernel without its coupling half, and the stand-alone coupling kernel, for the record
     def time_call(fn, reps):
         for _ in range(2):
             fn()
@@ -233,13 +261,26 @@ def main():
     ms_flux = time_call(lambda: B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream), reps)
     B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream)
     ms_cpl = time_call(lambda: B.rad_couple(h, I_b, fluid, dt, T_out, dT0, stream=stream), reps)
+    # roofline of the dominant kernel = the fused stage kernel k_stage (flux divergence + coupling in one launch): with
+    # caller-filled ghosts it is the only kernel of a step, so its average launch duration is the CUDA-event time of the
+    # timed region / launches
+    kernels_per_step = max(1, launches // max(1, args.steps))
     peak, peak_src = measured_peak()
     bpu = algorithmic_bytes_per_update(N)
-    achieved = bpu * updates / (ms_flux * 1e-3) / 1e9
-    roofline = {"kernel": "k_fluxdiv (fused spatial+angular flux divergence)", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_update": bpu,
-                "ms_per_launch": ms_flux, "coupling_ms_per_launch": ms_cpl,
-                "coupling_achieved_gbs": (16.0 + 104.0 / N) * updates / (ms_cpl * 1e-3) / 1e9}
+    achieved = bpu * updates / (ms * 1e-3) / 1e9
+    roofline = {"kernel": "k_stage (fused flux divergence + implicit coupling + mask, one launch per step)", "bound": "hbm",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_update": bpu, "design_bytes_per_update": design_bytes_per_update(N),
+                "design_frac": design_bytes_per_update(N) * updates / (ms * 1e-3) / 1e9 / peak,
+                "ms_per_launch": ms / kernels_per_step, "kernels_per_step": kernels_per_step,
+                "flux_divergence_only_ms": ms_flux, "standalone_coupling_kernel_ms": ms_cpl}
+    dfma = B.rad_probe_fp64(h)
+    slots = FP64_SLOTS_PER_UPDATE[True]
+    roofline_alu = {"kernel": roofline["kernel"], "bound": "alu", "unit": "TFLOP/s", "peak": 2.0 * dfma / 1e12,
+                    "peak_source": "measured live: rad_probe_fp64 (register-only DFMA kernel, CUDA events)",
+                    "achieved": 2.0 * slots * updates / (ms * 1e-3) / 1e12, "fp64_slots_per_update": slots,
+                    "note": "one FP64-pipe instruction slot per lane = 2 flop (DFMA-equivalent)"}
+    roofline_alu["frac"] = roofline_alu["achieved"] / roofline_alu["peak"]
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -256,10 +297,7 @@ def main():
             B.rad_stage_host(h, hI, hO, hfl, hop, 0.0, 1.0, dt, hT, hdT)
         torch.cuda.synchronize()
         w = (time.perf_counter() - w0) / nrep
-        if world > 1:
-            tt = torch.tensor([w], dtype=torch.float64, device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            w = float(tt.item())
+        w = max_over_ranks(w, world, "cuda")
         e2e = {"value": world * updates / w, "unit": UNIT, "h2d_bytes_per_step": int(hI.numel() * 8 + hfl.numel() * 8 + hop.numel() * 8),
                "d2h_bytes_per_step": int(hO.numel() * 8 + hT.numel() * 8 + hdT.numel() * 8), "ms_per_step": w * 1e3}
         del hI, hO
@@ -271,16 +309,21 @@ def main():
         return
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        nsub = args.ref_n
-        ups, sec = oracle_sample(cfg, nsub)
+        nsub = args.ref_n or 96
+        smp = OracleSample(cfg, nsub)
+        smp.run()
+        secs = [smp.run() for _ in range(2)]
+        sec = sum(secs)
+        ups = 2 * smp.updates / sec
         cpu = {"value": ups, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
-               "sample": f"{nsub}^3-cell sub-block (low corner, own ghosts) of {cfg}, {N} angles, one stage, {sec:.1f} s"}
-    line = {"metric": METRIC, "value": world * updates / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+               "sample": f"{nsub}^3-cell sub-block (low corner, own ghosts) of {cfg}, {N} angles, 2 timed stages after 1 warm-up, {sec:.1f} s"}
+    line = {"metric": METRIC, "value": whole_job_value(updates, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{cfg}: {c['angles']} angles={N}, {nn[0]}^3 cells + 2 ghosts, metric kind {c['metric']} a={c['a']}, box {c['box']}",
                        "updates_per_step": updates, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs (2 x %.2f GB) exceed L2; no flush" % (I_a.numel() * 8 / 1e9)},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_alu": roofline_alu,
+            "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

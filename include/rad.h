@@ -171,6 +171,11 @@ long long rad_ncells_total(const rad_ctx *);
 /* kernels launched by this context so far (bench.py's gpu_launches) */
 long long rad_launch_count(const rad_ctx *);
 
+/* Measurement helper (not part of the stage): the device's FP64 fused-multiply-add rate, in lane-level DFMA
+ * operations per second (x2 = flop/s), from a register-only kernel timed with CUDA events; synchronises.
+ * bench.py uses it as the denominator of the FP64 ("alu") roofline of the stage kernel. */
+rad_status rad_probe_fp64(rad_ctx *, double *dfma_per_sec /* HOST */);
+
 /* Text of the last error on this context (or of the last failed rad_create if ctx is NULL).  Never NULL. */
 const char *rad_last_error(const rad_ctx *);
 

@@ -19,7 +19,7 @@ NCELL, NFACE, MAXNBR = 52, 8, 6
  TAB_EDGE_MID, TAB_EDGE_NRM, TAB_CELL, TAB_FACE, TAB_FACE_SIGN, TAB_EDGE_SIGN, TAB_MAXSPEED) = range(17)
 
 EXPORTS = ["rad_create", "rad_stage", "rad_stage_host", "rad_fill_ghosts", "rad_transport", "rad_couple", "rad_moments",
-           "rad_get_table", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
+           "rad_get_table", "rad_probe_fp64", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
 
 
 class RadError(RuntimeError):
@@ -71,6 +71,7 @@ def lib():
         L.rad_couple.argtypes = [vp, vp, vp, d, vp, vp, ll, vp]
         L.rad_moments.argtypes = [vp, vp, C.c_int, vp, vp, vp]
         L.rad_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
+        L.rad_probe_fp64.argtypes = [vp, C.POINTER(C.c_double)]
         L.rad_ncells_total.argtypes = [vp]; L.rad_ncells_total.restype = C.c_longlong
         L.rad_launch_count.argtypes = [vp]; L.rad_launch_count.restype = C.c_longlong
         L.rad_last_error.argtypes = [vp]; L.rad_last_error.restype = C.c_char_p
@@ -172,6 +173,13 @@ def rad_couple(ctx, I, fluid, dt, T_out=None, dT0=None, count_noroot=False, stre
 
 def rad_moments(ctx, I, frame, fluid, out, stream=None):
     _check(ctx, lib().rad_moments(ctx, _dp(I), int(frame), _dp(fluid), _dp(out), _stream(stream)))
+
+
+def rad_probe_fp64(ctx):
+    """measured FP64 FMA rate of the context's device, lane-level DFMA operations per second"""
+    v = C.c_double(0.0)
+    _check(ctx, lib().rad_probe_fp64(ctx, C.byref(v)))
+    return v.value
 
 
 def rad_ncells_total(ctx):

@@ -331,6 +331,13 @@ rad_status rad_moments(rad_ctx *c, const double *I, int frame, const double *flu
     return RAD_OK;
 }
 
+rad_status rad_probe_fp64(rad_ctx *c, double *dfma_per_sec) {
+    if (!c || !dfma_per_sec) return fail(c, RAD_EINVAL, "rad_probe_fp64: NULL argument");
+    DeviceGuard guard(c->device);
+    if (rad::probe_dfma_rate(dfma_per_sec, &c->launches) != 0) return cuda_fail(c, "rad_probe_fp64");
+    return RAD_OK;
+}
+
 rad_status rad_get_table(rad_ctx *c, int which, void *host_out, size_t nbytes) {
     if (!c || !host_out) return fail(c, RAD_EINVAL, "rad_get_table: NULL argument");
     DeviceGuard guard(c->device);

@@ -96,5 +96,7 @@ int launch_stage_fused(const DeviceTables &t, const Params &p, const StageArgs &
 int launch_build_ke(const DeviceTables &t, double *ke, cudaStream_t s);
 int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed char *edge_sign, cudaStream_t s);
 int launch_maxspeed(const DeviceTables &t, double *out3, cudaStream_t s);
+// probe.cu: measured FP64 FMA rate of the current device (lane operations per second); 0 on success
+int probe_dfma_rate(double *dfma_per_sec, long long *launches);
 
 }  // namespace rad
