@@ -164,6 +164,7 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override cells per axis (same box)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-n", type=int, default=None, help="sub-block size of the oracle sample (default: 64 for --impl reference, 96 for the cpu_baseline leg)")
+    ap.add_argument("--recon", type=int, default=1, help="spatial reconstruction: 1 PLM (the workload's), 0 donor cell (diagnostic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -211,7 +212,7 @@ def main():
     T_out = torch.zeros(ncell, dtype=torch.float64, device="cuda"); dT0 = torch.zeros(4, ncell, dtype=torch.float64, device="cuda")
     h = B.rad_create(dict(kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg)),
                      dict(n=nn, x0=x0, dx=dx, bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3), c["angles"], (opac[0], opac[1], opac[2]),
-                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=1, renorm_fluid_weights=1, couple=1), local)
+                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=args.recon, renorm_fluid_weights=1, couple=1), local)
     vmax = float(B.rad_get_table(h, B.TAB_MAXSPEED).max())
     dt = W.CFL * min(dx) / vmax
     stream = torch.cuda.current_stream()

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of librad.so (include/rad.h): argument checking, context ownership, launches.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -58,6 +59,17 @@ bool upload(rad_ctx *c, const std::vector<T> &h, const T **dptr) {
 }
 
 bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+
+// the fused stage kernel: the tile-synchronous version (stage4.cu) where it serves the configuration, else the
+// warp-independent version (stage.cu).  RAD_STAGE_KERNEL=3 in the environment forces the latter (A/B measurements).
+int launch_fused(const rad::DeviceTables &t, const rad::Params &p, const rad::StageArgs &a, bool couple, cudaStream_t s) {
+    static const bool force_v3 = [] { const char *e = std::getenv("RAD_STAGE_KERNEL"); return e && e[0] == '3'; }();
+    if (!force_v3) {
+        const int nl = rad::launch_stage_tile(t, p, a, couple, s);
+        if (nl != 0) return nl;
+    }
+    return rad::launch_stage_fused(t, p, a, couple, s);
+}
 }  // namespace
 
 extern "C" {
@@ -226,7 +238,7 @@ rad_status rad_transport(rad_ctx *c, double *I_in, double *I_out, const double *
     if (st != RAD_OK) return st;
     rad::StageArgs a{};
     a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
-    int nl = rad::launch_stage_fused(c->dev, c->kp, a, false, (cudaStream_t)stream);
+    int nl = launch_fused(c->dev, c->kp, a, false, (cudaStream_t)stream);
     if (nl == 0) nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, (cudaStream_t)stream);
     if (nl < 0) return cuda_fail(c, "rad_transport");
     c->launches += nl;
@@ -271,7 +283,7 @@ rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, 
         a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
         a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
         a.T_out = T_out; a.dT0 = dT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
-        int nl = rad::launch_stage_fused(c->dev, c->kp, a, true, s);
+        int nl = launch_fused(c->dev, c->kp, a, true, s);
         if (nl < 0) return cuda_fail(c, "rad_stage");
         if (nl > 0) {
             c->launches += nl;
