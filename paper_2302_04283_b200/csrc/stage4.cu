@@ -31,21 +31,24 @@ constexpr int TY = 4, TZ = 3, NW = TY * TZ, NH = 4 * TZ + 4 * TY, RING = 5;
 struct Layout {
     int Np;   // row stride of intensity rows (even, >= N)
     int Kp;   // stride of the per-warp coefficient/flux buffers: 3 N + 2 (slot 3N is the always-zero flux)
-    int oR, oH, oK, oU, oN, oW, oD, oRec, oBar, total;
+    int Nt;   // length of the per-angle tables, padded to a whole number of warp iterations (lanes past N read benign entries)
+    int oR, oH, oK, oU, oUraw, oN, oW, oD, oRec, oBar, total;
 };
 __host__ __device__ inline Layout make_layout(int N) {
     Layout L;
     L.Np = (N + 1) & ~1;
     L.Kp = 3 * N + 2;
+    L.Nt = ((N + 31) / 32) * 32;
     L.oR = 0;
     L.oH = L.oR + RING * NW * L.Np;
     L.oK = L.oH + 2 * NH * L.Np;
     L.oU = L.oK + NW * L.Kp;
-    L.oN = L.oU + NW * 64;
-    L.oW = L.oN + 3 * L.Np;
-    L.oD = L.oW + L.Np;
-    L.oRec = L.oD + L.Np;          // uint4 per angle = 2 doubles
-    L.oBar = L.oRec + 2 * L.Np;    // 2 + NW mbarriers (8 bytes each)
+    L.oUraw = L.oU + NW * 64;
+    L.oN = L.oUraw + NW * 64;
+    L.oW = L.oN + 3 * L.Nt;
+    L.oD = L.oW + L.Nt;
+    L.oRec = L.oD + L.Nt;          // uint4 per angle = 2 doubles
+    L.oBar = L.oRec + 2 * L.Nt;    // 2 + NW mbarriers (8 bytes each)
     L.total = L.oBar + 2 + NW;
     return L;
 }
@@ -98,6 +101,18 @@ __device__ __forceinline__ FaceRec load_face_s(const double *f) {  // shared mem
     return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
 }
 
+// The same through volatile loads: the record is re-read at every use instead of being kept in 16 registers for the whole
+// step (five face records in registers are what made the kernel spill; a warp-uniform shared-memory read is one wavefront).
+__device__ __forceinline__ double2 lds_v2(uint32_t addr) {
+    double2 v;
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ FaceRec load_face_v(uint32_t addr) {
+    const double2 a = lds_v2(addr), b = lds_v2(addr + 16), c = lds_v2(addr + 32), d = lds_v2(addr + 48);
+    return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
+}
+
 // Upwind flux through a face (Eq.24), split into weight and face value: returns w = n^a n_0 / dx_a and sets
 // `up` to the reconstructed upwind intensity.  PLM: van Leer limited slope of the upwind cell (R7): with (far, mid, oth)
 // = (LL, L, R) for n^a > 0 and (RR, R, L) otherwise, the face value is mid + dl dr / (dl + dr), dl = mid - far,
@@ -118,30 +133,61 @@ __device__ __forceinline__ double face_w(const FaceRec &f, double n1, double n2,
     return __dmul_rn(na, n0);
 }
 
+// 8-byte asynchronous copy global -> shared (LDGSTS): the per-cell records are fetched one step ahead without holding
+// registers (a register prefetch would be spilled and the spill would wait for the load)
+__device__ __forceinline__ void cp_async8(uint32_t dst, const void *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// sums of four values over the warp, all lanes get all four: the first two butterfly steps halve the number of values a
+// lane carries instead of adding four values each (6 adds and 10 64-bit shuffles instead of 20 and 20)
+__device__ __forceinline__ void warp_sum4(double &a, double &b, double &c, double &d, int lane) {
+    const unsigned full = 0xffffffffu;
+    const bool u16 = (lane & 16) != 0;
+    double k0 = u16 ? c : a, k1 = u16 ? d : b;
+    k0 += __shfl_xor_sync(full, u16 ? a : c, 16);
+    k1 += __shfl_xor_sync(full, u16 ? b : d, 16);
+    const bool u8 = (lane & 8) != 0;
+    double k = u8 ? k1 : k0;
+    k += __shfl_xor_sync(full, u8 ? k0 : k1, 8);
+    k += __shfl_xor_sync(full, k, 4);
+    k += __shfl_xor_sync(full, k, 2);
+    k += __shfl_xor_sync(full, k, 1);
+    a = __shfl_sync(full, k, 0); b = __shfl_sync(full, k, 8); c = __shfl_sync(full, k, 16); d = __shfl_sync(full, k, 24);
+}
+
 // ------------------------------------------------------------------------------------------------------------------
 template <int NITER, bool PLM, bool COUPLE>
 __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, const Params p, const StageArgs a, const int KX) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = t.N;
     const Layout L = make_layout(N);
-    const int Np = L.Np, Kp = L.Kp;
+    const int Np = L.Np, Kp = L.Kp, Nt = L.Nt;
     double *sm = reinterpret_cast<double *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int wy = w % TY, wz = w / TY;
-    double *sR = sm + L.oR, *sH = sm + L.oH, *sK = sm + L.oK + w * Kp, *sU = sm + L.oU + w * 64;
+    double *sR = sm + L.oR, *sH = sm + L.oH, *sK = sm + L.oK + w * Kp, *sU = sm + L.oU + w * 64, *sUraw = sm + L.oUraw + w * 64;
     double *sN = sm + L.oN, *sWinv = sm + L.oW, *sDom = sm + L.oD;
     uint4 *sRec = reinterpret_cast<uint4 *>(sm + L.oRec);
     const uint32_t bar0 = smem_u32(sm + L.oBar);           // full[0], full[1], then kbar[w]
     const uint32_t kbar = bar0 + 8u * (2 + w);
     const uint32_t row_bytes = (uint32_t)N * 8u, ke_bytes = 3u * (uint32_t)N * 8u;
 
-    for (int q = tid; q < N; q += blockDim.x) {
-        sWinv[q] = t.winv[q];
-        sDom[q] = t.domega[q];
-        sRec[q] = reinterpret_cast<const uint4 *>(t.ang_rec)[q];
-        sN[q] = t.nhat[3 * q]; sN[Np + q] = t.nhat[3 * q + 1]; sN[2 * Np + q] = t.nhat[3 * q + 2];
+    // per-angle tables; entries past N (read by the idle lanes of the last iteration) are benign: direction of angle 0,
+    // zero weights, partner 0, pulls from the always-zero flux slot
+    for (int q = tid; q < Nt; q += blockDim.x) {
+        const int qa = q < N ? q : 0;
+        sWinv[q] = q < N ? t.winv[qa] : 0.0;
+        sDom[q] = q < N ? t.domega[qa] : 0.0;
+        uint4 rec = reinterpret_cast<const uint4 *>(t.ang_rec)[qa];
+        if (q >= N) { const unsigned z = 3u * (unsigned)N; rec = make_uint4(0u, z << 16, z | (z << 16), 0u); }
+        sRec[q] = rec;
+        sN[q] = t.nhat[3 * qa]; sN[Nt + q] = t.nhat[3 * qa + 1]; sN[2 * Nt + q] = t.nhat[3 * qa + 2];
     }
     if (lane == 0) { sK[3 * N] = 0.0; sK[3 * N + 1] = 0.0; }
+    sU[lane] = 0.0; sU[32 + lane] = 0.0;
     if (tid == 0) {
         for (int q = 0; q < 2 + NW; q++) mbar_init(bar0 + 8u * q, 1);
         fence_mbar_init();
@@ -206,36 +252,41 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
     }
 
     const double idx0 = t.inv_dx[0], idx1 = t.inv_dx[1], idx2 = t.inv_dx[2];
-    const int last_off = min((NITER - 1) * 32 + lane, N - 1);
     const bool last_valid = (NITER - 1) * 32 + lane < N;
 
-    // Warp-uniform records of a cell, gathered two per lane in one round trip and broadcast through shared memory:
+    // Warp-uniform records of a cell, gathered two per lane (cp.async, one step ahead) and broadcast through shared memory:
     //   sU[0..7] x face above, [8..15] y face below, [16..23] y face above, [24..31] z face below, [32..39] z face above
     //            (E parts multiplied by 1/dx of the face's axis),
-    //   [40] n^0, [41..44] n^0 E_0..E_3, [45] excised flag, [46..51] co-triad, [52..56] rho, T, u1', u2', u3',
+    //   [40] n^0, [41] excised flag, [42..45] n^0 E_0..E_3, [46..51] co-triad, [52..56] rho, T, u1', u2', u3',
     //   [57..59] alpha_P, alpha_E, alpha_s
     const double *ptrA = t.face, *ptrB = t.cell;
     int strideB = 0;
     double sclA = 1.0;
-    bool sclB_n0 = false;
+    bool sclB_n0 = false, haveB = false;
     if (active) {
         const long long c = c_first, cz = (long long)t.NI * t.NJ;
         const int g = lane >> 3, r = lane & 7;
         ptrA = t.face + ((g == 0 ? c + 1 : (g == 2 ? c + t.NI : c)) * 3 + (g == 0 ? 0 : (g == 3 ? 2 : 1))) * RAD_NFACE + r;
         if (r >= 4) sclA = g == 0 ? idx0 : (g == 3 ? idx2 : idx1);
-        ptrB = t.cell + c * RAD_NCELL;  // lanes 28..31: unused
+        ptrB = t.cell + c * RAD_NCELL;
         strideB = RAD_NCELL;
+        haveB = lane < 20;
         if (lane < 8) { ptrB = t.face + ((c + cz) * 3 + 2) * RAD_NFACE + lane; strideB = 3 * RAD_NFACE; }
-        else if (lane < 13) { ptrB += lane - 8; sclB_n0 = lane > 8; }
-        else if (lane == 13) ptrB += 50;
+        else if (lane == 8) ;                                            // n^0
+        else if (lane == 9) ptrB += 50;                                  // excised flag
+        else if (lane < 14) { ptrB += lane - 9; sclB_n0 = true; }        // E_0..E_3, stored multiplied by n^0
         else if (lane < 20) ptrB += 44 + (lane - 14);
         else if (COUPLE && p.couple && lane < 28) {
             ptrB = lane < 25 ? a.fluid + (long long)(lane - 20) * t.ncell + c : (lane == 25 ? a.aP : (lane == 26 ? a.aE : a.aS)) + c;
-            strideB = 1;
-        } else if (COUPLE && lane == 21) { ptrB = a.fluid + t.ncell + c; strideB = 1; }  // T_- is reported even when not coupling
+            strideB = 1; haveB = true;
+        } else if (COUPLE && lane == 21) { ptrB = a.fluid + t.ncell + c; strideB = 1; haveB = true; }  // T_- is reported even when not coupling
     }
-    double uA = 0.0, uB = 0.0;
-    if (active) { uA = __ldg(ptrA); uB = __ldg(ptrB); ptrA += 3 * RAD_NFACE; ptrB += strideB; }
+    const uint32_t rawA = smem_u32(sUraw + lane), rawB = smem_u32(sUraw + 32 + lane);
+    if (active) {
+        cp_async8(rawA, ptrA); ptrA += 3 * RAD_NFACE;
+        if (haveB) { cp_async8(rawB, ptrB); ptrB += strideB; }
+    }
+    cp_async_commit();
 
     // ---- flux through the lower x face of the first cell of this run (carried from then on)
     double carry[NITER];
@@ -247,17 +298,17 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
             f = {__ldg(fr), __ldg(fr + 1), __ldg(fr + 2), __ldg(fr + 3), __ldg(fr + 4) * idx0, __ldg(fr + 5) * idx0, __ldg(fr + 6) * idx0,
                  __ldg(fr + 7) * idx0};
         }
-        const double *r0 = sR + (0 * NW + w) * Np, *r1 = sR + (1 * NW + w) * Np, *r2 = sR + (2 * NW + w) * Np, *r3 = sR + (3 * NW + w) * Np;
+        const double *r0 = sR + (0 * NW + w) * Np + lane, *r1 = sR + (1 * NW + w) * Np + lane, *r2 = sR + (2 * NW + w) * Np + lane,
+                     *r3 = sR + (3 * NW + w) * Np + lane;
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
-            const int n = it < NITER - 1 ? it * 32 + lane : last_off;
+            const int n = it * 32 + lane;
             double up;
-            const double wgt = face_w<PLM>(f, sN[n], sN[Np + n], sN[2 * Np + n], PLM ? r0[n] : 0.0, r1[n], r2[n], PLM ? r3[n] : 0.0, up);
+            const double wgt = face_w<PLM>(f, sN[n], sN[Nt + n], sN[2 * Nt + n], PLM ? r0[it * 32] : 0.0, r1[it * 32], r2[it * 32],
+                                           PLM ? r3[it * 32] : 0.0, up);
             carry[it] = __dmul_rn(wgt, up);
         }
     }
-
-    const double thr_mask = p.n0_crit;  // |n_0| < n0_crit  <=>  |n^0 n_0| < n0_crit n^0
 
     for (int s = 0; s < nsteps; s++) {
         const int i = i_begin + s;
@@ -272,44 +323,54 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
         if (!active) continue;
 
         const long long c = c_first + s;
-        // ring slots of planes i-1, i, i+1, i+2 (plane i_begin + d lives in slot (d + 2) % 5)
-        const double *Rm1 = sR + (((s + 1) % RING) * NW) * Np, *R0 = sR + (((s + 2) % RING) * NW) * Np,
-                     *Rp1 = sR + (((s + 3) % RING) * NW) * Np, *Rp2 = sR + (((s + 4) % RING) * NW) * Np;
-        const double *Hc = sH + ((s & 1) * NH) * Np;
+        // ring slots of planes i-1, i, i+1, i+2 (plane i_begin + d lives in slot (d + 2) % 5); all pointers include the lane
+        const double *R0 = sR + (((s + 2) % RING) * NW) * Np + lane;
+        const double *Hc = sH + ((s & 1) * NH) * Np + lane;
         const double *own = R0 + w * Np;
+        const double *xm1 = sR + (((s + 1) % RING) * NW + w) * Np + lane, *xp1 = sR + (((s + 3) % RING) * NW + w) * Np + lane,
+                     *xp2 = sR + (((s + 4) % RING) * NW + w) * Np + lane;
 
-        // ---- uniform records of this cell -> shared memory; fetch the next cell's
+        // ---- uniform records of this cell: raw (landed by cp.async) -> scaled -> sU; fetch the next cell's
         {
-            const double nup0 = __shfl_sync(0xffffffffu, uB, 8);
+            cp_async_wait_all();
+            const double vA = sUraw[lane], vB = sUraw[32 + lane];
+            const double nup0 = __shfl_sync(0xffffffffu, vB, 8);
             __syncwarp();  // the previous step's readers of sU are done
-            sU[lane] = uA * sclA;
-            sU[32 + lane] = lane < 8 ? uB * ((lane >= 4) ? idx2 : 1.0) : (sclB_n0 ? uB * nup0 : uB);
-            if (more) { uA = __ldg(ptrA); uB = __ldg(ptrB); ptrA += 3 * RAD_NFACE; ptrB += strideB; }
+            sU[lane] = vA * sclA;
+            sU[32 + lane] = lane < 8 ? vB * ((lane >= 4) ? idx2 : 1.0) : (sclB_n0 ? vB * nup0 : vB);
+            if (more) {
+                cp_async8(rawA, ptrA); ptrA += 3 * RAD_NFACE;
+                if (haveB) { cp_async8(rawB, ptrB); ptrB += strideB; }
+            }
+            cp_async_commit();
         }
 
         // ---- angular fluxes (Eq.25, donor cell in angle): owners turn q_e into the edge flux in place
         double div[NITER];
         mbar_wait(kbar, s & 1);
+        {
+            const double *ownrow = own - lane;
 #pragma unroll
-        for (int it = 0; it < NITER; it++) {
-            const int n = it < NITER - 1 ? it * 32 + lane : last_off;
-            const uint4 rec = sRec[n];
-            const unsigned pj[3] = {rec.x & 0xffffu, rec.x >> 16, rec.y & 0xffffu};
-            double asum = 0.0;
+            for (int it = 0; it < NITER; it++) {
+                const int n = it * 32 + lane;
+                const uint4 rec = sRec[n];
+                const unsigned pj[3] = {rec.x & 0xffffu, rec.x >> 16, rec.y & 0xffffu};
+                double asum = 0.0;
 #pragma unroll
-            for (int jj = 0; jj < 3; jj++) {  // unused slots have q = 0
-                const double q = sK[jj * N + n];
-                const bool owner_up = (__double2loint(q) & 1) != 0;
-                const double G = q * own[owner_up ? (unsigned)n : pj[jj]];
-                asum += G;
-                if (it < NITER - 1 || last_valid) sK[jj * N + n] = G;
+                for (int jj = 0; jj < 3; jj++) {  // unused slots have q = 0
+                    const double q = sK[jj * N + n];
+                    const bool owner_up = (__double2loint(q) & 1) != 0;
+                    const double G = q * ownrow[owner_up ? (unsigned)n : pj[jj]];
+                    asum += G;
+                    if (it < NITER - 1 || last_valid) sK[jj * N + n] = G;
+                }
+                div[it] = asum;
             }
-            div[it] = asum;
         }
         __syncwarp();
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
-            const int n = it < NITER - 1 ? it * 32 + lane : last_off;
+            const int n = it * 32 + lane;
             const uint4 rec = sRec[n];
             const double asum = div[it] - ((sK[rec.y >> 16] + sK[rec.z & 0xffffu]) + sK[rec.z >> 16]);  // unused -> sK[3N] = 0
             div[it] = asum * sWinv[n];
@@ -322,51 +383,54 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
         }
 
         // ---- spatial fluxes (Eq.24), flux-divergence update of C = n^0 n_0 I (Eq.22, stage form R8), cons -> prim
-        const FaceRec fx = load_face_s(sU), fyl = load_face_s(sU + 8), fyh = load_face_s(sU + 16), fzl = load_face_s(sU + 24),
-                      fzh = load_face_s(sU + 32);
-        const double2 c01 = *reinterpret_cast<const double2 *>(sU + 40), c23 = *reinterpret_cast<const double2 *>(sU + 42),
-                      c45 = *reinterpret_cast<const double2 *>(sU + 44);
-        const double nup0 = c01.x, W0 = c01.y, W1 = c23.x, W2 = c23.y, W3 = c45.x;  // W = n^0 E: n^0 n_0 = W0 + W_b n^b
-        const bool excised = c45.y != 0.0;
+        const double2 c01 = *reinterpret_cast<const double2 *>(sU + 40);
+        const double nup0 = c01.x;
+        const bool excised = c01.y != 0.0;
         const double *nb[8];
 #pragma unroll
         for (int q = 0; q < 8; q++) nb[q] = ((nbHalo >> q) & 1u ? Hc : R0) + nbOff[q];
-        const double *xm1 = Rm1 + w * Np, *xp1 = Rp1 + w * Np, *xp2 = Rp2 + w * Np;
-        const double mbdt = -a.beta_dt, thr = thr_mask * nup0;
+        const double mbdt = -a.beta_dt, thr = p.n0_crit * nup0;  // |n_0| < n0_crit  <=>  |n^0 n_0| < n0_crit n^0
         double Is[NITER];
         unsigned maskbits = 0;
+        const uint32_t sUa = smem_u32(sU);
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
-            const int n = it < NITER - 1 ? it * 32 + lane : last_off;
-            const double n1 = sN[n], n2 = sN[Np + n], n3 = sN[2 * Np + n];
-            const double Iown = own[n];
+            const int n = it * 32 + lane, o = it * 32;
+            const double n1 = sN[n], n2 = sN[Nt + n], n3 = sN[2 * Nt + n];
+            const double Iown = own[o];
             double d = div[it], up;
             {   // x: flux through the upper face (the lower x face of cell i+1); the lower one is carried
-                const double wgt = face_w<PLM>(fx, n1, n2, n3, PLM ? xm1[n] : 0.0, Iown, xp1[n], PLM ? xp2[n] : 0.0, up);
+                const FaceRec fx = load_face_v(sUa);
+                const double wgt = face_w<PLM>(fx, n1, n2, n3, PLM ? xm1[o] : 0.0, Iown, xp1[o], PLM ? xp2[o] : 0.0, up);
                 const double F = __dmul_rn(wgt, up);
                 d += F - carry[it];
                 carry[it] = F;
             }
             {   // y: rows -2, -1, +1, +2 serve both faces
-                const double m2 = PLM ? nb[0][n] : 0.0, m1 = nb[1][n], p1 = nb[2][n], p2 = PLM ? nb[3][n] : 0.0;
-                const double wl = face_w<PLM>(fyl, n1, n2, n3, m2, m1, Iown, p1, up);
+                const double m2 = PLM ? nb[0][o] : 0.0, m1 = nb[1][o], p1 = nb[2][o], p2 = PLM ? nb[3][o] : 0.0;
+                const FaceRec fl = load_face_v(sUa + 64);
+                const double wl = face_w<PLM>(fl, n1, n2, n3, m2, m1, Iown, p1, up);
                 d = fma(-wl, up, d);
-                const double wh = face_w<PLM>(fyh, n1, n2, n3, m1, Iown, p1, p2, up);
+                const FaceRec fh = load_face_v(sUa + 128);
+                const double wh = face_w<PLM>(fh, n1, n2, n3, m1, Iown, p1, p2, up);
                 d = fma(wh, up, d);
             }
             {   // z
-                const double m2 = PLM ? nb[4][n] : 0.0, m1 = nb[5][n], p1 = nb[6][n], p2 = PLM ? nb[7][n] : 0.0;
-                const double wl = face_w<PLM>(fzl, n1, n2, n3, m2, m1, Iown, p1, up);
+                const double m2 = PLM ? nb[4][o] : 0.0, m1 = nb[5][o], p1 = nb[6][o], p2 = PLM ? nb[7][o] : 0.0;
+                const FaceRec fl = load_face_v(sUa + 192);
+                const double wl = face_w<PLM>(fl, n1, n2, n3, m2, m1, Iown, p1, up);
                 d = fma(-wl, up, d);
-                const double wh = face_w<PLM>(fzh, n1, n2, n3, m1, Iown, p1, p2, up);
+                const FaceRec fh = load_face_v(sUa + 256);
+                const double wh = face_w<PLM>(fh, n1, n2, n3, m1, Iown, p1, p2, up);
                 d = fma(wh, up, d);
             }
-            const double wgt = chain4(W0, W1, W2, W3, n1, n2, n3);  // n^0 n_0 at the cell centre
+            const double2 w01 = lds_v2(sUa + 8 * 42), w23 = lds_v2(sUa + 8 * 44);
+            const double wgt = chain4(w01.x, w01.y, w23.x, w23.y, n1, n2, n3);  // n^0 n_0 at the cell centre (sU[42..45] = n^0 E)
             if (fabs(wgt) < thr) maskbits |= 1u << it;
             double v = a.gam1 * Iown;
-            if (a.I0 != nullptr) v = fma(a.gam0, __ldg(a.I0 + c * N + n), v);
+            if (a.I0 != nullptr) v = fma(a.gam0, __ldg(a.I0 + c * N + min(n, N - 1)), v);
             v = fma(mbdt * d, fast_rcp(wgt), v);
-            Is[it] = excised ? 0.0 : v;
+            Is[it] = (excised || (it == NITER - 1 && !last_valid)) ? 0.0 : v;
         }
 
         if (COUPLE) {
@@ -390,14 +454,14 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
             double Wsum = 0.0, A1 = 0.0, A2 = 0.0, Em = 0.0;
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const int n = it < NITER - 1 ? it * 32 + lane : last_off;
-                const double n1 = sN[n], n2 = sN[Np + n], n3 = sN[2 * Np + n];
-                const double dom = (it < NITER - 1 || last_valid) ? sDom[n] : 0.0;
+                const int n = it * 32 + lane;
+                const double n1 = sN[n], n2 = sN[Nt + n], n3 = sN[2 * Nt + n];
+                const double dom = sDom[n];  // 0 for idle lanes
                 const double nbar = uh[0] - fma(uh[3], n3, fma(uh[2], n2, uh[1] * n1));  // n^0bar = -u_alpha n^alpha
                 const double dd = fma(nbar, aEdt, nup0);
                 const double rp = fast_rcp(nbar * dd);
                 const double rd = nbar * rp, rn = dd * rp, rn2 = rn * rn;
-                const double x = (nbar * nbar) * (Is[it] * dom);                          // Ibar dOmega_bar (Eq.38 summand)
+                const double x = (nbar * nbar) * (Is[it] * dom);                            // Ibar dOmega_bar (Eq.38 summand)
                 g1[it] = nup0 * rd;
                 g2r4[it] = rn2 * rp;
                 Em += x;
@@ -405,7 +469,7 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
                 A2 = fma(dom, rp, A2);                                                      // Eq.42b
                 Wsum = fma(dom, rn2, Wsum);
             }
-            Wsum = warp_sum(Wsum); A1 = warp_sum(A1); A2 = warp_sum(A2); Em = warp_sum(Em);
+            warp_sum4(Wsum, A1, A2, Em, lane);
             double Tp = Tm, src = 0.0;
             bool coupled = false, noroot = false;
             if (p.couple && enable) {
@@ -415,11 +479,7 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
                 const double B4 = A2 * aP * p.a_rad, om = 1.0 - A2 * aS;                   // Eq.50
                 const double B1 = Cv * om, Bp = A1 - om * Em;
                 double dTemp = 0.0;
-#ifdef RAD_EXP_NOQUARTIC
-                if (false) {
-#else
                 if (!quartic_delta(B4, B1, Bp, Tm, dTemp)) {
-#endif
                     noroot = true;
                 } else {
                     coupled = true;
@@ -433,9 +493,9 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
             double M0 = 0.0, M1 = 0.0, M2 = 0.0, M3 = 0.0;
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const int n = it < NITER - 1 ? it * 32 + lane : last_off;
-                const double n1 = sN[n], n2 = sN[Np + n], n3 = sN[2 * Np + n];
-                const double dom = (it < NITER - 1 || last_valid) ? sDom[n] : 0.0;
+                const int n = it * 32 + lane;
+                const double n1 = sN[n], n2 = sN[Nt + n], n3 = sN[2 * Nt + n];
+                const double dom = sDom[n];
                 const double Iold = Is[it];
                 double Inew = coupled ? fma(src, g2r4[it], g1[it] * Iold) : Iold;
                 const double wI = dom * (Inew - Iold);
@@ -443,22 +503,23 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage4(const DeviceTables t, con
                 if (thr > 0.0 && enable && ((maskbits >> it) & 1u)) Inew = 0.0;
                 Is[it] = Inew;
             }
-            M0 = warp_sum(M0); M1 = warp_sum(M1); M2 = warp_sum(M2); M3 = warp_sum(M3);
+            warp_sum4(M0, M1, M2, M3, lane);
             if (lane == 0) {
                 if (noroot && a.noroot) atomicAdd(a.noroot, 1ull);
                 if (a.T_out) a.T_out[c] = Tp;
                 if (a.dT0) {  // R^0_alpha = sum n^0 n_alpha I dOmega; n^0 n_0 = W_ahat n^ahat, n_i = theta^a_i n^a
-                    a.dT0[c] = -(W0 * M0 + W1 * M1 + W2 * M2 + W3 * M3);
+                    const double2 w01 = *reinterpret_cast<const double2 *>(sU + 42), w23 = *reinterpret_cast<const double2 *>(sU + 44);
+                    a.dT0[c] = -(w01.x * M0 + w01.y * M1 + w23.x * M2 + w23.y * M3);
                     a.dT0[t.ncell + c] = -(nup0 * (th[0] * M1));
                     a.dT0[2 * t.ncell + c] = -(nup0 * (th[1] * M1 + th[3] * M2));
                     a.dT0[3 * t.ncell + c] = -(nup0 * (th[2] * M1 + th[4] * M2 + th[5] * M3));
                 }
             }
         }
-        double *out = a.I_out + c * N;
+        double *out = a.I_out + c * N + lane;
 #pragma unroll
         for (int it = 0; it < NITER; it++)
-            if (it < NITER - 1 || last_valid) out[it * 32 + lane] = Is[it];
+            if (it < NITER - 1 || last_valid) out[it * 32] = Is[it];
     }
 }
 
