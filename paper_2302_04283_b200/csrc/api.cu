@@ -18,6 +18,7 @@ struct rad_ctx {
     rad::AngleTables host;
     rad::EdgeOwnership own;
     double *ke = nullptr;  // stored edge coefficients (owned)
+    double *rec = nullptr; // packed per-cell records of the stage kernel (owned)
     rad::DeviceTables dev{};
     rad::Params kp{};
     std::vector<void *> owned;  // device allocations to free
@@ -60,11 +61,16 @@ bool upload(rad_ctx *c, const std::vector<T> &h, const T **dptr) {
 
 bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
 
-// the fused stage kernel: the tile-synchronous version (stage4.cu) where it serves the configuration, else the
-// warp-independent version (stage.cu).  RAD_STAGE_KERNEL=3 in the environment forces the latter (A/B measurements).
+// the fused stage kernel: the angle-resident version (stage5.cu) where it serves the configuration, else the
+// tile-synchronous warp-per-cell version (stage4.cu), else the warp-independent version (stage.cu).
+// RAD_STAGE_KERNEL=4 / 3 in the environment forces the older versions (A/B measurements).
 int launch_fused(const rad::DeviceTables &t, const rad::Params &p, const rad::StageArgs &a, bool couple, cudaStream_t s) {
-    static const bool force_v3 = [] { const char *e = std::getenv("RAD_STAGE_KERNEL"); return e && e[0] == '3'; }();
-    if (!force_v3) {
+    static const int force = [] { const char *e = std::getenv("RAD_STAGE_KERNEL"); return e ? std::atoi(e) : 0; }();
+    if (force == 0 || force == 5) {
+        const int nl = rad::launch_stage_angle(t, p, a, couple, s);
+        if (nl != 0) return nl;
+    }
+    if (force != 3) {
         const int nl = rad::launch_stage_tile(t, p, a, couple, s);
         if (nl != 0) return nl;
     }
@@ -106,7 +112,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     if (!c) return fail(nullptr, RAD_ENOMEM, "rad_create: out of host memory");
     c->device = device; c->metric = *m; c->grid = *g; c->angles = *a; c->params = *p;
     if (o) c->opac = *o;
-    c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit;
+    c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit; c->kp.rgm1 = 1.0 / (p->gamma_gas - 1.0);
     c->kp.recon_space = p->recon_space; c->kp.renorm = p->renorm_fluid_weights; c->kp.couple = p->couple;
     std::string err;
     bool ok = (a->kind == 0) ? rad::build_latlon(a->nzeta, a->npsi, c->host, err)
@@ -139,7 +145,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
          upload(c, h.edge_lo, &t.edge_lo) && upload(c, h.edge_hi, &t.edge_hi) && upload(c, h.edge_len, &t.edge_len) &&
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
     // fused stage kernel: balanced edge ownership, per-angle records, 1/dOmega
-    t.fused_ok = 0; t.ang_rec = nullptr; t.winv = nullptr; t.own_edge = nullptr; t.ke = nullptr;
+    t.fused_ok = 0; t.ang_rec = nullptr; t.winv = nullptr; t.own_edge = nullptr; t.ke = nullptr; t.rec = nullptr;
     if (ok && h.N <= 192) {
         std::string oerr;
         if (rad::build_edge_ownership(h, c->own, oerr)) {
@@ -201,6 +207,19 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
         }
         c->launches += nl;
         t.ke = c->ke;
+        // packed per-cell records of the angle-resident stage kernel (stage5.cu)
+        if (cudaMalloc((void **)&c->rec, sizeof(double) * (size_t)t.ncell * RAD_STAGE_RECN) == cudaSuccess) {
+            nl = rad::launch_pack_rec(t, c->rec, 0);
+            if (nl < 0 || cudaDeviceSynchronize() != cudaSuccess) {
+                std::string msg = std::string("rad_create: stage records: ") + cudaGetErrorString(cudaGetLastError());
+                rad_destroy(c);
+                return fail(nullptr, RAD_ECUDA, msg);
+            }
+            c->launches += nl;
+            t.rec = c->rec;
+        } else {
+            cudaGetLastError();  // not fatal: the older stage kernel serves the context
+        }
     }
     *out = c;
     return RAD_OK;
@@ -213,6 +232,7 @@ void rad_destroy(rad_ctx *c) {
     for (int q = 0; q < 2; q++) if (c->scratch_I[q]) cudaFree(c->scratch_I[q]);
     if (c->scratch_small) cudaFree(c->scratch_small);
     if (c->ke) cudaFree(c->ke);
+    if (c->rec) cudaFree(c->rec);
     delete c;
 }
 

@@ -62,7 +62,9 @@ struct DeviceTables {
     const int *own_edge;     // [N][3]
     const double *ke;        // [n2][n1][n0][3][N] interior cells only, or nullptr (not stored)
     int fused_ok;            // 1 if the fused kernel can serve this angle grid
+    const double *rec;       // [ncell][RAD_STAGE_RECN] packed per-cell record of the angle-resident stage kernel (stage5.cu), or nullptr
 };
+#define RAD_STAGE_RECN 36
 
 // arguments of one stage (device pointers are the caller's)
 struct StageArgs {
@@ -76,6 +78,7 @@ struct StageArgs {
 
 struct Params {
     double gamma_gas, a_rad, n0_crit;
+    double rgm1;  // 1 / (gamma_gas - 1)
     int recon_space, renorm, couple;
 };
 
@@ -95,6 +98,9 @@ int launch_moments(const DeviceTables &t, const double *I, int frame, const doub
 int launch_stage_fused(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
 // tile-synchronous fused stage kernel (stage4.cu): 1 launched, 0 not served, -1 CUDA error
 int launch_stage_tile(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
+// angle-resident fused stage kernel (stage5.cu): 1 launched, 0 not served, -1 CUDA error; and its record builder
+int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
+int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s);
 int launch_build_ke(const DeviceTables &t, double *ke, cudaStream_t s);
 int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed char *edge_sign, cudaStream_t s);
 int launch_maxspeed(const DeviceTables &t, double *out3, cudaStream_t s);

@@ -1,0 +1,691 @@
+// stage5.cu -- the fused stage kernel, angle-resident version: spatial + angular flux divergence (Eq.22, 24, 25),
+// cons -> prim, locally implicit coupling (section 2.5), ergosphere mask, fluid increment
+// in ONE launch.
+//
+// Mapping:
+//   * a CTA owns a TY x TZ tile of cell columns in the y-z plane and marches along x through KX cells.  A cell is served
+//     by WPC warps; a thread keeps NITER FIXED angles for the whole march, so the angle's direction, solid angle and
+//     edge-ownership record live in registers, and so does the x stencil (I of planes i-1 .. i+2 is rotated, one new
+//     value per step) and the flux through the lower x face (carried).
+//   * every face flux is computed ONCE: a cell computes the flux through its upper y and z faces and publishes it in
+//     shared memory; the neighbour above takes it as its lower-face flux after the CTA barrier of the step (only the
+//     cells on the low edges of the tile compute their lower faces themselves).
+//   * shared memory is filled by bulk asynchronous copies (TMA, 1-D) two steps ahead, completion on two mbarriers: the
+//     tile's own rows (ring of 4 planes), the 2-deep halo rows of the current plane (2 buffers), the stored angular-edge
+//     coefficients of each cell (2 buffers; the owner of an edge overwrites the coefficient with the edge flux, the
+//     partner angle pulls it from there), and a packed per-cell geometry record (4 buffers).  One __syncthreads per step.
+//   * the coupling's angle sums are warp butterflies followed by a WPC-way exchange through shared memory under a
+//     named barrier private to the cell.
+#include <cstdlib>
+
+#include "async_copy.cuh"
+#include "stage_math.cuh"
+
+namespace rad {
+namespace {
+
+constexpr int RECN = RAD_STAGE_RECN;  // packed per-cell record, see k_pack_rec
+constexpr int USTR = 64;              // a cell's record slot in shared memory: [0..35] record, [36..43] lower y face,
+                                      // [44..51] lower z face, [52..59] rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s
+
+template <int TY_, int TZ_, int WPC_>
+struct Tile {
+    static constexpr int TY = TY_, TZ = TZ_, WPC = WPC_;
+    static constexpr int NC = TY * TZ, NH = 4 * TZ + 4 * TY, NR = 3 * NC + NH + TY + TZ, NT = NC * WPC * 32;
+    static constexpr int NFY = (TY - 1) * TZ, NFZ = TY * (TZ - 1);
+};
+
+struct Layout5 {
+    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oU, oRed, oRole, oBar, total;  // offsets in doubles
+};
+template <class T>
+__host__ __device__ inline Layout5 make_layout5(int N) {
+    Layout5 L;
+    L.Np = (N + 1) & ~1;
+    L.Kp = (3 * N + 3) & ~1;  // 3 N coefficients / fluxes + the always-zero slot 3N
+    L.oRing = 0;
+    L.oHalo = L.oRing + 4 * T::NC * L.Np;
+    L.oE = L.oHalo + 2 * T::NH * L.Np;
+    L.oFy = L.oE + 2 * T::NC * L.Kp;
+    L.oFz = L.oFy + 2 * T::NFY * L.Np;
+    L.oU = L.oFz + 2 * T::NFZ * L.Np;
+    L.oRed = L.oU + 4 * T::NC * USTR;
+    L.oRole = L.oRed + T::NC * (2 * T::WPC * 4 + 4);  // per cell: two sets of WPC partial sums, then (T_+, source, flag)
+    L.oBar = L.oRole + T::NR * 4;
+    L.total = L.oBar + 2;
+    return L;
+}
+
+// one bulk copy per step: what thread `r` of the CTA brings in for step u (source advances by `stride` doubles per step,
+// destination cycles through nbuf buffers `dstride` doubles apart)
+struct Role {
+    const double *src0;
+    int stride, dst0, dstride, nbufm1, boff, bytes;
+};
+static_assert(sizeof(Role) == 32, "Role is stored as four doubles");
+
+struct FaceRec {  // n^a = e0 + e_b n^b;  n_0 / dx_a = E0 + E_b n^b (the grid spacing is folded in)
+    double e0, e1, e2, e3, E0, E1, E2, E3;
+};
+__device__ __forceinline__ FaceRec load_face(const double *f) {  // warp-uniform address
+    const double2 a = *reinterpret_cast<const double2 *>(f), b = *reinterpret_cast<const double2 *>(f + 2),
+                  c = *reinterpret_cast<const double2 *>(f + 4), d = *reinterpret_cast<const double2 *>(f + 6);
+    return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
+}
+
+// Upwind flux n^a n_0 I / dx_a (Eq.24) through the face between cells L and R; qLL, qL, qR, qRR are the
+// intensities of the four cells around it.  PLM: van Leer limited slope of the upwind cell (R7): with (far, mid, oth)
+// = (LL, L, R) for n^a > 0 and (RR, R, L) otherwise, the face value is mid + dl dr / (dl + dr), dl = mid - far,
+// dr = oth - mid (the harmonic mean is odd under reversal, so one formula serves both signs).  Branch free; sign tests
+// are integer tests of the high word (na = +-0 -> the flux is 0 either way).
+template <bool PLM>
+__device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double n2, double n3, double qLL, double qL, double qR, double qRR) {
+    const double na = chain4(f.e0, f.e1, f.e2, f.e3, n1, n2, n3);
+    const double n0 = chain4(f.E0, f.E1, f.E2, f.E3, n1, n2, n3);
+    const bool pos = hi32(na) > 0;
+    double up = pos ? qL : qR;
+    if (PLM) {
+        const double far = pos ? qLL : qRR, oth = pos ? qR : qL;
+        const double dl = up - far, dr = oth - up, pr = dl * dr;
+        const double h = div3(pr, dl + dr);  // only used where pr > 0, i.e. dl + dr != 0
+        up += hi32(pr) > 0 ? h : 0.0;
+    }
+    return __dmul_rn(__dmul_rn(na, n0), up);
+}
+
+// sums of four values over the warp, all lanes get all four: the first two butterfly steps halve the number of values a
+// lane carries instead of adding four values each
+__device__ __forceinline__ void warp_sum4(double &a, double &b, double &c, double &d, int lane) {
+    const unsigned full = 0xffffffffu;
+    const bool u16 = (lane & 16) != 0;
+    double k0 = u16 ? c : a, k1 = u16 ? d : b;
+    k0 += __shfl_xor_sync(full, u16 ? a : c, 16);
+    k1 += __shfl_xor_sync(full, u16 ? b : d, 16);
+    const bool u8 = (lane & 8) != 0;
+    double k = u8 ? k1 : k0;
+    k += __shfl_xor_sync(full, u8 ? k0 : k1, 8);
+    k += __shfl_xor_sync(full, k, 4);
+    k += __shfl_xor_sync(full, k, 2);
+    k += __shfl_xor_sync(full, k, 1);
+    a = __shfl_sync(full, k, 0); b = __shfl_sync(full, k, 8); c = __shfl_sync(full, k, 16); d = __shfl_sync(full, k, 24);
+}
+
+// the four warp sums written to shared memory at `dst` (32 bytes) by the lanes that hold them after the butterfly
+__device__ __forceinline__ void warp_sum4_to(double a, double b, double c, double d, int lane, uint32_t dst) {
+    const unsigned full = 0xffffffffu;
+    const bool u16 = (lane & 16) != 0;
+    double k0 = u16 ? c : a, k1 = u16 ? d : b;
+    k0 += __shfl_xor_sync(full, u16 ? a : c, 16);
+    k1 += __shfl_xor_sync(full, u16 ? b : d, 16);
+    const bool u8 = (lane & 8) != 0;
+    double k = u8 ? k1 : k0;
+    k += __shfl_xor_sync(full, u8 ? k0 : k1, 8);
+    k += __shfl_xor_sync(full, k, 4);
+    k += __shfl_xor_sync(full, k, 2);
+    k += __shfl_xor_sync(full, k, 1);
+    if ((lane & 7) == 0) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dst + (uint32_t)lane), "d"(k) : "memory");  // lanes 0, 8, 16, 24 hold a, b, c, d
+}
+
+// the same over the WPC warps of a cell: partial sums through `red` ([WPC][4] doubles), summed by every thread in the
+// same order
+template <int WPC>
+__device__ __forceinline__ void cell_sum4(double &a, double &b, double &c, double &d, int lane, int wc, double *red, int barid) {
+    warp_sum4(a, b, c, d, lane);
+    if (WPC > 1) {
+        if (lane == 0) {
+            reinterpret_cast<double2 *>(red + wc * 4)[0] = make_double2(a, b);
+            reinterpret_cast<double2 *>(red + wc * 4)[1] = make_double2(c, d);
+        }
+        named_bar_sync(barid, WPC * 32);
+        a = b = c = d = 0.0;
+#pragma unroll
+        for (int q = 0; q < WPC; q++) {
+            const double2 v0 = reinterpret_cast<const double2 *>(red + q * 4)[0], v1 = reinterpret_cast<const double2 *>(red + q * 4)[1];
+            a += v0.x; b += v0.y; c += v1.x; d += v1.y;
+        }
+    }
+}
+
+// ---- shared-memory access through 32-bit addresses (bytes); `volatile` keeps the program order against barriers
+__device__ __forceinline__ double lds(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double2 lds2(uint32_t addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts(uint32_t addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
+__device__ __forceinline__ void sts2(uint32_t addr, double x, double y) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ FaceRec lds_face(uint32_t addr) {  // warp-uniform address
+    const double2 a = lds2(addr), b = lds2(addr + 16), c = lds2(addr + 32), d = lds2(addr + 48);
+    return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
+}
+
+// Quartic Eq.49 solved for the temperature change d = T_+ - T_- (R13), as quartic_delta (stage_math.cuh) with cheaper
+// scalar arithmetic: reciprocals by rcp3, the fourth root of the starting point from the hardware rsqrt seeds (the start
+// only has to be near the upper bound: g is convex and increasing, so Newton converges from either side after one step).
+__device__ __forceinline__ bool quartic_delta_fast(double B4, double B1, double Bp, double Tm, double &d) {
+    const double B0 = Bp - B1 * Tm;
+    if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return false;
+    const double rB1 = rcp3(B1);
+    if (B4 == 0.0) { d = -Bp * rB1; return true; }
+    const double y = -B0 * rcp3(B4);
+    double r1, r2;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r1) : "d"(y));
+    const double sy = y * r1;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r2) : "d"(sy));
+    double T0 = sy * r2;                         // ~ y^(1/4)
+    if (!(T0 > 0.0)) T0 = __longlong_as_double(0x7ff0000000000000ll);  // y outside the range of the approximation: the other bound alone
+    d = fmin(-B0 * rB1, T0) - Tm;
+    const double B44 = 4.0 * B4, aBp = fabs(Bp);
+    for (int it = 0; it < 60; it++) {
+        const double T = Tm + d, T2 = T * T, T3 = T2 * T, q = B4 * (T2 * T2);
+        const double g = q + fma(B1, d, Bp), gp = fma(B44, T3, B1);
+        const double rgp = rcp3(gp);  // gp >= B1 > 0, finite
+        const double dd = g * rgp;
+        d -= dd;
+        if (fabs(dd) <= 1e-15 * (fabs(d) + (aBp + q) * rgp)) break;
+    }
+    return true;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+template <int NITER, int WPC, int TY, int TZ, bool PLM, bool COUPLE>
+__global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
+    k_stage5(const DeviceTables t, const Params p, const StageArgs a, const Layout5 L, const int KX) {
+    using T = Tile<TY, TZ, WPC>;
+    constexpr int NC = T::NC, NH = T::NH, NR = T::NR;
+    constexpr uint32_t ITB = WPC * 32 * 8;  // byte distance between a thread's consecutive angles
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *sm = reinterpret_cast<double *>(smem_raw);
+    const uint32_t smb = smem_u32(sm);
+    const int N = t.N;
+    const int Np = L.Np, Kp = L.Kp;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int w = __shfl_sync(0xffffffffu, tid >> 5, 0);  // warp-uniform by construction
+    const int cs = w / WPC, wc = w - cs * WPC;
+    const int wy = cs % TY, wz = cs / TY;
+    const uint32_t bar0 = smb + 8u * L.oBar;
+    Role *roles = reinterpret_cast<Role *>(sm + L.oRole);
+
+    const int ng = t.ng;
+    const int j0 = blockIdx.y * TY + ng, k0 = blockIdx.z * TZ + ng;
+    const int j = j0 + wy, k = k0 + wz;
+    const bool active = j < t.n[1] + ng && k < t.n[2] + ng;
+    const int i_begin = blockIdx.x * KX + ng, i_end = min(i_begin + KX, t.n[0] + ng), nsteps = i_end - i_begin;
+    const long long c_first = ((long long)k * t.NJ + j) * t.NI + i_begin;
+
+    // ---- copy roles
+    if (tid < NR) {
+        Role r;
+        r.src0 = nullptr; r.stride = 0; r.dst0 = 0; r.dstride = 0; r.nbufm1 = 0; r.boff = 0; r.bytes = 0;
+        const int row_bytes = N * 8;
+        if (tid < NC + NH) {
+            int jj, kk;
+            if (tid < NC) { jj = j0 + tid % TY; kk = k0 + tid / TY; }
+            else {
+                const int h = tid - NC;
+                if (h < 4 * TZ) { const int hz = h >> 2, q = h & 3; kk = k0 + hz; jj = j0 + (q < 2 ? q - 2 : TY + q - 2); }
+                else { const int hh = h - 4 * TZ, hy = hh >> 2, q = hh & 3; jj = j0 + hy; kk = k0 + (q < 2 ? q - 2 : TZ + q - 2); }
+            }
+            if (jj < t.NJ && kk < t.NK) {
+                const long long c0 = ((long long)kk * t.NJ + jj) * t.NI + i_begin;
+                r.stride = N; r.bytes = row_bytes;
+                if (tid < NC) { r.src0 = a.I_in + (c0 + 2) * N; r.dst0 = L.oRing + tid * Np; r.dstride = NC * Np; r.nbufm1 = 3; r.boff = 2; }
+                else { r.src0 = a.I_in + c0 * N; r.dst0 = L.oHalo + (tid - NC) * Np; r.dstride = NH * Np; r.nbufm1 = 1; }
+            }
+        } else {
+            const int q = tid - NC - NH;
+            int kind, ccs;  // 0 edge coefficients, 1 cell record, 2 lower y face, 3 lower z face
+            if (q < NC) { kind = 0; ccs = q; }
+            else if (q < 2 * NC) { kind = 1; ccs = q - NC; }
+            else if (q < 2 * NC + TZ) { kind = 2; ccs = (q - 2 * NC) * TY; }
+            else { kind = 3; ccs = q - 2 * NC - TZ; }
+            const int jj = j0 + ccs % TY, kk = k0 + ccs / TY;
+            if (jj < t.n[1] + ng && kk < t.n[2] + ng) {
+                const long long c0 = ((long long)kk * t.NJ + jj) * t.NI + i_begin;
+                if (kind == 0) {
+                    const long long ci = ((long long)(kk - ng) * t.n[1] + (jj - ng)) * t.n[0] + (i_begin - ng);
+                    r.src0 = t.ke + ci * 3 * N; r.stride = 3 * N; r.dst0 = L.oE + ccs * Kp; r.dstride = NC * Kp; r.nbufm1 = 1; r.bytes = 3 * row_bytes;
+                } else {
+                    r.stride = RECN; r.dstride = NC * USTR; r.nbufm1 = 3;
+                    if (kind == 1) { r.src0 = t.rec + c0 * RECN; r.dst0 = L.oU + ccs * USTR; r.bytes = RECN * 8; }
+                    else if (kind == 2) { r.src0 = t.rec + (c0 - t.NI) * RECN + 8; r.dst0 = L.oU + ccs * USTR + 36; r.bytes = 64; }
+                    else { r.src0 = t.rec + (c0 - (long long)t.NI * t.NJ) * RECN + 16; r.dst0 = L.oU + ccs * USTR + 44; r.bytes = 64; }
+                }
+            }
+        }
+        roles[tid] = r;
+    }
+    if (wc == 0 && lane < 2) {  // the always-zero flux slot of both coefficient buffers
+        sm[L.oE + (lane * NC + cs) * Kp + 3 * N] = 0.0;
+        if (3 * N + 1 < Kp) sm[L.oE + (lane * NC + cs) * Kp + 3 * N + 1] = 0.0;
+    }
+    if (tid == 0) {
+        mbar_init(bar0, 1); mbar_init(bar0 + 8u, 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    uint32_t step_bytes = 0;
+    if (tid == 0) {
+        uint32_t own_bytes = 0;
+        for (int r = 0; r < NR; r++) { step_bytes += (uint32_t)roles[r].bytes; if (r < NC) own_bytes += (uint32_t)roles[r].bytes; }
+        mbar_expect_tx(bar0, step_bytes + own_bytes);
+        if (nsteps > 1) mbar_expect_tx(bar0 + 8u, step_bytes + own_bytes);
+    }
+    __syncthreads();
+    // everything step u needs that is not yet resident, signalled on full[u & 1]: own rows of plane u+2 (ring slot
+    // (u+2) & 3), halo rows of plane u, coefficients and records of the cells of plane u
+    auto issue = [&](int u) {
+        const Role r = roles[tid];
+        if (r.bytes) {
+            const int buf = (u + r.boff) & r.nbufm1;
+            bulk_g2s(smb + 8u * (uint32_t)(r.dst0 + buf * r.dstride), r.src0 + (long long)u * r.stride, (uint32_t)r.bytes, bar0 + 8u * (u & 1));
+        }
+    };
+    if (tid < NR) {
+        issue(0);
+        if (nsteps > 1) issue(1);
+        if (tid < NC) { issue(-2); if (nsteps > 1) issue(-1); }  // own rows of planes 0 and 1
+    }
+
+    // ---- the thread's angles: n = lane + 32 wc + 32 WPC it.  Only the last one can fall past N; such a slot is idle:
+    // it reads angle 0, has zero weights, pulls from the always-zero flux slot and stores nothing.
+    const int nbase = wc * 32 + lane;
+    const bool last_valid = nbase + (NITER - 1) * WPC * 32 < N;
+    const uint32_t lane8 = (uint32_t)nbase * 8u;                                      // byte offset of angle it: lane8 + it * ITB ...
+    const uint32_t last8 = last_valid ? lane8 + (NITER - 1) * ITB : 0u;              // ... except the last
+    unsigned rx[NITER], ry[NITER], rz[NITER];
+    double n1[NITER], n2[NITER], n3[NITER], dom[NITER], winv[NITER];
+#pragma unroll
+    for (int it = 0; it < NITER; it++) {
+        const bool v = it < NITER - 1 || last_valid;
+        const int n = v ? nbase + it * WPC * 32 : 0;
+        n1[it] = t.nhat[3 * n]; n2[it] = t.nhat[3 * n + 1]; n3[it] = t.nhat[3 * n + 2];
+        dom[it] = v ? t.domega[n] : 0.0;
+        winv[it] = v ? t.winv[n] : 0.0;
+        const uint4 rec = reinterpret_cast<const uint4 *>(t.ang_rec)[n];
+        const unsigned z = 3u * (unsigned)N;
+        rx[it] = v ? rec.x : 0u; ry[it] = v ? rec.y : (z << 16); rz[it] = v ? rec.z : (z | (z << 16));
+    }
+#define OFF8(it) ((it) < NITER - 1 ? lane8 + (uint32_t)(it) * ITB : last8)
+
+    // ---- x stencil and the flux through the lower x face of the first cell (carried from then on)
+    double xm1[NITER], x0[NITER], xp1[NITER], carry[NITER];
+#pragma unroll
+    for (int it = 0; it < NITER; it++) { xm1[it] = 0.0; x0[it] = 0.0; xp1[it] = 0.0; carry[it] = 0.0; }
+    const double *fptr = nullptr;  // fluid / opacity value this lane prefetches (lanes 0..7 of a cell's first warp)
+    if (active) {
+        const double *Ic = a.I_in + c_first * N;
+        const double *fr = t.rec + (c_first - 1) * RECN;
+        const FaceRec f = {__ldg(fr), __ldg(fr + 1), __ldg(fr + 2), __ldg(fr + 3), __ldg(fr + 4), __ldg(fr + 5), __ldg(fr + 6), __ldg(fr + 7)};
+#pragma unroll
+        for (int it = 0; it < NITER; it++) {
+            const int n = OFF8(it) >> 3;
+            const double xm2 = PLM ? __ldg(Ic - 2 * N + n) : 0.0;
+            xm1[it] = __ldg(Ic - N + n); x0[it] = __ldg(Ic + n); xp1[it] = __ldg(Ic + N + n);
+            carry[it] = face_flux<PLM>(f, n1[it], n2[it], n3[it], xm2, xm1[it], x0[it], xp1[it]);
+        }
+        if (COUPLE && wc == 0 && lane < 8) {
+            if (lane < 5) fptr = a.fluid + (long long)lane * t.ncell + c_first;
+            else if (p.couple) fptr = (lane == 5 ? a.aP : (lane == 6 ? a.aE : a.aS)) + c_first;
+            sts(smb + 8u * (uint32_t)(L.oU + cs * USTR + 52 + lane), fptr ? __ldg(fptr) : 0.0);
+        }
+    }
+    const int barid = 1 + cs;
+    // per-warp byte offsets of the eight stencil neighbours inside a ring plane / a halo buffer (bit q of nbHalo: halo)
+    uint32_t nbOff[8];
+    unsigned nbHalo = 0;
+#pragma unroll
+    for (int q = 0; q < 8; q++) {
+        const int dq = (q & 3) < 2 ? (q & 3) - 2 : (q & 3) - 1;  // -2, -1, +1, +2
+        int row;
+        if (q < 4) {
+            const int yy = wy + dq;
+            if (yy >= 0 && yy < TY) row = wz * TY + yy;
+            else { row = wz * 4 + (yy < 0 ? yy + 2 : yy - TY + 2); nbHalo |= 1u << q; }
+        } else {
+            const int zz = wz + dq;
+            if (zz >= 0 && zz < TZ) row = zz * TY + wy;
+            else { row = 4 * TZ + wy * 4 + (zz < 0 ? zz + 2 : zz - TZ + 2); nbHalo |= 1u << q; }
+        }
+        nbOff[q] = (uint32_t)(row * Np) * 8u;
+    }
+    const uint32_t ownOff = (uint32_t)(cs * Np) * 8u;
+    const uint32_t aRing = smb + 8u * L.oRing, aHalo = smb + 8u * L.oHalo, planeB = (uint32_t)(NC * Np) * 8u;
+    const uint32_t aE0 = smb + 8u * (uint32_t)(L.oE + cs * Kp), aU0 = smb + 8u * (uint32_t)(L.oU + cs * USTR);
+    const uint32_t aFy = smb + 8u * L.oFy, aFz = smb + 8u * L.oFz;
+    const uint32_t aRed = smb + 8u * (uint32_t)(L.oRed + cs * (2 * WPC * 4 + 4));
+    const uint32_t N8 = (uint32_t)N * 8u;
+    double *outp = a.I_out + c_first * N;
+    const double *I0p = a.I0 ? a.I0 + c_first * N : nullptr;
+
+    for (int s = 0; s < nsteps; s++) {
+        const int b = s & 1;
+        mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
+        if (tid == 0 && s + 2 < nsteps) mbar_expect_tx(bar0 + 8u * b, step_bytes);  // re-armed for step s+2 (copies start after the barrier below)
+        const uint32_t ringS = aRing + (uint32_t)(s & 3) * planeB;          // own rows of plane s
+        const uint32_t haloS = aHalo + (uint32_t)b * ((uint32_t)(NH * Np) * 8u);  // halo rows of plane s
+        const uint32_t aEb = aE0 + (uint32_t)b * ((uint32_t)(NC * Kp) * 8u);
+        const uint32_t aUb = aU0 + (uint32_t)(s & 3) * (NC * USTR * 8u);
+        double d[NITER], xp2[NITER], fnext = 0.0;
+#pragma unroll
+        for (int it = 0; it < NITER; it++) asm volatile("" : "+r"(rx[it]), "+r"(ry[it]), "+r"(rz[it]));  // unpack per step: the unpacked offsets would be spilled
+
+        if (active) {
+            if (COUPLE && fptr != nullptr && s + 1 < nsteps) fnext = __ldg(fptr + s + 1);
+            if (COUPLE && wc == 0) {
+                __syncwarp();  // the fluid values stored by lanes 0..7 at the end of the previous step
+                // tetrad-frame four-velocity of the fluid (R10), once per cell: u^ahat = theta^ahat_j u^j', u^0hat = sqrt(1 + |u|^2)
+                double uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
+                if (p.couple) {
+                    const double2 t0 = lds2(aUb + 8 * 30), t1 = lds2(aUb + 8 * 32), t2 = lds2(aUb + 8 * 34);
+                    const double2 f1 = lds2(aUb + 8 * 54);
+                    const double u3 = lds(aUb + 8 * 56);
+                    uh1 = t0.x * f1.x + t0.y * f1.y + t1.x * u3;
+                    uh2 = t1.y * f1.y + t2.x * u3;
+                    uh3 = t2.y * u3;
+                    uh0 = sqrt_ge1(1.0 + (uh1 * uh1 + uh2 * uh2 + uh3 * uh3));
+                }
+                if (lane == 0) { sts2(aUb + 8 * 60, uh0, uh1); sts2(aUb + 8 * 62, uh2, uh3); }
+            }
+            const uint32_t ownrow = ringS + ownOff;
+            const uint32_t newrow = aRing + (uint32_t)((s + 2) & 3) * planeB + ownOff;
+#pragma unroll
+            for (int it = 0; it < NITER; it++) xp2[it] = lds(newrow + OFF8(it));
+            // ---- angular fluxes (Eq.25, donor cell in angle): owners turn q_e into the edge flux in place
+#pragma unroll
+            for (int it = 0; it < NITER; it++) {
+                const unsigned pj[3] = {rx[it] & 0xffffu, rx[it] >> 16, ry[it] & 0xffffu};
+                const bool v = it < NITER - 1 || last_valid;
+                double asum = 0.0;
+#pragma unroll
+                for (int jj = 0; jj < 3; jj++) {  // unused slots have q = 0
+                    const uint32_t qa = aEb + (uint32_t)jj * N8 + OFF8(it);
+                    const double q = lds(qa);
+                    const bool owner_up = (__double2loint(q) & 1) != 0;
+                    const double G = q * lds(ownrow + (owner_up ? OFF8(it) : pj[jj] * 8u));
+                    asum += G;
+                    if (v) sts(qa, G);
+                }
+                d[it] = asum;
+            }
+            if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
+#pragma unroll
+            for (int it = 0; it < NITER; it++) {
+                const double pulled = (lds(aEb + (ry[it] >> 16) * 8u) + lds(aEb + (rz[it] & 0xffffu) * 8u)) + lds(aEb + (rz[it] >> 16) * 8u);  // unused -> slot 3N = 0
+                d[it] = (d[it] - pulled) * winv[it];
+            }
+            // ---- spatial fluxes (Eq.24).  x: the upper face; the lower one is carried
+            {
+                const FaceRec f = lds_face(aUb);
+#pragma unroll
+                for (int it = 0; it < NITER; it++) {
+                    const double F = face_flux<PLM>(f, n1[it], n2[it], n3[it], xm1[it], x0[it], xp1[it], xp2[it]);
+                    d[it] += F - carry[it];
+                    carry[it] = F;
+                }
+            }
+            // y and z: the upper face, published for the neighbour above; the lower face only on the low edge of the tile
+#pragma unroll
+            for (int ax = 1; ax <= 2; ax++) {
+                const int q0 = ax == 1 ? 0 : 4;
+                const uint32_t rm2 = ((nbHalo >> q0) & 1u ? haloS : ringS) + nbOff[q0], rm1 = ((nbHalo >> (q0 + 1)) & 1u ? haloS : ringS) + nbOff[q0 + 1],
+                               rp1 = ((nbHalo >> (q0 + 2)) & 1u ? haloS : ringS) + nbOff[q0 + 2], rp2 = ((nbHalo >> (q0 + 3)) & 1u ? haloS : ringS) + nbOff[q0 + 3];
+                const bool low_edge = (ax == 1 ? wy : wz) == 0, publish = ax == 1 ? wy < TY - 1 : wz < TZ - 1;
+                const uint32_t pub = ax == 1 ? aFy + (uint32_t)((b * T::NFY + wz * (TY - 1) + wy) * Np) * 8u : aFz + (uint32_t)((b * T::NFZ + wz * TY + wy) * Np) * 8u;
+                const FaceRec fh = lds_face(aUb + 64 * ax);
+                double m1[NITER], p1[NITER];
+#pragma unroll
+                for (int it = 0; it < NITER; it++) {
+                    m1[it] = lds(rm1 + OFF8(it)); p1[it] = lds(rp1 + OFF8(it));
+                    const double p2 = PLM ? lds(rp2 + OFF8(it)) : 0.0;
+                    const double F = face_flux<PLM>(fh, n1[it], n2[it], n3[it], m1[it], x0[it], p1[it], p2);
+                    d[it] += F;
+                    if (publish && (it < NITER - 1 || last_valid)) sts(pub + OFF8(it), F);
+                }
+                if (low_edge) {
+                    const FaceRec fl = lds_face(aUb + (ax == 1 ? 8 * 36 : 8 * 44));
+#pragma unroll
+                    for (int it = 0; it < NITER; it++) {
+                        const double m2 = PLM ? lds(rm2 + OFF8(it)) : 0.0;
+                        d[it] -= face_flux<PLM>(fl, n1[it], n2[it], n3[it], m2, m1[it], x0[it], p1[it]);
+                    }
+                }
+            }
+        }
+        __syncthreads();  // the fluxes of this plane are published; nobody reads the rows, halo and coefficients of plane s any more
+        if (s + 2 < nsteps && tid < NR) issue(s + 2);
+        if (!active) continue;
+
+        if (wy > 0) {
+            const uint32_t src = aFy + (uint32_t)((b * T::NFY + wz * (TY - 1) + wy - 1) * Np) * 8u;
+#pragma unroll
+            for (int it = 0; it < NITER; it++) d[it] -= lds(src + OFF8(it));
+        }
+        if (wz > 0) {
+            const uint32_t src = aFz + (uint32_t)((b * T::NFZ + (wz - 1) * TY + wy) * Np) * 8u;
+#pragma unroll
+            for (int it = 0; it < NITER; it++) d[it] -= lds(src + OFF8(it));
+        }
+        // ---- flux-divergence update of C = n^0 n_0 I (Eq.22, stage form R8), cons -> prim
+        const double2 c01 = lds2(aUb + 8 * 24);
+        const double nup0 = c01.x;
+        const bool excised = c01.y != 0.0;
+        const double2 w01 = lds2(aUb + 8 * 26), w23 = lds2(aUb + 8 * 28);  // n^0 E_alphahat
+        const double mbdt = -a.beta_dt, thr = p.n0_crit * nup0;  // |n_0| < n0_crit  <=>  |n^0 n_0| < n0_crit n^0
+        double Is[NITER];
+        unsigned maskbits = 0;
+#pragma unroll
+        for (int it = 0; it < NITER; it++) {
+            const double wgt = chain4(w01.x, w01.y, w23.x, w23.y, n1[it], n2[it], n3[it]);  // n^0 n_0 at the cell centre
+            if (fabs(wgt) < thr) maskbits |= 1u << it;
+            double v = a.gam1 * x0[it];
+            if (I0p != nullptr) v = fma(a.gam0, __ldg(I0p + (OFF8(it) >> 3)), v);
+            v = fma(mbdt * d[it], rcp3(wgt), v);
+            Is[it] = (excised || !(it < NITER - 1 || last_valid)) ? 0.0 : v;
+        }
+
+        if (COUPLE) {
+            // ---- locally implicit coupling (section 2.5, Eq.31-50), fluid increment, mask
+            const bool enable = !excised, docouple = p.couple && enable;
+            const double2 u01 = lds2(aUb + 8 * 60), u23 = lds2(aUb + 8 * 62);
+            const double uh0 = docouple ? u01.x : 1.0, uh1 = docouple ? u01.y : 0.0, uh2 = docouple ? u23.x : 0.0, uh3 = docouple ? u23.y : 0.0;
+            const double2 f3 = lds2(aUb + 8 * 58);              // alpha_E (absorption part), alpha_s
+            const double aEdt = (f3.x + f3.y) * a.beta_dt;      // Eq.33b
+            // sweep 1.  With dd = n^0 + n^0bar alpha_E dt, rp = 1/(n^0bar dd):  dOmega_bar = dOmega / n^0bar^2 (R11),
+            // Ibar dOmega_bar = n^0bar^2 Ihat dOmega,  A_1 = sum (n^0/dd) Ibar dOmega_bar, A_2 = dt/4pi sum dOmega rp (Eq.42),
+            // and Eq.40 back in the tetrad frame is  Ihat_+ = g1 Ihat_- + src / (dd n^0bar^3),  g1 = n^0 / dd.
+            double g1[NITER], g2r4[NITER];
+            double Wsum = 0.0, A1 = 0.0, A2 = 0.0, Em = 0.0;
+#pragma unroll
+            for (int it = 0; it < NITER; it++) {
+                const double nbar = uh0 - fma(uh3, n3[it], fma(uh2, n2[it], uh1 * n1[it]));  // n^0bar = -u_alpha n^alpha
+                const double dd = fma(nbar, aEdt, nup0);
+                const double rp = rcp3(nbar * dd);
+                const double rd = nbar * rp, rn = dd * rp, rn2 = rn * rn;
+                const double x = (nbar * nbar) * (Is[it] * dom[it]);                        // Ibar dOmega_bar (Eq.38 summand)
+                g1[it] = nup0 * rd;
+                g2r4[it] = rn2 * rp;
+                Em += x;
+                A1 = fma(g1[it], x, A1);                                                    // Eq.42a
+                A2 = fma(dom[it], rp, A2);                                                  // Eq.42b
+                Wsum = fma(dom[it], rn2, Wsum);
+            }
+            // the cell's first warp sums the partial sums, solves the quartic and hands (T_+, source, coupled) to the others
+            warp_sum4_to(Wsum, A1, A2, Em, lane, aRed + (uint32_t)wc * 32u);
+            if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
+            if (wc == 0) {
+                Wsum = A1 = A2 = Em = 0.0;
+#pragma unroll
+                for (int q = 0; q < WPC; q++) {
+                    const double2 v0 = lds2(aRed + q * 32), v1 = lds2(aRed + q * 32 + 16);
+                    Wsum += v0.x; A1 += v0.y; A2 += v1.x; Em += v1.y;
+                }
+                const double2 f0 = lds2(aUb + 8 * 52);          // rho, T_-
+                const double aP = lds(aUb + 8 * 57), aS = f3.y;
+                const double Tm = f0.y;
+                double Tp = Tm, src = 0.0, flag = 0.0;            // flag: 1 coupled, -1 no root
+                if (docouple) {
+                    const double scale = p.renorm ? kFourPi * rcp3(Wsum) : 1.0;             // R12
+                    A1 *= scale; Em *= scale; A2 *= scale * (a.beta_dt * kInvFourPi);
+                    const double Cv = f0.x * p.rgm1;
+                    const double B4 = A2 * aP * p.a_rad, om = 1.0 - A2 * aS;               // Eq.50
+                    const double B1 = Cv * om, Bp = A1 - om * Em;
+                    double dTemp = 0.0;
+                    if (!quartic_delta_fast(B4, B1, Bp, Tm, dTemp)) {
+                        flag = -1.0;
+                    } else {
+                        flag = 1.0;
+                        Tp = Tm + dTemp;
+                        const double Ep = Em - Cv * dTemp;                                  // Eq.48
+                        const double T2 = Tp * Tp;
+                        src = (aP * p.a_rad * T2 * T2 + aS * Ep) * (a.beta_dt * kInvFourPi);
+                    }
+                }
+                if (lane == 0) { sts2(aRed + WPC * 64, Tp, src); sts(aRed + WPC * 64 + 16, flag); }
+            }
+            if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
+            const double2 bc = lds2(aRed + WPC * 64);
+            const double flag = lds(aRed + WPC * 64 + 16);
+            const double src = bc.y;
+            const bool coupled = flag > 0.0;
+            // sweep 2: Eq.40, fluid increment through the tetrad-frame first moments of the change, mask
+            double M0 = 0.0, M1 = 0.0, M2 = 0.0, M3 = 0.0;
+#pragma unroll
+            for (int it = 0; it < NITER; it++) {
+                const double Iold = Is[it];
+                double Inew = coupled ? fma(src, g2r4[it], g1[it] * Iold) : Iold;
+                const double wI = dom[it] * (Inew - Iold);
+                M0 += wI; M1 = fma(wI, n1[it], M1); M2 = fma(wI, n2[it], M2); M3 = fma(wI, n3[it], M3);
+                if (thr > 0.0 && enable && ((maskbits >> it) & 1u)) Inew = 0.0;
+                Is[it] = Inew;
+            }
+            warp_sum4_to(M0, M1, M2, M3, lane, aRed + (uint32_t)(WPC + wc) * 32u);
+            if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
+            if (wc == 0 && lane == 0) {
+                M0 = M1 = M2 = M3 = 0.0;
+#pragma unroll
+                for (int q = 0; q < WPC; q++) {
+                    const double2 v0 = lds2(aRed + (WPC + q) * 32), v1 = lds2(aRed + (WPC + q) * 32 + 16);
+                    M0 += v0.x; M1 += v0.y; M2 += v1.x; M3 += v1.y;
+                }
+                const long long c = c_first + s;
+                if (flag < 0.0 && a.noroot) atomicAdd(a.noroot, 1ull);
+                if (a.T_out) a.T_out[c] = bc.x;
+                if (a.dT0) {  // R^0_alpha = sum n^0 n_alpha I dOmega; n^0 n_0 = W_ahat n^ahat, n_i = theta^a_i n^a
+                    const double2 t0 = lds2(aUb + 8 * 30), t1 = lds2(aUb + 8 * 32), t2 = lds2(aUb + 8 * 34);
+                    a.dT0[c] = -(w01.x * M0 + w01.y * M1 + w23.x * M2 + w23.y * M3);
+                    a.dT0[t.ncell + c] = -(nup0 * (t0.x * M1));
+                    a.dT0[2 * t.ncell + c] = -(nup0 * (t0.y * M1 + t1.y * M2));
+                    a.dT0[3 * t.ncell + c] = -(nup0 * (t1.x * M1 + t2.x * M2 + t2.y * M3));
+                }
+            }
+            if (wc == 0 && lane < 8 && s + 1 < nsteps) sts(aU0 + (uint32_t)((s + 1) & 3) * (NC * USTR * 8u) + 8u * (52 + lane), fnext);
+        }
+#pragma unroll
+        for (int it = 0; it < NITER; it++) {
+            if (it < NITER - 1 || last_valid) outp[OFF8(it) >> 3] = Is[it];
+            xm1[it] = x0[it]; x0[it] = xp1[it]; xp1[it] = xp2[it];
+        }
+        outp += N;
+        if (I0p != nullptr) I0p += N;
+    }
+#undef OFF8
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// packed per-cell record of the stage kernel, RECN doubles for EVERY cell of the array (ghosts included):
+//   [0..7]   upper x face (= lower x face of cell c+1): e^x_alphahat (4), E_alphahat / dx (4)   (rad.h face record, R6)
+//   [8..15]  upper y face, [16..23] upper z face, likewise with dy, dz
+//   [24] n^0   [25] excised flag   [26..29] n^0 E_alphahat (cell centre)   [30..35] co-triad
+// faces whose upper neighbour is outside the array are zero.
+__global__ void __launch_bounds__(256) k_pack_rec(const DeviceTables t, double *__restrict__ rec) {
+    const long long total = t.ncell * RECN;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        const long long c = idx / RECN;
+        const int m = (int)(idx - c * RECN);
+        const int i = (int)(c % t.NI), j = (int)((c / t.NI) % t.NJ), k = (int)(c / ((long long)t.NI * t.NJ));
+        double v = 0.0;
+        if (m < 24) {
+            const int ax = m >> 3, r = m & 7;
+            const bool inside = ax == 0 ? i + 1 < t.NI : (ax == 1 ? j + 1 < t.NJ : k + 1 < t.NK);
+            if (inside) {
+                const long long cu = c + (ax == 0 ? 1 : (ax == 1 ? (long long)t.NI : (long long)t.NI * t.NJ));
+                v = t.face[(cu * 3 + ax) * RAD_NFACE + r];
+                if (r >= 4) v *= t.inv_dx[ax];
+            }
+        } else {
+            const double *cg = t.cell + c * RAD_NCELL;
+            if (m == 24) v = cg[0];
+            else if (m == 25) v = cg[50];
+            else if (m < 30) v = cg[1 + (m - 26)] * cg[0];
+            else v = cg[44 + (m - 30)];
+        }
+        rec[idx] = v;
+    }
+}
+
+template <int NITER, int WPC, int TY, int TZ>
+int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
+    using T = Tile<TY, TZ, WPC>;
+    const Layout5 L = make_layout5<T>(t.N);
+    const size_t smem = sizeof(double) * (size_t)L.total;
+    if (smem > 227 * 1024) return 0;
+    // run length along x: long runs amortise the prologue, short runs fill the SMs of small grids; pick the candidate
+    // with the fewest CTA waves x (steps + prologue cost)
+    const long long tiles = (long long)((t.n[1] + TY - 1) / TY) * ((t.n[2] + TZ - 1) / TZ);
+    int KX = t.n[0];
+    double best = 1e300;
+    for (int cand = t.n[0];; cand = (cand + 1) / 2) {
+        const long long ctas = tiles * ((t.n[0] + cand - 1) / cand);
+        const double cost = (double)((ctas + 147) / 148) * (cand + 3);
+        if (cost < best) { best = cost; KX = cand; }
+        if (cand <= 4) break;
+    }
+    dim3 grid((t.n[0] + KX - 1) / KX, (t.n[1] + TY - 1) / TY, (t.n[2] + TZ - 1) / TZ);
+    if (grid.y > 65535 || grid.z > 65535) return 0;
+#define RAD_LAUNCH5(PLM, CPL)                                                                                          \
+    do {                                                                                                               \
+        if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, PLM, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
+        k_stage5<NITER, WPC, TY, TZ, PLM, CPL><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                                  \
+    } while (0)
+    if (p.recon_space == 1) { if (couple) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(true, false); }
+    else { if (couple) RAD_LAUNCH5(false, true); else RAD_LAUNCH5(false, false); }
+#undef RAD_LAUNCH5
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace
+
+// returns 1 (launched), 0 (this configuration is not served by this kernel), -1 (CUDA error)
+int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
+    if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr) return 0;
+    if (t.N & 1) return 0;  // rows must be multiples of 16 bytes for the bulk copies
+    if (((uintptr_t)a.I_in & 15) || ((uintptr_t)t.ke & 15) || ((uintptr_t)t.rec & 15)) return 0;
+    const int N = t.N;
+    if (N <= 32) return launch5<1, 1, 4, 2>(t, p, a, couple, s);
+    if (N <= 64) return launch5<1, 2, 4, 2>(t, p, a, couple, s);
+    if (N <= 96) return launch5<1, 3, 4, 2>(t, p, a, couple, s);
+    if (N <= 128) return launch5<2, 2, 4, 2>(t, p, a, couple, s);
+    if (N <= 192) {
+        static const int var = [] { const char *e = std::getenv("RAD_S5_VARIANT"); return e ? std::atoi(e) : 0; }();
+        if (var == 1) return launch5<2, 3, 3, 2>(t, p, a, couple, s);
+        if (var == 2) return launch5<2, 3, 4, 2>(t, p, a, couple, s);
+        if (var == 3) return launch5<3, 2, 3, 2>(t, p, a, couple, s);
+        return launch5<3, 2, 4, 2>(t, p, a, couple, s);
+    }
+    return 0;
+}
+
+int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s) {
+    k_pack_rec<<<148 * 8, 256, 0, s>>>(t, rec);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace rad

@@ -8,6 +8,7 @@
 namespace rad {
 
 constexpr double kFourPi = 12.566370614359172954;
+constexpr double kInvFourPi = 0.079577471545947667884;
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
