@@ -52,7 +52,7 @@ __host__ __device__ inline Layout5 make_layout5(int N) {
     L.oRed = L.oU + 4 * T::NC * USTR;
     L.oRole = L.oRed + T::NC * (2 * T::WPC * 4 + 4);  // per cell: two sets of WPC partial sums, then (T_+, source, flag)
     L.oBar = L.oRole + T::NR * 4;
-    L.total = L.oBar + 2;
+    L.total = L.oBar + 3;  // two mbarriers, then the bytes of one step's copies
     return L;
 }
 
@@ -181,15 +181,26 @@ __device__ __forceinline__ bool quartic_delta_fast(double B4, double B1, double 
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r2) : "d"(sy));
     double T0 = sy * r2;                         // ~ y^(1/4)
     if (!(T0 > 0.0)) T0 = __longlong_as_double(0x7ff0000000000000ll);  // y outside the range of the approximation: the other bound alone
-    d = fmin(-B0 * rB1, T0) - Tm;
     const double B44 = 4.0 * B4, aBp = fabs(Bp);
+    // start to the right of the root (g is convex and increasing there, Newton is then monotone): the upper bound
+    // min(-B0/B1, (-B0/B4)^(1/4)), or the Newton step from T_- (d = 0), which lands right of the root from either side
+    // and is much closer for cells near equilibrium
+    d = fmin(-B0 * rB1, T0) - Tm;
+    {
+        const double T2 = Tm * Tm, q = B4 * (T2 * T2);
+        const double d1 = -(q + Bp) * rcp3(fma(B44, T2 * Tm, B1));
+        d = fmin(d, d1);
+    }
     for (int it = 0; it < 60; it++) {
         const double T = Tm + d, T2 = T * T, T3 = T2 * T, q = B4 * (T2 * T2);
         const double g = q + fma(B1, d, Bp), gp = fma(B44, T3, B1);
         const double rgp = rcp3(gp);  // gp >= B1 > 0, finite
         const double dd = g * rgp;
         d -= dd;
-        if (fabs(dd) <= 1e-15 * (fabs(d) + (aBp + q) * rgp)) break;
+        // converged to rounding, or so close that this (quadratically convergent) step already was the last useful one:
+        // the error left is <= 1.5 dd^2 / T
+        const double add = fabs(dd);
+        if (add <= 1e-15 * (fabs(d) + (aBp + q) * rgp) || add <= 3e-9 * T) break;
     }
     return true;
 }
@@ -271,12 +282,12 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
         fence_mbar_init();
     }
     __syncthreads();
-    uint32_t step_bytes = 0;
     if (tid == 0) {
-        uint32_t own_bytes = 0;
+        uint32_t own_bytes = 0, step_bytes = 0;
         for (int r = 0; r < NR; r++) { step_bytes += (uint32_t)roles[r].bytes; if (r < NC) own_bytes += (uint32_t)roles[r].bytes; }
         mbar_expect_tx(bar0, step_bytes + own_bytes);
         if (nsteps > 1) mbar_expect_tx(bar0 + 8u, step_bytes + own_bytes);
+        *reinterpret_cast<uint32_t *>(sm + L.oBar + 2) = step_bytes;
     }
     __syncthreads();
     // everything step u needs that is not yet resident, signalled on full[u & 1]: own rows of plane u+2 (ring slot
@@ -319,7 +330,12 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     double xm1[NITER], x0[NITER], xp1[NITER], carry[NITER];
 #pragma unroll
     for (int it = 0; it < NITER; it++) { xm1[it] = 0.0; x0[it] = 0.0; xp1[it] = 0.0; carry[it] = 0.0; }
-    const double *fptr = nullptr;  // fluid / opacity value this lane prefetches (lanes 0..7 of a cell's first warp)
+    // lanes 0..7 of a cell's first warp prefetch rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s of the next cell
+    const bool pf_lane = COUPLE && active && wc == 0 && (lane < 5 || (lane < 8 && p.couple));
+    auto fluid_ptr = [&](int step) -> const double * {
+        const double *base = lane < 5 ? a.fluid + (long long)lane * t.ncell : (lane == 5 ? a.aP : (lane == 6 ? a.aE : a.aS));
+        return base + c_first + step;
+    };
     if (active) {
         const double *Ic = a.I_in + c_first * N;
         const double *fr = t.rec + (c_first - 1) * RECN;
@@ -331,11 +347,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
             xm1[it] = __ldg(Ic - N + n); x0[it] = __ldg(Ic + n); xp1[it] = __ldg(Ic + N + n);
             carry[it] = face_flux<PLM>(f, n1[it], n2[it], n3[it], xm2, xm1[it], x0[it], xp1[it]);
         }
-        if (COUPLE && wc == 0 && lane < 8) {
-            if (lane < 5) fptr = a.fluid + (long long)lane * t.ncell + c_first;
-            else if (p.couple) fptr = (lane == 5 ? a.aP : (lane == 6 ? a.aE : a.aS)) + c_first;
-            sts(smb + 8u * (uint32_t)(L.oU + cs * USTR + 52 + lane), fptr ? __ldg(fptr) : 0.0);
-        }
+        if (COUPLE && wc == 0 && lane < 8) sts(smb + 8u * (uint32_t)(L.oU + cs * USTR + 52 + lane), pf_lane ? __ldg(fluid_ptr(0)) : 0.0);
     }
     const int barid = 1 + cs;
     // per-warp byte offsets of the eight stencil neighbours inside a ring plane / a halo buffer (bit q of nbHalo: halo)
@@ -368,7 +380,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     for (int s = 0; s < nsteps; s++) {
         const int b = s & 1;
         mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
-        if (tid == 0 && s + 2 < nsteps) mbar_expect_tx(bar0 + 8u * b, step_bytes);  // re-armed for step s+2 (copies start after the barrier below)
+        if (tid == 0 && s + 2 < nsteps) mbar_expect_tx(bar0 + 8u * b, *reinterpret_cast<volatile uint32_t *>(sm + L.oBar + 2));  // re-armed for step s+2 (copies start after the barrier below)
         const uint32_t ringS = aRing + (uint32_t)(s & 3) * planeB;          // own rows of plane s
         const uint32_t haloS = aHalo + (uint32_t)b * ((uint32_t)(NH * Np) * 8u);  // halo rows of plane s
         const uint32_t aEb = aE0 + (uint32_t)b * ((uint32_t)(NC * Kp) * 8u);
@@ -378,7 +390,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
         for (int it = 0; it < NITER; it++) asm volatile("" : "+r"(rx[it]), "+r"(ry[it]), "+r"(rz[it]));  // unpack per step: the unpacked offsets would be spilled
 
         if (active) {
-            if (COUPLE && fptr != nullptr && s + 1 < nsteps) fnext = __ldg(fptr + s + 1);
+            if (pf_lane && s + 1 < nsteps) fnext = __ldg(fluid_ptr(s + 1));
             if (COUPLE && wc == 0) {
                 __syncwarp();  // the fluid values stored by lanes 0..7 at the end of the previous step
                 // tetrad-frame four-velocity of the fluid (R10), once per cell: u^ahat = theta^ahat_j u^j', u^0hat = sqrt(1 + |u|^2)
@@ -400,20 +412,24 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
             for (int it = 0; it < NITER; it++) xp2[it] = lds(newrow + OFF8(it));
             // ---- angular fluxes (Eq.25, donor cell in angle): owners turn q_e into the edge flux in place
 #pragma unroll
-            for (int it = 0; it < NITER; it++) {
+            for (int it = 0; it < NITER; it++) {  // loads first, stores last: the volatile accesses keep their order
                 const unsigned pj[3] = {rx[it] & 0xffffu, rx[it] >> 16, ry[it] & 0xffffu};
-                const bool v = it < NITER - 1 || last_valid;
-                double asum = 0.0;
+                const uint32_t qa = aEb + OFF8(it);
+                double q[3], G[3];
 #pragma unroll
-                for (int jj = 0; jj < 3; jj++) {  // unused slots have q = 0
-                    const uint32_t qa = aEb + (uint32_t)jj * N8 + OFF8(it);
-                    const double q = lds(qa);
-                    const bool owner_up = (__double2loint(q) & 1) != 0;
-                    const double G = q * lds(ownrow + (owner_up ? OFF8(it) : pj[jj] * 8u));
-                    asum += G;
-                    if (v) sts(qa, G);
+                for (int jj = 0; jj < 3; jj++) q[jj] = lds(qa + (uint32_t)jj * N8);  // unused slots have q = 0
+#pragma unroll
+                for (int jj = 0; jj < 3; jj++) {
+                    const bool owner_up = (__double2loint(q[jj]) & 1) != 0;
+                    G[jj] = lds(ownrow + (owner_up ? OFF8(it) : pj[jj] * 8u));
                 }
-                d[it] = asum;
+#pragma unroll
+                for (int jj = 0; jj < 3; jj++) G[jj] *= q[jj];
+                d[it] = (G[0] + G[1]) + G[2];
+                if (it < NITER - 1 || last_valid) {
+#pragma unroll
+                    for (int jj = 0; jj < 3; jj++) sts(qa + (uint32_t)jj * N8, G[jj]);
+                }
             }
             if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
 #pragma unroll
@@ -440,14 +456,21 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                 const bool low_edge = (ax == 1 ? wy : wz) == 0, publish = ax == 1 ? wy < TY - 1 : wz < TZ - 1;
                 const uint32_t pub = ax == 1 ? aFy + (uint32_t)((b * T::NFY + wz * (TY - 1) + wy) * Np) * 8u : aFz + (uint32_t)((b * T::NFZ + wz * TY + wy) * Np) * 8u;
                 const FaceRec fh = lds_face(aUb + 64 * ax);
-                double m1[NITER], p1[NITER];
+                double m1[NITER], p1[NITER], p2[NITER], F[NITER];
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
                     m1[it] = lds(rm1 + OFF8(it)); p1[it] = lds(rp1 + OFF8(it));
-                    const double p2 = PLM ? lds(rp2 + OFF8(it)) : 0.0;
-                    const double F = face_flux<PLM>(fh, n1[it], n2[it], n3[it], m1[it], x0[it], p1[it], p2);
-                    d[it] += F;
-                    if (publish && (it < NITER - 1 || last_valid)) sts(pub + OFF8(it), F);
+                    p2[it] = PLM ? lds(rp2 + OFF8(it)) : 0.0;
+                }
+#pragma unroll
+                for (int it = 0; it < NITER; it++) {
+                    F[it] = face_flux<PLM>(fh, n1[it], n2[it], n3[it], m1[it], x0[it], p1[it], p2[it]);
+                    d[it] += F[it];
+                }
+                if (publish) {
+#pragma unroll
+                    for (int it = 0; it < NITER; it++)
+                        if (it < NITER - 1 || last_valid) sts(pub + OFF8(it), F[it]);
                 }
                 if (low_edge) {
                     const FaceRec fl = lds_face(aUb + (ax == 1 ? 8 * 36 : 8 * 44));
