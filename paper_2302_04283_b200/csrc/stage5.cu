@@ -292,17 +292,18 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     __syncthreads();
     // everything step u needs that is not yet resident, signalled on full[u & 1]: own rows of plane u+2 (ring slot
     // (u+2) & 3), halo rows of plane u, coefficients and records of the cells of plane u
+    const int myrole = (tid >> 5) + (T::NT / 32) * lane;  // the copies of a step are spread over all warps (a warp issues its lanes' copies one by one)
     auto issue = [&](int u) {
-        const Role r = roles[tid];
+        const Role r = roles[myrole];
         if (r.bytes) {
             const int buf = (u + r.boff) & r.nbufm1;
             bulk_g2s(smb + 8u * (uint32_t)(r.dst0 + buf * r.dstride), r.src0 + (long long)u * r.stride, (uint32_t)r.bytes, bar0 + 8u * (u & 1));
         }
     };
-    if (tid < NR) {
+    if (myrole < NR) {
         issue(0);
         if (nsteps > 1) issue(1);
-        if (tid < NC) { issue(-2); if (nsteps > 1) issue(-1); }  // own rows of planes 0 and 1
+        if (myrole < NC) { issue(-2); if (nsteps > 1) issue(-1); }  // own rows of planes 0 and 1
     }
 
     // ---- the thread's angles: n = lane + 32 wc + 32 WPC it.  Only the last one can fall past N; such a slot is idle:
@@ -331,7 +332,8 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
 #pragma unroll
     for (int it = 0; it < NITER; it++) { xm1[it] = 0.0; x0[it] = 0.0; xp1[it] = 0.0; carry[it] = 0.0; }
     // lanes 0..7 of a cell's first warp prefetch rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s of the next cell
-    const bool pf_lane = COUPLE && active && wc == 0 && (lane < 5 || (lane < 8 && p.couple));
+    constexpr int WH = WPC - 1;  // the warp of a cell that does the per-cell chores (fluid prefetch, tetrad velocity, outputs); warp 0 solves the quartic
+    const bool pf_lane = COUPLE && active && wc == WH && (lane < 5 || (lane < 8 && p.couple));
     auto fluid_ptr = [&](int step) -> const double * {
         const double *base = lane < 5 ? a.fluid + (long long)lane * t.ncell : (lane == 5 ? a.aP : (lane == 6 ? a.aE : a.aS));
         return base + c_first + step;
@@ -347,7 +349,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
             xm1[it] = __ldg(Ic - N + n); x0[it] = __ldg(Ic + n); xp1[it] = __ldg(Ic + N + n);
             carry[it] = face_flux<PLM>(f, n1[it], n2[it], n3[it], xm2, xm1[it], x0[it], xp1[it]);
         }
-        if (COUPLE && wc == 0 && lane < 8) sts(smb + 8u * (uint32_t)(L.oU + cs * USTR + 52 + lane), pf_lane ? __ldg(fluid_ptr(0)) : 0.0);
+        if (COUPLE && wc == WH && lane < 8) sts(smb + 8u * (uint32_t)(L.oU + cs * USTR + 52 + lane), pf_lane ? __ldg(fluid_ptr(0)) : 0.0);
     }
     const int barid = 1 + cs;
     // per-warp byte offsets of the eight stencil neighbours inside a ring plane / a halo buffer (bit q of nbHalo: halo)
@@ -377,6 +379,31 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     double *outp = a.I_out + c_first * N;
     const double *I0p = a.I0 ? a.I0 + c_first * N : nullptr;
 
+    // T_+, the count of cells without a root and the fluid increment of step sp, by lane 0 of the cell's last warp, one
+    // cell barrier after the partial sums were written
+    auto emit = [&](int sp) {
+        const uint32_t aUp = aU0 + (uint32_t)(sp & 3) * (NC * USTR * 8u);
+        double M0 = 0.0, M1 = 0.0, M2 = 0.0, M3 = 0.0;
+#pragma unroll
+        for (int q = 0; q < WPC; q++) {
+            const double2 v0 = lds2(aRed + (WPC + q) * 32), v1 = lds2(aRed + (WPC + q) * 32 + 16);
+            M0 += v0.x; M1 += v0.y; M2 += v1.x; M3 += v1.y;
+        }
+        const double Tp = lds(aRed + WPC * 64), flag = lds(aRed + WPC * 64 + 16);
+        const long long c = c_first + sp;
+        if (flag < 0.0 && a.noroot) atomicAdd(a.noroot, 1ull);
+        if (a.T_out) a.T_out[c] = Tp;
+        if (a.dT0) {  // R^0_alpha = sum n^0 n_alpha I dOmega; n^0 n_0 = W_ahat n^ahat, n_i = theta^a_i n^a
+            const double nup0 = lds(aUp + 8 * 24);
+            const double2 w01 = lds2(aUp + 8 * 26), w23 = lds2(aUp + 8 * 28);
+            const double2 t0 = lds2(aUp + 8 * 30), t1 = lds2(aUp + 8 * 32), t2 = lds2(aUp + 8 * 34);
+            a.dT0[c] = -(w01.x * M0 + w01.y * M1 + w23.x * M2 + w23.y * M3);
+            a.dT0[t.ncell + c] = -(nup0 * (t0.x * M1));
+            a.dT0[2 * t.ncell + c] = -(nup0 * (t0.y * M1 + t1.y * M2));
+            a.dT0[3 * t.ncell + c] = -(nup0 * (t1.x * M1 + t2.x * M2 + t2.y * M3));
+        }
+    };
+
     for (int s = 0; s < nsteps; s++) {
         const int b = s & 1;
         mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
@@ -391,7 +418,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
 
         if (active) {
             if (pf_lane && s + 1 < nsteps) fnext = __ldg(fluid_ptr(s + 1));
-            if (COUPLE && wc == 0) {
+            if (COUPLE && wc == WH) {
                 __syncwarp();  // the fluid values stored by lanes 0..7 at the end of the previous step
                 // tetrad-frame four-velocity of the fluid (R10), once per cell: u^ahat = theta^ahat_j u^j', u^0hat = sqrt(1 + |u|^2)
                 double uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
@@ -432,6 +459,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                 }
             }
             if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
+            if (COUPLE && wc == WH && lane == 0 && s > 0) emit(s - 1);
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
                 const double pulled = (lds(aEb + (ry[it] >> 16) * 8u) + lds(aEb + (rz[it] & 0xffffu) * 8u)) + lds(aEb + (rz[it] >> 16) * 8u);  // unused -> slot 3N = 0
@@ -483,7 +511,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
             }
         }
         __syncthreads();  // the fluxes of this plane are published; nobody reads the rows, halo and coefficients of plane s any more
-        if (s + 2 < nsteps && tid < NR) issue(s + 2);
+        if (s + 2 < nsteps && myrole < NR) issue(s + 2);
         if (!active) continue;
 
         if (wy > 0) {
@@ -590,26 +618,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                 Is[it] = Inew;
             }
             warp_sum4_to(M0, M1, M2, M3, lane, aRed + (uint32_t)(WPC + wc) * 32u);
-            if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
-            if (wc == 0 && lane == 0) {
-                M0 = M1 = M2 = M3 = 0.0;
-#pragma unroll
-                for (int q = 0; q < WPC; q++) {
-                    const double2 v0 = lds2(aRed + (WPC + q) * 32), v1 = lds2(aRed + (WPC + q) * 32 + 16);
-                    M0 += v0.x; M1 += v0.y; M2 += v1.x; M3 += v1.y;
-                }
-                const long long c = c_first + s;
-                if (flag < 0.0 && a.noroot) atomicAdd(a.noroot, 1ull);
-                if (a.T_out) a.T_out[c] = bc.x;
-                if (a.dT0) {  // R^0_alpha = sum n^0 n_alpha I dOmega; n^0 n_0 = W_ahat n^ahat, n_i = theta^a_i n^a
-                    const double2 t0 = lds2(aUb + 8 * 30), t1 = lds2(aUb + 8 * 32), t2 = lds2(aUb + 8 * 34);
-                    a.dT0[c] = -(w01.x * M0 + w01.y * M1 + w23.x * M2 + w23.y * M3);
-                    a.dT0[t.ncell + c] = -(nup0 * (t0.x * M1));
-                    a.dT0[2 * t.ncell + c] = -(nup0 * (t0.y * M1 + t1.y * M2));
-                    a.dT0[3 * t.ncell + c] = -(nup0 * (t1.x * M1 + t2.x * M2 + t2.y * M3));
-                }
-            }
-            if (wc == 0 && lane < 8 && s + 1 < nsteps) sts(aU0 + (uint32_t)((s + 1) & 3) * (NC * USTR * 8u) + 8u * (52 + lane), fnext);
+            if (wc == WH && lane < 8 && s + 1 < nsteps) sts(aU0 + (uint32_t)((s + 1) & 3) * (NC * USTR * 8u) + 8u * (52 + lane), fnext);
         }
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
@@ -618,6 +627,10 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
         }
         outp += N;
         if (I0p != nullptr) I0p += N;
+    }
+    if (COUPLE && active) {
+        if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
+        if (wc == WH && lane == 0) emit(nsteps - 1);
     }
 #undef OFF8
 }
