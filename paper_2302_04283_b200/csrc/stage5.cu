@@ -36,7 +36,7 @@ struct Tile {
 };
 
 struct Layout5 {
-    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oU, oRed, oRole, oBar, total;  // offsets in doubles
+    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oFx, oU, oRed, oRole, oBar, total;  // offsets in doubles
 };
 template <class T>
 __host__ __device__ inline Layout5 make_layout5(int N) {
@@ -48,7 +48,8 @@ __host__ __device__ inline Layout5 make_layout5(int N) {
     L.oE = L.oHalo + 2 * T::NH * L.Np;
     L.oFy = L.oE + 2 * T::NC * L.Kp;
     L.oFz = L.oFy + 2 * T::NFY * L.Np;
-    L.oU = L.oFz + 2 * T::NFZ * L.Np;
+    L.oFx = L.oFz + 2 * T::NFZ * L.Np;  // the lower z face of cell (0,0), computed by cell (1,1) (load balance)
+    L.oU = L.oFx + 2 * L.Np;
     L.oRed = L.oU + 4 * T::NC * USTR;
     L.oRole = L.oRed + T::NC * (2 * T::WPC * 4 + 4);  // per cell: two sets of WPC partial sums, then (T_+, source, flag)
     L.oBar = L.oRole + T::NR * 4;
@@ -373,7 +374,11 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     const uint32_t ownOff = (uint32_t)(cs * Np) * 8u;
     const uint32_t aRing = smb + 8u * L.oRing, aHalo = smb + 8u * L.oHalo, planeB = (uint32_t)(NC * Np) * 8u;
     const uint32_t aE0 = smb + 8u * (uint32_t)(L.oE + cs * Kp), aU0 = smb + 8u * (uint32_t)(L.oU + cs * USTR);
-    const uint32_t aFy = smb + 8u * L.oFy, aFz = smb + 8u * L.oFz;
+    const uint32_t aFy = smb + 8u * L.oFy, aFz = smb + 8u * L.oFz, aFx = smb + 8u * L.oFx;
+    // load balance: cell (0,0) would compute five faces (x, upper y and z, lower y and z), cell (1,1) three; cell (1,1)
+    // takes over the lower z face of cell (0,0)
+    const bool helped = TY >= 2 && TZ >= 2 && j0 + 1 < t.n[1] + ng && k0 + 1 < t.n[2] + ng;
+    const bool is_helper = helped && cs == TY + 1, is_helpee = helped && cs == 0;
     const uint32_t aRed = smb + 8u * (uint32_t)(L.oRed + cs * (2 * WPC * 4 + 4));
     const uint32_t N8 = (uint32_t)N * 8u;
     double *outp = a.I_out + c_first * N;
@@ -500,7 +505,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                     for (int it = 0; it < NITER; it++)
                         if (it < NITER - 1 || last_valid) sts(pub + OFF8(it), F[it]);
                 }
-                if (low_edge) {
+                if (low_edge && !(ax == 2 && is_helpee)) {
                     const FaceRec fl = lds_face(aUb + (ax == 1 ? 8 * 36 : 8 * 44));
 #pragma unroll
                     for (int it = 0; it < NITER; it++) {
@@ -510,9 +515,29 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                 }
             }
         }
+        if (is_helper) {  // lower z face of cell (0,0): rows z-2, z-1 of column 0 are halo rows, z and z+1 ring rows
+            const uint32_t r_m2 = haloS + (uint32_t)((4 * TZ) * Np) * 8u, r_m1 = haloS + (uint32_t)((4 * TZ + 1) * Np) * 8u, r_0 = ringS,
+                           r_p1 = ringS + (uint32_t)(TY * Np) * 8u;
+            const FaceRec fl = lds_face(aUb - (uint32_t)cs * (USTR * 8u) + 8 * 44);
+            double q0[NITER], q1[NITER], q2[NITER], q3[NITER];
+#pragma unroll
+            for (int it = 0; it < NITER; it++) {
+                q0[it] = PLM ? lds(r_m2 + OFF8(it)) : 0.0; q1[it] = lds(r_m1 + OFF8(it)); q2[it] = lds(r_0 + OFF8(it)); q3[it] = lds(r_p1 + OFF8(it));
+            }
+#pragma unroll
+            for (int it = 0; it < NITER; it++) q0[it] = face_flux<PLM>(fl, n1[it], n2[it], n3[it], q0[it], q1[it], q2[it], q3[it]);
+#pragma unroll
+            for (int it = 0; it < NITER; it++)
+                if (it < NITER - 1 || last_valid) sts(aFx + (uint32_t)(b * Np) * 8u + OFF8(it), q0[it]);
+        }
         __syncthreads();  // the fluxes of this plane are published; nobody reads the rows, halo and coefficients of plane s any more
         if (s + 2 < nsteps && myrole < NR) issue(s + 2);
         if (!active) continue;
+
+        if (is_helpee) {
+#pragma unroll
+            for (int it = 0; it < NITER; it++) d[it] -= lds(aFx + (uint32_t)(b * Np) * 8u + OFF8(it));
+        }
 
         if (wy > 0) {
             const uint32_t src = aFy + (uint32_t)((b * T::NFY + wz * (TY - 1) + wy - 1) * Np) * 8u;
