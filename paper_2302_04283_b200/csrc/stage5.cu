@@ -21,9 +21,14 @@
 #include "async_copy.cuh"
 #include "stage_math.cuh"
 
+#ifndef RAD_S5_UNROLL
+#define RAD_S5_UNROLL 1
+#endif
+
 namespace rad {
 namespace {
 
+constexpr int kStepUnroll = RAD_S5_UNROLL;
 constexpr int RECN = RAD_STAGE_RECN;  // packed per-cell record, see k_pack_rec
 constexpr int USTR = 64;              // a cell's record slot in shared memory: [0..35] record, [36..43] lower y face,
                                       // [44..51] lower z face, [52..59] rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s
@@ -51,7 +56,7 @@ __host__ __device__ inline Layout5 make_layout5(int N) {
     L.oFx = L.oFz + 2 * T::NFZ * L.Np;  // the lower z face of cell (0,0), computed by cell (1,1) (load balance)
     L.oU = L.oFx + 2 * L.Np;
     L.oRed = L.oU + 4 * T::NC * USTR;
-    L.oRole = L.oRed + T::NC * (2 * T::WPC * 4 + 4);  // per cell: two sets of WPC partial sums, then (T_+, source, flag)
+    L.oRole = L.oRed + T::NC * (2 * T::WPC * 4 + 8);  // per cell: two sets of WPC partial sums, then (T_+, source, flag)
     L.oBar = L.oRole + T::NR * 4;
     L.total = L.oBar + 3;  // two mbarriers, then the bytes of one step's copies
     return L;
@@ -173,24 +178,25 @@ __device__ __forceinline__ FaceRec lds_face(uint32_t addr) {  // warp-uniform ad
 __device__ __forceinline__ bool quartic_delta_fast(double B4, double B1, double Bp, double Tm, double &d) {
     const double B0 = Bp - B1 * Tm;
     if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return false;
-    const double rB1 = rcp3(B1);
-    if (B4 == 0.0) { d = -Bp * rB1; return true; }
-    const double y = -B0 * rcp3(B4);
-    double r1, r2;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r1) : "d"(y));
-    const double sy = y * r1;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r2) : "d"(sy));
-    double T0 = sy * r2;                         // ~ y^(1/4)
-    if (!(T0 > 0.0)) T0 = __longlong_as_double(0x7ff0000000000000ll);  // y outside the range of the approximation: the other bound alone
+    if (B4 == 0.0) { d = -Bp * rcp3(B1); return true; }
     const double B44 = 4.0 * B4, aBp = fabs(Bp);
-    // start to the right of the root (g is convex and increasing there, Newton is then monotone): the upper bound
-    // min(-B0/B1, (-B0/B4)^(1/4)), or the Newton step from T_- (d = 0), which lands right of the root from either side
-    // and is much closer for cells near equilibrium
-    d = fmin(-B0 * rB1, T0) - Tm;
+    // start to the right of the root (g is convex and increasing there, Newton is then monotone): the Newton step from T_-
+    // (d = 0) lands right of the root from either side and is close for cells near equilibrium; where it lands far away
+    // (more than T_- beyond T_-) the upper bound min(-B0/B1, (-B0/B4)^(1/4)) caps it (fourth root from the hardware rsqrt
+    // seeds: the start only has to be near the bound)
     {
         const double T2 = Tm * Tm, q = B4 * (T2 * T2);
-        const double d1 = -(q + Bp) * rcp3(fma(B44, T2 * Tm, B1));
-        d = fmin(d, d1);
+        d = -(q + Bp) * rcp3(fma(B44, T2 * Tm, B1));
+    }
+    if (d > Tm) {
+        const double y = -B0 * rcp3(B4);
+        double r1, r2;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r1) : "d"(y));
+        const double sy = y * r1;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r2) : "d"(sy));
+        double T0 = sy * r2;                         // ~ y^(1/4)
+        if (!(T0 > 0.0)) T0 = __longlong_as_double(0x7ff0000000000000ll);  // y outside the range of the approximation: the other bound alone
+        d = fmin(d, fmin(-B0 * rcp3(B1), T0) - Tm);
     }
     for (int it = 0; it < 60; it++) {
         const double T = Tm + d, T2 = T * T, T3 = T2 * T, q = B4 * (T2 * T2);
@@ -379,11 +385,32 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     // takes over the lower z face of cell (0,0)
     const bool helped = TY >= 2 && TZ >= 2 && j0 + 1 < t.n[1] + ng && k0 + 1 < t.n[2] + ng;
     const bool is_helper = helped && cs == TY + 1, is_helpee = helped && cs == 0;
-    const uint32_t aRed = smb + 8u * (uint32_t)(L.oRed + cs * (2 * WPC * 4 + 4));
+    const uint32_t aRed = smb + 8u * (uint32_t)(L.oRed + cs * (2 * WPC * 4 + 8));
     const uint32_t N8 = (uint32_t)N * 8u;
     double *outp = a.I_out + c_first * N;
     const double *I0p = a.I0 ? a.I0 + c_first * N : nullptr;
 
+    // tetrad-frame four-velocity of the fluid in the cell of step u (R10), by the cell's last warp: u^ahat = theta^ahat_j u^j',
+    // u^0hat = sqrt(1 + |u|^2); needs the record and the fluid values of that cell in shared memory
+    auto tetrad = [&](int u) {
+        const uint32_t aUu = aU0 + (uint32_t)(u & 3) * (NC * USTR * 8u);
+        double uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
+        if (p.couple) {
+            const double2 t0 = lds2(aUu + 8 * 30), t1 = lds2(aUu + 8 * 32), t2 = lds2(aUu + 8 * 34);
+            const double2 f1 = lds2(aUu + 8 * 54);
+            const double u3 = lds(aUu + 8 * 56);
+            uh1 = t0.x * f1.x + t0.y * f1.y + t1.x * u3;
+            uh2 = t1.y * f1.y + t2.x * u3;
+            uh3 = t2.y * u3;
+            uh0 = sqrt_ge1(1.0 + (uh1 * uh1 + uh2 * uh2 + uh3 * uh3));
+        }
+        if (lane == 0) { sts2(aUu + 8 * 60, uh0, uh1); sts2(aUu + 8 * 62, uh2, uh3); }
+    };
+    if (COUPLE && active && wc == WH) {  // step 0: its record arrives with the first group of copies
+        mbar_wait(bar0, 0);
+        __syncwarp();
+        tetrad(0);
+    }
     // T_+, the count of cells without a root and the fluid increment of step sp, by lane 0 of the cell's last warp, one
     // cell barrier after the partial sums were written
     auto emit = [&](int sp) {
@@ -394,7 +421,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
             const double2 v0 = lds2(aRed + (WPC + q) * 32), v1 = lds2(aRed + (WPC + q) * 32 + 16);
             M0 += v0.x; M1 += v0.y; M2 += v1.x; M3 += v1.y;
         }
-        const double Tp = lds(aRed + WPC * 64), flag = lds(aRed + WPC * 64 + 16);
+        const double Tp = lds(aRed + WPC * 64 + (sp & 1) * 32), flag = lds(aRed + WPC * 64 + (sp & 1) * 32 + 16);
         const long long c = c_first + sp;
         if (flag < 0.0 && a.noroot) atomicAdd(a.noroot, 1ull);
         if (a.T_out) a.T_out[c] = Tp;
@@ -409,6 +436,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
         }
     };
 
+#pragma unroll(kStepUnroll)
     for (int s = 0; s < nsteps; s++) {
         const int b = s & 1;
         mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
@@ -423,21 +451,6 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
 
         if (active) {
             if (pf_lane && s + 1 < nsteps) fnext = __ldg(fluid_ptr(s + 1));
-            if (COUPLE && wc == WH) {
-                __syncwarp();  // the fluid values stored by lanes 0..7 at the end of the previous step
-                // tetrad-frame four-velocity of the fluid (R10), once per cell: u^ahat = theta^ahat_j u^j', u^0hat = sqrt(1 + |u|^2)
-                double uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
-                if (p.couple) {
-                    const double2 t0 = lds2(aUb + 8 * 30), t1 = lds2(aUb + 8 * 32), t2 = lds2(aUb + 8 * 34);
-                    const double2 f1 = lds2(aUb + 8 * 54);
-                    const double u3 = lds(aUb + 8 * 56);
-                    uh1 = t0.x * f1.x + t0.y * f1.y + t1.x * u3;
-                    uh2 = t1.y * f1.y + t2.x * u3;
-                    uh3 = t2.y * u3;
-                    uh0 = sqrt_ge1(1.0 + (uh1 * uh1 + uh2 * uh2 + uh3 * uh3));
-                }
-                if (lane == 0) { sts2(aUb + 8 * 60, uh0, uh1); sts2(aUb + 8 * 62, uh2, uh3); }
-            }
             const uint32_t ownrow = ringS + ownOff;
             const uint32_t newrow = aRing + (uint32_t)((s + 2) & 3) * planeB + ownOff;
 #pragma unroll
@@ -464,7 +477,6 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                 }
             }
             if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
-            if (COUPLE && wc == WH && lane == 0 && s > 0) emit(s - 1);
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
                 const double pulled = (lds(aEb + (ry[it] >> 16) * 8u) + lds(aEb + (rz[it] & 0xffffu) * 8u)) + lds(aEb + (rz[it] >> 16) * 8u);  // unused -> slot 3N = 0
@@ -624,11 +636,20 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                         src = (aP * p.a_rad * T2 * T2 + aS * Ep) * (a.beta_dt * kInvFourPi);
                     }
                 }
-                if (lane == 0) { sts2(aRed + WPC * 64, Tp, src); sts(aRed + WPC * 64 + 16, flag); }
+                if (lane == 0) { sts2(aRed + WPC * 64 + b * 32, Tp, src); sts(aRed + WPC * 64 + b * 32 + 16, flag); }
+            }
+            if (wc == WH) {  // meanwhile the cell's last warp writes the outputs of the previous step and prepares the next one
+                if (lane == 0 && s > 0) emit(s - 1);
+                if (s + 1 < nsteps) {
+                    if (lane < 8) sts(aU0 + (uint32_t)((s + 1) & 3) * (NC * USTR * 8u) + 8u * (52 + lane), fnext);
+                    mbar_wait(bar0 + 8u * (b ^ 1), ((s + 1) >> 1) & 1);  // the record of the next cell (copied two steps ahead)
+                    __syncwarp();
+                    tetrad(s + 1);
+                }
             }
             if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
-            const double2 bc = lds2(aRed + WPC * 64);
-            const double flag = lds(aRed + WPC * 64 + 16);
+            const double2 bc = lds2(aRed + WPC * 64 + b * 32);
+            const double flag = lds(aRed + WPC * 64 + b * 32 + 16);
             const double src = bc.y;
             const bool coupled = flag > 0.0;
             // sweep 2: Eq.40, fluid increment through the tetrad-frame first moments of the change, mask
@@ -643,7 +664,6 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
                 Is[it] = Inew;
             }
             warp_sum4_to(M0, M1, M2, M3, lane, aRed + (uint32_t)(WPC + wc) * 32u);
-            if (wc == WH && lane < 8 && s + 1 < nsteps) sts(aU0 + (uint32_t)((s + 1) & 3) * (NC * USTR * 8u) + 8u * (52 + lane), fnext);
         }
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
