@@ -9,7 +9,7 @@ before the timed region; the intensity arrays (2 x 2.98 GB) exceed L2 (126 MB), 
 
 One JSON line on stdout (rank 0).  `value` is device-timed (CUDA events on the launching stream, max over ranks);
 `e2e` is the same stage through rad_stage_host with pinned HOST buffers, copies inside the timed region;
-`roofline` is for the fused stage kernel (the only kernel of a step), from the CUDA-event time of the timed region; `cpu_baseline` is the oracle
+`roofline` is for the fused stage kernel k_stage5 (the only kernel of a step), from the CUDA-event time of the timed region; `cpu_baseline` is the oracle
 timed on the host cores on a bounded sub-block of the same workload.  With --gpus N > 1 (torchrun) every rank
 runs an independent replica of the block ("replicas only": the path has no collective), scaling = weak.
 """
@@ -36,14 +36,16 @@ def algorithmic_bytes_per_update(N):
 
 
 def design_bytes_per_update(N):
-    """what the kernel as built must move: the above without the 30 Ricci coefficients per cell (240 B) that the stored
-    design does not read, plus the stored angular-edge coefficients, 3 doubles per update"""
-    return 16.0 + 24.0 + 400.0 / N
+    """what the kernel as built must move: read I (8) + write I_+ (8) + the stored angular-edge coefficients (3 doubles per
+    update) + per cell 288 B packed record, ~48 B lower-face records of the tile edge,
+    64 B fluid and opacities, 40 B T_+ and fluid increment"""
+    return 16.0 + 24.0 + 440.0 / N
 
 
-# FP64-pipe instruction slots per update of the stage kernel as designed (DESIGN.md 'rooflines', table 'FP64 budget'),
-# counted per lane; one slot = one DFMA-equivalent issue = 2 flop of the measured DFMA peak
-FP64_SLOTS_PER_UPDATE = {True: 160.0, False: 113.0}  # with / without coupling
+# FP64-pipe instruction slots per update of the stage kernel (DESIGN.md 'rooflines'): FP64 warp instructions x 32 lanes /
+# updates, from the ncu instruction counts under profiles/ (idle lanes of the last angle group included); one slot = one
+# DFMA-equivalent issue = 2 flop of the measured DFMA peak
+FP64_SLOTS_PER_UPDATE = {True: 177.0, False: 118.0}  # with / without coupling
 
 
 class ClockSampler:
@@ -269,7 +271,7 @@ def main():
     peak, peak_src = measured_peak()
     bpu = algorithmic_bytes_per_update(N)
     achieved = bpu * updates / (ms * 1e-3) / 1e9
-    roofline = {"kernel": "k_stage (fused flux divergence + implicit coupling + mask, one launch per step)", "bound": "hbm",
+    roofline = {"kernel": "k_stage5 (fused flux divergence + implicit coupling + mask, one launch per step)", "bound": "hbm",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                 "algorithmic_bytes_per_update": bpu, "design_bytes_per_update": design_bytes_per_update(N),
                 "design_frac": design_bytes_per_update(N) * updates / (ms * 1e-3) / 1e9 / peak,
