@@ -752,13 +752,23 @@ int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &
     const int N = t.N;
     if (N <= 32) return launch5<1, 1, 4, 2>(t, p, a, couple, s);
     if (N <= 64) return launch5<1, 2, 4, 2>(t, p, a, couple, s);
-    if (N <= 96) return launch5<1, 3, 4, 2>(t, p, a, couple, s);
+    if (N <= 96) {
+        static const int var = [] { const char *e = std::getenv("RAD_S5_VARIANT"); return e ? std::atoi(e) : 0; }();
+        if (var == 1) return launch5<1, 3, 4, 2>(t, p, a, couple, s);
+        if (var == 2) return launch5<3, 1, 4, 4>(t, p, a, couple, s);
+        if (var == 3) return launch5<3, 1, 4, 2>(t, p, a, couple, s);
+        if (var == 4) return launch5<3, 1, 5, 2>(t, p, a, couple, s);
+        if (var == 5) return launch5<3, 1, 6, 2>(t, p, a, couple, s);
+        if (var == 6) return launch5<3, 1, 3, 4>(t, p, a, couple, s);
+        return launch5<3, 1, 4, 3>(t, p, a, couple, s);
+    }
     if (N <= 128) return launch5<2, 2, 4, 2>(t, p, a, couple, s);
     if (N <= 192) {
         static const int var = [] { const char *e = std::getenv("RAD_S5_VARIANT"); return e ? std::atoi(e) : 0; }();
         if (var == 1) return launch5<2, 3, 3, 2>(t, p, a, couple, s);
         if (var == 2) return launch5<2, 3, 4, 2>(t, p, a, couple, s);
         if (var == 3) return launch5<3, 2, 3, 2>(t, p, a, couple, s);
+        if (var == 4) return launch5<6, 1, 4, 2>(t, p, a, couple, s);
         return launch5<3, 2, 4, 2>(t, p, a, couple, s);
     }
     return 0;
