@@ -61,17 +61,13 @@ bool upload(rad_ctx *c, const std::vector<T> &h, const T **dptr) {
 
 bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
 
-// the fused stage kernel: the angle-resident version (stage5.cu) where it serves the configuration, else the
-// tile-synchronous warp-per-cell version (stage4.cu), else the warp-independent version (stage.cu).
-// RAD_STAGE_KERNEL=4 / 3 in the environment forces the older versions (A/B measurements).
+// the fused stage kernel: the angle-resident version (stage5.cu) where it serves the configuration (even N <= 192 that
+// fits shared memory), else the warp-independent version (stage.cu).  RAD_STAGE_KERNEL=3 in the environment forces the
+// latter (A/B measurements).
 int launch_fused(const rad::DeviceTables &t, const rad::Params &p, const rad::StageArgs &a, bool couple, cudaStream_t s) {
     static const int force = [] { const char *e = std::getenv("RAD_STAGE_KERNEL"); return e ? std::atoi(e) : 0; }();
     if (force == 0 || force == 5) {
         const int nl = rad::launch_stage_angle(t, p, a, couple, s);
-        if (nl != 0) return nl;
-    }
-    if (force != 3) {
-        const int nl = rad::launch_stage_tile(t, p, a, couple, s);
         if (nl != 0) return nl;
     }
     return rad::launch_stage_fused(t, p, a, couple, s);

@@ -96,8 +96,6 @@ int launch_moments(const DeviceTables &t, const double *I, int frame, const doub
 // fused stage kernel: flux divergence (+ coupling and mask when couple != 0) in one launch; returns 0 if this
 // configuration is not served (caller falls back to launch_fluxdiv + launch_coupling)
 int launch_stage_fused(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
-// tile-synchronous fused stage kernel (stage4.cu): 1 launched, 0 not served, -1 CUDA error
-int launch_stage_tile(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
 // angle-resident fused stage kernel (stage5.cu): 1 launched, 0 not served, -1 CUDA error; and its record builder
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s);

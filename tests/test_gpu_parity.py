@@ -294,3 +294,53 @@ def test_invariants_on_gpu(oracle, B):
         assert abs(e1 - e0) < 1e-12 * abs(e0) and e0 != 0
     finally:
         B.rad_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ full size, sampled
+@pytest.mark.parametrize("cfg,m,corners", [("C3", 6, [(0, 0, 0), (61, 62, 63), (122, 122, 122), (3, 120, 50)]),
+                                           ("C5", 5, [(0, 0, 0), (126, 127, 128), (251, 251, 251)])])
+def test_full_size_sampled(oracle, B, cfg, m, corners):
+    """BASELINE.json's full-size blocks in the launch configuration bench.py times (one rad_stage on the whole block), checked on
+    sampled sub-blocks: a cell's update reads at most 2 cells away, so the oracle run on m^3 cells whose 2-deep shell is cut
+    out of the full input must reproduce the GPU's values there.  Corners of the block, its middle and a tile-straddling
+    position are sampled (tiles are 4 x 2 / 4 x 3 cells in y-z)."""
+    c = W.CONFIGS[cfg]
+    nn, ng, x0, dx = W.grid(cfg)
+    N = W.n_angles(cfg)
+    h0 = B.rad_create(dict(kind=0), dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1)), c["angles"], None, dict(couple=0))
+    nhat = B.rad_get_table(h0, B.TAB_NHAT)
+    B.rad_destroy(h0)
+    inp = W.make_inputs(cfg, nhat, device="cuda")
+    shape = (nn[2] + 2 * ng, nn[1] + 2 * ng, nn[0] + 2 * ng)
+    I = inp["I"].reshape(-1, N).contiguous(); fluid = inp["fluid"].reshape(5, -1).contiguous(); opac = inp["opac"].reshape(3, -1).contiguous()
+    del inp
+    h = make_rad(B, cfg, opac)
+    try:
+        vmax = float(B.rad_get_table(h, B.TAB_MAXSPEED).max())
+        dt = W.CFL * min(dx) / vmax
+        O = torch.full_like(I, -7.0)
+        T = torch.zeros(I.shape[0], dtype=torch.float64, device="cuda"); dT0 = torch.zeros(4, I.shape[0], dtype=torch.float64, device="cuda")
+        nf = B.rad_stage(h, I, O, None, fluid, 0.0, 1.0, dt, T, dT0, count_noroot=True)
+        torch.cuda.synchronize()
+        assert nf == 0
+        A = oracle.Angles(*c["angles"])
+        I5 = I.reshape(shape + (N,)); O5 = O.reshape(shape + (N,))
+        f4 = fluid.reshape((5,) + shape); o4 = opac.reshape((3,) + shape); T3 = T.reshape(shape); d4 = dT0.reshape((4,) + shape)
+        for (ai, aj, ak) in corners:
+            sl = (slice(ak, ak + m + 2 * ng), slice(aj, aj + m + 2 * ng), slice(ai, ai + m + 2 * ng))
+            P = oracle.Problem(A, (m, m, m), (x0[0] + ai * dx[0], x0[1] + aj * dx[1], x0[2] + ak * dx[2]), dx, metric_kind=c["metric"], M=c["M"], a=c["a"],
+                               excise_r=W.excise_radius(cfg), bc_lo=(0, 0, 0), bc_hi=(0, 0, 0), gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD,
+                               n0_crit=W.N0_CRIT, recon_space=1, renorm=1, couple=1)
+            Is = I5[sl].cpu().numpy().reshape(-1, N).copy()
+            fs = f4[(slice(None),) + sl].cpu().numpy().reshape(5, -1).copy(); os_ = o4[(slice(None),) + sl].cpu().numpy().reshape(3, -1).copy()
+            out_o, T_o, dT0_o, nf_o = P.stage(Is, fs, os_, dt)
+            got = O5[sl].cpu().numpy().reshape(-1, N)
+            eI = rel_err_I(P.interior(got), P.interior(out_o))
+            eT = rel_err(P.interior(T3[sl].cpu().numpy().reshape(-1)), P.interior(T_o), 0.0)
+            R0 = np.abs(P.interior(P.moments(out_o, 1)[0]))
+            eD = max(rel_err(P.interior(d4[(q,) + sl].cpu().numpy().reshape(-1)), P.interior(dT0_o[q]), DT0_FLOOR * R0 + 1e-300) for q in range(4))
+            assert eI <= TOL_I and eT <= TOL_FLUID and eD <= TOL_FLUID, (cfg, (ai, aj, ak), eI, eT, eD)
+        # ghost cells of I_out are never written
+        assert float(O5[:ng].max()) == -7.0 and float(O5[:, :ng].max()) == -7.0 and float(O5[:, :, -ng:].max()) == -7.0
+    finally:
+        B.rad_destroy(h)
