@@ -158,6 +158,12 @@ __device__ __forceinline__ double lds(uint32_t addr) {
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
     return v;
 }
+// v = skip ? fallback : shared[addr]; lanes with `skip` take no part in the load (fewer bank conflicts for gathers)
+__device__ __forceinline__ double lds_unless(uint32_t addr, bool skip, double fallback) {
+    double v = fallback;
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@!p ld.shared.f64 %0, [%1];\n}" : "+d"(v) : "r"(addr), "r"((unsigned)skip));
+    return v;
+}
 __device__ __forceinline__ double2 lds2(uint32_t addr) {
     double2 v;
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
@@ -466,7 +472,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
 #pragma unroll
                 for (int jj = 0; jj < 3; jj++) {
                     const bool owner_up = (__double2loint(q[jj]) & 1) != 0;
-                    G[jj] = lds(ownrow + (owner_up ? OFF8(it) : pj[jj] * 8u));
+                    G[jj] = lds_unless(ownrow + pj[jj] * 8u, owner_up, x0[it]);  // the upwind intensity: the thread's own (in a register) or the partner's
                 }
 #pragma unroll
                 for (int jj = 0; jj < 3; jj++) G[jj] *= q[jj];
@@ -769,6 +775,7 @@ int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &
         if (var == 2) return launch5<2, 3, 4, 2>(t, p, a, couple, s);
         if (var == 3) return launch5<3, 2, 3, 2>(t, p, a, couple, s);
         if (var == 4) return launch5<6, 1, 4, 2>(t, p, a, couple, s);
+        if (var == 5) return launch5<6, 1, 3, 3>(t, p, a, couple, s);
         return launch5<3, 2, 4, 2>(t, p, a, couple, s);
     }
     return 0;
