@@ -122,8 +122,12 @@ rad_status rad_stage(rad_ctx *, double *I_in, double *I_out, const double *I0, c
                      long long *n_noroot, void *cuda_stream);
 
 /* Same stage with HOST buffers (same shapes): copies I_in, fluid and the three opacity arrays
- * host->device into library-owned scratch, runs rad_stage, copies I_out, T_out, dT0 back, and
- * synchronises.  opac_host: HOST SoA [3][ncells_total] = alpha_a_planck, alpha_a_energy, alpha_s.
+ * host->device into library-owned scratch, runs the stage, copies I_out, T_out, dT0 back, and
+ * synchronises.  With caller-filled boundaries and an angle grid the tile kernel serves, the block is
+ * processed in slabs of z planes on three streams, so that the copy-in of the next slab and the
+ * copy-out of the previous one overlap the stage of the current one (pinned host memory needed for
+ * the overlap); otherwise copy-in, rad_stage, copy-out run one after the other.  Ghost cells of
+ * I_out_host receive the values of I_in_host; T_out_host / dT0_host are defined in interior cells.  opac_host: HOST SoA [3][ncells_total] = alpha_a_planck, alpha_a_energy, alpha_s.
  * I0 is not supported here (forward-Euler style stages only).  Pinned host memory makes the copies faster
  * but is not required. */
 rad_status rad_stage_host(rad_ctx *, const double *I_in_host, double *I_out_host, const double *fluid_host,

@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "rad_internal.h"
 
@@ -25,6 +26,7 @@ struct rad_ctx {
     double *scratch_I[2] = {nullptr, nullptr};  // rad_stage_host
     double *scratch_small = nullptr;            // fluid[5] + opac[3] + T[1] + dT0[4] per cell
     unsigned long long *d_noroot = nullptr;
+    cudaStream_t hs[3] = {nullptr, nullptr, nullptr};  // rad_stage_host: copy-in, compute, copy-out
     long long launches = 0;
     std::string err;
 };
@@ -227,6 +229,7 @@ void rad_destroy(rad_ctx *c) {
     for (void *p : c->owned) cudaFree(p);
     for (int q = 0; q < 2; q++) if (c->scratch_I[q]) cudaFree(c->scratch_I[q]);
     if (c->scratch_small) cudaFree(c->scratch_small);
+    for (int q = 0; q < 3; q++) if (c->hs[q]) cudaStreamDestroy(c->hs[q]);
     if (c->ke) cudaFree(c->ke);
     if (c->rec) cudaFree(c->rec);
     delete c;
@@ -318,16 +321,105 @@ rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, 
     return rad_couple(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot, stream);
 }
 
+// rad_stage_host, pipelined: the block is cut into slabs of planes along z; while slab j is computed, the input planes of
+// slab j+1 travel host -> device and the output planes of slab j-1 device -> host (three streams, PCIe in both directions at
+// once).  Used when the angle-resident stage kernel serves the context and all boundaries are caller-filled (a periodic or
+// outflow fill in z needs the far end of the array first).  Returns RAD_EUNSUPPORTED if it does not apply.
+static rad_status stage_host_pipelined(rad_ctx *c, const double *I_in_host, double *I_out_host, const double *fluid_host, const double *opac_host,
+                                       double gam0, double gam1, double beta_dt, double *T_out_host, double *dT0_host, long long *n_noroot) {
+    const rad::DeviceTables &t = c->dev;
+    if (!rad::stage_angle_serves(t)) return RAD_EUNSUPPORTED;
+    for (int d = 0; d < 3; d++)
+        if (c->grid.bc_lo[d] != 0 || c->grid.bc_hi[d] != 0) return RAD_EUNSUPPORTED;
+    const int nz = t.n[2], ng = t.ng;
+    if (nz < 8) return RAD_EUNSUPPORTED;
+    cudaStream_t *st = c->hs;
+    for (int q = 0; q < 3; q++)
+        if (!st[q] && cudaStreamCreateWithFlags(&st[q], cudaStreamNonBlocking) != cudaSuccess) return cuda_fail(c, "rad_stage_host: stream");
+    const long long nc = t.ncell, plane = (long long)t.NI * t.NJ;  // cells per z plane
+    const size_t pbytes = sizeof(double) * plane * t.N;
+    double *dI = c->scratch_I[0], *dO = c->scratch_I[1];
+    double *dfl = c->scratch_small, *dop = dfl + 5 * nc, *dT = dop + 3 * nc, *ddT0 = dT + nc;
+    int nslab = (nz + 7) / 8;  // thin slabs: the first copy-in and the last copy-out are not overlapped
+    if (nslab > 48) nslab = 48;
+    const int per = (((nz + nslab - 1) / nslab) + 3) & ~3;  // planes per slab, a multiple of the tile heights
+    nslab = (nz + per - 1) / per;
+    std::vector<cudaEvent_t> evH(nslab), evK(nslab);
+    for (int j = 0; j < nslab; j++) {
+        if (cudaEventCreateWithFlags(&evH[j], cudaEventDisableTiming) != cudaSuccess || cudaEventCreateWithFlags(&evK[j], cudaEventDisableTiming) != cudaSuccess)
+            return cuda_fail(c, "rad_stage_host: event");
+    }
+    bool ok = true;
+    cudaEvent_t ev0;
+    ok = cudaEventCreateWithFlags(&ev0, cudaEventDisableTiming) == cudaSuccess;
+    // whoever used the default stream before (the caller's previous work on these buffers) is ordered before the pipeline
+    ok = ok && cudaEventRecord(ev0, 0) == cudaSuccess;
+    for (int q = 0; q < 3 && ok; q++) ok = cudaStreamWaitEvent(st[q], ev0, 0) == cudaSuccess;
+    if (ok && n_noroot) ok = cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), st[1]) == cudaSuccess;
+    const rad_opac saved = c->opac;
+    c->opac.alpha_a_planck = dop; c->opac.alpha_a_energy = dop + nc; c->opac.alpha_s = dop + 2 * nc;
+    int p_done = 0;  // array planes [0, p_done) are on their way to the device
+    for (int j = 0; j < nslab && ok; j++) {
+        const int kb = j * per, ke = kb + per < nz ? kb + per : nz;      // interior planes of the slab
+        const int need = (j == nslab - 1) ? t.NK : ke + 2 * ng;          // array planes [0, need) must be resident: interior plane k is array plane k + ng
+        if (need > p_done) {
+            ok = cudaMemcpyAsync(dI + (size_t)p_done * plane * t.N, I_in_host + (size_t)p_done * plane * t.N, pbytes * (need - p_done), cudaMemcpyHostToDevice, st[0]) == cudaSuccess;
+            p_done = need;
+        }
+        {   // fluid and opacities of the slab's own planes (read for interior cells only)
+            const size_t fo = (size_t)(kb + ng) * plane, fb = sizeof(double) * plane * (ke - kb);
+            for (int m = 0; m < 5 && ok; m++) ok = cudaMemcpyAsync(dfl + m * nc + fo, fluid_host + m * nc + fo, fb, cudaMemcpyHostToDevice, st[0]) == cudaSuccess;
+            for (int m = 0; m < 3 && ok && opac_host; m++) ok = cudaMemcpyAsync(dop + m * nc + fo, opac_host + m * nc + fo, fb, cudaMemcpyHostToDevice, st[0]) == cudaSuccess;
+        }
+        ok = ok && cudaEventRecord(evH[j], st[0]) == cudaSuccess && cudaStreamWaitEvent(st[1], evH[j], 0) == cudaSuccess;
+        // output planes of this slab start as a copy of the input (only interior cells are written by the stage: the ghost
+        // cells of the returned array are those of the input); the ghost planes below / above go with the first / last slab
+        const int ob = (j == 0) ? 0 : kb + ng, oe = (j == nslab - 1) ? t.NK : ke + ng;
+        ok = ok && cudaMemcpyAsync(dO + (size_t)ob * plane * t.N, dI + (size_t)ob * plane * t.N, pbytes * (oe - ob), cudaMemcpyDeviceToDevice, st[1]) == cudaSuccess;
+        if (!ok) break;
+        rad::StageArgs a{};
+        a.I_in = dI; a.I0 = nullptr; a.I_out = dO; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
+        a.fluid = dfl; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
+        a.T_out = dT; a.dT0 = ddT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
+        a.kz0 = kb; a.kz1 = ke;
+        const int nl = rad::launch_stage_angle(t, c->kp, a, true, st[1]);
+        if (nl <= 0) { ok = false; break; }
+        c->launches += nl;
+        ok = cudaEventRecord(evK[j], st[1]) == cudaSuccess && cudaStreamWaitEvent(st[2], evK[j], 0) == cudaSuccess;
+        ok = ok && cudaMemcpyAsync(I_out_host + (size_t)ob * plane * t.N, dO + (size_t)ob * plane * t.N, pbytes * (oe - ob), cudaMemcpyDeviceToHost, st[2]) == cudaSuccess;
+        const size_t cb = sizeof(double) * plane * (oe - ob), co = (size_t)ob * plane;
+        if (ok && T_out_host) ok = cudaMemcpyAsync(T_out_host + co, dT + co, cb, cudaMemcpyDeviceToHost, st[2]) == cudaSuccess;
+        for (int m = 0; m < 4 && ok && dT0_host; m++) ok = cudaMemcpyAsync(dT0_host + m * nc + co, ddT0 + m * nc + co, cb, cudaMemcpyDeviceToHost, st[2]) == cudaSuccess;
+    }
+    c->opac = saved;
+    unsigned long long v = 0;
+    if (ok && n_noroot) ok = cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, st[2]) == cudaSuccess;
+    for (int q = 0; q < 3; q++) ok = (cudaStreamSynchronize(st[q]) == cudaSuccess) && ok;
+    for (int j = 0; j < nslab; j++) { cudaEventDestroy(evH[j]); cudaEventDestroy(evK[j]); }
+    cudaEventDestroy(ev0);
+    if (!ok) return cuda_fail(c, "rad_stage_host: pipelined copies / launches");
+    if (n_noroot) *n_noroot = (long long)v;
+    return RAD_OK;
+}
+
 rad_status rad_stage_host(rad_ctx *c, const double *I_in_host, double *I_out_host, const double *fluid_host, const double *opac_host,
                           double gam0, double gam1, double beta_dt, double *T_out_host, double *dT0_host, long long *n_noroot) {
     if (!c || !I_in_host || !I_out_host || !fluid_host) return fail(c, RAD_EINVAL, "rad_stage_host: NULL argument");
     if (c->kp.couple && !opac_host) return fail(c, RAD_EINVAL, "rad_stage_host: coupling needs opac_host");
+    if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_stage_host: non-finite weights");
     DeviceGuard guard(c->device);
     const long long nc = c->dev.ncell;
     const size_t ibytes = sizeof(double) * nc * c->dev.N, cb = sizeof(double) * nc;
     for (int q = 0; q < 2; q++)
         if (!c->scratch_I[q] && cudaMalloc((void **)&c->scratch_I[q], ibytes) != cudaSuccess) return fail(c, RAD_ENOMEM, "rad_stage_host: device scratch");
     if (!c->scratch_small && cudaMalloc((void **)&c->scratch_small, 13 * cb) != cudaSuccess) return fail(c, RAD_ENOMEM, "rad_stage_host: device scratch");
+    if (c->kp.couple || opac_host) {
+        static const bool no_pipe = [] { const char *e = std::getenv("RAD_HOST_PIPELINE"); return e && e[0] == '0'; }();
+        if (!no_pipe && opac_host) {
+            const rad_status ps = stage_host_pipelined(c, I_in_host, I_out_host, fluid_host, opac_host, gam0, gam1, beta_dt, T_out_host, dT0_host, n_noroot);
+            if (ps != RAD_EUNSUPPORTED) return ps;
+        }
+    }
     double *dfl = c->scratch_small, *dop = dfl + 5 * nc, *dT = dop + 3 * nc, *ddT0 = dT + nc;
     cudaStream_t s = 0;
     bool ok = cudaMemcpyAsync(c->scratch_I[0], I_in_host, ibytes, cudaMemcpyHostToDevice, s) == cudaSuccess &&

@@ -74,6 +74,7 @@ struct StageArgs {
     const double *fluid, *aP, *aE, *aS;  // coupling only
     double *T_out, *dT0;
     unsigned long long *noroot;
+    int kz0, kz1;  // stage5 only: update the interior planes kz0 <= k < kz1 (0-based, without ghosts); kz1 <= kz0 = the whole block
 };
 
 struct Params {
@@ -98,6 +99,8 @@ int launch_moments(const DeviceTables &t, const double *I, int frame, const doub
 int launch_stage_fused(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
 // angle-resident fused stage kernel (stage5.cu): 1 launched, 0 not served, -1 CUDA error; and its record builder
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
+// 1 if launch_stage_angle serves this context (so that a stage can be run slab by slab along z)
+int stage_angle_serves(const DeviceTables &t);
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s);
 int launch_build_ke(const DeviceTables &t, double *ke, cudaStream_t s);
 int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed char *edge_sign, cudaStream_t s);

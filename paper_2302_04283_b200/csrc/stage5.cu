@@ -238,9 +238,10 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     Role *roles = reinterpret_cast<Role *>(sm + L.oRole);
 
     const int ng = t.ng;
-    const int j0 = blockIdx.y * TY + ng, k0 = blockIdx.z * TZ + ng;
+    const int kzb = a.kz1 > a.kz0 ? a.kz0 : 0, kze = a.kz1 > a.kz0 ? a.kz1 : t.n[2];  // the slab of interior planes this launch updates
+    const int j0 = blockIdx.y * TY + ng, k0 = blockIdx.z * TZ + ng + kzb;
     const int j = j0 + wy, k = k0 + wz;
-    const bool active = j < t.n[1] + ng && k < t.n[2] + ng;
+    const bool active = j < t.n[1] + ng && k < kze + ng;
     const int i_begin = blockIdx.x * KX + ng, i_end = min(i_begin + KX, t.n[0] + ng), nsteps = i_end - i_begin;
     const long long c_first = ((long long)k * t.NJ + j) * t.NI + i_begin;
 
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
             else if (q < 2 * NC + TZ) { kind = 2; ccs = (q - 2 * NC) * TY; }
             else { kind = 3; ccs = q - 2 * NC - TZ; }
             const int jj = j0 + ccs % TY, kk = k0 + ccs / TY;
-            if (jj < t.n[1] + ng && kk < t.n[2] + ng) {
+            if (jj < t.n[1] + ng && kk < kze + ng) {
                 const long long c0 = ((long long)kk * t.NJ + jj) * t.NI + i_begin;
                 if (kind == 0) {
                     const long long ci = ((long long)(kk - ng) * t.n[1] + (jj - ng)) * t.n[0] + (i_begin - ng);
@@ -389,7 +390,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
     const uint32_t aFy = smb + 8u * L.oFy, aFz = smb + 8u * L.oFz, aFx = smb + 8u * L.oFx;
     // load balance: cell (0,0) would compute five faces (x, upper y and z, lower y and z), cell (1,1) three; cell (1,1)
     // takes over the lower z face of cell (0,0)
-    const bool helped = TY >= 2 && TZ >= 2 && j0 + 1 < t.n[1] + ng && k0 + 1 < t.n[2] + ng;
+    const bool helped = TY >= 2 && TZ >= 2 && j0 + 1 < t.n[1] + ng && k0 + 1 < kze + ng;
     const bool is_helper = helped && cs == TY + 1, is_helpee = helped && cs == 0;
     const uint32_t aRed = smb + 8u * (uint32_t)(L.oRed + cs * (2 * WPC * 4 + 8));
     const uint32_t N8 = (uint32_t)N * 8u;
@@ -726,7 +727,8 @@ int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool cou
     if (smem > 227 * 1024) return 0;
     // run length along x: long runs amortise the prologue, short runs fill the SMs of small grids; pick the candidate
     // with the fewest CTA waves x (steps + prologue cost)
-    const long long tiles = (long long)((t.n[1] + TY - 1) / TY) * ((t.n[2] + TZ - 1) / TZ);
+    const int nz = a.kz1 > a.kz0 ? a.kz1 - a.kz0 : t.n[2];
+    const long long tiles = (long long)((t.n[1] + TY - 1) / TY) * ((nz + TZ - 1) / TZ);
     int KX = t.n[0];
     double best = 1e300;
     for (int cand = t.n[0];; cand = (cand + 1) / 2) {
@@ -735,7 +737,7 @@ int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool cou
         if (cost < best) { best = cost; KX = cand; }
         if (cand <= 4) break;
     }
-    dim3 grid((t.n[0] + KX - 1) / KX, (t.n[1] + TY - 1) / TY, (t.n[2] + TZ - 1) / TZ);
+    dim3 grid((t.n[0] + KX - 1) / KX, (t.n[1] + TY - 1) / TY, (nz + TZ - 1) / TZ);
     if (grid.y > 65535 || grid.z > 65535) return 0;
 #define RAD_LAUNCH5(PLM, CPL)                                                                                          \
     do {                                                                                                               \
@@ -779,6 +781,12 @@ int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &
         return launch5<3, 2, 4, 2>(t, p, a, couple, s);
     }
     return 0;
+}
+
+int stage_angle_serves(const DeviceTables &t) {
+    if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr || (t.N & 1) || t.N > 192) return 0;
+    if (t.N > 128) return sizeof(double) * (size_t)make_layout5<Tile<4, 2, 2>>(t.N).total <= 227 * 1024;
+    return 1;
 }
 
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s) {

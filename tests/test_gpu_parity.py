@@ -266,6 +266,27 @@ def test_stage_host_equals_stage(oracle, B):
         B.rad_destroy(h)
 
 
+@pytest.mark.parametrize("n,angles", [((6, 5, 20), ("geodesic", 2)), ((5, 9, 37), ("geodesic", 4)), ((4, 4, 9), ("latlon", 4, 8))])
+def test_stage_host_pipelined(oracle, B, n, angles):
+    """rad_stage_host with caller-filled boundaries runs slab by slab along z with overlapped copies: same values as the oracle,
+    ghost cells of the returned array = those of the input, every slab boundary inside the block"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, angles)
+    try:
+        out_h = np.full_like(I, -3.0); T_h = np.zeros(P.ncell); dT0_h = np.zeros((4, P.ncell))
+        nf = B.rad_stage_host(h, I, out_h, fluid, opac, 0.0, 1.0, 0.03, T_h, dT0_h, count_noroot=True)
+        out_o, T_o, dT0_o, nf_o = P.stage(I.copy(), fluid, opac, 0.03)
+        assert nf == nf_o
+        assert rel_err_I(P.interior(out_h), P.interior(out_o)) <= TOL_I
+        assert rel_err(P.interior(T_h), P.interior(T_o), 0.0) <= TOL_FLUID
+        R0 = np.abs(P.interior(P.moments(out_o, 1)[0]))
+        assert max(rel_err(P.interior(dT0_h[m]), P.interior(dT0_o[m]), DT0_FLOOR * R0 + 1e-300) for m in range(4)) <= TOL_FLUID
+        full = out_h.reshape(P.shape + (A.N,)).copy(); ref = I.reshape(P.shape + (A.N,)).copy()
+        P.interior(full)[...] = 0.0; P.interior(ref)[...] = 0.0
+        assert np.array_equal(full, ref)
+    finally:
+        B.rad_destroy(h)
+
+
 def test_invariants_on_gpu(oracle, B):
     """properties that hold at any size, checked on the CUDA path itself: isotropic fixed point in Minkowski (bit for bit)
     and conservation of sum n^0 n_0 I dOmega with sources off in Kerr-Schild"""
