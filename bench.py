@@ -42,6 +42,10 @@ def design_bytes_per_update(N):
     return 16.0 + 24.0 + 440.0 / N
 
 
+# DRAM bytes per launch of the stage kernel from the committed ncu --set full capture (dram__bytes_read.sum +
+# dram__bytes_write.sum; profiles/r1_k_stage5_ncu_full.md), for the workload it was taken on: (config, cells per axis, recon)
+NCU_TRAFFIC_BYTES = {("C3", None, 1): 15.86e9}
+
 # FP64-pipe instruction slots per update of the stage kernel: FP64 warp instructions x 32 lanes /
 # updates, from the ncu instruction counts under profiles/ (idle lanes of the last angle group included); one slot = one
 # DFMA-equivalent issue = 2 flop of the measured DFMA peak
@@ -272,7 +276,9 @@ def main():
     bpu = algorithmic_bytes_per_update(N)
     achieved = bpu * updates / (ms * 1e-3) / 1e9
     roofline = {"kernel": "k_stage5 (fused flux divergence + implicit coupling + mask, one launch per step)", "bound": "hbm",
-                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg, args.n, args.recon)),
+                "traffic_source": "ncu --set full capture, profiles/r1_k_stage5_ncu_full.md (bytes per launch)" if (cfg, args.n, args.recon) in NCU_TRAFFIC_BYTES else None,
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_update": bpu, "design_bytes_per_update": design_bytes_per_update(N),
                 "design_frac": design_bytes_per_update(N) * updates / (ms * 1e-3) / 1e9 / peak,
                 "ms_per_launch": ms / kernels_per_step, "kernels_per_step": kernels_per_step,
