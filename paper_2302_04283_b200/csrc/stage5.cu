@@ -219,8 +219,8 @@ __device__ __forceinline__ bool quartic_delta_fast(double B4, double B1, double 
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-template <int NITER, int WPC, int TY, int TZ, bool PLM, bool COUPLE>
-__global__ void __launch_bounds__(TY *TZ *WPC * 32, 1)
+template <int NITER, int WPC, int TY, int TZ, int MINB, bool PLM, bool COUPLE>
+__global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     k_stage5(const DeviceTables t, const Params p, const StageArgs a, const Layout5 L, const int KX) {
     using T = Tile<TY, TZ, WPC>;
     constexpr int NC = T::NC, NH = T::NH, NR = T::NR;
@@ -719,7 +719,7 @@ __global__ void __launch_bounds__(256) k_pack_rec(const DeviceTables t, double *
     }
 }
 
-template <int NITER, int WPC, int TY, int TZ>
+template <int NITER, int WPC, int TY, int TZ, int MINB = 1>
 int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
     using T = Tile<TY, TZ, WPC>;
     const Layout5 L = make_layout5<T>(t.N);
@@ -741,8 +741,8 @@ int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool cou
     if (grid.y > 65535 || grid.z > 65535) return 0;
 #define RAD_LAUNCH5(PLM, CPL)                                                                                          \
     do {                                                                                                               \
-        if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, PLM, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
-        k_stage5<NITER, WPC, TY, TZ, PLM, CPL><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                                  \
+        if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
+        k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                                  \
     } while (0)
     if (p.recon_space == 1) { if (couple) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(true, false); }
     else { if (couple) RAD_LAUNCH5(false, true); else RAD_LAUNCH5(false, false); }
@@ -778,6 +778,8 @@ int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &
         if (var == 3) return launch5<3, 2, 3, 2>(t, p, a, couple, s);
         if (var == 4) return launch5<6, 1, 4, 2>(t, p, a, couple, s);
         if (var == 5) return launch5<6, 1, 3, 3>(t, p, a, couple, s);
+        if (var == 6) return launch5<3, 2, 2, 2, 2>(t, p, a, couple, s);
+        if (var == 7) return launch5<3, 2, 3, 1, 2>(t, p, a, couple, s);
         return launch5<3, 2, 4, 2>(t, p, a, couple, s);
     }
     return 0;
