@@ -365,3 +365,25 @@ def test_full_size_sampled(oracle, B, cfg, m, corners):
         assert float(O5[:ng].max()) == -7.0 and float(O5[:, :ng].max()) == -7.0 and float(O5[:, :, -ng:].max()) == -7.0
     finally:
         B.rad_destroy(h)
+
+
+def test_three_stages_ping_pong(oracle, B):
+    """three consecutive stages with periodic boundaries, the two intensity buffers swapped after each (the caller's time loop):
+    the ghost fill of every stage works on the previous stage's output, the fluid temperature is carried along"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (9, 6, 5), ("geodesic", 3), bc=(1, 1, 1, 1, 1, 1))
+    try:
+        dA = dev(I); dB_ = torch.zeros_like(dA); dfl = dev(fluid)
+        dT = torch.zeros(P.ncell, dtype=torch.float64, device="cuda")
+        Io, fo = I.copy(), fluid.copy()
+        for step in range(3):
+            nf = B.rad_stage(h, dA, dB_, None, dfl, 0.0, 1.0, 0.04, dT, None, count_noroot=True)
+            out_o, T_o, _, nf_o = P.stage(Io, fo, opac, 0.04)
+            assert nf == nf_o == 0
+            assert rel_err_I(P.interior(dB_.cpu().numpy()), P.interior(out_o)) <= 3 * TOL_I, step
+            assert rel_err(P.interior(dT.cpu().numpy()), P.interior(T_o), 0.0) <= 3 * TOL_FLUID, step
+            dA, dB_ = dB_, dA
+            Io = out_o.copy()
+            Tin = P.interior(fo[1]); Tin[...] = P.interior(T_o)          # interior temperatures advance, ghosts keep theirs
+            P.interior(dfl[1].reshape(P.shape))[...] = torch.as_tensor(P.interior(T_o)).cuda()
+    finally:
+        B.rad_destroy(h)
