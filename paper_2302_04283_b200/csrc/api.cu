@@ -144,7 +144,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
     // fused stage kernel: balanced edge ownership, per-angle records, 1/dOmega
     t.fused_ok = 0; t.ang_rec = nullptr; t.winv = nullptr; t.own_edge = nullptr; t.ke = nullptr; t.rec = nullptr;
-    if (ok && h.N <= 192) {
+    if (ok && h.N <= 256) {
         std::string oerr;
         if (rad::build_edge_ownership(h, c->own, oerr)) {
             std::vector<short> rec((size_t)h.N * 8, 0);
@@ -287,7 +287,7 @@ rad_status rad_couple(rad_ctx *c, double *I, const double *fluid, double dt, dou
 rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
                      double beta_dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
     if (!c || !fluid) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
-    if (c->dev.fused_ok && c->dev.ke && c->dev.N <= 192) {
+    if (c->dev.fused_ok && c->dev.ke && c->dev.N <= 256) {
         // one launch: flux divergence + coupling + mask (stage.cu)
         if (!I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
         if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_stage: I_out must not alias I_in or I0 (the stencil reads old values)");

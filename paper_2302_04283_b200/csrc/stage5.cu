@@ -782,11 +782,13 @@ int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &
         if (var == 7) return launch5<3, 2, 3, 1, 2>(t, p, a, couple, s);
         return launch5<3, 2, 4, 2>(t, p, a, couple, s);
     }
+    if (N <= 256) return launch5<4, 2, 2, 2>(t, p, a, couple, s);  // geodesic level 5 (252 angles): 2 KB rows, 2 x 2 tiles
     return 0;
 }
 
 int stage_angle_serves(const DeviceTables &t) {
-    if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr || (t.N & 1) || t.N > 192) return 0;
+    if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr || (t.N & 1) || t.N > 256) return 0;
+    if (t.N > 192) return sizeof(double) * (size_t)make_layout5<Tile<2, 2, 2>>(t.N).total <= 227 * 1024;
     if (t.N > 128) return sizeof(double) * (size_t)make_layout5<Tile<4, 2, 2>>(t.N).total <= 227 * 1024;
     return 1;
 }
