@@ -471,6 +471,7 @@ struct orc_problem {
     const orc_angles *ang;
     double gamma_gas, a_rad, n0_crit;
     int recon_space, renorm, couple;
+    double tau_factor; /* constant of Eq.26; 0 = free-streaming flux Eq.24 */
     long long ncell;
     double *cell; /* [ncell][ORC_NCELL] */
     double *face; /* [ncell][3][ORC_NFACE]: lower face of each cell along each axis */
@@ -590,8 +591,13 @@ static double vl_slope(double qm, double q0, double qp) {
     double dl = q0 - qm, dr = qp - q0, pr = dl * dr;
     return (pr > 0.0) ? 2.0 * pr / (dl + dr) : 0.0;
 }
-/* Eq.24: flux of n^a n_0 I through the LOWER face of cell id[] along axis ax, angle n */
-static double face_flux(const orc_problem *P, const double *I, int ax, int i, int j, int k, int n) {
+/* Eq.24: flux of n^a n_0 I through the LOWER face of cell id[] along axis ax, angle n.
+ * With vel != NULL (tau_factor != 0): the optical-depth-aware flux of Eq.26-29.  vel[cell][5] holds the
+ * tetrad-frame fluid velocity u^alphahat (4) of each cell (its own cell-centre tetrad, R10) and alpha_E = alpha^a_E + alpha^s.
+ * Readings: R15 "interpolated to the interface" = arithmetic mean of the two adjacent cells; R16 the undefined
+ * v^0hat of Eq.26 = mean of the two cells' u^0hat; R17 g = (g_L + g_R)/2; R18 Delta t = beta dt of the stage, tau =
+ * tau_factor * alpha_E dt / v^0hat; G1 f = -expm1(-tau^2) (the sentence after Eq.27 defines expm1; Eq.27 as printed lacks it). */
+static double face_flux(const orc_problem *P, const double *I, int ax, int i, int j, int k, int n, const double *vel, double tau_dt) {
     int N = P->ang->N, st[3] = {0, 0, 0};
     st[ax] = 1;
     long long cR = cidx(P, k, j, i), cL = cidx(P, k - st[2], j - st[1], i - st[0]);
@@ -606,6 +612,17 @@ static double face_flux(const orc_problem *P, const double *I, int ax, int i, in
         Iup = qR;
         if (P->recon_space == 1) Iup = qR - 0.5 * vl_slope(qL, qR, I[cRR * N + n]);
     } else return 0.0;
+    if (vel) {
+        const double *vL = &vel[cL * 5], *vR = &vel[cR * 5];
+        double aE = 0.5 * (vL[4] + vR[4]), v0 = 0.5 * (vL[0] + vR[0]);               /* R15, R16 */
+        double tau = tau_dt * aE / v0;                                                /* Eq.26 */
+        double fint = -expm1(-tau * tau);                                             /* Eq.27 with G1 */
+        double nbL = vL[0] - (vL[1] * nh[0] + vL[2] * nh[1] + vL[3] * nh[2]);         /* n^0bar_L = -(u_alpha n^alpha)_L */
+        double nbR = vR[0] - (vR[1] * nh[0] + vR[2] * nh[1] + vR[3] * nh[2]);
+        double gL = -fint * (1.0 + 1.0 / nbL), gR = -fint * (1.0 + 1.0 / nbR);        /* Eq.29 */
+        double g = 0.5 * (gL + gR);                                                   /* R17 */
+        Iup *= (na > 0.0) ? (1.0 - gL + g) : (1.0 - gR + g);                          /* Eq.28 */
+    }
     return na * n0 * Iup;
 }
 /* pinned: c_e = -sum_{c=1..3} sum_{k=0..9} S[c][k] T_e[c][k], accumulated by fma from 0 in that order.
@@ -616,8 +633,8 @@ static double edge_coeff(const double *S, const double *T) {
     return -acc;
 }
 
-void orc_transport(const orc_problem *P, const double *I_in, const double *I0, double gam0, double gam1,
-                   double beta_dt, double *I_out) {
+static void transport_impl(const orc_problem *P, const double *I_in, const double *I0, double gam0, double gam1,
+                           double beta_dt, const double *vel, double tau_dt, double *I_out) {
     const orc_angles *A = P->ang;
     int N = A->N, E = A->E, ng = P->ng;
 #pragma omp parallel
@@ -643,9 +660,9 @@ void orc_transport(const orc_problem *P, const double *I_in, const double *I0, d
                         double nlo0 = contract4(cg + 17, nh); /* n_0 */
                         /* Eq.22: spatial flux divergence; uniform Cartesian grid with sqrt(-g)=1 => dA/dV = 1/dx */
                         double div = 0.0;
-                        div += (face_flux(P, I_in, 0, i + 1, j, k, n) - face_flux(P, I_in, 0, i, j, k, n)) / P->dx[0];
-                        div += (face_flux(P, I_in, 1, i, j + 1, k, n) - face_flux(P, I_in, 1, i, j, k, n)) / P->dx[1];
-                        div += (face_flux(P, I_in, 2, i, j, k + 1, n) - face_flux(P, I_in, 2, i, j, k, n)) / P->dx[2];
+                        div += (face_flux(P, I_in, 0, i + 1, j, k, n, vel, tau_dt) - face_flux(P, I_in, 0, i, j, k, n, vel, tau_dt)) / P->dx[0];
+                        div += (face_flux(P, I_in, 1, i, j + 1, k, n, vel, tau_dt) - face_flux(P, I_in, 1, i, j, k, n, vel, tau_dt)) / P->dx[1];
+                        div += (face_flux(P, I_in, 2, i, j, k + 1, n, vel, tau_dt) - face_flux(P, I_in, 2, i, j, k, n, vel, tau_dt)) / P->dx[2];
                         /* angular flux divergence: (1/dOmega) sum_e +-dlambda_e F_e, + where the edge normal points out of n */
                         double adiv = 0.0;
                         for (int s = 0; s < A->nnbr[n]; s++) {
@@ -664,6 +681,11 @@ void orc_transport(const orc_problem *P, const double *I_in, const double *I0, d
                 }
         free(Fe);
     }
+}
+
+void orc_transport(const orc_problem *P, const double *I_in, const double *I0, double gam0, double gam1,
+                   double beta_dt, double *I_out) {
+    transport_impl(P, I_in, I0, gam0, gam1, beta_dt, NULL, 0.0, I_out);
 }
 
 /* ======================================================================================
@@ -703,6 +725,37 @@ static void fluid_four_velocity(const double *cg, const double unorm[3], double 
     double gam = sqrt(1.0 + u2);
     ucon[0] = gam / alpha;
     for (int p = 0; p < 3; p++) ucon[p + 1] = unorm[p] - beta[p] * gam / alpha;
+}
+
+void orc_set_tau_factor(orc_problem *P, double tau_factor) { P->tau_factor = tau_factor; }
+
+/* vel[cell][5] for EVERY cell of the array (ghosts included: the faces of the outermost interior cells need their
+ * neighbours): tetrad-frame fluid velocity u^alphahat (R10, with the cell's own cell-centre tetrad; the same lines as in
+ * orc_coupling) and alpha_E = alpha^a_E + alpha^s (Eq.33b) */
+void orc_cell_velocity(const orc_problem *P, const double *fluid, const double *opac, double *vel) {
+    long long nc = P->ncell;
+#pragma omp parallel for schedule(static)
+    for (long long c = 0; c < nc; c++) {
+        const double *cg = &P->cell[c * ORC_NCELL], *Lw = cg + 17;
+        double unorm[3] = {fluid[2 * nc + c], fluid[3 * nc + c], fluid[4 * nc + c]}, ucon[4];
+        fluid_four_velocity(cg, unorm, ucon);
+        for (int ah = 0; ah < 4; ah++) {
+            double s = 0;
+            for (int b = 0; b < 4; b++) s += Lw[4 * b + ah] * ucon[b];
+            vel[c * 5 + ah] = (ah == 0 ? -1.0 : 1.0) * s;
+        }
+        vel[c * 5 + 4] = opac[1 * nc + c] + opac[2 * nc + c];
+    }
+}
+
+/* transport with the optical-depth-aware spatial flux of Eq.26-29 when tau_factor != 0 (else Eq.24) */
+void orc_transport_tau(const orc_problem *P, const double *I_in, const double *I0, double gam0, double gam1,
+                       double beta_dt, const double *fluid, const double *opac, double *I_out) {
+    if (P->tau_factor == 0.0 || !fluid || !opac) { transport_impl(P, I_in, I0, gam0, gam1, beta_dt, NULL, 0.0, I_out); return; }
+    double *vel = malloc(sizeof(double) * 5 * P->ncell);
+    orc_cell_velocity(P, fluid, opac, vel);
+    transport_impl(P, I_in, I0, gam0, gam1, beta_dt, vel, P->tau_factor * beta_dt, I_out);
+    free(vel);
 }
 
 long long orc_coupling(const orc_problem *P, double *I, const double *fluid, const double *opac, double dt,
@@ -809,7 +862,7 @@ long long orc_coupling(const orc_problem *P, double *I, const double *fluid, con
 long long orc_stage(const orc_problem *P, double *I_in, double *I_out, const double *I0, const double *fluid,
                     const double *opac, double gam0, double gam1, double beta_dt, double *T_out, double *dT0) {
     orc_fill_ghosts(P, I_in);
-    orc_transport(P, I_in, I0, gam0, gam1, beta_dt, I_out);
+    orc_transport_tau(P, I_in, I0, gam0, gam1, beta_dt, fluid, opac, I_out);
     return orc_coupling(P, I_out, fluid, opac, beta_dt, T_out, dT0);
 }
 

@@ -62,6 +62,13 @@ void orc_fill_ghosts(const orc_problem *, double *I);
 void orc_transport(const orc_problem *, const double *I_in, const double *I0, double gam0, double gam1,
                    double beta_dt, double *I_out);
 
+/* ---- NEXT-1: optical-depth-aware spatial flux (Eq.26-29).  tau_factor = the constant of Eq.26; 0 (default)
+ * = Eq.24.  orc_stage uses it through orc_transport_tau; fluid and opac must then be valid in the ghost cells too. ---- */
+void orc_set_tau_factor(orc_problem *, double tau_factor);
+void orc_cell_velocity(const orc_problem *, const double *fluid, const double *opac, double *vel /* [ncells_total][5] */);
+void orc_transport_tau(const orc_problem *, const double *I_in, const double *I0, double gam0, double gam1,
+                       double beta_dt, const double *fluid, const double *opac, double *I_out);
+
 /* ---- a4-a6: coupling (Eq.31-50) in place on I (interior), then the n_0 mask.
  * fluid: SoA [5][ncells_total] = rho, T, u1', u2', u3'.  opac: SoA [3][ncells_total] =
  * alpha_a_planck, alpha_a_energy, alpha_s.  T_out[ncells_total], dT0[4][ncells_total] (may be NULL).

@@ -59,6 +59,9 @@ def lib():
         L.orc_coupling.argtypes = [vp, vp, vp, vp, C.c_double, vp, vp]
         L.orc_stage.restype = C.c_longlong
         L.orc_stage.argtypes = [vp, vp, vp, vp, vp, vp, C.c_double, C.c_double, C.c_double, vp, vp]
+        L.orc_set_tau_factor.argtypes = [vp, C.c_double]
+        L.orc_cell_velocity.argtypes = [vp, vp, vp, vp]
+        L.orc_transport_tau.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_double, vp, vp, vp]
         L.orc_moments.argtypes = [vp, vp, C.c_int, vp, vp]
         L.orc_upwind_tables.argtypes = [vp, vp, vp]
         L.orc_edge_coeffs.argtypes = [vp, C.c_longlong, vp, vp]
@@ -117,7 +120,7 @@ class Problem:
     """Grid + metric + angles + parameters; the oracle's stage, moments and tables."""
 
     def __init__(self, angles, n, x0, dx, metric_kind=0, M=1.0, a=0.0, excise_r=0.0, ng=2, bc_lo=(0, 0, 0), bc_hi=(0, 0, 0),
-                 gamma_gas=5.0 / 3.0, a_rad=1.0, n0_crit=0.1, recon_space=1, renorm=1, couple=1):
+                 gamma_gas=5.0 / 3.0, a_rad=1.0, n0_crit=0.1, recon_space=1, renorm=1, couple=1, tau_factor=0.0):
         L = lib()
         self.angles = angles
         self.n = tuple(int(v) for v in n); self.ng = ng
@@ -128,6 +131,8 @@ class Problem:
         self.h = L.orc_create(metric_kind, M, a, excise_r, i3(*self.n), ng, d3(*x0), d3(*dx), i3(*bc_lo), i3(*bc_hi), angles.h,
                               gamma_gas, a_rad, n0_crit, recon_space, renorm, couple)
         self.ncell = L.orc_ncells_total(self.h)
+        self.tau_factor = float(tau_factor)
+        L.orc_set_tau_factor(self.h, self.tau_factor)   # constant of Eq.26; 0 = free-streaming flux Eq.24
 
     def __del__(self):
         try:
@@ -148,6 +153,18 @@ class Problem:
         I_in = _f64(I_in); out = np.zeros_like(I_in)
         lib().orc_transport(self.h, _p(I_in), _p(None if I0 is None else _f64(I0)), gam0, gam1, beta_dt, _p(out))
         return out
+
+    def transport_tau(self, I_in, beta_dt, fluid, opac, I0=None, gam0=0.0, gam1=1.0):
+        """transport with the optical-depth-aware flux of Eq.26-29 (tau_factor != 0); fluid/opac valid in ghosts too"""
+        I_in = _f64(I_in); out = np.zeros_like(I_in)
+        lib().orc_transport_tau(self.h, _p(I_in), _p(None if I0 is None else _f64(I0)), gam0, gam1, beta_dt, _p(_f64(fluid)), _p(_f64(opac)), _p(out))
+        return out
+
+    def cell_velocity(self, fluid, opac):
+        """[ncell][5]: tetrad-frame u^alphahat and alpha_E of every cell"""
+        vel = np.zeros((self.ncell, 5))
+        lib().orc_cell_velocity(self.h, _p(_f64(fluid)), _p(_f64(opac)), _p(vel))
+        return vel
 
     def coupling(self, I, fluid, opac, dt):
         """in place on I.  returns (T_out, dT0, n_noroot)."""
