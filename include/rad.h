@@ -88,7 +88,10 @@ typedef struct {
     int recon_angle;          /* 0 donor cell; others RAD_EUNSUPPORTED */
     int renorm_fluid_weights; /* R12: 1 = rescale fluid-frame solid angles to sum to 4 pi */
     int couple;               /* 0 = transport only, 1 = with implicit coupling (section 2.5) */
-    double tau_factor;        /* constant of Eq.26; only 0 (free-streaming flux, Eq.24) is implemented */
+    double tau_factor;        /* constant of Eq.26: 0 = free-streaming spatial flux (Eq.24); > 0 = optical-depth-aware flux
+                                 (Eq.26-29; readings R15-R18, G1 in DESIGN.md).  Then rad_stage reads fluid and opacities in the first
+                                 ghost layer too, runs as separate kernels (velocity table, flux divergence, coupling), and
+                                 rad_transport returns RAD_ESTATE (the flux needs the fluid state) */
     int recompute_edge_coeffs; /* stored-versus-recomputed angular geometry:
                                   0 = the angular-edge coefficients dlambda_e c_e n_0e (Eq.16-17, Eq.25) are built once
                                       in rad_create and stored, 3 N doubles per interior cell (adds 24 B per
@@ -99,8 +102,8 @@ typedef struct {
 
 /* Build a context: angle tables on the host (section 2.6), geometry tables on the device (section 2.1-2.2,
  * one kernel launch; synchronises the device once).  `device` is the CUDA ordinal.
- * Errors: RAD_EINVAL (NULL, ng != 2, n < 1, non-finite or non-positive dx, bad enum), RAD_EUNSUPPORTED
- * (recon_angle != 0, tau_factor != 0), RAD_ENOMEM, RAD_ECUDA.  On error *out is NULL. */
+ * Errors: RAD_EINVAL (NULL, ng != 2, n < 1, non-finite or non-positive dx, bad enum, tau_factor < 0), RAD_EUNSUPPORTED
+ * (recon_angle != 0), RAD_ENOMEM, RAD_ECUDA.  On error *out is NULL. */
 rad_status rad_create(const rad_metric *, const rad_grid *, const rad_angles *, const rad_opac *,
                       const rad_params *, int device, rad_ctx **out);
 

@@ -20,6 +20,7 @@ struct rad_ctx {
     rad::EdgeOwnership own;
     double *ke = nullptr;  // stored edge coefficients (owned)
     double *rec = nullptr; // packed per-cell records of the stage kernel (owned)
+    double *vel = nullptr; // optical-depth-aware flux: {u^alphahat, alpha_E} per cell (owned, allocated on first use)
     rad::DeviceTables dev{};
     rad::Params kp{};
     std::vector<void *> owned;  // device allocations to free
@@ -95,7 +96,8 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
         return fail(nullptr, RAD_EINVAL, "rad_create: bad gamma_gas / a_rad / n0_crit");
     if (p->recon_space < 0 || p->recon_space > 1) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: recon_space must be 0 (DC) or 1 (PLM)");
     if (p->recon_angle != 0) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: only donor-cell angular reconstruction is implemented");
-    if (p->tau_factor != 0.0) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: only tau_factor = 0 (Eq.24) is implemented");
+    if (!std::isfinite(p->tau_factor) || p->tau_factor < 0.0) return fail(nullptr, RAD_EINVAL, "rad_create: tau_factor must be finite and >= 0");
+    if (p->tau_factor != 0.0 && (!o || !o->alpha_a_energy || !o->alpha_s)) return fail(nullptr, RAD_EINVAL, "rad_create: tau_factor != 0 needs opacities");
     if (p->couple && (!o || !o->alpha_a_planck || !o->alpha_a_energy || !o->alpha_s)) return fail(nullptr, RAD_EINVAL, "rad_create: coupling needs opacities");
 
     int ndev = 0;
@@ -110,7 +112,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     if (!c) return fail(nullptr, RAD_ENOMEM, "rad_create: out of host memory");
     c->device = device; c->metric = *m; c->grid = *g; c->angles = *a; c->params = *p;
     if (o) c->opac = *o;
-    c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit; c->kp.rgm1 = 1.0 / (p->gamma_gas - 1.0);
+    c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit; c->kp.rgm1 = 1.0 / (p->gamma_gas - 1.0); c->kp.tau_factor = p->tau_factor;
     c->kp.recon_space = p->recon_space; c->kp.renorm = p->renorm_fluid_weights; c->kp.couple = p->couple;
     std::string err;
     bool ok = (a->kind == 0) ? rad::build_latlon(a->nzeta, a->npsi, c->host, err)
@@ -232,6 +234,7 @@ void rad_destroy(rad_ctx *c) {
     for (int q = 0; q < 3; q++) if (c->hs[q]) cudaStreamDestroy(c->hs[q]);
     if (c->ke) cudaFree(c->ke);
     if (c->rec) cudaFree(c->rec);
+    if (c->vel) cudaFree(c->vel);
     delete c;
 }
 
@@ -252,6 +255,7 @@ rad_status rad_transport(rad_ctx *c, double *I_in, double *I_out, const double *
     if (!c || !I_in || !I_out) return fail(c, RAD_EINVAL, "rad_transport: NULL argument");
     if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_transport: I_out must not alias I_in or I0 (the stencil reads old values)");
     if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_transport: non-finite weights");
+    if (c->kp.tau_factor != 0.0) return fail(c, RAD_ESTATE, "rad_transport: with tau_factor != 0 the spatial flux needs the fluid state (Eq.26-29): use rad_stage");
     DeviceGuard guard(c->device);
     rad_status st = rad_fill_ghosts(c, I_in, stream);
     if (st != RAD_OK) return st;
@@ -287,6 +291,26 @@ rad_status rad_couple(rad_ctx *c, double *I, const double *fluid, double dt, dou
 rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
                      double beta_dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
     if (!c || !fluid) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
+    if (c->kp.tau_factor != 0.0) {
+        // optical-depth-aware spatial flux (Eq.26-29): velocity table of all cells, then the two-kernel path
+        if (!I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
+        if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_stage: I_out must not alias I_in or I0 (the stencil reads old values)");
+        if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_stage: non-finite weights");
+        if (!c->opac.alpha_a_energy || !c->opac.alpha_s) return fail(c, RAD_ESTATE, "rad_stage: context has no opacities");
+        DeviceGuard guard(c->device);
+        cudaStream_t s = (cudaStream_t)stream;
+        if (!c->vel && cudaMalloc((void **)&c->vel, sizeof(double) * 5 * (size_t)c->dev.ncell) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(c, RAD_ENOMEM, "rad_stage: no device memory for the velocity table");
+        }
+        rad_status st = rad_fill_ghosts(c, I_in, stream);
+        if (st != RAD_OK) return st;
+        int nl = rad::launch_cell_velocity(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->vel, s);
+        if (nl > 0) { c->launches += nl; nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, s, c->vel, c->kp.tau_factor * beta_dt); }
+        if (nl < 0) return cuda_fail(c, "rad_stage (optical-depth-aware flux)");
+        c->launches += nl;
+        return rad_couple(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot, stream);
+    }
     if (c->dev.fused_ok && c->dev.ke && c->dev.N <= 256) {
         // one launch: flux divergence + coupling + mask (stage.cu)
         if (!I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
@@ -328,7 +352,7 @@ rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, 
 static rad_status stage_host_pipelined(rad_ctx *c, const double *I_in_host, double *I_out_host, const double *fluid_host, const double *opac_host,
                                        double gam0, double gam1, double beta_dt, double *T_out_host, double *dT0_host, long long *n_noroot) {
     const rad::DeviceTables &t = c->dev;
-    if (!rad::stage_angle_serves(t)) return RAD_EUNSUPPORTED;
+    if (!rad::stage_angle_serves(t) || c->kp.tau_factor != 0.0) return RAD_EUNSUPPORTED;
     for (int d = 0; d < 3; d++)
         if (c->grid.bc_lo[d] != 0 || c->grid.bc_hi[d] != 0) return RAD_EUNSUPPORTED;
     const int nz = t.n[2], ng = t.ng;

@@ -80,6 +80,7 @@ struct StageArgs {
 struct Params {
     double gamma_gas, a_rad, n0_crit;
     double rgm1;  // 1 / (gamma_gas - 1)
+    double tau_factor;  // constant of Eq.26; 0 = free-streaming flux (Eq.24)
     int recon_space, renorm, couple;
 };
 
@@ -88,7 +89,9 @@ int launch_geometry(const rad_metric &m, const rad_grid &g, double *cell, double
                     cudaStream_t s);
 int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_hi[3], double *I, cudaStream_t s);
 int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, const double *I0, double gam0,
-                   double gam1, double beta_dt, double *I_out, cudaStream_t s);
+                   double gam1, double beta_dt, double *I_out, cudaStream_t s, const double *vel = nullptr, double tau_dt = 0.0);
+// optical-depth-aware flux (NEXT-1, Eq.26-29): per-cell {u^alphahat, alpha_E} of every cell, vel[ncell][5]
+int launch_cell_velocity(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double *vel, cudaStream_t s);
 int launch_coupling(const DeviceTables &t, const Params &p, double *I, const double *fluid, const double *aP,
                     const double *aE, const double *aS, double dt, double *T_out, double *dT0,
                     unsigned long long *noroot, cudaStream_t s);

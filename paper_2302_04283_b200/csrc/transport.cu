@@ -60,9 +60,13 @@ __device__ __forceinline__ double vl_slope(double qm, double q0, double qp) {
     return pr > 0.0 ? 2.0 * pr / (dl + dr) : 0.0;
 }
 
-// flux through the face whose record is `f`, between cells L (lower) and R (upper) along a stride `st`
-template <bool PLM>
-__device__ __forceinline__ double face_flux(const double *f, double n1, double n2, double n3, const double *__restrict__ pR, long long st) {
+// flux through the face whose record is `f`, between cells L (lower) and R (upper) along a stride `st`.
+// TAU: the optical-depth-aware flux of Eq.26-29 (readings R15-R18, G1 in DESIGN.md): vL, vR = {u^alphahat (4),
+// alpha_E} of the two cells, tau = tau_dt (alpha_E,L + alpha_E,R)/2 / ((u^0hat_L + u^0hat_R)/2), f = -expm1(-tau^2),
+// g_L/R = -f (1 + 1/n^0bar_L/R), g = (g_L + g_R)/2, the upwind intensity is multiplied by 1 - g_up + g.
+template <bool PLM, bool TAU>
+__device__ __forceinline__ double face_flux(const double *f, double n1, double n2, double n3, const double *__restrict__ pR, long long st,
+                                            const double *__restrict__ vL, const double *__restrict__ vR, double tau_dt) {
     const double na = chain4(f, n1, n2, n3), n0 = chain4(f + 4, n1, n2, n3);
     double up;
     if (na > 0.0) {
@@ -76,12 +80,37 @@ __device__ __forceinline__ double face_flux(const double *f, double n1, double n
     } else {
         return 0.0;
     }
+    if (TAU) {
+        const double aE = 0.5 * (vL[4] + vR[4]), v0 = 0.5 * (vL[0] + vR[0]);
+        const double tau = tau_dt * aE / v0;                                         // Eq.26
+        const double fint = -expm1(-tau * tau);                                      // Eq.27 (G1)
+        const double nbL = vL[0] - (vL[1] * n1 + vL[2] * n2 + vL[3] * n3);           // n^0bar_L
+        const double nbR = vR[0] - (vR[1] * n1 + vR[2] * n2 + vR[3] * n3);
+        const double gL = -fint * (1.0 + 1.0 / nbL), gR = -fint * (1.0 + 1.0 / nbR);  // Eq.29
+        const double g = 0.5 * (gL + gR);
+        up *= (na > 0.0) ? (1.0 - gL + g) : (1.0 - gR + g);                          // Eq.28
+    }
     return na * n0 * up;
 }
 
-template <bool PLM>
+// tetrad-frame fluid velocity and alpha_E of EVERY cell (ghosts included), vel[cell][5], for the optical-depth-aware flux:
+// u^ahat = theta^ahat_j u^j' (co-triad of the cell record), u^0hat = sqrt(1 + |u^ahat|^2) (R10), alpha_E = alpha^a_E + alpha^s
+__global__ void __launch_bounds__(256) k_cell_velocity(DeviceTables t, const double *__restrict__ fluid, const double *__restrict__ aE,
+                                                       const double *__restrict__ aS, double *__restrict__ vel) {
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < t.ncell; c += (long long)gridDim.x * blockDim.x) {
+        const double *th = t.cell + c * RAD_NCELL + 44;
+        const double u1 = fluid[2 * t.ncell + c], u2 = fluid[3 * t.ncell + c], u3 = fluid[4 * t.ncell + c];
+        const double h1 = th[0] * u1 + th[1] * u2 + th[2] * u3, h2 = th[3] * u2 + th[4] * u3, h3 = th[5] * u3;
+        vel[5 * c] = sqrt(1.0 + (h1 * h1 + h2 * h2 + h3 * h3));
+        vel[5 * c + 1] = h1; vel[5 * c + 2] = h2; vel[5 * c + 3] = h3;
+        vel[5 * c + 4] = aE[c] + aS[c];
+    }
+}
+
+template <bool PLM, bool TAU>
 __global__ void __launch_bounds__(256) k_fluxdiv_v1(DeviceTables t, const double *__restrict__ I_in, const double *__restrict__ I0,
-                                                   double gam0, double gam1, double beta_dt, double *__restrict__ I_out) {
+                                                   double gam0, double gam1, double beta_dt, double *__restrict__ I_out,
+                                                   const double *__restrict__ vel, double tau_dt) {
     extern __shared__ double smem[];
     const int N = t.N, E = t.E;
     double *sCell = smem;                 // [CX][36]: n^0, E[4], S[30], excised
@@ -139,9 +168,13 @@ __global__ void __launch_bounds__(256) k_fluxdiv_v1(DeviceTables t, const double
         const double *p = I_in + c * N + n;
         const long long sx = N;
         double div = 0.0;
-        div += (face_flux<PLM>(sFx + (cl + 1) * 8, n1, n2, n3, p + sx, sx) - face_flux<PLM>(sFx + cl * 8, n1, n2, n3, p, sx)) * t.inv_dx[0];
-        div += (face_flux<PLM>(sFy + CX * 8 + cl * 8, n1, n2, n3, p + sy * N, sy * N) - face_flux<PLM>(sFy + cl * 8, n1, n2, n3, p, sy * N)) * t.inv_dx[1];
-        div += (face_flux<PLM>(sFz + CX * 8 + cl * 8, n1, n2, n3, p + sz * N, sz * N) - face_flux<PLM>(sFz + cl * 8, n1, n2, n3, p, sz * N)) * t.inv_dx[2];
+        const double *vc = TAU ? vel + 5 * c : nullptr;  // this cell's velocity record; the neighbours' are 5 * stride away
+        div += (face_flux<PLM, TAU>(sFx + (cl + 1) * 8, n1, n2, n3, p + sx, sx, vc, vc + 5, tau_dt) -
+                face_flux<PLM, TAU>(sFx + cl * 8, n1, n2, n3, p, sx, vc - 5, vc, tau_dt)) * t.inv_dx[0];
+        div += (face_flux<PLM, TAU>(sFy + CX * 8 + cl * 8, n1, n2, n3, p + sy * N, sy * N, vc, vc + 5 * sy, tau_dt) -
+                face_flux<PLM, TAU>(sFy + cl * 8, n1, n2, n3, p, sy * N, vc - 5 * sy, vc, tau_dt)) * t.inv_dx[1];
+        div += (face_flux<PLM, TAU>(sFz + CX * 8 + cl * 8, n1, n2, n3, p + sz * N, sz * N, vc, vc + 5 * sz, tau_dt) -
+                face_flux<PLM, TAU>(sFz + cl * 8, n1, n2, n3, p, sz * N, vc - 5 * sz, vc, tau_dt)) * t.inv_dx[2];
         double adiv = 0.0;
 #pragma unroll
         for (int s = 0; s < RAD_MAXNBR; s++) {
@@ -172,18 +205,25 @@ int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_h
     return launches;
 }
 
+int launch_cell_velocity(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double *vel, cudaStream_t s) {
+    k_cell_velocity<<<148 * 4, 256, 0, s>>>(t, fluid, aE, aS, vel);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+// vel != nullptr: optical-depth-aware flux (Eq.26-29) with tau_dt = tau_factor * beta_dt
 int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, const double *I0, double gam0, double gam1,
-                   double beta_dt, double *I_out, cudaStream_t s) {
+                   double beta_dt, double *I_out, cudaStream_t s, const double *vel, double tau_dt) {
     const int nxb = (t.n[0] + CX - 1) / CX;
     const long long blocks = (long long)nxb * t.n[1] * t.n[2];
     const size_t smem = sizeof(double) * (CX * 36 + (CX + 1) * 8 + 4 * CX * 8 + (size_t)CX * t.E);
-    if (p.recon_space == 1) {
-        cudaFuncSetAttribute(k_fluxdiv_v1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        k_fluxdiv_v1<true><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out);
-    } else {
-        cudaFuncSetAttribute(k_fluxdiv_v1<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        k_fluxdiv_v1<false><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out);
-    }
+#define RAD_LAUNCH_FD(PLM, TAU)                                                                                     \
+    do {                                                                                                            \
+        cudaFuncSetAttribute(k_fluxdiv_v1<PLM, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+        k_fluxdiv_v1<PLM, TAU><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out, vel, tau_dt); \
+    } while (0)
+    if (p.recon_space == 1) { if (vel) RAD_LAUNCH_FD(true, true); else RAD_LAUNCH_FD(true, false); }
+    else { if (vel) RAD_LAUNCH_FD(false, true); else RAD_LAUNCH_FD(false, false); }
+#undef RAD_LAUNCH_FD
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -61,7 +61,10 @@ def test_no_gpu_means_error_not_fallback(so):
     assert e.value.status == 4  # RAD_EUNSUPPORTED
     with pytest.raises(B.RadError) as e:
         B.rad_create(dict(kind=0), grid, ("latlon", 2, 4), None, dict(couple=0, tau_factor=1.0))
-    assert e.value.status == 4
+    assert e.value.status == 1  # RAD_EINVAL: the optical-depth-aware flux (Eq.26-29) needs opacities
+    with pytest.raises(B.RadError) as e:
+        B.rad_create(dict(kind=0), grid, ("latlon", 2, 4), None, dict(couple=0, tau_factor=-1.0))
+    assert e.value.status == 1
     with pytest.raises(B.RadError) as e:
         B.rad_create(dict(kind=0), grid, ("latlon", 2, 4), None, dict(couple=1))
     assert e.value.status == 1  # coupling needs opacities

@@ -387,3 +387,28 @@ def test_three_stages_ping_pong(oracle, B):
             P.interior(dfl[1].reshape(P.shape))[...] = torch.as_tensor(P.interior(T_o)).cuda()
     finally:
         B.rad_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-1: Eq.26-29
+@pytest.mark.parametrize("n,angles,kind,tau", [((7, 6, 5), ("geodesic", 2), 1, 2.0), ((9, 4, 6), ("geodesic", 4), 1, 0.5), ((5, 5, 5), ("latlon", 4, 8), 0, 10.0)])
+def test_optical_depth_flux_parity(oracle, B, n, angles, kind, tau):
+    """stage with the optical-depth-aware spatial flux (tau_factor != 0): CUDA path against the oracle, same tolerances"""
+    A = oracle.Angles(*angles)
+    P = oracle.Problem(A, n, (3.0, 2.0, 1.0), (0.3, 0.25, 0.2), metric_kind=kind, M=1.0, a=0.9 if kind else 0.0, tau_factor=tau)
+    rng = np.random.default_rng(7)
+    nc = P.ncell
+    I = np.exp(rng.normal(size=(nc, A.N)))
+    fluid = np.stack([rng.uniform(0.5, 2, nc), rng.uniform(0.3, 1.5, nc)] + [rng.uniform(-0.4, 0.4, nc) for _ in range(3)])
+    opac = np.stack([rng.uniform(0.1, 30, nc)] * 2 + [rng.uniform(0.1, 30, nc)])
+    d_opac = dev(opac)
+    h = B.rad_create(dict(kind=kind, M=1.0, a=0.9 if kind else 0.0), dict(n=n, x0=(3.0, 2.0, 1.0), dx=(0.3, 0.25, 0.2)), angles,
+                     (d_opac[0], d_opac[1], d_opac[2]), dict(tau_factor=tau))
+    try:
+        got, ref = compare_stage(B, A, P, h, I, fluid, opac, 0.02)
+        free = oracle.Problem(A, n, (3.0, 2.0, 1.0), (0.3, 0.25, 0.2), metric_kind=kind, M=1.0, a=0.9 if kind else 0.0).stage(I.copy(), fluid, opac, 0.02)[0]
+        assert np.abs(P.interior(ref) - P.interior(free)).max() > 1e-6   # the flux factor did something
+        with pytest.raises(B.RadError) as e:   # the transport half alone has no fluid state
+            B.rad_transport(h, dev(I), torch.zeros_like(dev(I)), None, 0.0, 1.0, 0.02)
+        assert e.value.status == 5
+    finally:
+        B.rad_destroy(h)
