@@ -115,14 +115,14 @@ class OracleSample:
     """the oracle, as it stands, on the nsub^3 cells at the low corner of the workload's block (same spacing, own ghosts,
     same input recipe); built once, each run() is one full stage on the same inputs"""
 
-    def __init__(self, cfg, nsub):
+    def __init__(self, cfg, nsub, tau_factor=0.0):
         from oracle import rad_oracle as O
         from paper_2302_04283_b200 import workloads as W
         c = W.CONFIGS[cfg]
         A = O.Angles(*c["angles"])
         nn, ng, x0, dx = W.grid(cfg, sub=nsub)
         self.P = O.Problem(A, nn, x0, dx, metric_kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg),
-                           bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3)
+                           bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3, tau_factor=tau_factor)
         inp = W.make_inputs(cfg, A.nhat, sub=nsub)
         self.I = inp["I"].numpy().reshape(-1, A.N).copy()
         self.fluid = inp["fluid"].numpy().reshape(5, -1).copy(); self.opac = inp["opac"].numpy().reshape(3, -1).copy()
@@ -146,7 +146,7 @@ def run_reference(args):
     nsub = args.ref_n or 64
     N = W.n_angles(cfg)
     cores = os.cpu_count()
-    smp = OracleSample(cfg, nsub)
+    smp = OracleSample(cfg, nsub, args.tau_factor)
     for _ in range(args.warmup):
         smp.run()
     times = [smp.run() for _ in range(args.steps)]
@@ -171,6 +171,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-n", type=int, default=None, help="sub-block size of the oracle sample (default: 64 for --impl reference, 96 for the cpu_baseline leg)")
     ap.add_argument("--recon", type=int, default=1, help="spatial reconstruction: 1 PLM (the workload's), 0 donor cell (diagnostic)")
+    ap.add_argument("--tau-factor", type=float, default=0.0, help="constant of Eq.26: > 0 times the stage with the optical-depth-aware flux (NEXT-1; separate kernels)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -218,7 +219,7 @@ def main():
     T_out = torch.zeros(ncell, dtype=torch.float64, device="cuda"); dT0 = torch.zeros(4, ncell, dtype=torch.float64, device="cuda")
     h = B.rad_create(dict(kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg)),
                      dict(n=nn, x0=x0, dx=dx, bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3), c["angles"], (opac[0], opac[1], opac[2]),
-                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=args.recon, renorm_fluid_weights=1, couple=1), local)
+                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=args.recon, renorm_fluid_weights=1, couple=1, tau_factor=args.tau_factor), local)
     vmax = float(B.rad_get_table(h, B.TAB_MAXSPEED).max())
     dt = W.CFL * min(dx) / vmax
     stream = torch.cuda.current_stream()
@@ -265,8 +266,10 @@ def main():
         return a.elapsed_time(b) / reps
 
     reps = max(3, args.steps)
-    ms_flux = time_call(lambda: B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream), reps)
-    B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream)
+    ms_flux = None
+    if args.tau_factor == 0.0:  # (with the optical-depth-aware flux the transport half alone has no fluid state)
+        ms_flux = time_call(lambda: B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream), reps)
+        B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream)
     ms_cpl = time_call(lambda: B.rad_couple(h, I_b, fluid, dt, T_out, dT0, stream=stream), reps)
     # roofline of the dominant kernel = the fused stage kernel k_stage (flux divergence + coupling in one launch): with
     # caller-filled ghosts it is the only kernel of a step, so its average launch duration is the CUDA-event time of the
@@ -275,7 +278,9 @@ def main():
     peak, peak_src = measured_peak()
     bpu = algorithmic_bytes_per_update(N)
     achieved = bpu * updates / (ms * 1e-3) / 1e9
-    roofline = {"kernel": "k_stage5 (fused flux divergence + implicit coupling + mask, one launch per step)", "bound": "hbm",
+    kname = "k_stage5 (fused flux divergence + implicit coupling + mask, one launch per step)" if args.tau_factor == 0.0 else \
+        "k_cell_velocity + k_fluxdiv_v1 (Eq.26-29 flux) + k_coupling_w: the step's three kernels together"
+    roofline = {"kernel": kname, "bound": "hbm",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg, args.n, args.recon)),
                 "traffic_source": "ncu --set full capture, profiles/r1_k_stage5_ncu_full.md (bytes per launch)" if (cfg, args.n, args.recon) in NCU_TRAFFIC_BYTES else None,
                 "peak_source": peak_src,
@@ -285,7 +290,7 @@ def main():
                 "flux_divergence_only_ms": ms_flux, "standalone_coupling_kernel_ms": ms_cpl}
     dfma = B.rad_probe_fp64(h)
     slots = FP64_SLOTS_PER_UPDATE[True]
-    roofline_alu = {"kernel": roofline["kernel"], "bound": "alu", "unit": "TFLOP/s", "peak": 2.0 * dfma / 1e12,
+    roofline_alu = {"kernel": kname, "bound": "alu", "unit": "TFLOP/s", "peak": 2.0 * dfma / 1e12,
                     "peak_source": "measured live: rad_probe_fp64 (register-only DFMA kernel, CUDA events)",
                     "achieved": 2.0 * slots * updates / (ms * 1e-3) / 1e12, "fp64_slots_per_update": slots,
                     "note": "one FP64-pipe instruction slot per lane = 2 flop (DFMA-equivalent)"}
@@ -319,7 +324,7 @@ def main():
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         nsub = args.ref_n or 96
-        smp = OracleSample(cfg, nsub)
+        smp = OracleSample(cfg, nsub, args.tau_factor)
         smp.run()
         secs = [smp.run() for _ in range(2)]
         sec = sum(secs)
@@ -329,7 +334,7 @@ def main():
     line = {"metric": METRIC, "value": whole_job_value(updates, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{cfg}: {c['angles']} angles={N}, {nn[0]}^3 cells + 2 ghosts, metric kind {c['metric']} a={c['a']}, box {c['box']}",
-                       "updates_per_step": updates, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "updates_per_step": updates, "tau_factor": args.tau_factor, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs (2 x %.2f GB) exceed L2; no flush" % (I_a.numel() * 8 / 1e9)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_alu": roofline_alu,
             "cpu_baseline": cpu}
