@@ -306,7 +306,31 @@ rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, 
         rad_status st = rad_fill_ghosts(c, I_in, stream);
         if (st != RAD_OK) return st;
         int nl = rad::launch_cell_velocity(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->vel, s);
-        if (nl > 0) { c->launches += nl; nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, s, c->vel, c->kp.tau_factor * beta_dt); }
+        if (nl < 0) return cuda_fail(c, "rad_stage (velocity table)");
+        c->launches += nl;
+        static const bool split = [] { const char *e = std::getenv("RAD_TAU_SPLIT"); return e && e[0] == '1'; }();
+        if (!split && c->kp.couple && c->opac.alpha_a_planck) {
+            // fused warp-per-cell stage kernel (stage.cu) with the Eq.28 factor; serves N <= 192 with stored coefficients
+            if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
+            rad::StageArgs a{};
+            a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
+            a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
+            a.T_out = T_out; a.dT0 = dT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
+            a.vel = c->vel; a.tau_dt = c->kp.tau_factor * beta_dt;
+            nl = rad::launch_stage_fused(c->dev, c->kp, a, true, s);
+            if (nl < 0) return cuda_fail(c, "rad_stage (optical-depth-aware flux, fused)");
+            if (nl > 0) {
+                c->launches += nl;
+                if (n_noroot) {
+                    unsigned long long v = 0;
+                    if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+                        return cuda_fail(c, "rad_stage: readback");
+                    *n_noroot = (long long)v;
+                }
+                return RAD_OK;
+            }
+        }
+        nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, s, c->vel, c->kp.tau_factor * beta_dt);
         if (nl < 0) return cuda_fail(c, "rad_stage (optical-depth-aware flux)");
         c->launches += nl;
         return rad_couple(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot, stream);

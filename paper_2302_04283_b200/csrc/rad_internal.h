@@ -74,6 +74,8 @@ struct StageArgs {
     const double *fluid, *aP, *aE, *aS;  // coupling only
     double *T_out, *dT0;
     unsigned long long *noroot;
+    const double *vel;  // stage.cu only: optical-depth-aware flux (Eq.26-29), {u^alphahat, alpha_E} per cell, or nullptr (Eq.24)
+    double tau_dt;      // tau_factor * beta_dt
     int kz0, kz1;  // stage5 only: update the interior planes kz0 <= k < kz1 (0-based, without ghosts); kz1 <= kz0 = the whole block
 };
 

@@ -60,9 +60,12 @@ __device__ __forceinline__ FaceRec load_face_s(const double *f) {  // shared mem
 // (far, mid, oth) = (LL, L, R) for n^a > 0 and (RR, R, L) otherwise, the face value is mid + dl dr / (dl + dr),
 // dl = mid - far, dr = oth - mid (the harmonic mean is odd under reversal, so one formula serves both signs).
 // Branch free; the two products are never contracted, so the two cells that share a face get the same bits.
-template <bool PLM>
+// TAU: optical-depth-aware flux (Eq.26-29; readings R15-R18, G1 in DESIGN.md).  With G_c = -(1 + 1/n^0bar_c) per cell and
+// angle and f the interpolating factor of the face, g_L/R = f G_L/R, g = (g_L + g_R)/2, and the factor of Eq.28,
+// 1 - g_up + g, is 1 + (f/2) (G_R - G_L) for n^a > 0 and 1 + (f/2) (G_L - G_R) otherwise; fh = f/2.
+template <bool PLM, bool TAU>
 __device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double n2, double n3, double qLL, double qL, double qR,
-                                            double qRR) {
+                                            double qRR, double GL = 0.0, double GR = 0.0, double fh = 0.0) {
     const double na = chain4(f.e0, f.e1, f.e2, f.e3, n1, n2, n3);
     const double n0 = chain4(f.E0, f.E1, f.E2, f.E3, n1, n2, n3);
     const bool pos = na > 0.0;
@@ -73,7 +76,19 @@ __device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double 
         const double h = pr * fast_rcp(dl + dr);
         up += pr > 0.0 ? h : 0.0;
     }
+    if (TAU) up *= fma(fh, pos ? GR - GL : GL - GR, 1.0);
     return __dmul_rn(__dmul_rn(na, n0), up);  // n^a = 0 gives 0 for finite intensities
+}
+
+// G = -(1 + 1/n^0bar) of one cell for one angle; v = {u^0hat, u^1hat, u^2hat, u^3hat} of the cell (Eq.29)
+__device__ __forceinline__ double tau_G(const double *v, double n1, double n2, double n3) {
+    const double nb = v[0] - (v[1] * n1 + v[2] * n2 + v[3] * n3);
+    return -(1.0 + fast_rcp(nb));
+}
+// f/2 of a face between cells L and R (Eq.26-27): vL, vR = {u^alphahat (4), alpha_E}
+__device__ __forceinline__ double tau_fh(const double *vL, const double *vR, double tau_dt) {
+    const double tau = tau_dt * (0.5 * (vL[4] + vR[4])) / (0.5 * (vL[0] + vR[0]));
+    return -0.5 * expm1(-tau * tau);
 }
 
 // v[it] = row[angle of (lane, it)]; lanes past the last angle re-read angle N-1 (last_off)
@@ -87,7 +102,7 @@ __device__ __forceinline__ void load_row(const double *__restrict__ row, int lan
 __device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
-template <int NITER, bool PLM, bool COUPLE>
+template <int NITER, bool PLM, bool COUPLE, bool TAU>
 __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, const Params p, const StageArgs a, const int KX) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = t.N, Np = (N + 2) & ~1;  // even, > N: slot N of a row is scratch
@@ -96,8 +111,8 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, cons
     double *sm = reinterpret_cast<double *>(smem_raw);
     double *sI = sm + (size_t)w * 4 * Np;                    // [Np]    this warp's cell, all angles
     double *sG = sI + Np;                                    // [3*N+1] fluxes of owned edges, position j*N + n; [3N] = 0
-    double *sU = sm + (size_t)NW * 4 * Np + (size_t)w * 64;  // [64] this cell's warp-uniform records (see below)
-    double *sWinv = sm + (size_t)NW * (4 * Np + 64);         // [Np] 1/dOmega
+    double *sU = sm + (size_t)NW * 4 * Np + (size_t)w * 128;  // [128] this cell's warp-uniform records (see below)
+    double *sWinv = sm + (size_t)NW * (4 * Np + 128);         // [Np] 1/dOmega
     double *sDom = sWinv + Np;                               // [Np] dOmega
     uint4 *sRec = reinterpret_cast<uint4 *>(sDom + Np);      // [N]  {own_partner[3], pull_pos[3]} as uint16
     for (int q = threadIdx.x; q < N; q += blockDim.x) {
@@ -130,8 +145,16 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, cons
         double qLL[NITER], qL[NITER], qR[NITER], qRR[NITER];
         load_row<NITER>(Ic - N, lane, last_off, qL); load_row<NITER>(Ic, lane, last_off, qR);
         if (PLM) { load_row<NITER>(Ic - 2 * N, lane, last_off, qLL); load_row<NITER>(Ic + N, lane, last_off, qRR); }
+        double vL[5] = {1.0, 0.0, 0.0, 0.0, 0.0}, vR[5] = {1.0, 0.0, 0.0, 0.0, 0.0}, fh = 0.0;
+        if (TAU) {
 #pragma unroll
-        for (int it = 0; it < NITER; it++) carry[it] = face_flux<PLM>(f, n1[it], n2[it], n3[it], PLM ? qLL[it] : 0.0, qL[it], qR[it], PLM ? qRR[it] : 0.0);
+            for (int r = 0; r < 5; r++) { vL[r] = __ldg(a.vel + 5 * (c - 1) + r); vR[r] = __ldg(a.vel + 5 * c + r); }
+            fh = tau_fh(vL, vR, a.tau_dt);
+        }
+#pragma unroll
+        for (int it = 0; it < NITER; it++)
+            carry[it] = face_flux<PLM, TAU>(f, n1[it], n2[it], n3[it], PLM ? qLL[it] : 0.0, qL[it], qR[it], PLM ? qRR[it] : 0.0,
+                                            TAU ? tau_G(vL, n1[it], n2[it], n3[it]) : 0.0, TAU ? tau_G(vR, n1[it], n2[it], n3[it]) : 0.0, fh);
     }
 
     // Warp-uniform records of a cell, gathered two per lane in one round trip and broadcast through shared memory:
@@ -179,14 +202,28 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, cons
             double q0[NITER], q1[NITER], q2[NITER];
             const double uA = __ldg(ptrA), uB = __ldg(ptrB);
             ptrA += 3 * RAD_NFACE; ptrB += strideB;
+            double uV = 0.0;  // TAU: {u^alphahat, alpha_E} of this cell and its +x, -y, +y, -z, +z neighbours, one double per lane
+            if (TAU && lane < 30) {
+                const int q = lane / 5;
+                const long long cq = c + (q == 1 ? 1 : (q == 2 ? -(long long)t.NI : (q == 3 ? (long long)t.NI : (q == 4 ? -(long long)t.NI * t.NJ : (q == 5 ? (long long)t.NI * t.NJ : 0)))));
+                uV = __ldg(a.vel + 5 * cq + (lane - 5 * q));
+            }
             load_row<NITER>(Ic, lane, last_off, Iown);
             load_row<NITER>(kec, lane, last_off, q0); load_row<NITER>(kec + N, lane, last_off, q1); load_row<NITER>(kec + 2 * N, lane, last_off, q2);
             __syncwarp();  // the previous step's readers of sI / sG / sU are done
             sU[lane] = uA; sU[32 + lane] = uB;
+            if (TAU) sU[64 + lane] = uV;
 #pragma unroll
             for (int it = 0; it < NITER; it++)
                 if (it < NITER - 1 || last_valid) sI[it * 32 + lane] = Iown[it];
             __syncwarp();
+            if (TAU) {  // f/2 of the five faces computed below: x above (0,1), y below (2,0), y above (0,3), z below (4,0), z above (0,5)
+                if (lane < 5) {
+                    const int L = lane == 1 ? 2 : (lane == 3 ? 4 : 0), R = lane == 0 ? 1 : (lane == 2 ? 3 : (lane == 4 ? 5 : 0));
+                    sU[96 + lane] = tau_fh(sU + 64 + 5 * L, sU + 64 + 5 * R, a.tau_dt);
+                }
+                __syncwarp();
+            }
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
                 const int n = it < NITER - 1 ? it * 32 + lane : last_off;
@@ -212,6 +249,9 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, cons
                 div[it] = asum * sWinv[n];
             }
         }
+        double G0[NITER];  // TAU: G of this cell per angle
+#pragma unroll
+        for (int it = 0; it < NITER; it++) G0[it] = TAU ? tau_G(sU + 64, n1[it], n2[it], n3[it]) : 0.0;
         // ---- x: flux through the upper face (the lower x face of cell i+1); the lower one is carried
         {
             const FaceRec f = load_face_s(sU);
@@ -220,7 +260,8 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, cons
             if (PLM) { load_row<NITER>(Ic - N, lane, last_off, qLL); load_row<NITER>(Ic + 2 * N, lane, last_off, qRR); }
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const double F = face_flux<PLM>(f, n1[it], n2[it], n3[it], PLM ? qLL[it] : 0.0, Iown[it], qR[it], PLM ? qRR[it] : 0.0);
+                const double F = face_flux<PLM, TAU>(f, n1[it], n2[it], n3[it], PLM ? qLL[it] : 0.0, Iown[it], qR[it], PLM ? qRR[it] : 0.0, G0[it],
+                                                     TAU ? tau_G(sU + 69, n1[it], n2[it], n3[it]) : 0.0, TAU ? sU[96] : 0.0);
                 div[it] = fma(F - carry[it], idx0, div[it]);
                 carry[it] = F;
             }
@@ -236,8 +277,9 @@ __global__ void __launch_bounds__(NW * 32, 1) k_stage(const DeviceTables t, cons
             if (PLM) { load_row<NITER>(Ic - 2 * st, lane, last_off, m2); load_row<NITER>(Ic + 2 * st, lane, last_off, p2); }
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const double Flo = face_flux<PLM>(flo, n1[it], n2[it], n3[it], PLM ? m2[it] : 0.0, m1[it], Iown[it], p1[it]);
-                const double Fhi = face_flux<PLM>(fhi, n1[it], n2[it], n3[it], m1[it], Iown[it], p1[it], PLM ? p2[it] : 0.0);
+                const double Glo = TAU ? tau_G(sU + (ax == 1 ? 74 : 84), n1[it], n2[it], n3[it]) : 0.0, Ghi = TAU ? tau_G(sU + (ax == 1 ? 79 : 89), n1[it], n2[it], n3[it]) : 0.0;
+                const double Flo = face_flux<PLM, TAU>(flo, n1[it], n2[it], n3[it], PLM ? m2[it] : 0.0, m1[it], Iown[it], p1[it], Glo, G0[it], TAU ? sU[ax == 1 ? 97 : 99] : 0.0);
+                const double Fhi = face_flux<PLM, TAU>(fhi, n1[it], n2[it], n3[it], m1[it], Iown[it], p1[it], PLM ? p2[it] : 0.0, G0[it], Ghi, TAU ? sU[ax == 1 ? 98 : 100] : 0.0);
                 div[it] = fma(Fhi - Flo, idx, div[it]);
             }
         }
@@ -329,15 +371,20 @@ __global__ void __launch_bounds__(256) k_build_ke(const DeviceTables t, double *
 
 size_t stage_smem_bytes(int N) {
     const int Np = (N + 2) & ~1;
-    return sizeof(double) * ((size_t)NW * (4 * Np + 64) + 2 * (size_t)Np) + sizeof(uint4) * (size_t)N;
+    return sizeof(double) * ((size_t)NW * (4 * Np + 128) + 2 * (size_t)Np) + sizeof(uint4) * (size_t)N;
 }
 
 template <int NITER>
 int launch_niter(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, dim3 grid, size_t smem, int KX, cudaStream_t s) {
 #define RAD_LAUNCH(PLM, CPL)                                                                                         \
     do {                                                                                                             \
-        if (cudaFuncSetAttribute(k_stage<NITER, PLM, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
-        k_stage<NITER, PLM, CPL><<<grid, NW * 32, smem, s>>>(t, p, a, KX);                                            \
+        if (a.vel != nullptr) {                                                                                      \
+            if (cudaFuncSetAttribute(k_stage<NITER, PLM, CPL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
+            k_stage<NITER, PLM, CPL, true><<<grid, NW * 32, smem, s>>>(t, p, a, KX);                                   \
+        } else {                                                                                                     \
+            if (cudaFuncSetAttribute(k_stage<NITER, PLM, CPL, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
+            k_stage<NITER, PLM, CPL, false><<<grid, NW * 32, smem, s>>>(t, p, a, KX);                                  \
+        }                                                                                                            \
     } while (0)
     if (p.recon_space == 1) { if (couple) RAD_LAUNCH(true, true); else RAD_LAUNCH(true, false); }
     else { if (couple) RAD_LAUNCH(false, true); else RAD_LAUNCH(false, false); }
