@@ -412,3 +412,26 @@ def test_optical_depth_flux_parity(oracle, B, n, angles, kind, tau):
         assert e.value.status == 5
     finally:
         B.rad_destroy(h)
+
+
+def test_optical_depth_flux_host_path_and_periodic(oracle, B):
+    """tau_factor != 0 through rad_stage_host (not pipelined: the flux needs the neighbours' fluid state) with periodic ghosts of I"""
+    A = oracle.Angles("geodesic", 3)
+    n, x0, dx = (6, 5, 9), (0.0, 0.0, 0.0), (0.2, 0.2, 0.2)
+    P = oracle.Problem(A, n, x0, dx, metric_kind=0, bc_lo=(1, 1, 1), bc_hi=(1, 1, 1), tau_factor=4.0)
+    rng = np.random.default_rng(3)
+    nc = P.ncell
+    I = np.exp(rng.normal(size=(nc, A.N)))
+    fluid = np.stack([rng.uniform(0.5, 2, nc), rng.uniform(0.3, 1.5, nc)] + [rng.uniform(-0.4, 0.4, nc) for _ in range(3)])
+    opac = np.stack([rng.uniform(0.1, 30, nc)] * 2 + [rng.uniform(0.1, 30, nc)])
+    d_opac = dev(opac)
+    h = B.rad_create(dict(kind=0), dict(n=n, x0=x0, dx=dx, bc_lo=(1, 1, 1), bc_hi=(1, 1, 1)), ("geodesic", 3), (d_opac[0], d_opac[1], d_opac[2]), dict(tau_factor=4.0))
+    try:
+        out_h = np.zeros_like(I); T_h = np.zeros(nc); dT0_h = np.zeros((4, nc))
+        nf = B.rad_stage_host(h, I, out_h, fluid, opac, 0.0, 1.0, 0.03, T_h, dT0_h, count_noroot=True)
+        out_o, T_o, dT0_o, nf_o = P.stage(I.copy(), fluid, opac, 0.03)
+        assert nf == nf_o
+        assert rel_err_I(P.interior(out_h), P.interior(out_o)) <= TOL_I
+        assert rel_err(P.interior(T_h), P.interior(T_o), 0.0) <= TOL_FLUID
+    finally:
+        B.rad_destroy(h)
