@@ -279,7 +279,7 @@ def main():
     bpu = algorithmic_bytes_per_update(N)
     achieved = bpu * updates / (ms * 1e-3) / 1e9
     kname = "k_stage5 (fused flux divergence + implicit coupling + mask, one launch per step)" if args.tau_factor == 0.0 else \
-        "k_cell_velocity + k_stage<TAU> (stage.cu: fused flux divergence with the Eq.28 factor + coupling): the step's two kernels together"
+        "k_tau_table + k_stage5<TAU> (tile kernel with the Eq.28 factor): the step's two kernels together"
     roofline = {"kernel": kname, "bound": "hbm",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg, args.n, args.recon)),
                 "traffic_source": "ncu --set full capture, profiles/r1_k_stage5_ncu_full.md (bytes per launch)" if (cfg, args.n, args.recon) in NCU_TRAFFIC_BYTES else None,

@@ -90,7 +90,7 @@ typedef struct {
     int couple;               /* 0 = transport only, 1 = with implicit coupling (section 2.5) */
     double tau_factor;        /* constant of Eq.26: 0 = free-streaming spatial flux (Eq.24); > 0 = optical-depth-aware flux
                                  (Eq.26-29; readings R15-R18, G1 in DESIGN.md).  Then rad_stage reads fluid and opacities in the first
-                                 ghost layer too, runs as a velocity-table kernel plus the warp-per-cell fused stage kernel, and
+                                 ghost layer too, runs as a per-cell table kernel plus the stage kernel, and
                                  rad_transport returns RAD_ESTATE (the flux needs the fluid state) */
     int recompute_edge_coeffs; /* stored-versus-recomputed angular geometry:
                                   0 = the angular-edge coefficients dlambda_e c_e n_0e (Eq.16-17, Eq.25) are built once

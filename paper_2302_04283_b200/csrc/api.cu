@@ -20,6 +20,7 @@ struct rad_ctx {
     rad::EdgeOwnership own;
     double *ke = nullptr;  // stored edge coefficients (owned)
     double *rec = nullptr; // packed per-cell records of the stage kernel (owned)
+    double *vel8 = nullptr; // optical-depth-aware flux in the tile kernel: {u^alphahat, f/2 of the upper faces} per cell (owned, allocated on first use)
     double *vel = nullptr; // optical-depth-aware flux: {u^alphahat, alpha_E} per cell (owned, allocated on first use)
     rad::DeviceTables dev{};
     rad::Params kp{};
@@ -235,6 +236,7 @@ void rad_destroy(rad_ctx *c) {
     if (c->ke) cudaFree(c->ke);
     if (c->rec) cudaFree(c->rec);
     if (c->vel) cudaFree(c->vel);
+    if (c->vel8) cudaFree(c->vel8);
     delete c;
 }
 
@@ -305,11 +307,39 @@ rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, 
         }
         rad_status st = rad_fill_ghosts(c, I_in, stream);
         if (st != RAD_OK) return st;
+        static const int tau_path = [] { const char *e = std::getenv("RAD_TAU_PATH"); return e ? std::atoi(e) : 0; }();  // 5 / 3 / 2: force a path (A/B runs)
+        if ((tau_path == 0 || tau_path == 5) && c->kp.couple && c->opac.alpha_a_planck && rad::stage_angle_serves(c->dev)) {
+            // the tile kernel (stage5.cu) with the Eq.28 factor: per-cell table {u^alphahat, f/2 of the upper faces}, then one launch
+            if (!c->vel8 && cudaMalloc((void **)&c->vel8, sizeof(double) * 8 * (size_t)c->dev.ncell) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(c, RAD_ENOMEM, "rad_stage: no device memory for the velocity table");
+            }
+            int nl5 = rad::launch_tau_table(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->kp.tau_factor * beta_dt, c->vel8, s);
+            if (nl5 < 0) return cuda_fail(c, "rad_stage (velocity table)");
+            c->launches += nl5;
+            if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
+            rad::StageArgs a{};
+            a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
+            a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
+            a.T_out = T_out; a.dT0 = dT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
+            a.vel8 = c->vel8;
+            nl5 = rad::launch_stage_angle(c->dev, c->kp, a, true, s);
+            if (nl5 < 0) return cuda_fail(c, "rad_stage (optical-depth-aware flux, tile kernel)");
+            if (nl5 > 0) {
+                c->launches += nl5;
+                if (n_noroot) {
+                    unsigned long long v = 0;
+                    if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+                        return cuda_fail(c, "rad_stage: readback");
+                    *n_noroot = (long long)v;
+                }
+                return RAD_OK;
+            }
+        }
         int nl = rad::launch_cell_velocity(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->vel, s);
         if (nl < 0) return cuda_fail(c, "rad_stage (velocity table)");
         c->launches += nl;
-        static const bool split = [] { const char *e = std::getenv("RAD_TAU_SPLIT"); return e && e[0] == '1'; }();
-        if (!split && c->kp.couple && c->opac.alpha_a_planck) {
+        if (tau_path != 2 && c->kp.couple && c->opac.alpha_a_planck) {
             // fused warp-per-cell stage kernel (stage.cu) with the Eq.28 factor; serves N <= 192 with stored coefficients
             if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
             rad::StageArgs a{};

@@ -76,6 +76,7 @@ struct StageArgs {
     unsigned long long *noroot;
     const double *vel;  // stage.cu only: optical-depth-aware flux (Eq.26-29), {u^alphahat, alpha_E} per cell, or nullptr (Eq.24)
     double tau_dt;      // tau_factor * beta_dt
+    const double *vel8; // stage5.cu only: optical-depth-aware flux, per cell {u^alphahat (4), f/2 of the upper x, y, z faces, pad}, or nullptr
     int kz0, kz1;  // stage5 only: update the interior planes kz0 <= k < kz1 (0-based, without ghosts); kz1 <= kz0 = the whole block
 };
 
@@ -106,6 +107,8 @@ int launch_stage_fused(const DeviceTables &t, const Params &p, const StageArgs &
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
 // 1 if launch_stage_angle serves this context (so that a stage can be run slab by slab along z)
 int stage_angle_serves(const DeviceTables &t);
+// TAU table of the angle-resident kernel: vel8[ncell][8], see k_tau_table (stage5.cu)
+int launch_tau_table(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double tau_dt, double *vel8, cudaStream_t s);
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s);
 int launch_build_ke(const DeviceTables &t, double *ke, cudaStream_t s);
 int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed char *edge_sign, cudaStream_t s);

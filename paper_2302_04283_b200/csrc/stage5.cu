@@ -33,15 +33,17 @@ constexpr int RECN = RAD_STAGE_RECN;  // packed per-cell record, see k_pack_rec
 constexpr int USTR = 64;              // a cell's record slot in shared memory: [0..35] record, [36..43] lower y face,
                                       // [44..51] lower z face, [52..59] rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s
 
-template <int TY_, int TZ_, int WPC_>
+template <int TY_, int TZ_, int WPC_, bool TAU_ = false>
 struct Tile {
     static constexpr int TY = TY_, TZ = TZ_, WPC = WPC_;
-    static constexpr int NC = TY * TZ, NH = 4 * TZ + 4 * TY, NR = 3 * NC + NH + TY + TZ, NT = NC * WPC * 32;
+    static constexpr bool TAU = TAU_;  // optical-depth-aware flux (Eq.26-29): per-cell velocity records of the tile and its 1-deep halo
+    static constexpr int NVH = 2 * TZ + 2 * TY;  // halo cells at distance 1 (no corners)
+    static constexpr int NC = TY * TZ, NH = 4 * TZ + 4 * TY, NR0 = 3 * NC + NH + TY + TZ, NR = NR0 + (TAU ? NC + NVH : 0), NT = NC * WPC * 32;
     static constexpr int NFY = (TY - 1) * TZ, NFZ = TY * (TZ - 1);
 };
 
 struct Layout5 {
-    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oFx, oU, oRed, oRole, oBar, total;  // offsets in doubles
+    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oFx, oU, oRed, oRole, oV, oVh, oBar, total;  // offsets in doubles
 };
 template <class T>
 __host__ __device__ inline Layout5 make_layout5(int N) {
@@ -57,7 +59,9 @@ __host__ __device__ inline Layout5 make_layout5(int N) {
     L.oU = L.oFx + 2 * L.Np;
     L.oRed = L.oU + 4 * T::NC * USTR;
     L.oRole = L.oRed + T::NC * (2 * T::WPC * 4 + 8);  // per cell: two sets of WPC partial sums, then (T_+, source, flag)
-    L.oBar = L.oRole + T::NR * 4;
+    L.oV = L.oRole + T::NR * 4;                       // TAU: velocity records (8 doubles) of the own cells, 4 buffers
+    L.oVh = L.oV + (T::TAU ? 4 * T::NC * 8 : 0);      // ... and of the halo cells at distance 1, 2 buffers
+    L.oBar = L.oVh + (T::TAU ? 2 * T::NVH * 8 : 0);
     L.total = L.oBar + 3;  // two mbarriers, then the bytes of one step's copies
     return L;
 }
@@ -84,8 +88,11 @@ __device__ __forceinline__ FaceRec load_face(const double *f) {  // warp-uniform
 // = (LL, L, R) for n^a > 0 and (RR, R, L) otherwise, the face value is mid + dl dr / (dl + dr), dl = mid - far,
 // dr = oth - mid (the harmonic mean is odd under reversal, so one formula serves both signs).  Branch free; sign tests
 // are integer tests of the high word (na = +-0 -> the flux is 0 either way).
-template <bool PLM>
-__device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double n2, double n3, double qLL, double qL, double qR, double qRR) {
+// TAU (Eq.26-29; readings R15-R18, G1 in DESIGN.md): with G = -(1 + 1/n^0bar) of the two cells for this angle and fh = f/2 of the
+// face, the factor 1 - g_up + g of Eq.28 is 1 + fh (G_R - G_L) for n^a > 0 and 1 + fh (G_L - G_R) otherwise.
+template <bool PLM, bool TAU = false>
+__device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double n2, double n3, double qLL, double qL, double qR, double qRR,
+                                            double GL = 0.0, double GR = 0.0, double fh = 0.0) {
     const double na = chain4(f.e0, f.e1, f.e2, f.e3, n1, n2, n3);
     const double n0 = chain4(f.E0, f.E1, f.E2, f.E3, n1, n2, n3);
     const bool pos = hi32(na) > 0;
@@ -96,7 +103,13 @@ __device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double 
         const double h = div3(pr, dl + dr);  // only used where pr > 0, i.e. dl + dr != 0
         up += hi32(pr) > 0 ? h : 0.0;
     }
+    if (TAU) up *= fma(fh, pos ? GR - GL : GL - GR, 1.0);
     return __dmul_rn(__dmul_rn(na, n0), up);
+}
+
+// TAU: G = -(1 + 1/n^0bar) of a cell for one angle, n^0bar = u^0hat - u^ahat n^ahat (Eq.29)
+__device__ __forceinline__ double tau_G(double u0, double u1, double u2, double u3, double n1, double n2, double n3) {
+    return -(1.0 + rcp3(u0 - (u1 * n1 + u2 * n2 + u3 * n3)));
 }
 
 // sums of four values over the warp, all lanes get all four: the first two butterfly steps halve the number of values a
@@ -219,10 +232,10 @@ __device__ __forceinline__ bool quartic_delta_fast(double B4, double B1, double 
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-template <int NITER, int WPC, int TY, int TZ, int MINB, bool PLM, bool COUPLE>
+template <int NITER, int WPC, int TY, int TZ, int MINB, bool PLM, bool COUPLE, bool TAU>
 __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     k_stage5(const DeviceTables t, const Params p, const StageArgs a, const Layout5 L, const int KX) {
-    using T = Tile<TY, TZ, WPC>;
+    using T = Tile<TY, TZ, WPC, TAU>;
     constexpr int NC = T::NC, NH = T::NH, NR = T::NR;
     constexpr uint32_t ITB = WPC * 32 * 8;  // byte distance between a thread's consecutive angles
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -263,6 +276,21 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 r.stride = N; r.bytes = row_bytes;
                 if (tid < NC) { r.src0 = a.I_in + (c0 + 2) * N; r.dst0 = L.oRing + tid * Np; r.dstride = NC * Np; r.nbufm1 = 3; r.boff = 2; }
                 else { r.src0 = a.I_in + c0 * N; r.dst0 = L.oHalo + (tid - NC) * Np; r.dstride = NH * Np; r.nbufm1 = 1; }
+            }
+        } else if (TAU && tid >= T::NR0) {
+            // velocity records (8 doubles: u^alphahat, f/2 of the three upper faces, pad) of plane u: the own cells (4 buffers) and
+            // the halo cells at distance 1 (2 buffers; index: y halo wz * 2 + {below, above}, z halo 2 TZ + wy * 2 + {below, above})
+            const int q = tid - T::NR0;
+            int jj, kk;
+            if (q < NC) { jj = j0 + q % TY; kk = k0 + q / TY; r.dst0 = L.oV + q * 8; r.dstride = NC * 8; r.nbufm1 = 3; }
+            else {
+                const int h = q - NC;
+                if (h < 2 * TZ) { kk = k0 + (h >> 1); jj = (h & 1) ? j0 + TY : j0 - 1; }
+                else { jj = j0 + ((h - 2 * TZ) >> 1); kk = ((h - 2 * TZ) & 1) ? k0 + TZ : k0 - 1; }
+                r.dst0 = L.oVh + h * 8; r.dstride = T::NVH * 8; r.nbufm1 = 1;
+            }
+            if (jj < t.NJ && kk < t.NK) {
+                r.src0 = a.vel8 + (((long long)kk * t.NJ + jj) * t.NI + i_begin) * 8; r.stride = 8; r.bytes = 64;
             }
         } else {
             const int q = tid - NC - NH;
@@ -361,7 +389,14 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             const int n = OFF8(it) >> 3;
             const double xm2 = PLM ? __ldg(Ic - 2 * N + n) : 0.0;
             xm1[it] = __ldg(Ic - N + n); x0[it] = __ldg(Ic + n); xp1[it] = __ldg(Ic + N + n);
-            carry[it] = face_flux<PLM>(f, n1[it], n2[it], n3[it], xm2, xm1[it], x0[it], xp1[it]);
+            double GL = 0.0, GR = 0.0, fhx = 0.0;
+            if (TAU) {
+                const double *vL = a.vel8 + (c_first - 1) * 8, *vR = a.vel8 + c_first * 8;
+                GL = tau_G(__ldg(vL), __ldg(vL + 1), __ldg(vL + 2), __ldg(vL + 3), n1[it], n2[it], n3[it]);
+                GR = tau_G(__ldg(vR), __ldg(vR + 1), __ldg(vR + 2), __ldg(vR + 3), n1[it], n2[it], n3[it]);
+                fhx = __ldg(vL + 4);
+            }
+            carry[it] = face_flux<PLM, TAU>(f, n1[it], n2[it], n3[it], xm2, xm1[it], x0[it], xp1[it], GL, GR, fhx);
         }
         if (COUPLE && wc == WH && lane < 8) sts(smb + 8u * (uint32_t)(L.oU + cs * USTR + 52 + lane), pf_lane ? __ldg(fluid_ptr(0)) : 0.0);
     }
@@ -447,6 +482,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     for (int s = 0; s < nsteps; s++) {
         const int b = s & 1;
         mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
+        if (TAU && s + 1 < nsteps) mbar_wait(bar0 + 8u * (b ^ 1), ((s + 1) >> 1) & 1);  // the velocity records of plane s+1 (x face above)
         if (tid == 0 && s + 2 < nsteps) mbar_expect_tx(bar0 + 8u * b, *reinterpret_cast<volatile uint32_t *>(sm + L.oBar + 2));  // re-armed for step s+2 (copies start after the barrier below)
         const uint32_t ringS = aRing + (uint32_t)(s & 3) * planeB;          // own rows of plane s
         const uint32_t haloS = aHalo + (uint32_t)b * ((uint32_t)(NH * Np) * 8u);  // halo rows of plane s
@@ -490,11 +526,27 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 d[it] = (d[it] - pulled) * winv[it];
             }
             // ---- spatial fluxes (Eq.24).  x: the upper face; the lower one is carried
+            double G0[NITER];  // TAU: G of this cell per angle
+            const uint32_t vOwn = smb + 8u * (uint32_t)(L.oV + ((s & 3) * NC + cs) * 8), vHal = smb + 8u * (uint32_t)(L.oVh + b * T::NVH * 8);
+            double2 own46 = make_double2(0.0, 0.0);  // f/2 of the upper x and y faces
+            double own6 = 0.0;                       // ... and of the upper z face
+            if (TAU) {
+                const double2 u01 = lds2(vOwn), u23 = lds2(vOwn + 16);
+                own46 = lds2(vOwn + 32); own6 = lds(vOwn + 48);
+#pragma unroll
+                for (int it = 0; it < NITER; it++) G0[it] = tau_G(u01.x, u01.y, u23.x, u23.y, n1[it], n2[it], n3[it]);
+            }
             {
                 const FaceRec f = lds_face(aUb);
+                double2 x01 = make_double2(1.0, 0.0), x23 = make_double2(0.0, 0.0);
+                if (TAU) {
+                    if (s + 1 < nsteps) { const uint32_t vXp = smb + 8u * (uint32_t)(L.oV + (((s + 1) & 3) * NC + cs) * 8); x01 = lds2(vXp); x23 = lds2(vXp + 16); }
+                    else { const double *vg = a.vel8 + (c_first + s + 1) * 8; x01 = make_double2(__ldg(vg), __ldg(vg + 1)); x23 = make_double2(__ldg(vg + 2), __ldg(vg + 3)); }
+                }
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
-                    const double F = face_flux<PLM>(f, n1[it], n2[it], n3[it], xm1[it], x0[it], xp1[it], xp2[it]);
+                    const double F = face_flux<PLM, TAU>(f, n1[it], n2[it], n3[it], xm1[it], x0[it], xp1[it], xp2[it], TAU ? G0[it] : 0.0,
+                                                         TAU ? tau_G(x01.x, x01.y, x23.x, x23.y, n1[it], n2[it], n3[it]) : 0.0, own46.x);
                     d[it] += F - carry[it];
                     carry[it] = F;
                 }
@@ -508,6 +560,13 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 const bool low_edge = (ax == 1 ? wy : wz) == 0, publish = ax == 1 ? wy < TY - 1 : wz < TZ - 1;
                 const uint32_t pub = ax == 1 ? aFy + (uint32_t)((b * T::NFY + wz * (TY - 1) + wy) * Np) * 8u : aFz + (uint32_t)((b * T::NFZ + wz * TY + wy) * Np) * 8u;
                 const FaceRec fh = lds_face(aUb + 64 * ax);
+                double2 q01 = make_double2(1.0, 0.0), q23 = make_double2(0.0, 0.0);  // TAU: velocity of the cell above along this axis
+                if (TAU) {
+                    const bool inside = ax == 1 ? wy + 1 < TY : wz + 1 < TZ;
+                    const uint32_t vq = inside ? vOwn + (uint32_t)(ax == 1 ? 1 : TY) * 64u : vHal + (uint32_t)(ax == 1 ? wz * 2 + 1 : 2 * TZ + wy * 2 + 1) * 64u;
+                    q01 = lds2(vq); q23 = lds2(vq + 16);
+                }
+                const double fhu = ax == 1 ? own46.y : own6;
                 double m1[NITER], p1[NITER], p2[NITER], F[NITER];
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
@@ -516,7 +575,8 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 }
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
-                    F[it] = face_flux<PLM>(fh, n1[it], n2[it], n3[it], m1[it], x0[it], p1[it], p2[it]);
+                    F[it] = face_flux<PLM, TAU>(fh, n1[it], n2[it], n3[it], m1[it], x0[it], p1[it], p2[it], TAU ? G0[it] : 0.0,
+                                                TAU ? tau_G(q01.x, q01.y, q23.x, q23.y, n1[it], n2[it], n3[it]) : 0.0, fhu);
                     d[it] += F[it];
                 }
                 if (publish) {
@@ -526,10 +586,17 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 }
                 if (low_edge && !(ax == 2 && is_helpee)) {
                     const FaceRec fl = lds_face(aUb + (ax == 1 ? 8 * 36 : 8 * 44));
+                    double2 l01 = make_double2(1.0, 0.0), l23 = make_double2(0.0, 0.0);
+                    double fhl = 0.0;  // TAU: the cell below is a halo cell; f/2 of this face is its upper-face entry
+                    if (TAU) {
+                        const uint32_t vq = vHal + (uint32_t)(ax == 1 ? wz * 2 : 2 * TZ + wy * 2) * 64u;
+                        l01 = lds2(vq); l23 = lds2(vq + 16); fhl = lds(vq + (ax == 1 ? 40 : 48));
+                    }
 #pragma unroll
                     for (int it = 0; it < NITER; it++) {
                         const double m2 = PLM ? lds(rm2 + OFF8(it)) : 0.0;
-                        d[it] -= face_flux<PLM>(fl, n1[it], n2[it], n3[it], m2, m1[it], x0[it], p1[it]);
+                        d[it] -= face_flux<PLM, TAU>(fl, n1[it], n2[it], n3[it], m2, m1[it], x0[it], p1[it],
+                                                     TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0, TAU ? G0[it] : 0.0, fhl);
                     }
                 }
             }
@@ -544,7 +611,16 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 q0[it] = PLM ? lds(r_m2 + OFF8(it)) : 0.0; q1[it] = lds(r_m1 + OFF8(it)); q2[it] = lds(r_0 + OFF8(it)); q3[it] = lds(r_p1 + OFF8(it));
             }
 #pragma unroll
-            for (int it = 0; it < NITER; it++) q0[it] = face_flux<PLM>(fl, n1[it], n2[it], n3[it], q0[it], q1[it], q2[it], q3[it]);
+            double2 l01 = make_double2(1.0, 0.0), l23 = make_double2(0.0, 0.0), r01 = l01, r23 = l23;
+            double fhl = 0.0;
+            if (TAU) {  // cell (0,0) and the halo cell below it in z
+                const uint32_t vl = smb + 8u * (uint32_t)(L.oVh + (b * T::NVH + 2 * TZ) * 8), vr = smb + 8u * (uint32_t)(L.oV + ((s & 3) * NC) * 8);
+                l01 = lds2(vl); l23 = lds2(vl + 16); fhl = lds(vl + 48); r01 = lds2(vr); r23 = lds2(vr + 16);
+            }
+#pragma unroll
+            for (int it = 0; it < NITER; it++)
+                q0[it] = face_flux<PLM, TAU>(fl, n1[it], n2[it], n3[it], q0[it], q1[it], q2[it], q3[it], TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0,
+                                             TAU ? tau_G(r01.x, r01.y, r23.x, r23.y, n1[it], n2[it], n3[it]) : 0.0, fhl);
 #pragma unroll
             for (int it = 0; it < NITER; it++)
                 if (it < NITER - 1 || last_valid) sts(aFx + (uint32_t)(b * Np) * 8u + OFF8(it), q0[it]);
@@ -719,9 +795,9 @@ __global__ void __launch_bounds__(256) k_pack_rec(const DeviceTables t, double *
     }
 }
 
-template <int NITER, int WPC, int TY, int TZ, int MINB = 1>
-int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
-    using T = Tile<TY, TZ, WPC>;
+template <int NITER, int WPC, int TY, int TZ, int MINB, bool TAU>
+int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
+    using T = Tile<TY, TZ, WPC, TAU>;
     const Layout5 L = make_layout5<T>(t.N);
     const size_t smem = sizeof(double) * (size_t)L.total;
     if (smem > 227 * 1024) return 0;
@@ -741,13 +817,52 @@ int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool cou
     if (grid.y > 65535 || grid.z > 65535) return 0;
 #define RAD_LAUNCH5(PLM, CPL)                                                                                          \
     do {                                                                                                               \
-        if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
-        k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                                  \
+        if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
+        k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL, TAU><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                                  \
     } while (0)
-    if (p.recon_space == 1) { if (couple) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(true, false); }
+    if (TAU) {  // the optical-depth-aware flux is only reached through rad_stage (with the coupling half)
+        if (p.recon_space == 1) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(false, true);
+    } else if (p.recon_space == 1) { if (couple) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(true, false); }
     else { if (couple) RAD_LAUNCH5(false, true); else RAD_LAUNCH5(false, false); }
 #undef RAD_LAUNCH5
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+template <int NITER, int WPC, int TY, int TZ, int MINB = 1>
+int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
+    if (a.vel8 != nullptr) return launch5t<NITER, WPC, TY, TZ, MINB, true>(t, p, a, couple, s);
+    return launch5t<NITER, WPC, TY, TZ, MINB, false>(t, p, a, couple, s);
+}
+
+// TAU: per-cell record of the optical-depth-aware flux for EVERY cell (ghosts included), 8 doubles: tetrad-frame fluid velocity
+// u^alphahat (R10), f/2 = -expm1(-tau^2)/2 of the cell's upper x, y, z faces (Eq.26-27 with R15, R16, R18, G1; 0 where the upper
+// neighbour is outside the array), pad.  One launch per stage (the fluid state and beta dt change).
+__device__ __forceinline__ void cell_u(const DeviceTables &t, const double *__restrict__ fluid, long long c, double (&u)[4]) {
+    const double *th = t.cell + c * RAD_NCELL + 44;
+    const double u1 = fluid[2 * t.ncell + c], u2 = fluid[3 * t.ncell + c], u3 = fluid[4 * t.ncell + c];
+    u[1] = th[0] * u1 + th[1] * u2 + th[2] * u3; u[2] = th[3] * u2 + th[4] * u3; u[3] = th[5] * u3;
+    u[0] = sqrt(1.0 + (u[1] * u[1] + u[2] * u[2] + u[3] * u[3]));
+}
+__global__ void __launch_bounds__(256) k_tau_table(const DeviceTables t, const double *__restrict__ fluid, const double *__restrict__ aE,
+                                                   const double *__restrict__ aS, double tau_dt, double *__restrict__ vel8) {
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < t.ncell; c += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(c % t.NI), j = (int)((c / t.NI) % t.NJ), k = (int)(c / ((long long)t.NI * t.NJ));
+        double u[4], un[4];
+        cell_u(t, fluid, c, u);
+        const double ae = aE[c] + aS[c];
+        double out[8] = {u[0], u[1], u[2], u[3], 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+        for (int ax = 0; ax < 3; ax++) {
+            const bool inside = ax == 0 ? i + 1 < t.NI : (ax == 1 ? j + 1 < t.NJ : k + 1 < t.NK);
+            if (!inside) continue;
+            const long long cu = c + (ax == 0 ? 1 : (ax == 1 ? (long long)t.NI : (long long)t.NI * t.NJ));
+            cell_u(t, fluid, cu, un);
+            const double tau = tau_dt * (0.5 * (ae + (aE[cu] + aS[cu]))) / (0.5 * (u[0] + un[0]));
+            out[4 + ax] = -0.5 * expm1(-tau * tau);
+        }
+#pragma unroll
+        for (int q = 0; q < 8; q++) vel8[c * 8 + q] = out[q];
+    }
 }
 
 }  // namespace
@@ -756,7 +871,7 @@ int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool cou
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
     if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr) return 0;
     if (t.N & 1) return 0;  // rows must be multiples of 16 bytes for the bulk copies
-    if (((uintptr_t)a.I_in & 15) || ((uintptr_t)t.ke & 15) || ((uintptr_t)t.rec & 15)) return 0;
+    if (((uintptr_t)a.I_in & 15) || ((uintptr_t)t.ke & 15) || ((uintptr_t)t.rec & 15) || ((uintptr_t)a.vel8 & 15)) return 0;
     const int N = t.N;
     if (N <= 32) return launch5<1, 1, 4, 2>(t, p, a, couple, s);
     if (N <= 64) return launch5<1, 2, 4, 2>(t, p, a, couple, s);
@@ -791,6 +906,11 @@ int stage_angle_serves(const DeviceTables &t) {
     if (t.N > 192) return sizeof(double) * (size_t)make_layout5<Tile<2, 2, 2>>(t.N).total <= 227 * 1024;
     if (t.N > 128) return sizeof(double) * (size_t)make_layout5<Tile<4, 2, 2>>(t.N).total <= 227 * 1024;
     return 1;
+}
+
+int launch_tau_table(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double tau_dt, double *vel8, cudaStream_t s) {
+    k_tau_table<<<148 * 4, 256, 0, s>>>(t, fluid, aE, aS, tau_dt, vel8);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s) {
