@@ -12,7 +12,10 @@
  *
  * Parity unpinned (no external anchor; the oracle IS the definition): R1 lat-lon centres,
  * R3 geodesic index order, R2 triad order, R6 face-centre evaluation, R7 limiter form,
- * R12 renorm flag, R13 failure policy, R14 mask placement.  Everything else is pinned by
+ * R12 renorm flag, R13 failure policy, R14 mask placement; and in the optical-depth-aware flux
+ * (face_flux with vel != NULL, Eq.26-29): the sign and form of g_L/R (Eq.29) and the readings
+ * R15-R17 -- its limits (tau = 0, tau -> 0 quadratically, uniform flow, saturation) and
+ * conservation ARE pinned (tests/test_oracle_tauflux.py).  Everything else is pinned by
  * tests/test_oracle_*.py (-m "not gpu").
  */
 #include "rad_oracle.h"

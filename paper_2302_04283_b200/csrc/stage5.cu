@@ -15,7 +15,10 @@
 //     coefficients of each cell (2 buffers; the owner of an edge overwrites the coefficient with the edge flux, the
 //     partner angle pulls it from there), and a packed per-cell geometry record (4 buffers).  One __syncthreads per step.
 //   * the coupling's angle sums are warp butterflies followed by a WPC-way exchange through shared memory under a
-//     named barrier private to the cell.
+//     named barrier private to the cell; the cell's first warp solves the quartic while its last warp writes the previous
+//     step's outputs and prepares the next cell's fluid velocity.
+//   * TAU (template): the optical-depth-aware spatial flux of Eq.26-29 -- a per-cell table (k_tau_table) of u^alphahat and f/2
+//     of the upper faces comes in with the other copies for the tile's cells and the halo cells at distance 1.
 #include <cstdlib>
 
 #include "async_copy.cuh"
