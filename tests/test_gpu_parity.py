@@ -435,3 +435,34 @@ def test_optical_depth_flux_host_path_and_periodic(oracle, B):
         assert rel_err(P.interior(T_h), P.interior(T_o), 0.0) <= TOL_FLUID
     finally:
         B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_random_configurations(oracle, B, seed):
+    """randomised sweep: angle grid, block shape (long x runs, partial tiles), metric, boundary codes, reconstruction, fluid-frame
+    weight flag, mask, optical-depth factor -- every case within the stage tolerances"""
+    import random
+    rnd = random.Random(seed)
+    angs = [("geodesic", 1), ("geodesic", 2), ("geodesic", 3), ("geodesic", 4), ("geodesic", 5), ("latlon", 4, 8), ("latlon", 5, 16), ("latlon", 2, 4), ("latlon", 6, 10)]
+    for case in range(25):
+        ang = rnd.choice(angs); n = (rnd.randint(1, 40 if seed == 3 else 14), rnd.randint(1, 11), rnd.randint(1, 11))
+        kind = rnd.choice([0, 1, 1]); a = rnd.choice([0.0, 0.5, 0.9]) if kind else 0.0
+        bc = tuple(rnd.choice([0, 1, 2]) for _ in range(6)); tau = rnd.choice([0.0, 0.0, 0.7, 5.0])
+        params = dict(recon_space=rnd.choice([0, 1, 1]), renorm_fluid_weights=rnd.choice([0, 1]), n0_crit=rnd.choice([0.0, 0.1]), couple=1)
+        dx = (rnd.uniform(0.15, 0.4), rnd.uniform(0.15, 0.4), rnd.uniform(0.15, 0.4))
+        A = oracle.Angles(*ang)
+        P = oracle.Problem(A, n, (3.0, 2.0, 1.0), dx, metric_kind=kind, M=1.0, a=a, bc_lo=bc[:3], bc_hi=bc[3:], recon_space=params["recon_space"],
+                           renorm=params["renorm_fluid_weights"], couple=1, n0_crit=params["n0_crit"], tau_factor=tau)
+        rng = np.random.default_rng(1000 * seed + case); nc = P.ncell
+        I = np.exp(rng.normal(size=(nc, A.N)))
+        fluid = np.stack([rng.uniform(0.5, 2, nc), rng.uniform(0.3, 1.5, nc)] + [rng.uniform(-0.4, 0.4, nc) for _ in range(3)])
+        opac = np.stack([rng.uniform(0.1, 30, nc)] * 2 + [rng.uniform(0.1, 30, nc)])
+        d_opac = dev(opac)
+        h = B.rad_create(dict(kind=kind, M=1.0, a=a), dict(n=n, x0=(3.0, 2.0, 1.0), dx=dx, bc_lo=bc[:3], bc_hi=bc[3:]), ang,
+                         (d_opac[0], d_opac[1], d_opac[2]), dict(params, tau_factor=tau))
+        try:
+            compare_stage(B, A, P, h, I, fluid, opac, rnd.uniform(0.01, 0.05))
+        except AssertionError as e:
+            raise AssertionError((case, ang, n, kind, a, bc, tau, params, str(e)))
+        finally:
+            B.rad_destroy(h)
