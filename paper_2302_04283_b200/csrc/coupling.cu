@@ -8,6 +8,10 @@
 // dT^0_alpha = -sum_n n^0 n_alpha (I_+ - I*) dOmega_n with a second shuffle tree.
 #include "stage_math.cuh"
 
+#ifndef RAD_MOM_CTAS
+#define RAD_MOM_CTAS 8
+#endif
+
 namespace rad {
 namespace {
 
@@ -232,6 +236,97 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta) k_moments(DeviceTables t, c
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// moments, leaner version: persistent warps, the angle set in registers, one cell per warp iteration.
+// By linearity every frame's moments follow from the ten tetrad-frame sums M^{ab} = sum_n I dOmega ntil^a ntil^b,
+// ntil = (1, n^1hat, n^2hat, n^3hat): 13 FP64 operations per angle instead of ~35, all loads of a row issued together;
+// the per-cell transform (tetrad e^mu_ahat for frame 0, n_alpha rows for frame 1, boost Eq.13-14 for frame 3) is done
+// once per cell after the warp reduction.
+// ------------------------------------------------------------------------------------------------
+template <int NITER>
+__global__ void __launch_bounds__(256) k_moments_t(DeviceTables t, const double *__restrict__ I, int frame, const double *__restrict__ fluid,
+                                                   double *__restrict__ out) {
+    const int lane = threadIdx.x & 31, N = t.N;
+    const long long nwarp = (long long)gridDim.x * (blockDim.x >> 5), nint = (long long)t.n[0] * t.n[1] * t.n[2];
+    double n1[NITER], n2[NITER], n3[NITER], dom[NITER];
+    int off[NITER];
+#pragma unroll
+    for (int it = 0; it < NITER; it++) {
+        const int n = it * 32 + lane;
+        const bool v = n < N;
+        off[it] = v ? n : 0;
+        n1[it] = t.nhat[3 * off[it]]; n2[it] = t.nhat[3 * off[it] + 1]; n3[it] = t.nhat[3 * off[it] + 2];
+        dom[it] = v ? t.domega[n] : 0.0;
+    }
+    for (long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); wid < nint; wid += nwarp) {
+        const int i = (int)(wid % t.n[0]) + t.ng, j = (int)((wid / t.n[0]) % t.n[1]) + t.ng, k = (int)(wid / ((long long)t.n[0] * t.n[1])) + t.ng;
+        const long long c = ((long long)k * t.NJ + j) * t.NI + i;
+        const double *row = I + c * N;
+        double w[NITER];
+#pragma unroll
+        for (int it = 0; it < NITER; it++) w[it] = row[off[it]];
+        double m[10];
+#pragma unroll
+        for (int q = 0; q < 10; q++) m[q] = 0.0;
+#pragma unroll
+        for (int it = 0; it < NITER; it++) {
+            const double w0 = w[it] * dom[it], w1 = w0 * n1[it], w2 = w0 * n2[it], w3 = w0 * n3[it];
+            m[0] += w0; m[1] += w1; m[2] += w2; m[3] += w3;
+            m[4] = fma(w1, n1[it], m[4]); m[5] = fma(w1, n2[it], m[5]); m[6] = fma(w1, n3[it], m[6]);
+            m[7] = fma(w2, n2[it], m[7]); m[8] = fma(w2, n3[it], m[8]); m[9] = fma(w3, n3[it], m[9]);
+        }
+#pragma unroll
+        for (int q = 0; q < 10; q++) m[q] = warp_sum(m[q]);
+        if (lane != 0) continue;
+        const double *cg = t.cell + c * RAD_NCELL;
+        // full symmetric M[a][b]
+        const double M[4][4] = {{m[0], m[1], m[2], m[3]}, {m[1], m[4], m[5], m[6]}, {m[2], m[5], m[7], m[8]}, {m[3], m[6], m[8], m[9]}};
+        if (frame == 2) {
+#pragma unroll
+            for (int q = 0; q < 10; q++) out[q * t.ncell + c] = m[q];
+        } else if (frame == 1) {  // R^0_alpha = n^0 sum n_alpha I dOmega; n_0 = E_ahat ntil^ahat, n_i = theta^a_i n^a
+            const double nup0 = cg[0];
+            out[c] = nup0 * (cg[1] * m[0] + cg[2] * m[1] + cg[3] * m[2] + cg[4] * m[3]);
+            out[t.ncell + c] = nup0 * (cg[44] * m[1]);
+            out[2 * t.ncell + c] = nup0 * (cg[45] * m[1] + cg[47] * m[2]);
+            out[3 * t.ncell + c] = nup0 * (cg[46] * m[1] + cg[48] * m[2] + cg[49] * m[3]);
+        } else if (frame == 0) {  // R^{mu nu} = e^mu_a e^nu_b M^{ab}; e^0_0 = n^0, e^i_0 = -beta^i n^0, e^i_a = triad (upper triangular, R2)
+            const double nup0 = cg[0];
+            const double E[4][4] = {{nup0, 0.0, 0.0, 0.0}, {-cg[35] * nup0, cg[38], cg[39], cg[40]}, {-cg[36] * nup0, 0.0, cg[41], cg[42]}, {-cg[37] * nup0, 0.0, 0.0, cg[43]}};
+            double EM[4][4];
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++)
+#pragma unroll
+                for (int b = 0; b < 4; b++) EM[mu][b] = E[mu][0] * M[0][b] + E[mu][1] * M[1][b] + E[mu][2] * M[2][b] + E[mu][3] * M[3][b];
+            int q = 0;
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++)
+#pragma unroll
+                for (int nu = mu; nu < 4; nu++) {
+                    out[q * t.ncell + c] = EM[mu][0] * E[nu][0] + EM[mu][1] * E[nu][1] + EM[mu][2] * E[nu][2] + EM[mu][3] * E[nu][3];
+                    q++;
+                }
+        } else {  // fluid frame (Eq.13-14 with G2): nbar^0 = u^0 - u_a n^a, nbar^a = n^a + u^a (u_b n^b / (1 + u^0) - 1)
+            double uh[4];
+            tetrad_velocity_rec(cg, fluid[2 * t.ncell + c], fluid[3 * t.ncell + c], fluid[4 * t.ncell + c], uh);
+            const double r = 1.0 / (1.0 + uh[0]);
+            double L[4][4];
+            L[0][0] = uh[0]; L[0][1] = -uh[1]; L[0][2] = -uh[2]; L[0][3] = -uh[3];
+#pragma unroll
+            for (int a = 1; a < 4; a++) {
+                L[a][0] = -uh[a];
+#pragma unroll
+                for (int b = 1; b < 4; b++) L[a][b] = (a == b ? 1.0 : 0.0) + uh[a] * uh[b] * r;
+            }
+            double LM[4];  // Lambda^0_a M^{ab}
+#pragma unroll
+            for (int b = 0; b < 4; b++) LM[b] = L[0][0] * M[0][b] + L[0][1] * M[1][b] + L[0][2] * M[2][b] + L[0][3] * M[3][b];
+#pragma unroll
+            for (int q = 0; q < 4; q++) out[q * t.ncell + c] = LM[0] * L[q][0] + LM[1] * L[q][1] + LM[2] * L[q][2] + LM[3] * L[q][3];
+        }
+    }
+}
+
 }  // namespace
 
 int launch_coupling(const DeviceTables &t, const Params &p, double *I, const double *fluid, const double *aP, const double *aE,
@@ -255,7 +350,18 @@ int launch_coupling(const DeviceTables &t, const Params &p, double *I, const dou
 int launch_moments(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out, cudaStream_t s) {
     const long long nint = (long long)t.n[0] * t.n[1] * t.n[2];
     const long long blocks = (nint + kWarpsPerCta - 1) / kWarpsPerCta;
-    k_moments<<<(unsigned)blocks, 32 * kWarpsPerCta, 0, s>>>(t, I, frame, fluid, out);
+    const int grid = 148 * RAD_MOM_CTAS;
+    switch ((t.N + 31) / 32) {
+        case 1: k_moments_t<1><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        case 2: k_moments_t<2><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        case 3: k_moments_t<3><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        case 4: k_moments_t<4><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        case 5: k_moments_t<5><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        case 6: k_moments_t<6><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        case 7: k_moments_t<7><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        case 8: k_moments_t<8><<<grid, 256, 0, s>>>(t, I, frame, fluid, out); break;
+        default: k_moments<<<(unsigned)blocks, 32 * kWarpsPerCta, 0, s>>>(t, I, frame, fluid, out);  // N > 256: per-angle version
+    }
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
