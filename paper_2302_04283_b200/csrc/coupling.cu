@@ -236,6 +236,27 @@ __global__ void __launch_bounds__(32 * kWarpsPerCta) k_moments(DeviceTables t, c
     }
 }
 
+// sums of ten values over the warp, delivered to every lane: a transposing butterfly (at distance 16, 8, 4, 2 a lane keeps half of
+// the values it carries and hands the other half to its partner), 16 + 10 shuffles instead of 50
+__device__ __forceinline__ void warp_sum10(double (&m)[10], int lane) {
+    const unsigned full = 0xffffffffu;
+    double a[16];
+#pragma unroll
+    for (int q = 0; q < 16; q++) a[q] = q < 10 ? m[q] : 0.0;
+    double b[8], c[4], d[2];
+    const bool h16 = (lane & 16) != 0, h8 = (lane & 8) != 0, h4 = (lane & 4) != 0, h2 = (lane & 2) != 0;
+#pragma unroll
+    for (int q = 0; q < 8; q++) b[q] = (h16 ? a[8 + q] : a[q]) + __shfl_xor_sync(full, h16 ? a[q] : a[8 + q], 16);
+#pragma unroll
+    for (int q = 0; q < 4; q++) c[q] = (h8 ? b[4 + q] : b[q]) + __shfl_xor_sync(full, h8 ? b[q] : b[4 + q], 8);
+#pragma unroll
+    for (int q = 0; q < 2; q++) d[q] = (h4 ? c[2 + q] : c[q]) + __shfl_xor_sync(full, h4 ? c[q] : c[2 + q], 4);
+    double e = (h2 ? d[1] : d[0]) + __shfl_xor_sync(full, h2 ? d[0] : d[1], 2);
+    e += __shfl_xor_sync(full, e, 1);  // lanes 2q, 2q+1 hold the sum of value q
+#pragma unroll
+    for (int q = 0; q < 10; q++) m[q] = __shfl_sync(full, e, 2 * q);
+}
+
 // ------------------------------------------------------------------------------------------------
 // moments, leaner version: persistent warps, the angle set in registers, one cell per warp iteration.
 // By linearity every frame's moments follow from the ten tetrad-frame sums M^{ab} = sum_n I dOmega ntil^a ntil^b,
@@ -275,8 +296,7 @@ __global__ void __launch_bounds__(256) k_moments_t(DeviceTables t, const double 
             m[4] = fma(w1, n1[it], m[4]); m[5] = fma(w1, n2[it], m[5]); m[6] = fma(w1, n3[it], m[6]);
             m[7] = fma(w2, n2[it], m[7]); m[8] = fma(w2, n3[it], m[8]); m[9] = fma(w3, n3[it], m[9]);
         }
-#pragma unroll
-        for (int q = 0; q < 10; q++) m[q] = warp_sum(m[q]);
+        warp_sum10(m, lane);
         if (lane != 0) continue;
         const double *cg = t.cell + c * RAD_NCELL;
         // full symmetric M[a][b]
