@@ -9,7 +9,7 @@
 #include "stage_math.cuh"
 
 #ifndef RAD_MOM_CTAS
-#define RAD_MOM_CTAS 8
+#define RAD_MOM_CTAS 6
 #endif
 
 namespace rad {
@@ -265,36 +265,32 @@ __device__ __forceinline__ void warp_sum10(double (&m)[10], int lane) {
 // once per cell after the warp reduction.
 // ------------------------------------------------------------------------------------------------
 template <int NITER>
-__global__ void __launch_bounds__(256) k_moments_t(DeviceTables t, const double *__restrict__ I, int frame, const double *__restrict__ fluid,
+__global__ void __launch_bounds__(256, 3) k_moments_t(DeviceTables t, const double *__restrict__ I, int frame, const double *__restrict__ fluid,
                                                    double *__restrict__ out) {
     const int lane = threadIdx.x & 31, N = t.N;
     const long long nwarp = (long long)gridDim.x * (blockDim.x >> 5), nint = (long long)t.n[0] * t.n[1] * t.n[2];
-    double n1[NITER], n2[NITER], n3[NITER], dom[NITER];
-    int off[NITER];
-#pragma unroll
-    for (int it = 0; it < NITER; it++) {
-        const int n = it * 32 + lane;
-        const bool v = n < N;
-        off[it] = v ? n : 0;
-        n1[it] = t.nhat[3 * off[it]]; n2[it] = t.nhat[3 * off[it] + 1]; n3[it] = t.nhat[3 * off[it] + 2];
-        dom[it] = v ? t.domega[n] : 0.0;
-    }
+    // per-angle table {dOmega, n^1hat, n^2hat, n^3hat} in shared memory (registers are for warps in flight: the kernel is latency bound)
+    __shared__ double4 sAng[NITER * 32];
+    for (int q = threadIdx.x; q < NITER * 32; q += blockDim.x)
+        sAng[q] = q < N ? make_double4(t.domega[q], t.nhat[3 * q], t.nhat[3 * q + 1], t.nhat[3 * q + 2]) : make_double4(0.0, 0.0, 0.0, 0.0);
+    __syncthreads();
     for (long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); wid < nint; wid += nwarp) {
         const int i = (int)(wid % t.n[0]) + t.ng, j = (int)((wid / t.n[0]) % t.n[1]) + t.ng, k = (int)(wid / ((long long)t.n[0] * t.n[1])) + t.ng;
         const long long c = ((long long)k * t.NJ + j) * t.NI + i;
         const double *row = I + c * N;
         double w[NITER];
 #pragma unroll
-        for (int it = 0; it < NITER; it++) w[it] = row[off[it]];
+        for (int it = 0; it < NITER; it++) w[it] = row[min(it * 32 + lane, N - 1)];
         double m[10];
 #pragma unroll
         for (int q = 0; q < 10; q++) m[q] = 0.0;
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
-            const double w0 = w[it] * dom[it], w1 = w0 * n1[it], w2 = w0 * n2[it], w3 = w0 * n3[it];
+            const double4 an = sAng[it * 32 + lane];  // dOmega = 0 for the idle slots of the last group
+            const double w0 = w[it] * an.x, w1 = w0 * an.y, w2 = w0 * an.z, w3 = w0 * an.w;
             m[0] += w0; m[1] += w1; m[2] += w2; m[3] += w3;
-            m[4] = fma(w1, n1[it], m[4]); m[5] = fma(w1, n2[it], m[5]); m[6] = fma(w1, n3[it], m[6]);
-            m[7] = fma(w2, n2[it], m[7]); m[8] = fma(w2, n3[it], m[8]); m[9] = fma(w3, n3[it], m[9]);
+            m[4] = fma(w1, an.y, m[4]); m[5] = fma(w1, an.z, m[5]); m[6] = fma(w1, an.w, m[6]);
+            m[7] = fma(w2, an.z, m[7]); m[8] = fma(w2, an.w, m[8]); m[9] = fma(w3, an.w, m[9]);
         }
         warp_sum10(m, lane);
         if (lane != 0) continue;
