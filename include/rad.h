@@ -97,7 +97,11 @@ typedef struct {
                                       in rad_create and stored, 3 N doubles per interior cell (adds 24 B per
                                       intensity update of HBM traffic, removes ~100 FP64 operations per update);
                                   1 = not stored: every stage recomputes them from the Ricci rotation coefficients
-                                      (no extra memory; the stage then runs as two kernels and is FP64-bound). */
+                                      (no extra memory; the generic flux-divergence kernel recomputes them and is FP64-bound). */
+    int vel_estimate;          /* radiation-dominated velocity estimate (Eq.51-55; reading G8 in DESIGN.md):
+                                  1 = in cells where Ebar exceeds rho + u_gas the coupling uses the fluid velocity of Eq.55
+                                      (blend of the gas velocity and the radiation velocity of Eq.51 with the clamped
+                                      fractions of Eq.54) instead of the pre-coupling velocity; 0 = always the pre-coupling velocity */
 } rad_params;
 
 /* Build a context: angle tables on the host (section 2.6), geometry tables on the device (section 2.1-2.2,

@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.environ.get("RAD_LIBRAD_PATH") or os.path.join(_HERE, "librad.so")  # override: an experimental build of the same ABI
+_SO = os.path.join(_HERE, "librad.so")
 NCELL, NFACE, MAXNBR = 52, 8, 6
 
 (TAB_NANG, TAB_NEDGE, TAB_NHAT, TAB_DOMEGA, TAB_NNBR, TAB_NBR, TAB_NBR_EDGE, TAB_EDGE_LO, TAB_EDGE_HI, TAB_EDGE_LEN,
@@ -49,7 +49,7 @@ class _Opac(C.Structure):
 class _Params(C.Structure):
     _fields_ = [("gamma_gas", C.c_double), ("a_rad", C.c_double), ("n0_crit", C.c_double), ("recon_space", C.c_int),
                 ("recon_angle", C.c_int), ("renorm_fluid_weights", C.c_int), ("couple", C.c_int), ("tau_factor", C.c_double),
-                ("recompute_edge_coeffs", C.c_int)]
+                ("recompute_edge_coeffs", C.c_int), ("vel_estimate", C.c_int)]
 
 
 _lib = None
@@ -129,7 +129,7 @@ def rad_create(metric, grid, angles, opac, params, device=0):
     o = _Opac(*(_dp(x) for x in opac)) if opac is not None else None
     p = _Params(float(params.get("gamma_gas", 5.0 / 3.0)), float(params.get("a_rad", 1.0)), float(params.get("n0_crit", 0.1)),
                 int(params.get("recon_space", 1)), int(params.get("recon_angle", 0)), int(params.get("renorm_fluid_weights", 1)),
-                int(params.get("couple", 1)), float(params.get("tau_factor", 0.0)), int(params.get("recompute_edge_coeffs", 0)))
+                int(params.get("couple", 1)), float(params.get("tau_factor", 0.0)), int(params.get("recompute_edge_coeffs", 0)), int(params.get("vel_estimate", 0)))
     h = C.c_void_p()
     st = lib().rad_create(C.byref(m), C.byref(g), C.byref(a), C.byref(o) if o is not None else None, C.byref(p), int(device), C.byref(h))
     _check(None, st)

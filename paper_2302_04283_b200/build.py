@@ -23,16 +23,25 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
 
 
-def build(force=False, verbose=False, out=None, extra=()):
-    """out/extra: an experimental build (other -D flags) written somewhere else; the default build is librad.so"""
-    if out is not None:
-        subprocess.check_call([NVCC] + FLAGS + list(extra) + ["-shared", "-o", out] + sources())
-        return out
-    deps = sources() + glob.glob(os.path.join(CSRC, "*.h")) + [os.path.join(ROOT, "include", "rad.h"), os.path.abspath(__file__)]
+def _compile(args):
+    src, obj, flags = args
+    subprocess.check_call([NVCC] + flags + ["-c", src, "-o", obj])
+    return obj
+
+
+def build(force=False, verbose=False):
+    """compile every source of csrc/ (in parallel, one object per file) and link librad.so next to this file"""
+    deps = sources() + glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(ROOT, "include", "rad.h"), os.path.abspath(__file__)]
     if not force and os.path.exists(SO) and os.path.getmtime(SO) >= max(os.path.getmtime(d) for d in deps):
         return SO
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-shared", "-o", SO] + sources()
-    subprocess.check_call(cmd)
+    import concurrent.futures
+    import tempfile
+    flags = FLAGS + (["-Xptxas", "-v"] if verbose else [])
+    with tempfile.TemporaryDirectory() as tmp:
+        jobs = [(s, os.path.join(tmp, os.path.basename(s) + ".o"), flags) for s in sources()]
+        with concurrent.futures.ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 1)) as ex:
+            objs = list(ex.map(_compile, jobs))
+        subprocess.check_call([NVCC] + FLAGS + ["-shared", "-o", SO] + objs)
     return SO
 
 

@@ -1,7 +1,6 @@
 // api.cu -- the C ABI of librad.so (include/rad.h): argument checking, context ownership, launches.
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -34,7 +33,7 @@ struct rad_ctx {
 };
 
 namespace {
-std::string g_create_err;
+thread_local std::string g_create_err;  // text of the last failed rad_create of the calling thread
 
 struct DeviceGuard {
     int prev = -1;
@@ -65,17 +64,16 @@ bool upload(rad_ctx *c, const std::vector<T> &h, const T **dptr) {
 
 bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
 
-// the fused stage kernel: the angle-resident version (stage5.cu) where it serves the configuration (even N <= 192 that
-// fits shared memory), else the warp-independent version (stage.cu).  RAD_STAGE_KERNEL=3 in the environment forces the
-// latter (A/B measurements).
-int launch_fused(const rad::DeviceTables &t, const rad::Params &p, const rad::StageArgs &a, bool couple, cudaStream_t s) {
-    static const int force = [] { const char *e = std::getenv("RAD_STAGE_KERNEL"); return e ? std::atoi(e) : 0; }();
-    if (force == 0 || force == 5) {
-        const int nl = rad::launch_stage_angle(t, p, a, couple, s);
-        if (nl != 0) return nl;
-    }
-    return rad::launch_stage_fused(t, p, a, couple, s);
+// the count of cells without a root (R13) back to the host, if asked for: synchronises the stream
+rad_status read_noroot(rad_ctx *c, long long *n_noroot, cudaStream_t s, const char *where) {
+    if (!n_noroot) return RAD_OK;
+    unsigned long long v = 0;
+    if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+        return cuda_fail(c, where);
+    *n_noroot = (long long)v;
+    return RAD_OK;
 }
+
 }  // namespace
 
 extern "C" {
@@ -115,6 +113,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     if (o) c->opac = *o;
     c->kp.gamma_gas = p->gamma_gas; c->kp.a_rad = p->a_rad; c->kp.n0_crit = p->n0_crit; c->kp.rgm1 = 1.0 / (p->gamma_gas - 1.0); c->kp.tau_factor = p->tau_factor;
     c->kp.recon_space = p->recon_space; c->kp.renorm = p->renorm_fluid_weights; c->kp.couple = p->couple;
+    c->kp.vel_estimate = p->vel_estimate;
     std::string err;
     bool ok = (a->kind == 0) ? rad::build_latlon(a->nzeta, a->npsi, c->host, err)
             : (a->kind == 1) ? rad::build_geodesic(a->nlev, c->host, err) : (err = "bad angle grid kind", false);
@@ -125,6 +124,11 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     t.N = h.N; t.E = h.E; t.ng = g->ng;
     for (int d = 0; d < 3; d++) { t.n[d] = g->n[d]; t.inv_dx[d] = 1.0 / g->dx[d]; }
     t.NI = g->n[0] + 2 * g->ng; t.NJ = g->n[1] + 2 * g->ng; t.NK = g->n[2] + 2 * g->ng;
+    if (cudaDeviceGetAttribute(&t.sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&t.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) != cudaSuccess) {
+        delete c;
+        return cuda_fail(nullptr, "rad_create: device attributes");
+    }
     t.ncell = (long long)t.NI * t.NJ * t.NK;
     // derived angle tables: pinned products T[e][c][k] = N^c * (n^alpha n^beta), and per-angle signed edge weights
     std::vector<double> edge_T((size_t)h.E * 30), nbr_w((size_t)h.N * RAD_MAXNBR, 0.0);
@@ -253,21 +257,70 @@ rad_status rad_fill_ghosts(rad_ctx *c, double *I, void *stream) {
     return RAD_OK;
 }
 
+// The two halves of a stage on one stream (no argument checks: the callers did them).
+// transport: ghost fill, then the tile kernel (stage5.cu) where it serves the context, else the generic flux-divergence kernel
+// (transport.cu).  `fluid` != nullptr with tau_factor != 0 selects the optical-depth-aware flux (Eq.26-29).
+static rad_status run_transport(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
+                                double beta_dt, cudaStream_t s, int kz0 = 0, int kz1 = 0, bool fill = true) {
+    if (fill) {
+        rad_status st = rad_fill_ghosts(c, I_in, s);
+        if (st != RAD_OK) return st;
+    }
+    const bool tau = c->kp.tau_factor != 0.0;
+    rad::StageArgs a{};
+    a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt; a.kz0 = kz0; a.kz1 = kz1;
+    if (rad::stage_angle_serves(c->dev)) {
+        if (tau) {  // per-cell table {u^alphahat, f/2 of the upper faces}
+            if (!c->vel8 && cudaMalloc((void **)&c->vel8, sizeof(double) * 8 * (size_t)c->dev.ncell) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(c, RAD_ENOMEM, "rad_stage: no device memory for the velocity table");
+            }
+            const int nt = rad::launch_tau_table(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->kp.tau_factor * beta_dt, c->vel8, s);
+            if (nt < 0) return cuda_fail(c, "rad_stage (velocity table)");
+            c->launches += nt;
+            a.vel8 = c->vel8;
+        }
+        const int nl = rad::launch_stage_angle(c->dev, c->kp, a, false, s);
+        if (nl < 0) return cuda_fail(c, "rad_stage (tile kernel)");
+        if (nl > 0) { c->launches += nl; return RAD_OK; }
+    }
+    if (kz1 > kz0) return fail(c, RAD_EUNSUPPORTED, "slab-wise transport needs the tile kernel");
+    const double *vel = nullptr;
+    if (tau) {  // generic path: per-cell {u^alphahat, alpha_E}
+        if (!c->vel && cudaMalloc((void **)&c->vel, sizeof(double) * 5 * (size_t)c->dev.ncell) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(c, RAD_ENOMEM, "rad_stage: no device memory for the velocity table");
+        }
+        const int nv = rad::launch_cell_velocity(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->vel, s);
+        if (nv < 0) return cuda_fail(c, "rad_stage (velocity table)");
+        c->launches += nv;
+        vel = c->vel;
+    }
+    const int nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, s, vel, c->kp.tau_factor * beta_dt);
+    if (nl < 0) return cuda_fail(c, "rad_stage (flux divergence)");
+    c->launches += nl;
+    return RAD_OK;
+}
+
+// coupling + mask + fluid increment in place on I: the streaming kernel (stream.cu) where it serves, else the generic one (coupling.cu)
+static rad_status run_coupling(rad_ctx *c, double *I, const double *fluid, double dt, double *T_out, double *dT0, bool count, cudaStream_t s,
+                               int kz0 = 0, int kz1 = 0) {
+    unsigned long long *cnt = count ? c->d_noroot : nullptr;
+    int nl = rad::launch_couple_stream(c->dev, c->kp, I, fluid, c->opac.alpha_a_planck, c->opac.alpha_a_energy, c->opac.alpha_s, dt, T_out, dT0, cnt, s, kz0, kz1);
+    if (nl == 0 && kz1 > kz0) return fail(c, RAD_EUNSUPPORTED, "slab-wise coupling needs the streaming kernel");
+    if (nl == 0) nl = rad::launch_coupling(c->dev, c->kp, I, fluid, c->opac.alpha_a_planck, c->opac.alpha_a_energy, c->opac.alpha_s, dt, T_out, dT0, cnt, s);
+    if (nl < 0) return cuda_fail(c, "rad_couple");
+    c->launches += nl;
+    return RAD_OK;
+}
+
 rad_status rad_transport(rad_ctx *c, double *I_in, double *I_out, const double *I0, double gam0, double gam1, double beta_dt, void *stream) {
     if (!c || !I_in || !I_out) return fail(c, RAD_EINVAL, "rad_transport: NULL argument");
     if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_transport: I_out must not alias I_in or I0 (the stencil reads old values)");
     if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_transport: non-finite weights");
     if (c->kp.tau_factor != 0.0) return fail(c, RAD_ESTATE, "rad_transport: with tau_factor != 0 the spatial flux needs the fluid state (Eq.26-29): use rad_stage");
     DeviceGuard guard(c->device);
-    rad_status st = rad_fill_ghosts(c, I_in, stream);
-    if (st != RAD_OK) return st;
-    rad::StageArgs a{};
-    a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
-    int nl = launch_fused(c->dev, c->kp, a, false, (cudaStream_t)stream);
-    if (nl == 0) nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, (cudaStream_t)stream);
-    if (nl < 0) return cuda_fail(c, "rad_transport");
-    c->launches += nl;
-    return RAD_OK;
+    return run_transport(c, I_in, I_out, I0, nullptr, gam0, gam1, beta_dt, (cudaStream_t)stream);
 }
 
 rad_status rad_couple(rad_ctx *c, double *I, const double *fluid, double dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
@@ -277,126 +330,26 @@ rad_status rad_couple(rad_ctx *c, double *I, const double *fluid, double dt, dou
     DeviceGuard guard(c->device);
     cudaStream_t s = (cudaStream_t)stream;
     if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_couple: memset");
-    int nl = rad::launch_coupling(c->dev, c->kp, I, fluid, c->opac.alpha_a_planck, c->opac.alpha_a_energy, c->opac.alpha_s, dt, T_out, dT0,
-                                  n_noroot ? c->d_noroot : nullptr, s);
-    if (nl < 0) return cuda_fail(c, "rad_couple");
-    c->launches += nl;
-    if (n_noroot) {
-        unsigned long long v = 0;
-        if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
-            return cuda_fail(c, "rad_couple: readback");
-        *n_noroot = (long long)v;
-    }
-    return RAD_OK;
+    rad_status st = run_coupling(c, I, fluid, dt, T_out, dT0, n_noroot != nullptr, s);
+    if (st != RAD_OK) return st;
+    return read_noroot(c, n_noroot, s, "rad_couple: readback");
 }
 
 rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
                      double beta_dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
-    if (!c || !fluid) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
-    if (c->kp.tau_factor != 0.0) {
-        // optical-depth-aware spatial flux (Eq.26-29): velocity table of all cells, then the two-kernel path
-        if (!I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
-        if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_stage: I_out must not alias I_in or I0 (the stencil reads old values)");
-        if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_stage: non-finite weights");
-        if (!c->opac.alpha_a_energy || !c->opac.alpha_s) return fail(c, RAD_ESTATE, "rad_stage: context has no opacities");
-        DeviceGuard guard(c->device);
-        cudaStream_t s = (cudaStream_t)stream;
-        if (!c->vel && cudaMalloc((void **)&c->vel, sizeof(double) * 5 * (size_t)c->dev.ncell) != cudaSuccess) {
-            cudaGetLastError();
-            return fail(c, RAD_ENOMEM, "rad_stage: no device memory for the velocity table");
-        }
-        rad_status st = rad_fill_ghosts(c, I_in, stream);
-        if (st != RAD_OK) return st;
-        static const int tau_path = [] { const char *e = std::getenv("RAD_TAU_PATH"); return e ? std::atoi(e) : 0; }();  // 5 / 3 / 2: force a path (A/B runs)
-        if ((tau_path == 0 || tau_path == 5) && c->kp.couple && c->opac.alpha_a_planck && rad::stage_angle_serves(c->dev)) {
-            // the tile kernel (stage5.cu) with the Eq.28 factor: per-cell table {u^alphahat, f/2 of the upper faces}, then one launch
-            if (!c->vel8 && cudaMalloc((void **)&c->vel8, sizeof(double) * 8 * (size_t)c->dev.ncell) != cudaSuccess) {
-                cudaGetLastError();
-                return fail(c, RAD_ENOMEM, "rad_stage: no device memory for the velocity table");
-            }
-            int nl5 = rad::launch_tau_table(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->kp.tau_factor * beta_dt, c->vel8, s);
-            if (nl5 < 0) return cuda_fail(c, "rad_stage (velocity table)");
-            c->launches += nl5;
-            if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
-            rad::StageArgs a{};
-            a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
-            a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
-            a.T_out = T_out; a.dT0 = dT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
-            a.vel8 = c->vel8;
-            nl5 = rad::launch_stage_angle(c->dev, c->kp, a, true, s);
-            if (nl5 < 0) return cuda_fail(c, "rad_stage (optical-depth-aware flux, tile kernel)");
-            if (nl5 > 0) {
-                c->launches += nl5;
-                if (n_noroot) {
-                    unsigned long long v = 0;
-                    if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
-                        return cuda_fail(c, "rad_stage: readback");
-                    *n_noroot = (long long)v;
-                }
-                return RAD_OK;
-            }
-        }
-        int nl = rad::launch_cell_velocity(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->vel, s);
-        if (nl < 0) return cuda_fail(c, "rad_stage (velocity table)");
-        c->launches += nl;
-        if (tau_path != 2 && c->kp.couple && c->opac.alpha_a_planck) {
-            // fused warp-per-cell stage kernel (stage.cu) with the Eq.28 factor; serves N <= 192 with stored coefficients
-            if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
-            rad::StageArgs a{};
-            a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
-            a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
-            a.T_out = T_out; a.dT0 = dT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
-            a.vel = c->vel; a.tau_dt = c->kp.tau_factor * beta_dt;
-            nl = rad::launch_stage_fused(c->dev, c->kp, a, true, s);
-            if (nl < 0) return cuda_fail(c, "rad_stage (optical-depth-aware flux, fused)");
-            if (nl > 0) {
-                c->launches += nl;
-                if (n_noroot) {
-                    unsigned long long v = 0;
-                    if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
-                        return cuda_fail(c, "rad_stage: readback");
-                    *n_noroot = (long long)v;
-                }
-                return RAD_OK;
-            }
-        }
-        nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, s, c->vel, c->kp.tau_factor * beta_dt);
-        if (nl < 0) return cuda_fail(c, "rad_stage (optical-depth-aware flux)");
-        c->launches += nl;
-        return rad_couple(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot, stream);
-    }
-    if (c->dev.fused_ok && c->dev.ke && c->dev.N <= 256) {
-        // one launch: flux divergence + coupling + mask (stage.cu)
-        if (!I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
-        if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_stage: I_out must not alias I_in or I0 (the stencil reads old values)");
-        if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_stage: non-finite weights");
-        if (c->kp.couple && (!c->opac.alpha_a_planck || !c->opac.alpha_a_energy || !c->opac.alpha_s)) return fail(c, RAD_ESTATE, "rad_stage: context has no opacities");
-        DeviceGuard guard(c->device);
-        cudaStream_t s = (cudaStream_t)stream;
-        rad_status st = rad_fill_ghosts(c, I_in, stream);
-        if (st != RAD_OK) return st;
-        if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
-        rad::StageArgs a{};
-        a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
-        a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
-        a.T_out = T_out; a.dT0 = dT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
-        int nl = launch_fused(c->dev, c->kp, a, true, s);
-        if (nl < 0) return cuda_fail(c, "rad_stage");
-        if (nl > 0) {
-            c->launches += nl;
-            if (n_noroot) {
-                unsigned long long v = 0;
-                if (cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
-                    return cuda_fail(c, "rad_stage: readback");
-                *n_noroot = (long long)v;
-            }
-            return RAD_OK;
-        }
-        // not served: fall through to the two-kernel path (ghosts are already filled; filling twice is harmless)
-    }
-    rad_status st = rad_transport(c, I_in, I_out, I0, gam0, gam1, beta_dt, stream);
+    if (!c || !fluid || !I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage: NULL argument");
+    if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_stage: I_out must not alias I_in or I0 (the stencil reads old values)");
+    if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_stage: non-finite weights");
+    if ((c->kp.couple || c->kp.tau_factor != 0.0) && (!c->opac.alpha_a_planck || !c->opac.alpha_a_energy || !c->opac.alpha_s))
+        return fail(c, RAD_ESTATE, "rad_stage: context has no opacities");
+    DeviceGuard guard(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
+    rad_status st = run_transport(c, I_in, I_out, I0, fluid, gam0, gam1, beta_dt, s);
     if (st != RAD_OK) return st;
-    return rad_couple(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot, stream);
+    st = run_coupling(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot != nullptr, s);
+    if (st != RAD_OK) return st;
+    return read_noroot(c, n_noroot, s, "rad_stage: readback");
 }
 
 // rad_stage_host, pipelined: the block is cut into slabs of planes along z; while slab j is computed, the input planes of
@@ -406,7 +359,7 @@ rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, 
 static rad_status stage_host_pipelined(rad_ctx *c, const double *I_in_host, double *I_out_host, const double *fluid_host, const double *opac_host,
                                        double gam0, double gam1, double beta_dt, double *T_out_host, double *dT0_host, long long *n_noroot) {
     const rad::DeviceTables &t = c->dev;
-    if (!rad::stage_angle_serves(t) || c->kp.tau_factor != 0.0) return RAD_EUNSUPPORTED;
+    if (!rad::stage_angle_serves(t) || !rad::stream_serves(t, c->scratch_I[1]) || c->kp.tau_factor != 0.0) return RAD_EUNSUPPORTED;
     for (int d = 0; d < 3; d++)
         if (c->grid.bc_lo[d] != 0 || c->grid.bc_hi[d] != 0) return RAD_EUNSUPPORTED;
     const int nz = t.n[2], ng = t.ng;
@@ -420,22 +373,20 @@ static rad_status stage_host_pipelined(rad_ctx *c, const double *I_in_host, doub
     double *dfl = c->scratch_small, *dop = dfl + 5 * nc, *dT = dop + 3 * nc, *ddT0 = dT + nc;
     int nslab = (nz + 7) / 8;  // thin slabs: the first copy-in and the last copy-out are not overlapped
     if (nslab > 48) nslab = 48;
-    const int per = (((nz + nslab - 1) / nslab) + 3) & ~3;  // planes per slab, a multiple of the tile heights
+    const int per = (((nz + nslab - 1) / nslab) + 11) / 12 * 12;  // planes per slab, a multiple of every tile height (TZ = 2, 3)
     nslab = (nz + per - 1) / per;
-    std::vector<cudaEvent_t> evH(nslab), evK(nslab);
-    for (int j = 0; j < nslab; j++) {
-        if (cudaEventCreateWithFlags(&evH[j], cudaEventDisableTiming) != cudaSuccess || cudaEventCreateWithFlags(&evK[j], cudaEventDisableTiming) != cudaSuccess)
-            return cuda_fail(c, "rad_stage_host: event");
-    }
-    bool ok = true;
-    cudaEvent_t ev0;
-    ok = cudaEventCreateWithFlags(&ev0, cudaEventDisableTiming) == cudaSuccess;
-    // whoever used the default stream before (the caller's previous work on these buffers) is ordered before the pipeline
+    std::vector<cudaEvent_t> evH(nslab, nullptr), evK(nslab, nullptr);
+    cudaEvent_t ev0 = nullptr;
+    bool ok = cudaEventCreateWithFlags(&ev0, cudaEventDisableTiming) == cudaSuccess;
+    for (int j = 0; j < nslab && ok; j++)
+        ok = cudaEventCreateWithFlags(&evH[j], cudaEventDisableTiming) == cudaSuccess && cudaEventCreateWithFlags(&evK[j], cudaEventDisableTiming) == cudaSuccess;
+    // the caller's earlier work on these buffers (legacy default stream) is ordered before the pipeline
     ok = ok && cudaEventRecord(ev0, 0) == cudaSuccess;
     for (int q = 0; q < 3 && ok; q++) ok = cudaStreamWaitEvent(st[q], ev0, 0) == cudaSuccess;
     if (ok && n_noroot) ok = cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), st[1]) == cudaSuccess;
     const rad_opac saved = c->opac;
     c->opac.alpha_a_planck = dop; c->opac.alpha_a_energy = dop + nc; c->opac.alpha_s = dop + 2 * nc;
+    bool launch_failed = false;
     int p_done = 0;  // array planes [0, p_done) are on their way to the device
     for (int j = 0; j < nslab && ok; j++) {
         const int kb = j * per, ke = kb + per < nz ? kb + per : nz;      // interior planes of the slab
@@ -455,14 +406,8 @@ static rad_status stage_host_pipelined(rad_ctx *c, const double *I_in_host, doub
         const int ob = (j == 0) ? 0 : kb + ng, oe = (j == nslab - 1) ? t.NK : ke + ng;
         ok = ok && cudaMemcpyAsync(dO + (size_t)ob * plane * t.N, dI + (size_t)ob * plane * t.N, pbytes * (oe - ob), cudaMemcpyDeviceToDevice, st[1]) == cudaSuccess;
         if (!ok) break;
-        rad::StageArgs a{};
-        a.I_in = dI; a.I0 = nullptr; a.I_out = dO; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
-        a.fluid = dfl; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
-        a.T_out = dT; a.dT0 = ddT0; a.noroot = n_noroot ? c->d_noroot : nullptr;
-        a.kz0 = kb; a.kz1 = ke;
-        const int nl = rad::launch_stage_angle(t, c->kp, a, true, st[1]);
-        if (nl <= 0) { ok = false; break; }
-        c->launches += nl;
+        if (run_transport(c, dI, dO, nullptr, dfl, gam0, gam1, beta_dt, st[1], kb, ke, false) != RAD_OK ||
+            run_coupling(c, dO, dfl, beta_dt, dT, ddT0, n_noroot != nullptr, st[1], kb, ke) != RAD_OK) { launch_failed = true; break; }
         ok = cudaEventRecord(evK[j], st[1]) == cudaSuccess && cudaStreamWaitEvent(st[2], evK[j], 0) == cudaSuccess;
         ok = ok && cudaMemcpyAsync(I_out_host + (size_t)ob * plane * t.N, dO + (size_t)ob * plane * t.N, pbytes * (oe - ob), cudaMemcpyDeviceToHost, st[2]) == cudaSuccess;
         const size_t cb = sizeof(double) * plane * (oe - ob), co = (size_t)ob * plane;
@@ -473,9 +418,10 @@ static rad_status stage_host_pipelined(rad_ctx *c, const double *I_in_host, doub
     unsigned long long v = 0;
     if (ok && n_noroot) ok = cudaMemcpyAsync(&v, c->d_noroot, sizeof(v), cudaMemcpyDeviceToHost, st[2]) == cudaSuccess;
     for (int q = 0; q < 3; q++) ok = (cudaStreamSynchronize(st[q]) == cudaSuccess) && ok;
-    for (int j = 0; j < nslab; j++) { cudaEventDestroy(evH[j]); cudaEventDestroy(evK[j]); }
-    cudaEventDestroy(ev0);
-    if (!ok) return cuda_fail(c, "rad_stage_host: pipelined copies / launches");
+    for (int j = 0; j < nslab; j++) { if (evH[j]) cudaEventDestroy(evH[j]); if (evK[j]) cudaEventDestroy(evK[j]); }
+    if (ev0) cudaEventDestroy(ev0);
+    if (launch_failed) return RAD_ECUDA;  // text already set by the failing launch
+    if (!ok) return cuda_fail(c, "rad_stage_host: pipelined copies");
     if (n_noroot) *n_noroot = (long long)v;
     return RAD_OK;
 }
@@ -490,10 +436,12 @@ rad_status rad_stage_host(rad_ctx *c, const double *I_in_host, double *I_out_hos
     const size_t ibytes = sizeof(double) * nc * c->dev.N, cb = sizeof(double) * nc;
     for (int q = 0; q < 2; q++)
         if (!c->scratch_I[q] && cudaMalloc((void **)&c->scratch_I[q], ibytes) != cudaSuccess) return fail(c, RAD_ENOMEM, "rad_stage_host: device scratch");
-    if (!c->scratch_small && cudaMalloc((void **)&c->scratch_small, 13 * cb) != cudaSuccess) return fail(c, RAD_ENOMEM, "rad_stage_host: device scratch");
+    if (!c->scratch_small) {
+        if (cudaMalloc((void **)&c->scratch_small, 13 * cb) != cudaSuccess) return fail(c, RAD_ENOMEM, "rad_stage_host: device scratch");
+        if (cudaMemset(c->scratch_small, 0, 13 * cb) != cudaSuccess) return cuda_fail(c, "rad_stage_host: memset");  // ghost entries of T_out / dT0 are returned as 0
+    }
     if (c->kp.couple || opac_host) {
-        static const bool no_pipe = [] { const char *e = std::getenv("RAD_HOST_PIPELINE"); return e && e[0] == '0'; }();
-        if (!no_pipe && opac_host) {
+        if (opac_host) {
             const rad_status ps = stage_host_pipelined(c, I_in_host, I_out_host, fluid_host, opac_host, gam0, gam1, beta_dt, T_out_host, dT0_host, n_noroot);
             if (ps != RAD_EUNSUPPORTED) return ps;
         }
@@ -523,7 +471,8 @@ rad_status rad_moments(rad_ctx *c, const double *I, int frame, const double *flu
     if (frame < 0 || frame > 3) return fail(c, RAD_EINVAL, "rad_moments: frame must be 0..3");
     if (frame == 3 && !fluid) return fail(c, RAD_EINVAL, "rad_moments: fluid frame needs fluid");
     DeviceGuard guard(c->device);
-    int nl = rad::launch_moments(c->dev, I, frame, fluid, out, (cudaStream_t)stream);
+    int nl = rad::launch_moments_stream(c->dev, I, frame, fluid, out, (cudaStream_t)stream);
+    if (nl == 0) nl = rad::launch_moments(c->dev, I, frame, fluid, out, (cudaStream_t)stream);
     if (nl < 0) return cuda_fail(c, "rad_moments");
     c->launches += nl;
     return RAD_OK;

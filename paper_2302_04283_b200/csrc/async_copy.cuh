@@ -36,6 +36,28 @@ __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier
 // barrier among the `nthreads` threads that use the same id (1..15; 0 is __syncthreads)
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 
+// ---- shared-memory access through 32-bit addresses (bytes); `volatile` keeps the program order against barriers
+__device__ __forceinline__ double lds(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+// v = skip ? fallback : shared[addr]; lanes with `skip` take no part in the load (fewer bank conflicts for gathers)
+__device__ __forceinline__ double lds_unless(uint32_t addr, bool skip, double fallback) {
+    double v = fallback;
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@!p ld.shared.f64 %0, [%1];\n}" : "+d"(v) : "r"(addr), "r"((unsigned)skip));
+    return v;
+}
+__device__ __forceinline__ double2 lds2(uint32_t addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts(uint32_t addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
+__device__ __forceinline__ void sts2(uint32_t addr, double x, double y) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(x), "d"(y) : "memory");
+}
+
 __device__ __forceinline__ int hi32(double x) { return __double2hiint(x); }
 
 __device__ __forceinline__ double rcp_seed(double d) {  // MUFU.RCP64H: ~2^-20 relative

@@ -40,6 +40,7 @@ struct DeviceTables {
     int N, E;
     int n[3], ng, NI, NJ, NK;
     long long ncell;
+    int sms, smem_optin;  // device: SM count and the opt-in shared memory per CTA (bytes), queried once in rad_create
     double inv_dx[3];
     // angle tables
     const double *nhat;      // [N][3]
@@ -55,7 +56,7 @@ struct DeviceTables {
     // geometry
     const double *cell;  // [ncell][RAD_NCELL]
     const double *face;  // [ncell][3][RAD_NFACE]
-    // fused stage kernel (stage.cu): per-angle record {own_partner[3], pull_pos[3], 0, 0} as 8 x int16 (16 B),
+    // fused stage kernel (stage5.cu): per-angle record {own_partner[3], pull_pos[3], 0, 0} as 8 x int16 (16 B),
     // 1/dOmega, the owned edge ids, and the stored edge coefficients
     const short *ang_rec;    // [N][8]
     const double *winv;      // [N]
@@ -74,9 +75,7 @@ struct StageArgs {
     const double *fluid, *aP, *aE, *aS;  // coupling only
     double *T_out, *dT0;
     unsigned long long *noroot;
-    const double *vel;  // stage.cu only: optical-depth-aware flux (Eq.26-29), {u^alphahat, alpha_E} per cell, or nullptr (Eq.24)
-    double tau_dt;      // tau_factor * beta_dt
-    const double *vel8; // stage5.cu only: optical-depth-aware flux, per cell {u^alphahat (4), f/2 of the upper x, y, z faces, pad}, or nullptr
+    const double *vel8; // optical-depth-aware flux (Eq.26-29): per cell {u^alphahat (4), f/2 of the upper x, y, z faces, pad}, or nullptr (Eq.24)
     int kz0, kz1;  // stage5 only: update the interior planes kz0 <= k < kz1 (0-based, without ghosts); kz1 <= kz0 = the whole block
 };
 
@@ -85,6 +84,7 @@ struct Params {
     double rgm1;  // 1 / (gamma_gas - 1)
     double tau_factor;  // constant of Eq.26; 0 = free-streaming flux (Eq.24)
     int recon_space, renorm, couple;
+    int vel_estimate;  // 1: radiation-dominated velocity estimate Eq.51-55 in the coupling (NEXT-2)
 };
 
 // kernel launchers (each returns the number of kernels it launched, or -1 after setting a CUDA error)
@@ -100,10 +100,14 @@ int launch_coupling(const DeviceTables &t, const Params &p, double *I, const dou
                     unsigned long long *noroot, cudaStream_t s);
 int launch_moments(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out,
                    cudaStream_t s);
-// fused stage kernel: flux divergence (+ coupling and mask when couple != 0) in one launch; returns 0 if this
-// configuration is not served (caller falls back to launch_fluxdiv + launch_coupling)
-int launch_stage_fused(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
-// angle-resident fused stage kernel (stage5.cu): 1 launched, 0 not served, -1 CUDA error; and its record builder
+// streaming versions (stream.cu; even N, 16-byte aligned I): 1 launched, 0 not served, -1 CUDA error
+int stream_serves(const DeviceTables &t, const void *I);
+int launch_couple_stream(const DeviceTables &t, const Params &p, double *I, const double *fluid, const double *aP, const double *aE, const double *aS,
+                         double dt, double *T_out, double *dT0, unsigned long long *noroot, cudaStream_t s, int kz0 = 0, int kz1 = 0);
+int launch_moments_stream(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out, cudaStream_t s);
+// angle-resident fused stage kernel (stage5.cu): flux divergence (+ coupling and mask when couple != 0) in one launch:
+// 1 launched, 0 this configuration is not served (caller falls back to launch_fluxdiv + launch_coupling), -1 CUDA error;
+// and its record builder
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
 // 1 if launch_stage_angle serves this context (so that a stage can be run slab by slab along z)
 int stage_angle_serves(const DeviceTables &t);

@@ -19,19 +19,12 @@
 //     step's outputs and prepares the next cell's fluid velocity.
 //   * TAU (template): the optical-depth-aware spatial flux of Eq.26-29 -- a per-cell table (k_tau_table) of u^alphahat and f/2
 //     of the upper faces comes in with the other copies for the tile's cells and the halo cells at distance 1.
-#include <cstdlib>
-
 #include "async_copy.cuh"
 #include "stage_math.cuh"
-
-#ifndef RAD_S5_UNROLL
-#define RAD_S5_UNROLL 1
-#endif
 
 namespace rad {
 namespace {
 
-constexpr int kStepUnroll = RAD_S5_UNROLL;
 constexpr int RECN = RAD_STAGE_RECN;  // packed per-cell record, see k_pack_rec
 constexpr int USTR = 64;              // a cell's record slot in shared memory: [0..35] record, [36..43] lower y face,
                                       // [44..51] lower z face, [52..59] rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s
@@ -80,34 +73,46 @@ static_assert(sizeof(Role) == 32, "Role is stored as four doubles");
 struct FaceRec {  // n^a = e0 + e_b n^b;  n_0 / dx_a = E0 + E_b n^b (the grid spacing is folded in)
     double e0, e1, e2, e3, E0, E1, E2, E3;
 };
-__device__ __forceinline__ FaceRec load_face(const double *f) {  // warp-uniform address
-    const double2 a = *reinterpret_cast<const double2 *>(f), b = *reinterpret_cast<const double2 *>(f + 2),
-                  c = *reinterpret_cast<const double2 *>(f + 4), d = *reinterpret_cast<const double2 *>(f + 6);
-    return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
-}
-
 // Upwind flux n^a n_0 I / dx_a (Eq.24) through the face between cells L and R; qLL, qL, qR, qRR are the
-// intensities of the four cells around it.  PLM: van Leer limited slope of the upwind cell (R7): with (far, mid, oth)
-// = (LL, L, R) for n^a > 0 and (RR, R, L) otherwise, the face value is mid + dl dr / (dl + dr), dl = mid - far,
-// dr = oth - mid (the harmonic mean is odd under reversal, so one formula serves both signs).  Branch free; sign tests
-// are integer tests of the high word (na = +-0 -> the flux is 0 either way).
+// intensities of the four cells around it.  PLM: van Leer limited slope of the upwind cell (R7): with (far, up, oth)
+// = (LL, L, R) for n^a >= 0 and (RR, R, L) otherwise, the face value is up + dl dr / (dl + dr), dl = up - far,
+// dr = oth - up (the harmonic mean is odd under reversal, so one formula serves both signs).  oth - up = +-(qR - qL): the
+// difference is formed once and its sign bit flipped with the sign bit of n^a.  Branch free; sign tests are integer tests
+// of the high word (n^a = +-0 -> the flux is 0 either way).  The limited slope is added under a predicate, so a slope
+// that is not used (dl dr <= 0, where dl + dr may be 0) never reaches the result.
 // TAU (Eq.26-29; readings R15-R18, G1 in DESIGN.md): with G = -(1 + 1/n^0bar) of the two cells for this angle and fh = f/2 of the
 // face, the factor 1 - g_up + g of Eq.28 is 1 + fh (G_R - G_L) for n^a > 0 and 1 + fh (G_L - G_R) otherwise.
+struct FaceGeom {  // n^a and n_0 / dx_a of one face for one angle
+    double na, n0;
+    bool neg;       // n^a < 0 (or -0): the upper cell is upwind
+    int flip;       // the sign bit of n^a
+};
+__device__ __forceinline__ FaceGeom face_geom(const FaceRec &f, double n1, double n2, double n3) {
+    FaceGeom g;
+    g.na = chain4(f.e0, f.e1, f.e2, f.e3, n1, n2, n3);
+    g.n0 = chain4(f.E0, f.E1, f.E2, f.E3, n1, n2, n3);
+    g.neg = hi32(g.na) < 0;
+    g.flip = hi32(g.na) & (int)0x80000000;
+    return g;
+}
+// up = the upwind one of (qL, qR), far = the cell behind it, D = qR - qL
+template <bool PLM, bool TAU = false>
+__device__ __forceinline__ double face_value(const FaceGeom &g, double up, double far, double D, double GL = 0.0, double GR = 0.0, double fh = 0.0) {
+    if (PLM) {
+        const double dl = up - far, dr = __hiloint2double(__double2hiint(D) ^ g.flip, __double2loint(D)), pr = dl * dr;
+        const double h = div3(pr, dl + dr);  // only used where pr > 0, i.e. dl + dr != 0
+        if (hi32(pr) > 0) up += h;
+    }
+    if (TAU) up *= fma(fh, g.neg ? GL - GR : GR - GL, 1.0);
+    return __dmul_rn(__dmul_rn(g.na, g.n0), up);
+}
+// all four intensities in registers (x faces)
 template <bool PLM, bool TAU = false>
 __device__ __forceinline__ double face_flux(const FaceRec &f, double n1, double n2, double n3, double qLL, double qL, double qR, double qRR,
                                             double GL = 0.0, double GR = 0.0, double fh = 0.0) {
-    const double na = chain4(f.e0, f.e1, f.e2, f.e3, n1, n2, n3);
-    const double n0 = chain4(f.E0, f.E1, f.E2, f.E3, n1, n2, n3);
-    const bool pos = hi32(na) > 0;
-    double up = pos ? qL : qR;
-    if (PLM) {
-        const double far = pos ? qLL : qRR, oth = pos ? qR : qL;
-        const double dl = up - far, dr = oth - up, pr = dl * dr;
-        const double h = div3(pr, dl + dr);  // only used where pr > 0, i.e. dl + dr != 0
-        up += hi32(pr) > 0 ? h : 0.0;
-    }
-    if (TAU) up *= fma(fh, pos ? GR - GL : GL - GR, 1.0);
-    return __dmul_rn(__dmul_rn(na, n0), up);
+    const FaceGeom g = face_geom(f, n1, n2, n3);
+    const double up = g.neg ? qR : qL, far = PLM ? (g.neg ? qRR : qLL) : 0.0;
+    return face_value<PLM, TAU>(g, up, far, qR - qL, GL, GR, fh);
 }
 
 // TAU: G = -(1 + 1/n^0bar) of a cell for one angle, n^0bar = u^0hat - u^ahat n^ahat (Eq.29)
@@ -115,24 +120,8 @@ __device__ __forceinline__ double tau_G(double u0, double u1, double u2, double 
     return -(1.0 + rcp3(u0 - (u1 * n1 + u2 * n2 + u3 * n3)));
 }
 
-// sums of four values over the warp, all lanes get all four: the first two butterfly steps halve the number of values a
-// lane carries instead of adding four values each
-__device__ __forceinline__ void warp_sum4(double &a, double &b, double &c, double &d, int lane) {
-    const unsigned full = 0xffffffffu;
-    const bool u16 = (lane & 16) != 0;
-    double k0 = u16 ? c : a, k1 = u16 ? d : b;
-    k0 += __shfl_xor_sync(full, u16 ? a : c, 16);
-    k1 += __shfl_xor_sync(full, u16 ? b : d, 16);
-    const bool u8 = (lane & 8) != 0;
-    double k = u8 ? k1 : k0;
-    k += __shfl_xor_sync(full, u8 ? k0 : k1, 8);
-    k += __shfl_xor_sync(full, k, 4);
-    k += __shfl_xor_sync(full, k, 2);
-    k += __shfl_xor_sync(full, k, 1);
-    a = __shfl_sync(full, k, 0); b = __shfl_sync(full, k, 8); c = __shfl_sync(full, k, 16); d = __shfl_sync(full, k, 24);
-}
-
-// the four warp sums written to shared memory at `dst` (32 bytes) by the lanes that hold them after the butterfly
+// sums of four values over the warp, written to shared memory at `dst` (32 bytes) by the lanes that hold them after the
+// butterfly: the first two steps halve the number of values a lane carries instead of adding four values each
 __device__ __forceinline__ void warp_sum4_to(double a, double b, double c, double d, int lane, uint32_t dst) {
     const unsigned full = 0xffffffffu;
     const bool u16 = (lane & 16) != 0;
@@ -148,90 +137,9 @@ __device__ __forceinline__ void warp_sum4_to(double a, double b, double c, doubl
     if ((lane & 7) == 0) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dst + (uint32_t)lane), "d"(k) : "memory");  // lanes 0, 8, 16, 24 hold a, b, c, d
 }
 
-// the same over the WPC warps of a cell: partial sums through `red` ([WPC][4] doubles), summed by every thread in the
-// same order
-template <int WPC>
-__device__ __forceinline__ void cell_sum4(double &a, double &b, double &c, double &d, int lane, int wc, double *red, int barid) {
-    warp_sum4(a, b, c, d, lane);
-    if (WPC > 1) {
-        if (lane == 0) {
-            reinterpret_cast<double2 *>(red + wc * 4)[0] = make_double2(a, b);
-            reinterpret_cast<double2 *>(red + wc * 4)[1] = make_double2(c, d);
-        }
-        named_bar_sync(barid, WPC * 32);
-        a = b = c = d = 0.0;
-#pragma unroll
-        for (int q = 0; q < WPC; q++) {
-            const double2 v0 = reinterpret_cast<const double2 *>(red + q * 4)[0], v1 = reinterpret_cast<const double2 *>(red + q * 4)[1];
-            a += v0.x; b += v0.y; c += v1.x; d += v1.y;
-        }
-    }
-}
-
-// ---- shared-memory access through 32-bit addresses (bytes); `volatile` keeps the program order against barriers
-__device__ __forceinline__ double lds(uint32_t addr) {
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-    return v;
-}
-// v = skip ? fallback : shared[addr]; lanes with `skip` take no part in the load (fewer bank conflicts for gathers)
-__device__ __forceinline__ double lds_unless(uint32_t addr, bool skip, double fallback) {
-    double v = fallback;
-    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %2, 0;\n@!p ld.shared.f64 %0, [%1];\n}" : "+d"(v) : "r"(addr), "r"((unsigned)skip));
-    return v;
-}
-__device__ __forceinline__ double2 lds2(uint32_t addr) {
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ void sts(uint32_t addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
-__device__ __forceinline__ void sts2(uint32_t addr, double x, double y) {
-    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(x), "d"(y) : "memory");
-}
 __device__ __forceinline__ FaceRec lds_face(uint32_t addr) {  // warp-uniform address
     const double2 a = lds2(addr), b = lds2(addr + 16), c = lds2(addr + 32), d = lds2(addr + 48);
     return {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
-}
-
-// Quartic Eq.49 solved for the temperature change d = T_+ - T_- (R13), as quartic_delta (stage_math.cuh) with cheaper
-// scalar arithmetic: reciprocals by rcp3, the fourth root of the starting point from the hardware rsqrt seeds (the start
-// only has to be near the upper bound: g is convex and increasing, so Newton converges from either side after one step).
-__device__ __forceinline__ bool quartic_delta_fast(double B4, double B1, double Bp, double Tm, double &d) {
-    const double B0 = Bp - B1 * Tm;
-    if (!(B0 < 0.0) || !(B1 > 0.0) || !(B4 >= 0.0) || !isfinite(B0) || !isfinite(B1) || !isfinite(B4)) return false;
-    if (B4 == 0.0) { d = -Bp * rcp3(B1); return true; }
-    const double B44 = 4.0 * B4, aBp = fabs(Bp);
-    // start to the right of the root (g is convex and increasing there, Newton is then monotone): the Newton step from T_-
-    // (d = 0) lands right of the root from either side and is close for cells near equilibrium; where it lands far away
-    // (more than T_- beyond T_-) the upper bound min(-B0/B1, (-B0/B4)^(1/4)) caps it (fourth root from the hardware rsqrt
-    // seeds: the start only has to be near the bound)
-    {
-        const double T2 = Tm * Tm, q = B4 * (T2 * T2);
-        d = -(q + Bp) * rcp3(fma(B44, T2 * Tm, B1));
-    }
-    if (d > Tm) {
-        const double y = -B0 * rcp3(B4);
-        double r1, r2;
-        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r1) : "d"(y));
-        const double sy = y * r1;
-        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r2) : "d"(sy));
-        double T0 = sy * r2;                         // ~ y^(1/4)
-        if (!(T0 > 0.0)) T0 = __longlong_as_double(0x7ff0000000000000ll);  // y outside the range of the approximation: the other bound alone
-        d = fmin(d, fmin(-B0 * rcp3(B1), T0) - Tm);
-    }
-    for (int it = 0; it < 60; it++) {
-        const double T = Tm + d, T2 = T * T, T3 = T2 * T, q = B4 * (T2 * T2);
-        const double g = q + fma(B1, d, Bp), gp = fma(B44, T3, B1);
-        const double rgp = rcp3(gp);  // gp >= B1 > 0, finite
-        const double dd = g * rgp;
-        d -= dd;
-        // converged to rounding, or so close that this (quadratically convergent) step already was the last useful one:
-        // the error left is <= 1.5 dd^2 / T
-        const double add = fabs(dd);
-        if (add <= 1e-15 * (fabs(d) + (aBp + q) * rgp) || add <= 3e-9 * T) break;
-    }
-    return true;
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -481,7 +389,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         }
     };
 
-#pragma unroll(kStepUnroll)
+#pragma unroll 1
     for (int s = 0; s < nsteps; s++) {
         const int b = s & 1;
         mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
@@ -570,16 +478,20 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                     q01 = lds2(vq); q23 = lds2(vq + 16);
                 }
                 const double fhu = ax == 1 ? own46.y : own6;
-                double m1[NITER], p1[NITER], p2[NITER], F[NITER];
+                // the upper face lies between this cell (x0, in a register) and the cell above (p1); the cell behind the upwind one
+                // (below: m1, above: p2) is loaded from the row the sign of n^a selects
+                FaceGeom gu[NITER];
+                double p1[NITER], far[NITER], F[NITER];
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
-                    m1[it] = lds(rm1 + OFF8(it)); p1[it] = lds(rp1 + OFF8(it));
-                    p2[it] = PLM ? lds(rp2 + OFF8(it)) : 0.0;
+                    gu[it] = face_geom(fh, n1[it], n2[it], n3[it]);
+                    p1[it] = lds(rp1 + OFF8(it));
+                    far[it] = PLM ? lds((gu[it].neg ? rp2 : rm1) + OFF8(it)) : 0.0;
                 }
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
-                    F[it] = face_flux<PLM, TAU>(fh, n1[it], n2[it], n3[it], m1[it], x0[it], p1[it], p2[it], TAU ? G0[it] : 0.0,
-                                                TAU ? tau_G(q01.x, q01.y, q23.x, q23.y, n1[it], n2[it], n3[it]) : 0.0, fhu);
+                    F[it] = face_value<PLM, TAU>(gu[it], gu[it].neg ? p1[it] : x0[it], far[it], p1[it] - x0[it], TAU ? G0[it] : 0.0,
+                                                 TAU ? tau_G(q01.x, q01.y, q23.x, q23.y, n1[it], n2[it], n3[it]) : 0.0, fhu);
                     d[it] += F[it];
                 }
                 if (publish) {
@@ -596,10 +508,12 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                         l01 = lds2(vq); l23 = lds2(vq + 16); fhl = lds(vq + (ax == 1 ? 40 : 48));
                     }
 #pragma unroll
-                    for (int it = 0; it < NITER; it++) {
-                        const double m2 = PLM ? lds(rm2 + OFF8(it)) : 0.0;
-                        d[it] -= face_flux<PLM, TAU>(fl, n1[it], n2[it], n3[it], m2, m1[it], x0[it], p1[it],
-                                                     TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0, TAU ? G0[it] : 0.0, fhl);
+                    for (int it = 0; it < NITER; it++) {  // the lower face: between the cell below (m1) and this one
+                        const FaceGeom gl = face_geom(fl, n1[it], n2[it], n3[it]);
+                        const double m1 = lds(rm1 + OFF8(it));
+                        const double farl = PLM ? (gl.neg ? p1[it] : lds_unless(rm2 + OFF8(it), gl.neg, 0.0)) : 0.0;
+                        d[it] -= face_value<PLM, TAU>(gl, gl.neg ? x0[it] : m1, farl, x0[it] - m1,
+                                                      TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0, TAU ? G0[it] : 0.0, fhl);
                     }
                 }
             }
@@ -608,22 +522,21 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             const uint32_t r_m2 = haloS + (uint32_t)((4 * TZ) * Np) * 8u, r_m1 = haloS + (uint32_t)((4 * TZ + 1) * Np) * 8u, r_0 = ringS,
                            r_p1 = ringS + (uint32_t)(TY * Np) * 8u;
             const FaceRec fl = lds_face(aUb - (uint32_t)cs * (USTR * 8u) + 8 * 44);
-            double q0[NITER], q1[NITER], q2[NITER], q3[NITER];
-#pragma unroll
-            for (int it = 0; it < NITER; it++) {
-                q0[it] = PLM ? lds(r_m2 + OFF8(it)) : 0.0; q1[it] = lds(r_m1 + OFF8(it)); q2[it] = lds(r_0 + OFF8(it)); q3[it] = lds(r_p1 + OFF8(it));
-            }
-#pragma unroll
             double2 l01 = make_double2(1.0, 0.0), l23 = make_double2(0.0, 0.0), r01 = l01, r23 = l23;
             double fhl = 0.0;
             if (TAU) {  // cell (0,0) and the halo cell below it in z
                 const uint32_t vl = smb + 8u * (uint32_t)(L.oVh + (b * T::NVH + 2 * TZ) * 8), vr = smb + 8u * (uint32_t)(L.oV + ((s & 3) * NC) * 8);
                 l01 = lds2(vl); l23 = lds2(vl + 16); fhl = lds(vl + 48); r01 = lds2(vr); r23 = lds2(vr + 16);
             }
+            double q0[NITER];
 #pragma unroll
-            for (int it = 0; it < NITER; it++)
-                q0[it] = face_flux<PLM, TAU>(fl, n1[it], n2[it], n3[it], q0[it], q1[it], q2[it], q3[it], TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0,
-                                             TAU ? tau_G(r01.x, r01.y, r23.x, r23.y, n1[it], n2[it], n3[it]) : 0.0, fhl);
+            for (int it = 0; it < NITER; it++) {
+                const FaceGeom gl = face_geom(fl, n1[it], n2[it], n3[it]);
+                const double q1 = lds(r_m1 + OFF8(it)), q2 = lds(r_0 + OFF8(it));
+                const double farl = PLM ? lds((gl.neg ? r_p1 : r_m2) + OFF8(it)) : 0.0;
+                q0[it] = face_value<PLM, TAU>(gl, gl.neg ? q2 : q1, farl, q2 - q1, TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0,
+                                              TAU ? tau_G(r01.x, r01.y, r23.x, r23.y, n1[it], n2[it], n3[it]) : 0.0, fhl);
+            }
 #pragma unroll
             for (int it = 0; it < NITER; it++)
                 if (it < NITER - 1 || last_valid) sts(aFx + (uint32_t)(b * Np) * 8u + OFF8(it), q0[it]);
@@ -712,7 +625,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                     const double B4 = A2 * aP * p.a_rad, om = 1.0 - A2 * aS;               // Eq.50
                     const double B1 = Cv * om, Bp = A1 - om * Em;
                     double dTemp = 0.0;
-                    if (!quartic_delta_fast(B4, B1, Bp, Tm, dTemp)) {
+                    if (!quartic_delta(B4, B1, Bp, Tm, dTemp)) {
                         flag = -1.0;
                     } else {
                         flag = 1.0;
@@ -803,7 +716,7 @@ int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, bool co
     using T = Tile<TY, TZ, WPC, TAU>;
     const Layout5 L = make_layout5<T>(t.N);
     const size_t smem = sizeof(double) * (size_t)L.total;
-    if (smem > 227 * 1024) return 0;
+    if (smem > (size_t)t.smem_optin) return 0;
     // run length along x: long runs amortise the prologue, short runs fill the SMs of small grids; pick the candidate
     // with the fewest CTA waves x (steps + prologue cost)
     const int nz = a.kz1 > a.kz0 ? a.kz1 - a.kz0 : t.n[2];
@@ -812,7 +725,7 @@ int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, bool co
     double best = 1e300;
     for (int cand = t.n[0];; cand = (cand + 1) / 2) {
         const long long ctas = tiles * ((t.n[0] + cand - 1) / cand);
-        const double cost = (double)((ctas + 147) / 148) * (cand + 3);
+        const double cost = (double)((ctas + t.sms - 1) / t.sms) * (cand + 3);
         if (cost < best) { best = cost; KX = cand; }
         if (cand <= 4) break;
     }
@@ -823,9 +736,7 @@ int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, bool co
         if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
         k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL, TAU><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                                  \
     } while (0)
-    if (TAU) {  // the optical-depth-aware flux is only reached through rad_stage (with the coupling half)
-        if (p.recon_space == 1) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(false, true);
-    } else if (p.recon_space == 1) { if (couple) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(true, false); }
+    if (p.recon_space == 1) { if (couple) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(true, false); }
     else { if (couple) RAD_LAUNCH5(false, true); else RAD_LAUNCH5(false, false); }
 #undef RAD_LAUNCH5
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
@@ -870,54 +781,44 @@ __global__ void __launch_bounds__(256) k_tau_table(const DeviceTables t, const d
 
 }  // namespace
 
+// The tile shape per number of angles (the A/B runs behind these choices are in
+// profiles/r1_k_stage5_ncu_full.md).  CALL(NITER, WPC, TY, TZ): NITER * WPC * 32 >= N angle slots per cell.
+#define RAD_S5_DISPATCH(N, CALL)                 \
+    do {                                         \
+        if ((N) <= 32) CALL(1, 1, 4, 2);         \
+        else if ((N) <= 64) CALL(1, 2, 4, 2);    \
+        else if ((N) <= 96) CALL(3, 1, 4, 3);    \
+        else if ((N) <= 128) CALL(2, 2, 4, 2);   \
+        else if ((N) <= 192) CALL(3, 2, 4, 2);   \
+        else CALL(4, 2, 2, 2);                   \
+    } while (0)
+
 // returns 1 (launched), 0 (this configuration is not served by this kernel), -1 (CUDA error)
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
-    if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr) return 0;
-    if (t.N & 1) return 0;  // rows must be multiples of 16 bytes for the bulk copies
-    if (((uintptr_t)a.I_in & 15) || ((uintptr_t)t.ke & 15) || ((uintptr_t)t.rec & 15) || ((uintptr_t)a.vel8 & 15)) return 0;
-    const int N = t.N;
-    if (N <= 32) return launch5<1, 1, 4, 2>(t, p, a, couple, s);
-    if (N <= 64) return launch5<1, 2, 4, 2>(t, p, a, couple, s);
-    if (N <= 96) {
-        static const int var = [] { const char *e = std::getenv("RAD_S5_VARIANT"); return e ? std::atoi(e) : 0; }();
-        if (var == 1) return launch5<1, 3, 4, 2>(t, p, a, couple, s);
-        if (var == 2) return launch5<3, 1, 4, 4>(t, p, a, couple, s);
-        if (var == 3) return launch5<3, 1, 4, 2>(t, p, a, couple, s);
-        if (var == 4) return launch5<3, 1, 5, 2>(t, p, a, couple, s);
-        if (var == 5) return launch5<3, 1, 6, 2>(t, p, a, couple, s);
-        if (var == 6) return launch5<3, 1, 3, 4>(t, p, a, couple, s);
-        return launch5<3, 1, 4, 3>(t, p, a, couple, s);
-    }
-    if (N <= 128) return launch5<2, 2, 4, 2>(t, p, a, couple, s);
-    if (N <= 192) {
-        static const int var = [] { const char *e = std::getenv("RAD_S5_VARIANT"); return e ? std::atoi(e) : 0; }();
-        if (var == 1) return launch5<2, 3, 3, 2>(t, p, a, couple, s);
-        if (var == 2) return launch5<2, 3, 4, 2>(t, p, a, couple, s);
-        if (var == 3) return launch5<3, 2, 3, 2>(t, p, a, couple, s);
-        if (var == 4) return launch5<6, 1, 4, 2>(t, p, a, couple, s);
-        if (var == 5) return launch5<6, 1, 3, 3>(t, p, a, couple, s);
-        if (var == 6) return launch5<3, 2, 2, 2, 2>(t, p, a, couple, s);
-        if (var == 7) return launch5<3, 2, 3, 1, 2>(t, p, a, couple, s);
-        return launch5<3, 2, 4, 2>(t, p, a, couple, s);
-    }
-    if (N <= 256) return launch5<4, 2, 2, 2>(t, p, a, couple, s);  // geodesic level 5 (252 angles): 2 KB rows, 2 x 2 tiles
+    if (!stage_angle_serves(t)) return 0;
+    if (((uintptr_t)a.I_in & 15) || ((uintptr_t)a.vel8 & 15)) return 0;  // rows are brought in by 16-byte bulk copies
+#define RAD_S5_CALL(NITER, WPC, TY, TZ) return launch5<NITER, WPC, TY, TZ>(t, p, a, couple, s)
+    RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
+#undef RAD_S5_CALL
     return 0;
 }
 
 int stage_angle_serves(const DeviceTables &t) {
-    if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr || (t.N & 1) || t.N > 256) return 0;
-    if (t.N > 192) return sizeof(double) * (size_t)make_layout5<Tile<2, 2, 2>>(t.N).total <= 227 * 1024;
-    if (t.N > 128) return sizeof(double) * (size_t)make_layout5<Tile<4, 2, 2>>(t.N).total <= 227 * 1024;
-    return 1;
+    if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr || (t.N & 1) || t.N > 256) return 0;  // rows must be multiples of 16 bytes
+    if (((uintptr_t)t.ke & 15) || ((uintptr_t)t.rec & 15)) return 0;
+#define RAD_S5_CALL(NITER, WPC, TY, TZ) return sizeof(double) * (size_t)make_layout5<Tile<TY, TZ, WPC, false>>(t.N).total <= (size_t)t.smem_optin
+    RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
+#undef RAD_S5_CALL
+    return 0;
 }
 
 int launch_tau_table(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double tau_dt, double *vel8, cudaStream_t s) {
-    k_tau_table<<<148 * 4, 256, 0, s>>>(t, fluid, aE, aS, tau_dt, vel8);
+    k_tau_table<<<t.sms * 4, 256, 0, s>>>(t, fluid, aE, aS, tau_dt, vel8);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s) {
-    k_pack_rec<<<148 * 8, 256, 0, s>>>(t, rec);
+    k_pack_rec<<<t.sms * 8, 256, 0, s>>>(t, rec);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

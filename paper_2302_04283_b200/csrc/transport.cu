@@ -3,6 +3,7 @@
 // Paper: section 2.3-2.4.  Eq.24 spatial upwind flux, Eq.25 angular upwind flux, Eq.22 update
 // of C = n^0 n_0 I, then I* = C*/(n^0 n_0) (P:L79).  Intensities are I[cell][angle], angle innermost.
 #include <math.h>
+#include <stdint.h>
 
 #include "rad_internal.h"
 
@@ -12,7 +13,7 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 // ghost fill: one launch per axis, in x, y, z order so that edges and corners are filled
 // ------------------------------------------------------------------------------------------------
-__global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int NK, int ng, int axis, int nint, int bc_lo, int bc_hi) {
+__global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int NK, int ng, int axis, int nint, int bc_lo, int bc_hi, int vec2) {
     // one CTA per ghost cell of this axis' two slabs; threads over angles
     const int dims[3] = {NI, NJ, NK};
     int d[3];
@@ -37,7 +38,7 @@ __global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int
     const long long cd = ((long long)d[2] * NJ + d[1]) * NI + d[0], cs = ((long long)s[2] * NJ + s[1]) * NI + s[0];
     const double2 *ps = reinterpret_cast<const double2 *>(I + cs * N);
     double2 *pd = reinterpret_cast<double2 *>(I + cd * N);
-    if ((N & 1) == 0) {
+    if (vec2) {  // rows are 16-byte aligned: N even and the array itself aligned
         for (int n = threadIdx.x; n < N / 2; n += blockDim.x) pd[n] = ps[n];
     } else {
         for (int n = threadIdx.x; n < N; n += blockDim.x) I[cd * N + n] = I[cs * N + n];
@@ -198,7 +199,7 @@ int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_h
         long long ext[3] = {t.NI, t.NJ, t.NK};
         ext[ax] = 2 * t.ng;
         const long long blocks = ext[0] * ext[1] * ext[2];
-        k_fill_ghosts<<<(unsigned)blocks, 64, 0, s>>>(I, t.N, t.NI, t.NJ, t.NK, t.ng, ax, t.n[ax], bc_lo[ax], bc_hi[ax]);
+        k_fill_ghosts<<<(unsigned)blocks, 64, 0, s>>>(I, t.N, t.NI, t.NJ, t.NK, t.ng, ax, t.n[ax], bc_lo[ax], bc_hi[ax], (t.N & 1) == 0 && ((uintptr_t)I & 15) == 0);
         if (cudaGetLastError() != cudaSuccess) return -1;
         launches++;
     }
@@ -206,7 +207,7 @@ int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_h
 }
 
 int launch_cell_velocity(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double *vel, cudaStream_t s) {
-    k_cell_velocity<<<148 * 4, 256, 0, s>>>(t, fluid, aE, aS, vel);
+    k_cell_velocity<<<t.sms * 4, 256, 0, s>>>(t, fluid, aE, aS, vel);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
