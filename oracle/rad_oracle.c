@@ -34,6 +34,7 @@ static const double PI = 3.14159265358979323846;
  * ==================================================================================== */
 struct orc_angles {
     int N, E;
+    int kind, nzeta, npsi; /* 0 latitude-longitude (nzeta x npsi), 1 geodesic */
     double *nhat;    /* [N][3]  unit directions n^ahat, Eq.15b-d */
     double *domega;  /* [N]     Delta Omega */
     int *nnbr;       /* [N] */
@@ -125,6 +126,7 @@ orc_angles *orc_angles_latlon(int nzeta, int npsi) {
     orc_angles *A = calloc(1, sizeof(*A));
     int N = nzeta * npsi;
     ang_alloc(A, N, 2 * N + 4);
+    A->kind = 0; A->nzeta = nzeta; A->npsi = npsi;
     double dpsi = 2.0 * PI / npsi;
     for (int l = 0; l < nzeta; l++) {
         double muf0 = 1.0 - 2.0 * l / nzeta, muf1 = 1.0 - 2.0 * (l + 1) / nzeta;
@@ -193,6 +195,7 @@ orc_angles *orc_angles_geodesic(int nlev) {
     int L = nlev, N = 10 * L * L + 2, NT = 20 * L * L;
     orc_angles *A = calloc(1, sizeof(*A));
     ang_alloc(A, N, 3 * N);
+    A->kind = 1;
     /* icosahedron: north pole V0, upper ring U_k = V_{1+k}, lower ring L_k = V_{6+k}, south pole V11 */
     double V[12][3];
     double cr = 2.0 / sqrt(5.0), sr = 1.0 / sqrt(5.0);
@@ -475,6 +478,10 @@ struct orc_problem {
     double gamma_gas, a_rad, n0_crit;
     int recon_space, renorm, couple;
     double tau_factor; /* constant of Eq.26; 0 = free-streaming flux Eq.24 */
+    int recon_angle;   /* 0 donor cell, 1 PLM on the latitude-longitude grid incl. across the poles */
+    int vel_estimate;  /* 1: radiation-dominated velocity estimate Eq.51-55 */
+    int dt0_literal;   /* 0: dT^0_alpha = -sum n^0 n_alpha (I_+ - I*) dOmega; 1: -(R^0_alpha[I_+] - R^0_alpha[I*]) formed from two sums */
+    int *mirror;       /* [3][N] angle whose direction is n with component a flipped (reflecting boundary, bc code 3), or -1 */
     long long ncell;
     double *cell; /* [ncell][ORC_NCELL] */
     double *face; /* [ncell][3][ORC_NFACE]: lower face of each cell along each axis */
@@ -530,6 +537,20 @@ orc_problem *orc_create(int kind, double M, double a, double excise_r, const int
     P->cell = malloc(sizeof(double) * P->ncell * ORC_NCELL);
     P->face = malloc(sizeof(double) * P->ncell * 3 * ORC_NFACE);
     P->excised = calloc(P->ncell, sizeof(int));
+    /* R20 (reflecting wall): the image of direction n under a reflection that flips tetrad component a is the grid
+     * angle whose direction vector equals n-hat with that component negated; -1 where the grid has no such angle */
+    P->mirror = malloc(sizeof(int) * 3 * ang->N);
+    for (int ax = 0; ax < 3; ax++)
+        for (int n = 0; n < ang->N; n++) {
+            double want[3] = {ang->nhat[3 * n], ang->nhat[3 * n + 1], ang->nhat[3 * n + 2]};
+            want[ax] = -want[ax];
+            int found = -1;
+            for (int m = 0; m < ang->N && found < 0; m++) {
+                double d0 = ang->nhat[3 * m] - want[0], d1 = ang->nhat[3 * m + 1] - want[1], d2 = ang->nhat[3 * m + 2] - want[2];
+                if (fabs(d0) < 1e-12 && fabs(d1) < 1e-12 && fabs(d2) < 1e-12) found = m;
+            }
+            P->mirror[ax * ang->N + n] = found;
+        }
 #pragma omp parallel for schedule(static)
     for (int k = 0; k < P->NK; k++)
         for (int j = 0; j < P->NJ; j++)
@@ -554,7 +575,7 @@ orc_problem *orc_create(int kind, double M, double a, double excise_r, const int
             }
     return P;
 }
-void orc_destroy(orc_problem *P) { if (!P) return; free(P->cell); free(P->face); free(P->excised); free(P); }
+void orc_destroy(orc_problem *P) { if (!P) return; free(P->cell); free(P->face); free(P->excised); free(P->mirror); free(P); }
 long long orc_ncells_total(const orc_problem *P) { return P->ncell; }
 void orc_get_geometry(const orc_problem *P, double *cell, double *face, int *excised) {
     if (cell) memcpy(cell, P->cell, sizeof(double) * P->ncell * ORC_NCELL);
@@ -571,15 +592,26 @@ void orc_fill_ghosts(const orc_problem *P, double *I) {
     int N = P->ang->N, ng = P->ng, dims[3] = {P->NI, P->NJ, P->NK};
     for (int ax = 0; ax < 3; ax++)
         for (int k = 0; k < P->NK; k++) for (int j = 0; j < P->NJ; j++) for (int i = 0; i < P->NI; i++) {
-            int id[3] = {i, j, k}, src[3] = {i, j, k}, q = id[ax], nint = P->n[ax];
+            int id[3] = {i, j, k}, src[3] = {i, j, k}, q = id[ax], nint = P->n[ax], bc;
             int wrap = ng + (((q - ng) % nint) + nint) % nint; /* periodic image inside the interior (also for nint < ng) */
             if (q < ng) {
-                if (P->bc_lo[ax] == 1) src[ax] = wrap; else if (P->bc_lo[ax] == 2) src[ax] = ng; else continue;
+                bc = P->bc_lo[ax];
+                if (bc == 1) src[ax] = wrap; else if (bc == 2) src[ax] = ng; else if (bc == 3) src[ax] = 2 * ng - 1 - q; else continue;
             } else if (q >= dims[ax] - ng) {
-                if (P->bc_hi[ax] == 1) src[ax] = wrap; else if (P->bc_hi[ax] == 2) src[ax] = ng + nint - 1; else continue;
+                bc = P->bc_hi[ax];
+                if (bc == 1) src[ax] = wrap; else if (bc == 2) src[ax] = ng + nint - 1; else if (bc == 3) src[ax] = 2 * (dims[ax] - ng) - 1 - q; else continue;
             } else continue;
-            memcpy(&I[cidx(P, k, j, i) * N], &I[cidx(P, src[2], src[1], src[0]) * N], sizeof(double) * N);
+            double *dst = &I[cidx(P, k, j, i) * N];
+            const double *sp = &I[cidx(P, src[2], src[1], src[0]) * N];
+            if (bc == 3) { /* R20: mirror cell across the wall, direction with the normal component flipped */
+                for (int n = 0; n < N; n++) { int m = P->mirror[ax * N + n]; dst[n] = (m >= 0) ? sp[m] : 0.0; }
+            } else memcpy(dst, sp, sizeof(double) * N);
         }
+}
+/* 1 if every angle has its mirror image under the flip of component ax on this angle grid */
+int orc_has_mirror(const orc_problem *P, int ax) {
+    for (int n = 0; n < P->ang->N; n++) if (P->mirror[ax * P->ang->N + n] < 0) return 0;
+    return 1;
 }
 
 /* ======================================================================================
@@ -594,6 +626,31 @@ static double vl_slope(double qm, double q0, double qp) {
     double dl = q0 - qm, dr = qp - q0, pr = dl * dr;
     return (pr > 0.0) ? 2.0 * pr / (dl + dr) : 0.0;
 }
+/* PPM (Colella & Woodward 1984, cited P:L276) on uniform spacing, as used for cell-centred variables without characteristic
+ * tracing: the monotonised parabola of cell 0 from the five values q[-2..2]; returns its values at the lower (qm) and upper (qp)
+ * face.  CW84 Eq.1.6-1.8: interface value q_{1/2} = q_0 + (q_1 - q_0)/2 - (dq_1 - dq_0)/6 with van Leer-limited average slopes
+ * dq = min(|q_{+1} - q_{-1}|/2, 2|q_{+1} - q_0|, 2|q_0 - q_{-1}|) sgn(q_{+1} - q_{-1}) at non-extrema, 0 at extrema;
+ * CW84 Eq.1.10: flatten at extrema, pull the far face in where the parabola overshoots. */
+static double ppm_dq(double qm, double q0, double qp) {
+    double dl = q0 - qm, dr = qp - q0;
+    if (dl * dr <= 0.0) return 0.0;
+    double d = 0.5 * (qp - qm), lim = fmin(2.0 * fabs(dl), 2.0 * fabs(dr));
+    return (d > 0.0 ? 1.0 : -1.0) * fmin(fabs(d), lim);
+}
+static void ppm_states(const double q[5], double *qm_out, double *qp_out) {
+    double dqm = ppm_dq(q[0], q[1], q[2]), dq0 = ppm_dq(q[1], q[2], q[3]), dqp = ppm_dq(q[2], q[3], q[4]);
+    double qm = q[1] + 0.5 * (q[2] - q[1]) - (dq0 - dqm) / 6.0; /* value at the lower face */
+    double qp = q[2] + 0.5 * (q[3] - q[2]) - (dqp - dq0) / 6.0; /* value at the upper face */
+    double q0 = q[2];
+    if ((qp - q0) * (q0 - qm) <= 0.0) { qm = q0; qp = q0; }
+    else {
+        double dq = qp - qm, q6 = 6.0 * (q0 - 0.5 * (qm + qp));
+        if (dq * q6 > dq * dq) qm = 3.0 * q0 - 2.0 * qp;
+        else if (-dq * dq > dq * q6) qp = 3.0 * q0 - 2.0 * qm;
+    }
+    *qm_out = qm; *qp_out = qp;
+}
+
 /* Eq.24: flux of n^a n_0 I through the LOWER face of cell id[] along axis ax, angle n.
  * With vel != NULL (tau_factor != 0): the optical-depth-aware flux of Eq.26-29.  vel[cell][5] holds the
  * tetrad-frame fluid velocity u^alphahat (4) of each cell (its own cell-centre tetrad, R10) and alpha_E = alpha^a_E + alpha^s.
@@ -611,9 +668,19 @@ static double face_flux(const orc_problem *P, const double *I, int ax, int i, in
     if (na > 0.0) {
         Iup = qL;
         if (P->recon_space == 1) Iup = qL + 0.5 * vl_slope(I[cLL * N + n], qL, qR);
+        else if (P->recon_space == 2) { /* upper-face value of the parabola of cell L */
+            long long c3 = cidx(P, k - 3 * st[2], j - 3 * st[1], i - 3 * st[0]);
+            double q[5] = {I[c3 * N + n], I[cLL * N + n], qL, qR, I[cRR * N + n]}, qm;
+            ppm_states(q, &qm, &Iup);
+        }
     } else if (na < 0.0) {
         Iup = qR;
         if (P->recon_space == 1) Iup = qR - 0.5 * vl_slope(qL, qR, I[cRR * N + n]);
+        else if (P->recon_space == 2) { /* lower-face value of the parabola of cell R */
+            long long c3 = cidx(P, k + 2 * st[2], j + 2 * st[1], i + 2 * st[0]);
+            double q[5] = {I[cLL * N + n], qL, qR, I[cRR * N + n], I[c3 * N + n]}, qp;
+            ppm_states(q, &Iup, &qp);
+        }
     } else return 0.0;
     if (vel) {
         const double *vL = &vel[cL * 5], *vR = &vel[cR * 5];
@@ -628,6 +695,28 @@ static double face_flux(const orc_problem *P, const double *I, int ax, int i, in
     }
     return na * n0 * Iup;
 }
+/* R21: PLM in angle on the latitude-longitude grid.  "Reconstruction on latitude/longitude grids uses the same
+ * algorithms as spatial reconstruction": the van Leer slope of R7 in index space along zeta and along psi.  The neighbours of
+ * cell (l, m) along zeta are (l -+ 1, m); beyond a pole the row continues on the far side of the sphere, in cell
+ * (l, m + N_psi/2) of the same row l (the paper's example: (0,4), (0,0), (1,0), (2,0) for N_psi = 8); along psi the grid is
+ * periodic.  I is a scalar: no sign change across the poles.  Returns the value of cell u at its face in slot `slot`
+ * (0 zeta-, 1 zeta+, 2 psi-, 3 psi+). */
+static double latlon_face_value(const orc_angles *A, const double *Ic, int u, int slot) {
+    int np = A->npsi, l = u / np, m = u % np, lo, hi;
+    if (slot < 2) {
+        int across = l * np + (m + np / 2) % np;
+        lo = (l > 0) ? (l - 1) * np + m : across;
+        hi = (l + 1 < A->nzeta) ? (l + 1) * np + m : across;
+    } else {
+        lo = l * np + (m + np - 1) % np;
+        hi = l * np + (m + 1) % np;
+    }
+    double s = vl_slope(Ic[lo], Ic[u], Ic[hi]);
+    return (slot & 1) ? Ic[u] + 0.5 * s : Ic[u] - 0.5 * s;
+}
+/* for the pins: value of cell u at its face in `slot`, from the row Ic[N] of one spatial cell */
+double orc_latlon_face_value(const orc_angles *A, const double *Ic, int u, int slot) { return latlon_face_value(A, Ic, u, slot); }
+
 /* pinned: c_e = -sum_{c=1..3} sum_{k=0..9} S[c][k] T_e[c][k], accumulated by fma from 0 in that order.
  * = a(n_e) . N_e with a^c = -omega^c_{alpha beta} n^alpha n^beta  (R5; Eq.16b,c) */
 static double edge_coeff(const double *S, const double *T) {
@@ -654,7 +743,13 @@ static void transport_impl(const orc_problem *P, const double *I_in, const doubl
                     for (int e = 0; e < E; e++) {
                         double ce = edge_coeff(cg + 33, &A->edge_T[30 * e]);
                         double n0e = contract4(cg + 17, &A->edge_mid[3 * e]); /* n_0 at the edge direction, cell-centre tetrad */
-                        double Iup = (ce > 0.0) ? I_in[c * N + A->edge_lo[e]] : I_in[c * N + A->edge_hi[e]];
+                        int up = (ce > 0.0) ? A->edge_lo[e] : A->edge_hi[e];
+                        double Iup = I_in[c * N + up];
+                        if (P->recon_angle == 1 && ce != 0.0) { /* R21: the upwind cell's PLM value at this edge */
+                            int slot = 0;
+                            while (A->nbr_edge[up * ORC_MAXNBR + slot] != e) slot++;
+                            Iup = latlon_face_value(A, &I_in[c * N], up, slot);
+                        }
                         Fe[e] = (ce == 0.0) ? 0.0 : ce * n0e * Iup;
                     }
                     for (int n = 0; n < N; n++) {
@@ -731,6 +826,17 @@ static void fluid_four_velocity(const double *cg, const double unorm[3], double 
 }
 
 void orc_set_tau_factor(orc_problem *P, double tau_factor) { P->tau_factor = tau_factor; }
+/* options: 0 recon_angle (0 DC, 1 lat-lon PLM; returns -1 if the angle grid is not lat-lon with even N_psi), 1 vel_estimate,
+ * 2 dt0_literal */
+int orc_set_option(orc_problem *P, int which, int value) {
+    if (which == 0) {
+        if (value == 1 && (P->ang->kind != 0 || (P->ang->npsi & 1))) return -1;
+        P->recon_angle = value;
+    } else if (which == 1) P->vel_estimate = value;
+    else if (which == 2) P->dt0_literal = value;
+    else return -1;
+    return 0;
+}
 
 /* vel[cell][5] for EVERY cell of the array (ghosts included: the faces of the outermost interior cells need their
  * neighbours): tetrad-frame fluid velocity u^alphahat (R10, with the cell's own cell-centre tetrad; the same lines as in
@@ -759,6 +865,55 @@ void orc_transport_tau(const orc_problem *P, const double *I_in, const double *I
     orc_cell_velocity(P, fluid, opac, vel);
     transport_impl(P, I_in, I0, gam0, gam1, beta_dt, vel, P->tau_factor * beta_dt, I_out);
     free(vel);
+}
+
+/* NEXT-2: radiation-dominated velocity estimate (Eq.51-55).  Inputs: the tetrad-frame intensities of one cell
+ * (after transport), the gas four-velocity uh[4] in the tetrad frame, rho, T, the absorptivities, dt.  If Ebar (fluid-frame
+ * radiation energy density for the gas velocity, Eq.38 in covariant form u_a u_b R^{ab}) exceeds rho + u_gas, uh is
+ * replaced by the blend of Eq.55 and 1 is returned; else uh is left alone and 0 is returned.
+ * Readings: G8 -- Eq.54 as printed has u^ahat in the denominator; taken as f^a = G^a dt / (T_rad^{0a} - T_gas^{0a}),
+ * the fraction of the momentum gap the force closes in dt (the printed form diverges for a gas at rest and lets the sign of
+ * u^a decide the clamp); a vanishing denominator gives f^a = 0.  R19 -- |v_rad|^2 is capped at 1 - 1e-12 so that the
+ * "associated four-velocity" exists for a single beam; u^0hat of the blend from normalisation.  T in Eq.53 is the
+ * pre-coupling gas temperature.  Optional outputs for the pins: G[4] (Eq.53), fr[3] (Eq.54, clamped), Rt[10] (R^{ahat bhat}). */
+static int velocity_estimate(const orc_problem *P, const double *Ic, double uh[4], double rho, double Tm, double aP, double aEa,
+                             double aS, double dt, double *G_out, double *fr_out, double *R_out) {
+    const orc_angles *A = P->ang;
+    int N = A->N;
+    double R[4][4] = {{0}};
+    for (int n = 0; n < N; n++) {
+        const double *nh = &A->nhat[3 * n];
+        double n4[4] = {1.0, nh[0], nh[1], nh[2]}, w = Ic[n] * A->domega[n];
+        for (int a = 0; a < 4; a++) for (int b = 0; b < 4; b++) R[a][b] += w * n4[a] * n4[b]; /* Eq.45 in the tetrad frame */
+    }
+    if (R_out) { int q = 0; for (int a = 0; a < 4; a++) for (int b = a; b < 4; b++) R_out[q++] = R[a][b]; }
+    double ul[4] = {-uh[0], uh[1], uh[2], uh[3]}; /* u_ahat */
+    double uR[4], Ebar = 0;
+    for (int a = 0; a < 4; a++) { uR[a] = 0; for (int b = 0; b < 4; b++) uR[a] += ul[b] * R[a][b]; }
+    for (int a = 0; a < 4; a++) Ebar += ul[a] * uR[a];
+    double ugas = rho * Tm / (P->gamma_gas - 1.0), pgas = rho * Tm; /* k_B/(mu m_p) = 1 */
+    double emis = aP * P->a_rad * Tm * Tm * Tm * Tm + aS * Ebar, aE = aEa + aS;
+    double G[4];
+    for (int a = 0; a < 4; a++) G[a] = -emis * uh[a] - aE * uR[a]; /* Eq.53 */
+    if (G_out) for (int a = 0; a < 4; a++) G_out[a] = G[a];
+    if (fr_out) for (int a = 0; a < 3; a++) fr_out[a] = 0.0;
+    if (!(Ebar > rho + ugas) || !(R[0][0] > 0.0)) return 0;
+    double v[3] = {R[0][1] / R[0][0], R[0][2] / R[0][0], R[0][3] / R[0][0]}; /* Eq.51 */
+    double vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+    if (vv > 1.0 - 1e-12) vv = 1.0 - 1e-12; /* R19 */
+    double W = 1.0 / sqrt(1.0 - vv), ur[4] = {W, W * v[0], W * v[1], W * v[2]};
+    double wgas = rho + ugas + pgas, un[4];
+    for (int a = 1; a < 4; a++) {
+        double Tgas = wgas * uh[0] * uh[a], Trad = wgas * ur[0] * ur[a]; /* Eq.52 */
+        double den = Trad - Tgas, f = (den != 0.0) ? G[a] * dt / den : 0.0; /* Eq.54 with G8 */
+        if (!(f > 0.0)) f = 0.0;
+        if (f > 1.0) f = 1.0;
+        if (fr_out) fr_out[a - 1] = f;
+        un[a] = (1.0 - f) * uh[a] + f * ur[a]; /* Eq.55 */
+    }
+    uh[1] = un[1]; uh[2] = un[2]; uh[3] = un[3];
+    uh[0] = sqrt(1.0 + (un[1] * un[1] + un[2] * un[2] + un[3] * un[3]));
+    return 1;
 }
 
 long long orc_coupling(const orc_problem *P, double *I, const double *fluid, const double *opac, double dt,
@@ -796,6 +951,7 @@ long long orc_coupling(const orc_problem *P, double *I, const double *fluid, con
                             for (int b = 0; b < 4; b++) s += Lw[4 * b + ah] * ucon[b];
                             uh[ah] = (ah == 0 ? -1.0 : 1.0) * s;
                         }
+                        if (P->vel_estimate) velocity_estimate(P, Ic, uh, rho, Tm, aP, aEa, aS, dt, NULL, NULL, NULL); /* Eq.51-55 */
                         /* per angle: n^0bar = -u_alpha n^alpha = u^0hat - u^ahat n^ahat (Eq.14a,b);
                          * R11: Ibar = (n^0bar)^4 Ihat, dOmega_bar = dOmega / (n^0bar)^2 */
                         double W = 0;
@@ -829,24 +985,24 @@ long long orc_coupling(const orc_problem *P, double *I, const double *fluid, con
                             Tp = Tm + dT;
                             double Ep = Em - Cv * dT;                      /* Eq.48 */
                             double src = aP * P->a_rad * Tp * Tp * Tp * Tp + aS * Ep;
-                            /* R0_alpha before */
-                            double Rb[4] = {0, 0, 0, 0}, Ra[4] = {0, 0, 0, 0};
+                            /* subtract the change of R^0_alpha from T^0_alpha.  SURVEY O5: the change is formed angle by angle,
+                             * dT^0_alpha = -sum_n n^0 n_alpha (Ihat_+ - I*) dOmega_n; with dt0_literal the two sums R^0_alpha[I*] and
+                             * R^0_alpha[Ihat_+] are formed first and subtracted (the same number up to the rounding of two N-term sums). */
+                            double Rb[4] = {0, 0, 0, 0}, Ra[4] = {0, 0, 0, 0}, dR[4] = {0, 0, 0, 0};
                             for (int n = 0; n < N; n++) {
                                 const double *nh = &A->nhat[3 * n];
-                                for (int m = 0; m < 4; m++) Rb[m] += nup0 * contract4(Lw + 4 * m, nh) * Ic[n] * A->domega[n];
-                            }
-                            for (int n = 0; n < N; n++) {
                                 double dn = nup0 + n0bar[n] * aE * dt;
                                 double Ibp = (nup0 * Ibm[n] + n0bar[n] * dt / (4.0 * PI) * src) / dn; /* Eq.40 */
                                 double n2 = n0bar[n] * n0bar[n];
-                                Ic[n] = Ibp / (n2 * n2);
+                                double Inew = Ibp / (n2 * n2), Iold = Ic[n];
+                                for (int m = 0; m < 4; m++) {
+                                    double wgt = nup0 * contract4(Lw + 4 * m, nh) * A->domega[n]; /* n^0 n_alpha dOmega */
+                                    Rb[m] += wgt * Iold; Ra[m] += wgt * Inew;
+                                    dR[m] += wgt * (Inew - Iold);
+                                }
+                                Ic[n] = Inew;
                             }
-                            for (int n = 0; n < N; n++) {
-                                const double *nh = &A->nhat[3 * n];
-                                for (int m = 0; m < 4; m++) Ra[m] += nup0 * contract4(Lw + 4 * m, nh) * Ic[n] * A->domega[n];
-                            }
-                            /* subtract the change of R^0_alpha from T^0_alpha */
-                            if (dT0) for (int m = 0; m < 4; m++) dT0[m * nc + c] = -(Ra[m] - Rb[m]);
+                            if (dT0) for (int m = 0; m < 4; m++) dT0[m * nc + c] = P->dt0_literal ? -(Ra[m] - Rb[m]) : -dR[m];
                         }
                     }
                     (void)coupled;
@@ -860,6 +1016,13 @@ long long orc_coupling(const orc_problem *P, double *I, const double *fluid, con
         free(n0bar); free(dOmb); free(Ibm);
     }
     return nfail;
+}
+
+/* Eq.51-55 for one cell, for the pins: u_inout[4] tetrad-frame gas velocity in, estimate out; G[4], fr[3], R[10] as in
+ * velocity_estimate.  returns 1 if the cell is radiation dominated (the blend was applied) */
+int orc_velocity_estimate_cell(const orc_problem *P, const double *Icell, double *u_inout, double rho, double Tm, double aP, double aEa,
+                               double aS, double dt, double *G, double *fr, double *R) {
+    return velocity_estimate(P, Icell, u_inout, rho, Tm, aP, aEa, aS, dt, G, fr, R);
 }
 
 long long orc_stage(const orc_problem *P, double *I_in, double *I_out, const double *I0, const double *fluid,

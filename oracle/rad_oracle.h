@@ -69,6 +69,16 @@ void orc_cell_velocity(const orc_problem *, const double *fluid, const double *o
 void orc_transport_tau(const orc_problem *, const double *I_in, const double *I0, double gam0, double gam1,
                        double beta_dt, const double *fluid, const double *opac, double *I_out);
 
+/* ---- options set after create: which = 0 recon_angle (0 donor cell, 1 PLM on the latitude-longitude grid incl. across the poles,
+ * P:L280; -1 is returned if the grid is not lat-lon with even N_psi), 1 vel_estimate (Eq.51-55), 2 dt0_literal
+ * (dT^0_alpha as the difference of two sums instead of the sum of differences).  recon_space = 2 (PPM) needs ng = 3.
+ * Boundary code 3 = reflecting wall with the angle-mirror permutation (R20). ---- */
+int orc_set_option(orc_problem *, int which, int value);
+int orc_has_mirror(const orc_problem *, int axis);
+double orc_latlon_face_value(const orc_angles *, const double *Icell, int u, int slot /* 0 zeta-, 1 zeta+, 2 psi-, 3 psi+ */);
+int orc_velocity_estimate_cell(const orc_problem *, const double *Icell, double *u_inout, double rho, double Tm, double aP, double aEa,
+                               double aS, double dt, double *G, double *fr, double *R);
+
 /* ---- a4-a6: coupling (Eq.31-50) in place on I (interior), then the n_0 mask.
  * fluid: SoA [5][ncells_total] = rho, T, u1', u2', u3'.  opac: SoA [3][ncells_total] =
  * alpha_a_planck, alpha_a_energy, alpha_s.  T_out[ncells_total], dT0[4][ncells_total] (may be NULL).

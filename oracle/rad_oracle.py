@@ -63,6 +63,11 @@ def lib():
         L.orc_cell_velocity.argtypes = [vp, vp, vp, vp]
         L.orc_transport_tau.argtypes = [vp, vp, vp, C.c_double, C.c_double, C.c_double, vp, vp, vp]
         L.orc_moments.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.orc_set_option.argtypes = [vp, C.c_int, C.c_int]
+        L.orc_has_mirror.argtypes = [vp, C.c_int]
+        L.orc_latlon_face_value.restype = C.c_double
+        L.orc_latlon_face_value.argtypes = [vp, vp, C.c_int, C.c_int]
+        L.orc_velocity_estimate_cell.argtypes = [vp, vp, vp] + [C.c_double] * 6 + [vp, vp, vp]
         L.orc_upwind_tables.argtypes = [vp, vp, vp]
         L.orc_edge_coeffs.argtypes = [vp, C.c_longlong, vp, vp]
         L.orc_max_speed.restype = C.c_double
@@ -100,6 +105,11 @@ class Angles:
                             _p(self.edge_lo), _p(self.edge_hi), _p(self.edge_len), _p(self.edge_mid),
                             _p(self.edge_nrm), _p(self.edge_T))
 
+    def latlon_face_value(self, Icell, u, slot):
+        """R21: PLM value of angle cell u at its face in slot (0 zeta-, 1 zeta+, 2 psi-, 3 psi+) from one spatial cell's row"""
+        Icell = _f64(Icell)
+        return lib().orc_latlon_face_value(self.h, _p(Icell), int(u), int(slot))
+
     def __del__(self):
         try:
             lib().orc_angles_free(self.h)
@@ -120,7 +130,8 @@ class Problem:
     """Grid + metric + angles + parameters; the oracle's stage, moments and tables."""
 
     def __init__(self, angles, n, x0, dx, metric_kind=0, M=1.0, a=0.0, excise_r=0.0, ng=2, bc_lo=(0, 0, 0), bc_hi=(0, 0, 0),
-                 gamma_gas=5.0 / 3.0, a_rad=1.0, n0_crit=0.1, recon_space=1, renorm=1, couple=1, tau_factor=0.0):
+                 gamma_gas=5.0 / 3.0, a_rad=1.0, n0_crit=0.1, recon_space=1, renorm=1, couple=1, tau_factor=0.0, recon_angle=0,
+                 vel_estimate=0, dt0_literal=0):
         L = lib()
         self.angles = angles
         self.n = tuple(int(v) for v in n); self.ng = ng
@@ -133,6 +144,14 @@ class Problem:
         self.ncell = L.orc_ncells_total(self.h)
         self.tau_factor = float(tau_factor)
         L.orc_set_tau_factor(self.h, self.tau_factor)   # constant of Eq.26; 0 = free-streaming flux Eq.24
+        if recon_space == 2 and ng < 3:
+            raise ValueError("PPM needs ng = 3")
+        for which, val in ((0, recon_angle), (1, vel_estimate), (2, dt0_literal)):
+            if L.orc_set_option(self.h, which, int(val)) != 0:
+                raise ValueError("option %d = %d is not available on this angle grid" % (which, val))
+        for d in range(3):
+            if (bc_lo[d] == 3 or bc_hi[d] == 3) and not L.orc_has_mirror(self.h, d):
+                raise ValueError("reflecting boundary along axis %d: the angle grid is not symmetric under that reflection" % d)
 
     def __del__(self):
         try:
@@ -183,6 +202,13 @@ class Problem:
                              gam0, gam1, beta_dt, _p(T), _p(dT0))
         return out, T, dT0, nf
 
+    def velocity_estimate_cell(self, Icell, uh, rho, Tm, aP, aEa, aS, dt):
+        """Eq.51-55 for one cell: returns (applied, u_estimate[4], G[4], f[3], R[10])"""
+        Icell = _f64(Icell); u = _f64(np.array(uh, dtype=np.float64).copy())
+        G = np.zeros(4); fr = np.zeros(3); R = np.zeros(10)
+        ap = lib().orc_velocity_estimate_cell(self.h, _p(Icell), _p(u), rho, Tm, aP, aEa, aS, dt, _p(G), _p(fr), _p(R))
+        return bool(ap), u, G, fr, R
+
     def moments(self, I, frame, fluid=None):
         ncomp = 10 if frame in (0, 2) else 4
         out = np.zeros((ncomp, self.ncell))
@@ -208,6 +234,15 @@ class Problem:
         ax = (C.c_double * 3)()
         v = lib().orc_max_speed(self.h, ax)
         return v, tuple(ax)
+
+    def mirror(self, axis):
+        """angle permutation of the reflection that flips tetrad component `axis` (R20), -1 where the grid has no image"""
+        out = np.zeros(self.N, np.int32)
+        for n in range(self.N):
+            want = self.angles.nhat[n].copy(); want[axis] = -want[axis]
+            d = np.abs(self.angles.nhat - want).max(1)
+            out[n] = int(d.argmin()) if d.min() < 1e-12 else -1
+        return out
 
     def interior(self, a):
         """view of the interior of an array whose leading dims are (NK,NJ,NI) flattened or not."""
