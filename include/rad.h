@@ -14,7 +14,7 @@
  *
  * Arrays
  *  - Grid: uniform Cartesian, n[0..2] interior cells along x,y,z, ng = 2 ghost cells per side
- *    (PLM needs two).  NI = n[0]+2ng etc.  Cell (k,j,i) has flat index c = (k*NJ + j)*NI + i.
+ *    (PLM needs two; PPM three).  NI = n[0]+2ng etc.  Cell (k,j,i) has flat index c = (k*NJ + j)*NI + i.
  *  - Intensity I[c][n]: angle index n innermost (contiguous), N = number of angles.  FP64.
  *  - Per-cell scalars are SoA: field[f][c].
  */
@@ -65,14 +65,28 @@ typedef struct {
 } rad_metric;
 
 typedef struct {
-    int n[3], ng;           /* interior cells per axis; ng must be 2 */
+    int n[3], ng;           /* interior cells per axis; ghost cells per side: 2, or 3 (needed by recon_space = 2, PPM) */
     double x0[3], dx[3];    /* lower corner of the interior and cell sizes */
-    int bc_lo[3], bc_hi[3]; /* 0 caller-filled, 1 periodic, 2 outflow (copy of nearest interior cell) */
+    int bc_lo[3], bc_hi[3]; /* 0 caller-filled, 1 periodic, 2 outflow (copy of nearest interior cell),
+                               3 reflecting wall: ghost cell = mirror cell across the wall, with the intensity of
+                               the direction whose wall-normal tetrad component is flipped (reading R20); needs an angle
+                               grid that is symmetric under that flip (every lat-lon grid with even npsi; the geodesic
+                               grid for the y axis only), else rad_create returns RAD_EUNSUPPORTED */
 } rad_grid;
 
 typedef struct {
-    int kind; /* 0 latitude-longitude (nzeta x npsi), 1 geodesic (level nlev) */
+    int kind; /* 0 latitude-longitude (nzeta x npsi), 1 geodesic (level nlev),
+                 2 explicit tables (any grid the paper allows) */
     int nzeta, npsi, nlev;
+    /* kind 2, all HOST, copied at create.  nang angles; per angle: unit direction nhat[nang][3] (Eq.15b-d), solid angle
+     * domega[nang], number of neighbours nnbr[nang] (<= RAD_MAXNBR), neighbour list nbr[nang][RAD_MAXNBR] (-1 = none; both
+     * angles of an edge must list each other); per (angle, slot): the edge's arc length edge_len[nang][RAD_MAXNBR]
+     * (Delta lambda, Eq.20f), unit vector to its midpoint edge_mid[nang][RAD_MAXNBR][3] and in-sphere unit normal
+     * edge_nrm[nang][RAD_MAXNBR][3] pointing from the angle to that neighbour.  An edge's data are read from the entry of
+     * its lower-numbered angle.  Errors: RAD_EINVAL (NULL, non-unit nhat, non-positive domega, asymmetric lists). */
+    int nang;
+    const double *nhat, *domega, *edge_len, *edge_mid, *edge_nrm;
+    const int *nnbr, *nbr;
 } rad_angles;
 
 typedef struct { /* fluid-frame absorptivities, DEVICE, each [ncells_total], NOT owned;
@@ -84,8 +98,11 @@ typedef struct {
     double gamma_gas;         /* adiabatic index Gamma (Eq.48); k_B/(mu m_p) = 1 */
     double a_rad;             /* radiation constant (Eq.34) */
     double n0_crit;           /* Ihat is zeroed where |n_0| < n0_crit; <= 0 disables */
-    int recon_space;          /* 0 donor cell, 1 PLM van Leer */
-    int recon_angle;          /* 0 donor cell; others RAD_EUNSUPPORTED */
+    int recon_space;          /* 0 donor cell, 1 PLM van Leer, 2 PPM Colella & Woodward (needs ng = 3; runs in the
+                                 generic flux-divergence kernel) */
+    int recon_angle;          /* 0 donor cell; 1 PLM on the latitude-longitude grid, across the poles as P:L280 spells
+                                 out (reading R21; lat-lon grids with even npsi only, else RAD_EUNSUPPORTED; generic kernel).
+                                 MAPR on the geodesic grid is not implemented: its sources are not in the paper */
     int renorm_fluid_weights; /* R12: 1 = rescale fluid-frame solid angles to sum to 4 pi */
     int couple;               /* 0 = transport only, 1 = with implicit coupling (section 2.5) */
     double tau_factor;        /* constant of Eq.26: 0 = free-streaming spatial flux (Eq.24); > 0 = optical-depth-aware flux
@@ -106,8 +123,9 @@ typedef struct {
 
 /* Build a context: angle tables on the host (section 2.6), geometry tables on the device (section 2.1-2.2,
  * one kernel launch; synchronises the device once).  `device` is the CUDA ordinal.
- * Errors: RAD_EINVAL (NULL, ng != 2, n < 1, non-finite or non-positive dx, bad enum, tau_factor < 0), RAD_EUNSUPPORTED
- * (recon_angle != 0), RAD_ENOMEM, RAD_ECUDA.  On error *out is NULL. */
+ * Errors: RAD_EINVAL (NULL, ng not 2 or 3, PPM with ng = 2, n < 1, non-finite or non-positive dx, bad enum, tau_factor < 0),
+ * RAD_EUNSUPPORTED (recon_angle = 1 or a reflecting wall on an angle grid that does not allow it), RAD_ENOMEM, RAD_ECUDA.
+ * On error *out is NULL. */
 rad_status rad_create(const rad_metric *, const rad_grid *, const rad_angles *, const rad_opac *,
                       const rad_params *, int device, rad_ctx **out);
 
@@ -173,7 +191,13 @@ typedef enum {
     RAD_TAB_FACE = 13,      /* double[ncells_total][3][RAD_NFACE] */
     RAD_TAB_FACE_SIGN = 14, /* signed char[ncells_total][3][N]: sgn n^a at each cell's lower faces (upwind index, Eq.24) */
     RAD_TAB_EDGE_SIGN = 15, /* signed char[ncells_total][E]: sgn c_e (upwind index, Eq.25) */
-    RAD_TAB_MAXSPEED = 16   /* double[3]: max over faces and angles of |n^a / n^0| per axis (for the CFL step, R9) */
+    RAD_TAB_MAXSPEED = 16,  /* double[3]: max over faces and angles of |n^a / n^0| per axis (for the CFL step, R9) */
+    /* the upwind decisions as the stage kernel itself takes them (RAD_ESTATE if the context does not run the tile kernel): */
+    RAD_TAB_OWN_EDGE = 17,  /* int[N][3]: unique edge id owned by angle n in slot j, -1 = none (balanced ownership) */
+    RAD_TAB_KE = 18,        /* double[n2][n1][n0][3][N] (interior cells): stored edge coefficient of the edge angle n owns in slot j,
+                               +-dlambda_e c_e n_0e; its lowest mantissa bit = 1 if the owner is the upwind end (Eq.25) */
+    RAD_TAB_STAGE_FACE_SIGN = 19 /* signed char[ncells_total][3][N]: sgn n^a at each cell's UPPER faces, from the kernel's own face
+                                    evaluation on its packed records (Eq.24) */
 } rad_table;
 rad_status rad_get_table(rad_ctx *, int which, void *host_out, size_t nbytes);
 

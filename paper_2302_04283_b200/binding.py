@@ -16,7 +16,8 @@ _SO = os.path.join(_HERE, "librad.so")
 NCELL, NFACE, MAXNBR = 52, 8, 6
 
 (TAB_NANG, TAB_NEDGE, TAB_NHAT, TAB_DOMEGA, TAB_NNBR, TAB_NBR, TAB_NBR_EDGE, TAB_EDGE_LO, TAB_EDGE_HI, TAB_EDGE_LEN,
- TAB_EDGE_MID, TAB_EDGE_NRM, TAB_CELL, TAB_FACE, TAB_FACE_SIGN, TAB_EDGE_SIGN, TAB_MAXSPEED) = range(17)
+ TAB_EDGE_MID, TAB_EDGE_NRM, TAB_CELL, TAB_FACE, TAB_FACE_SIGN, TAB_EDGE_SIGN, TAB_MAXSPEED, TAB_OWN_EDGE, TAB_KE,
+ TAB_STAGE_FACE_SIGN) = range(20)
 
 EXPORTS = ["rad_create", "rad_stage", "rad_stage_host", "rad_fill_ghosts", "rad_transport", "rad_couple", "rad_moments",
            "rad_get_table", "rad_probe_fp64", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
@@ -39,7 +40,9 @@ class _Grid(C.Structure):
 
 
 class _Angles(C.Structure):
-    _fields_ = [("kind", C.c_int), ("nzeta", C.c_int), ("npsi", C.c_int), ("nlev", C.c_int)]
+    _fields_ = [("kind", C.c_int), ("nzeta", C.c_int), ("npsi", C.c_int), ("nlev", C.c_int), ("nang", C.c_int),
+                ("nhat", C.c_void_p), ("domega", C.c_void_p), ("edge_len", C.c_void_p), ("edge_mid", C.c_void_p), ("edge_nrm", C.c_void_p),
+                ("nnbr", C.c_void_p), ("nbr", C.c_void_p)]
 
 
 class _Opac(C.Structure):
@@ -119,13 +122,23 @@ def _check(ctx, st):
 
 def rad_create(metric, grid, angles, opac, params, device=0):
     """metric: dict(kind, M, a, excise_r, cell_tab, face_tab); grid: dict(n, x0, dx, bc_lo, bc_hi[, ng]);
-    angles: ("latlon", nzeta, npsi) or ("geodesic", nlev); opac: (alpha_a_planck, alpha_a_energy, alpha_s) CUDA
+    angles: ("latlon", nzeta, npsi), ("geodesic", nlev) or ("explicit", dict(nhat, domega, nnbr, nbr, edge_len, edge_mid, edge_nrm)); opac: (alpha_a_planck, alpha_a_energy, alpha_s) CUDA
     tensors or None; params: dict of rad_params fields.  Returns an opaque handle."""
     m = _Metric(int(metric.get("kind", 0)), float(metric.get("M", 1.0)), float(metric.get("a", 0.0)), float(metric.get("excise_r", 0.0)),
                 _dp(metric.get("cell_tab")), _dp(metric.get("face_tab")))
     i3, d3 = C.c_int * 3, C.c_double * 3
     g = _Grid(i3(*grid["n"]), int(grid.get("ng", 2)), d3(*grid["x0"]), d3(*grid["dx"]), i3(*grid.get("bc_lo", (0, 0, 0))), i3(*grid.get("bc_hi", (0, 0, 0))))
-    a = _Angles(0, int(angles[1]), int(angles[2]), 0) if angles[0] == "latlon" else _Angles(1, 0, 0, int(angles[1]))
+    keep = []
+    if angles[0] == "latlon":
+        a = _Angles(0, int(angles[1]), int(angles[2]), 0)
+    elif angles[0] == "geodesic":
+        a = _Angles(1, 0, 0, int(angles[1]))
+    else:  # ("explicit", dict of host tables): see rad_angles kind 2 in rad.h
+        tb = angles[1]
+        f64 = lambda k: np.ascontiguousarray(tb[k], dtype=np.float64)
+        i32 = lambda k: np.ascontiguousarray(tb[k], dtype=np.int32)
+        keep = [f64("nhat"), f64("domega"), f64("edge_len"), f64("edge_mid"), f64("edge_nrm"), i32("nnbr"), i32("nbr")]
+        a = _Angles(2, 0, 0, 0, int(keep[1].shape[0]), *[C.c_void_p(x.ctypes.data) for x in keep])
     o = _Opac(*(_dp(x) for x in opac)) if opac is not None else None
     p = _Params(float(params.get("gamma_gas", 5.0 / 3.0)), float(params.get("a_rad", 1.0)), float(params.get("n0_crit", 0.1)),
                 int(params.get("recon_space", 1)), int(params.get("recon_angle", 0)), int(params.get("renorm_fluid_weights", 1)),
@@ -190,8 +203,8 @@ def rad_launch_count(ctx):
     return lib().rad_launch_count(ctx)
 
 
-def rad_get_table(ctx, which):
-    """host numpy copy of one of the library's tables (see rad_table in rad.h)"""
+def rad_get_table(ctx, which, n_interior=None):
+    """host numpy copy of one of the library's tables (see rad_table in rad.h); TAB_KE needs n_interior = number of interior cells"""
     L = lib()
 
     def get(w, shape, dtype):
@@ -206,5 +219,6 @@ def rad_get_table(ctx, which):
             TAB_NBR_EDGE: ((N, MAXNBR), np.int32), TAB_EDGE_LO: ((E,), np.int32), TAB_EDGE_HI: ((E,), np.int32),
             TAB_EDGE_LEN: ((E,), np.float64), TAB_EDGE_MID: ((E, 3), np.float64), TAB_EDGE_NRM: ((E, 3), np.float64),
             TAB_CELL: ((nc, NCELL), np.float64), TAB_FACE: ((nc, 3, NFACE), np.float64), TAB_FACE_SIGN: ((nc, 3, N), np.int8),
-            TAB_EDGE_SIGN: ((nc, E), np.int8), TAB_MAXSPEED: ((3,), np.float64)}
+            TAB_EDGE_SIGN: ((nc, E), np.int8), TAB_MAXSPEED: ((3,), np.float64), TAB_OWN_EDGE: ((N, 3), np.int32),
+            TAB_KE: ((n_interior or 0, 3, N), np.float64), TAB_STAGE_FACE_SIGN: ((nc, 3, N), np.int8)}
     return get(which, *spec[which])

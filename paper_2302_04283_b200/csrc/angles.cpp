@@ -244,4 +244,43 @@ bool build_geodesic(int nlev, AngleTables &t, std::string &err) {
     return true;
 }
 
+// Explicit angle grid (rad_angles kind 2: any grid of cells with centres, solid angles and edges): the caller gives per
+// angle the direction, the solid angle, the neighbour list, and per (angle, slot) the edge's arc length, unit midpoint and in-sphere
+// normal pointing from the angle to that neighbour.  Unique edges are enumerated by (n ascending, slot ascending) with the neighbour
+// index above n (the order of the geodesic builder); an edge's data are taken from its lower angle's entry.
+bool build_explicit(int N, const double *nhat, const double *domega, const int *nnbr, const int *nbr, const double *edge_len,
+                    const double *edge_mid, const double *edge_nrm, AngleTables &t, std::string &err) {
+    if (N < 1 || !nhat || !domega || !nnbr || !nbr || !edge_len || !edge_mid || !edge_nrm) { err = "explicit angle grid: missing table"; return false; }
+    reserve(t, N);
+    for (int n = 0; n < N; n++) {
+        double r2 = 0.0;
+        for (int c = 0; c < 3; c++) { t.nhat[3 * n + c] = nhat[3 * n + c]; r2 += nhat[3 * n + c] * nhat[3 * n + c]; }
+        if (!(std::fabs(r2 - 1.0) < 1e-12) || !(domega[n] > 0.0) || !std::isfinite(domega[n])) { err = "explicit angle grid: nhat must be unit vectors and domega positive"; return false; }
+        t.domega[n] = domega[n];
+        if (nnbr[n] < 0 || nnbr[n] > RAD_MAXNBR) { err = "explicit angle grid: nnbr out of range"; return false; }
+        t.nnbr[n] = nnbr[n];
+        for (int s = 0; s < RAD_MAXNBR; s++) {
+            const int m = nbr[n * RAD_MAXNBR + s];
+            if (m < -1 || m >= N || m == n || (s >= nnbr[n] && m != -1)) { err = "explicit angle grid: bad neighbour index"; return false; }
+        }
+    }
+    for (int n = 0; n < N; n++)
+        for (int s = 0; s < RAD_MAXNBR; s++) {
+            const int m = nbr[n * RAD_MAXNBR + s];
+            if (m < 0 || m < n) continue;
+            int sm = -1;  // the neighbour's matching slot: the first one that lists n and is not paired yet
+            for (int q = 0; q < RAD_MAXNBR && sm < 0; q++)
+                if (nbr[m * RAD_MAXNBR + q] == n && t.nbr_edge[m * RAD_MAXNBR + q] < 0) sm = q;
+            if (sm < 0) { err = "explicit angle grid: neighbour lists are not symmetric"; return false; }
+            const size_t q = (size_t)n * RAD_MAXNBR + s;
+            if (!std::isfinite(edge_len[q]) || edge_len[q] < 0.0) { err = "explicit angle grid: bad edge length"; return false; }
+            push_edge(t, n, s, m, sm, edge_len[q], {edge_mid[3 * q], edge_mid[3 * q + 1], edge_mid[3 * q + 2]},
+                      {edge_nrm[3 * q], edge_nrm[3 * q + 1], edge_nrm[3 * q + 2]});
+        }
+    for (int n = 0; n < N; n++)
+        for (int s = 0; s < RAD_MAXNBR; s++)
+            if (nbr[n * RAD_MAXNBR + s] >= 0 && t.nbr_edge[n * RAD_MAXNBR + s] < 0) { err = "explicit angle grid: neighbour lists are not symmetric"; return false; }
+    return true;
+}
+
 }  // namespace rad

@@ -82,19 +82,23 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
                       int device, rad_ctx **out) {
     if (out) *out = nullptr;
     if (!m || !g || !a || !p || !out) return fail(nullptr, RAD_EINVAL, "rad_create: NULL argument");
-    if (g->ng != 2) return fail(nullptr, RAD_EINVAL, "rad_create: ng must be 2");
+    if (g->ng != 2 && g->ng != 3) return fail(nullptr, RAD_EINVAL, "rad_create: ng must be 2 or 3");
     for (int d = 0; d < 3; d++) {
         if (g->n[d] < 1) return fail(nullptr, RAD_EINVAL, "rad_create: n[d] must be >= 1");
         if (!finite_pos(g->dx[d]) || !std::isfinite(g->x0[d])) return fail(nullptr, RAD_EINVAL, "rad_create: bad x0/dx");
-        if (g->bc_lo[d] < 0 || g->bc_lo[d] > 2 || g->bc_hi[d] < 0 || g->bc_hi[d] > 2) return fail(nullptr, RAD_EINVAL, "rad_create: bad boundary code");
+        if (g->bc_lo[d] < 0 || g->bc_lo[d] > 3 || g->bc_hi[d] < 0 || g->bc_hi[d] > 3) return fail(nullptr, RAD_EINVAL, "rad_create: bad boundary code");
+        if ((g->bc_lo[d] == 3 || g->bc_hi[d] == 3) && g->n[d] < g->ng) return fail(nullptr, RAD_EINVAL, "rad_create: a reflecting wall needs n[d] >= ng");
     }
     if (m->kind < 0 || m->kind > 2) return fail(nullptr, RAD_EINVAL, "rad_create: bad metric kind");
     if (m->kind == 1 && (!finite_pos(m->M) || !std::isfinite(m->a) || std::fabs(m->a) > m->M)) return fail(nullptr, RAD_EINVAL, "rad_create: bad M or a");
     if (m->kind == 2 && (!m->cell_tab || !m->face_tab)) return fail(nullptr, RAD_EINVAL, "rad_create: tabulated metric needs cell_tab and face_tab");
     if (!(p->gamma_gas > 1.0) || !std::isfinite(p->gamma_gas) || !std::isfinite(p->a_rad) || p->a_rad < 0.0 || !std::isfinite(p->n0_crit))
         return fail(nullptr, RAD_EINVAL, "rad_create: bad gamma_gas / a_rad / n0_crit");
-    if (p->recon_space < 0 || p->recon_space > 1) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: recon_space must be 0 (DC) or 1 (PLM)");
-    if (p->recon_angle != 0) return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: only donor-cell angular reconstruction is implemented");
+    if (p->recon_space < 0 || p->recon_space > 2) return fail(nullptr, RAD_EINVAL, "rad_create: recon_space must be 0 (DC), 1 (PLM) or 2 (PPM)");
+    if (p->recon_space == 2 && g->ng < 3) return fail(nullptr, RAD_EINVAL, "rad_create: PPM needs ng = 3");
+    if (p->recon_angle < 0 || p->recon_angle > 1) return fail(nullptr, RAD_EINVAL, "rad_create: recon_angle must be 0 (DC) or 1 (lat-lon PLM)");
+    if (p->recon_angle == 1 && (a->kind != 0 || (a->npsi & 1)))
+        return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: PLM in angle needs a latitude-longitude grid with even npsi (MAPR on the geodesic grid is not implemented)");
     if (!std::isfinite(p->tau_factor) || p->tau_factor < 0.0) return fail(nullptr, RAD_EINVAL, "rad_create: tau_factor must be finite and >= 0");
     if (p->tau_factor != 0.0 && (!o || !o->alpha_a_energy || !o->alpha_s)) return fail(nullptr, RAD_EINVAL, "rad_create: tau_factor != 0 needs opacities");
     if (p->couple && (!o || !o->alpha_a_planck || !o->alpha_a_energy || !o->alpha_s)) return fail(nullptr, RAD_EINVAL, "rad_create: coupling needs opacities");
@@ -116,12 +120,33 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     c->kp.vel_estimate = p->vel_estimate;
     std::string err;
     bool ok = (a->kind == 0) ? rad::build_latlon(a->nzeta, a->npsi, c->host, err)
-            : (a->kind == 1) ? rad::build_geodesic(a->nlev, c->host, err) : (err = "bad angle grid kind", false);
+            : (a->kind == 1) ? rad::build_geodesic(a->nlev, c->host, err)
+            : (a->kind == 2) ? rad::build_explicit(a->nang, a->nhat, a->domega, a->nnbr, a->nbr, a->edge_len, a->edge_mid, a->edge_nrm, c->host, err)
+                             : (err = "bad angle grid kind", false);
     if (!ok) { delete c; return fail(nullptr, RAD_EINVAL, "rad_create: " + err); }
 
+    c->angles.nhat = c->angles.domega = c->angles.edge_len = c->angles.edge_mid = c->angles.edge_nrm = nullptr;  // the caller's tables are not kept
+    c->angles.nnbr = c->angles.nbr = nullptr;
     rad::DeviceTables &t = c->dev;
     const rad::AngleTables &h = c->host;
     t.N = h.N; t.E = h.E; t.ng = g->ng;
+    t.recon_angle = p->recon_angle; t.nzeta = a->kind == 0 ? a->nzeta : 0; t.npsi = a->kind == 0 ? a->npsi : 0;
+    // reflecting walls (R20): the angle whose direction is n-hat with component a flipped, for every axis that has such a wall
+    std::vector<int> mirror((size_t)3 * h.N, 0);
+    bool any_wall = false;
+    for (int d = 0; d < 3; d++) {
+        if (g->bc_lo[d] != 3 && g->bc_hi[d] != 3) continue;
+        any_wall = true;
+        for (int n = 0; n < h.N; n++) {
+            double want[3] = {h.nhat[3 * n], h.nhat[3 * n + 1], h.nhat[3 * n + 2]};
+            want[d] = -want[d];
+            int found = -1;
+            for (int m = 0; m < h.N && found < 0; m++)
+                if (std::fabs(h.nhat[3 * m] - want[0]) < 1e-12 && std::fabs(h.nhat[3 * m + 1] - want[1]) < 1e-12 && std::fabs(h.nhat[3 * m + 2] - want[2]) < 1e-12) found = m;
+            if (found < 0) { delete c; return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: reflecting wall: the angle grid is not symmetric under the flip of that direction component"); }
+            mirror[(size_t)d * h.N + n] = found;
+        }
+    }
     for (int d = 0; d < 3; d++) { t.n[d] = g->n[d]; t.inv_dx[d] = 1.0 / g->dx[d]; }
     t.NI = g->n[0] + 2 * g->ng; t.NJ = g->n[1] + 2 * g->ng; t.NK = g->n[2] + 2 * g->ng;
     if (cudaDeviceGetAttribute(&t.sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
@@ -149,9 +174,12 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
     ok = upload(c, h.nhat, &t.nhat) && upload(c, h.domega, &t.domega) && upload(c, h.nnbr, &t.nnbr) && upload(c, h.nbr_edge, &t.nbr_edge) &&
          upload(c, h.edge_lo, &t.edge_lo) && upload(c, h.edge_hi, &t.edge_hi) && upload(c, h.edge_len, &t.edge_len) &&
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
+    t.mirror = nullptr;
+    if (ok && any_wall) ok = upload(c, mirror, &t.mirror);
     // fused stage kernel: balanced edge ownership, per-angle records, 1/dOmega
     t.fused_ok = 0; t.ang_rec = nullptr; t.winv = nullptr; t.own_edge = nullptr; t.ke = nullptr; t.rec = nullptr;
-    if (ok && h.N <= 256) {
+    const bool tile_cfg = g->ng == 2 && p->recon_space <= 1 && p->recon_angle == 0;  // what the tile kernel (stage5.cu) implements
+    if (ok && h.N <= 256 && tile_cfg) {
         std::string oerr;
         if (rad::build_edge_ownership(h, c->own, oerr)) {
             std::vector<short> rec((size_t)h.N * 8, 0);
@@ -196,6 +224,10 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
         return fail(nullptr, RAD_ECUDA, msg);
     }
     c->metric.cell_tab = nullptr; c->metric.face_tab = nullptr;
+    if (p->vel_estimate && p->couple && !rad::stream_serves(t, nullptr)) {
+        rad_destroy(c);
+        return fail(nullptr, RAD_EUNSUPPORTED, "rad_create: vel_estimate needs an even number of angles that fits the streaming coupling kernel's shared memory");
+    }
     // stored edge coefficients q_e per (interior cell, owned edge): 3 N doubles per cell
     if (t.fused_ok && !p->recompute_edge_coeffs) {
         const size_t bytes = sizeof(double) * (size_t)g->n[0] * g->n[1] * g->n[2] * 3 * h.N;
@@ -316,6 +348,8 @@ static rad_status run_coupling(rad_ctx *c, double *I, const double *fluid, doubl
     unsigned long long *cnt = count ? c->d_noroot : nullptr;
     int nl = rad::launch_couple_stream(c->dev, c->kp, I, fluid, c->opac.alpha_a_planck, c->opac.alpha_a_energy, c->opac.alpha_s, dt, T_out, dT0, cnt, s, kz0, kz1);
     if (nl == 0 && kz1 > kz0) return fail(c, RAD_EUNSUPPORTED, "slab-wise coupling needs the streaming kernel");
+    if (nl == 0 && c->kp.vel_estimate && c->kp.couple)
+        return fail(c, RAD_EUNSUPPORTED, "the velocity estimate (Eq.51-55) runs in the streaming coupling kernel: it needs a 16-byte aligned intensity array");
     if (nl == 0) nl = rad::launch_coupling(c->dev, c->kp, I, fluid, c->opac.alpha_a_planck, c->opac.alpha_a_energy, c->opac.alpha_s, dt, T_out, dT0, cnt, s);
     if (nl < 0) return cuda_fail(c, "rad_couple");
     c->launches += nl;
@@ -522,6 +556,15 @@ rad_status rad_get_table(rad_ctx *c, int which, void *host_out, size_t nbytes) {
         case RAD_TAB_FACE_SIGN: need = (size_t)t.ncell * 3 * t.N; break;
         case RAD_TAB_EDGE_SIGN: need = (size_t)t.ncell * t.E; break;
         case RAD_TAB_MAXSPEED: need = 3 * sizeof(double); break;
+        case RAD_TAB_OWN_EDGE:
+            if (!t.fused_ok) return fail(c, RAD_ESTATE, "rad_get_table: this context does not run the tile kernel");
+            src = c->own.own_edge.data(); need = sizeof(int) * 3 * h.N; break;
+        case RAD_TAB_KE:
+            if (!t.ke) return fail(c, RAD_ESTATE, "rad_get_table: this context stores no edge coefficients");
+            need = sizeof(double) * (size_t)t.n[0] * t.n[1] * t.n[2] * 3 * h.N; break;
+        case RAD_TAB_STAGE_FACE_SIGN:
+            if (!t.rec) return fail(c, RAD_ESTATE, "rad_get_table: this context does not run the tile kernel");
+            need = (size_t)t.ncell * 3 * t.N; break;
         default: return fail(c, RAD_EINVAL, "rad_get_table: unknown table");
     }
     if (nbytes != need) {
@@ -530,8 +573,9 @@ rad_status rad_get_table(rad_ctx *c, int which, void *host_out, size_t nbytes) {
         return fail(c, RAD_EINVAL, buf);
     }
     if (src) { memcpy(host_out, src, need); return RAD_OK; }
-    if (which == RAD_TAB_CELL || which == RAD_TAB_FACE) {
-        if (cudaMemcpy(host_out, which == RAD_TAB_CELL ? t.cell : t.face, need, cudaMemcpyDeviceToHost) != cudaSuccess) return cuda_fail(c, "rad_get_table");
+    if (which == RAD_TAB_CELL || which == RAD_TAB_FACE || which == RAD_TAB_KE) {
+        const void *dsrc = which == RAD_TAB_CELL ? (const void *)t.cell : (which == RAD_TAB_FACE ? (const void *)t.face : (const void *)t.ke);
+        if (cudaMemcpy(host_out, dsrc, need, cudaMemcpyDeviceToHost) != cudaSuccess) return cuda_fail(c, "rad_get_table");
         return RAD_OK;
     }
     void *tmp = nullptr;
@@ -539,6 +583,7 @@ rad_status rad_get_table(rad_ctx *c, int which, void *host_out, size_t nbytes) {
     int nl = 0;
     if (which == RAD_TAB_FACE_SIGN) nl = rad::launch_sign_tables(t, (signed char *)tmp, nullptr, 0);
     else if (which == RAD_TAB_EDGE_SIGN) nl = rad::launch_sign_tables(t, nullptr, (signed char *)tmp, 0);
+    else if (which == RAD_TAB_STAGE_FACE_SIGN) nl = rad::launch_stage_face_signs(t, (signed char *)tmp, 0);
     else nl = rad::launch_maxspeed(t, (double *)tmp, 0);
     bool ok = nl >= 0 && cudaMemcpy(host_out, tmp, need, cudaMemcpyDeviceToHost) == cudaSuccess;
     cudaFree(tmp);

@@ -34,6 +34,8 @@ bool build_edge_ownership(const AngleTables &a, EdgeOwnership &out, std::string 
 
 bool build_latlon(int nzeta, int npsi, AngleTables &out, std::string &err);
 bool build_geodesic(int nlev, AngleTables &out, std::string &err);
+bool build_explicit(int N, const double *nhat, const double *domega, const int *nnbr, const int *nbr, const double *edge_len,
+                    const double *edge_mid, const double *edge_nrm, AngleTables &out, std::string &err);
 
 // Everything the kernels read besides the caller's arrays (device pointers).
 struct DeviceTables {
@@ -63,6 +65,9 @@ struct DeviceTables {
     const int *own_edge;     // [N][3]
     const double *ke;        // [n2][n1][n0][3][N] interior cells only, or nullptr (not stored)
     int fused_ok;            // 1 if the fused kernel can serve this angle grid
+    const int *mirror;       // [3][N] angle image under the flip of tetrad component a (reflecting walls, R20), or nullptr
+    int recon_angle;         // 0 donor cell, 1 PLM on the latitude-longitude grid (R21)
+    int nzeta, npsi;         // latitude-longitude grid shape (recon_angle == 1)
     const double *rec;       // [ncell][RAD_STAGE_RECN] packed per-cell record of the angle-resident stage kernel (stage5.cu), or nullptr
 };
 #define RAD_STAGE_RECN 36
@@ -114,6 +119,7 @@ int stage_angle_serves(const DeviceTables &t);
 // TAU table of the angle-resident kernel: vel8[ncell][8], see k_tau_table (stage5.cu)
 int launch_tau_table(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double tau_dt, double *vel8, cudaStream_t s);
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s);
+int launch_stage_face_signs(const DeviceTables &t, signed char *out, cudaStream_t s);  // 0 if the context has no stage records
 int launch_build_ke(const DeviceTables &t, double *ke, cudaStream_t s);
 int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed char *edge_sign, cudaStream_t s);
 int launch_maxspeed(const DeviceTables &t, double *out3, cudaStream_t s);

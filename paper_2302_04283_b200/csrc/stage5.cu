@@ -711,6 +711,20 @@ __global__ void __launch_bounds__(256) k_pack_rec(const DeviceTables t, double *
     }
 }
 
+// Parity helper: the upwind decision of the stage kernel itself for the three UPPER faces of every cell -- face_geom() on the packed
+// records, exactly what k_stage5 evaluates -- as sgn n^a: -1 where the kernel takes the upper cell as upwind, +1 the lower, 0 for n^a = 0.
+__global__ void __launch_bounds__(256) k_stage_face_signs(const DeviceTables t, signed char *__restrict__ out) {
+    const long long total = t.ncell * 3 * t.N;
+    for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
+        const int n = (int)(q % t.N);
+        const long long cf = q / t.N;  // cell * 3 + axis
+        const double *r = t.rec + (cf / 3) * RECN + (cf % 3) * 8;
+        const FaceRec f = {r[0], r[1], r[2], r[3], r[4], r[5], r[6], r[7]};
+        const FaceGeom g = face_geom(f, t.nhat[3 * n], t.nhat[3 * n + 1], t.nhat[3 * n + 2]);
+        out[q] = g.na == 0.0 ? 0 : (g.neg ? -1 : 1);
+    }
+}
+
 template <int NITER, int WPC, int TY, int TZ, int MINB, bool TAU>
 int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
     using T = Tile<TY, TZ, WPC, TAU>;
@@ -814,6 +828,12 @@ int stage_angle_serves(const DeviceTables &t) {
 
 int launch_tau_table(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double tau_dt, double *vel8, cudaStream_t s) {
     k_tau_table<<<t.sms * 4, 256, 0, s>>>(t, fluid, aE, aS, tau_dt, vel8);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+int launch_stage_face_signs(const DeviceTables &t, signed char *out, cudaStream_t s) {
+    if (t.rec == nullptr) return 0;
+    k_stage_face_signs<<<t.sms * 8, 256, 0, s>>>(t, out);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -564,7 +564,8 @@ size_t moments_smem(int N) { return sizeof(double) * (4 * (size_t)N + (size_t)kW
 
 }  // namespace
 
-// 1 if the streaming kernels serve this angle grid and these arrays: rows must be multiples of 16 bytes (bulk copies)
+// 1 if the streaming kernels serve this angle grid and these arrays: rows must be multiples of 16 bytes (bulk copies).
+// I == nullptr asks about the angle grid alone.
 int stream_serves(const DeviceTables &t, const void *I) {
     return (t.N & 1) == 0 && ((uintptr_t)I & 15) == 0 && couple_smem(t.N) <= (size_t)t.smem_optin;
 }

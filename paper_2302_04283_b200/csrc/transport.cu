@@ -13,7 +13,10 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 // ghost fill: one launch per axis, in x, y, z order so that edges and corners are filled
 // ------------------------------------------------------------------------------------------------
-__global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int NK, int ng, int axis, int nint, int bc_lo, int bc_hi, int vec2) {
+// bc: 0 caller-filled, 1 periodic, 2 outflow, 3 reflecting wall: mirror cell across the wall, direction with the wall-normal tetrad
+// component flipped (R20); mirror[N] = that angle permutation for this axis
+__global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int NK, int ng, int axis, int nint, int bc_lo, int bc_hi, int vec2,
+                              const int *__restrict__ mirror) {
     // one CTA per ghost cell of this axis' two slabs; threads over angles
     const int dims[3] = {NI, NJ, NK};
     int d[3];
@@ -32,13 +35,16 @@ __global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int
     if (bc == 0) return;
     int src = q;
     if (bc == 1) src = ng + (((q - ng) % nint) + nint) % nint;
+    else if (bc == 3) src = low ? 2 * ng - 1 - q : 2 * (dims[axis] - ng) - 1 - q;
     else src = low ? ng : ng + nint - 1;
     int s[3] = {d[0], d[1], d[2]};
     s[axis] = src;
     const long long cd = ((long long)d[2] * NJ + d[1]) * NI + d[0], cs = ((long long)s[2] * NJ + s[1]) * NI + s[0];
     const double2 *ps = reinterpret_cast<const double2 *>(I + cs * N);
     double2 *pd = reinterpret_cast<double2 *>(I + cd * N);
-    if (vec2) {  // rows are 16-byte aligned: N even and the array itself aligned
+    if (bc == 3) {
+        for (int n = threadIdx.x; n < N; n += blockDim.x) I[cd * N + n] = I[cs * N + mirror[n]];
+    } else if (vec2) {  // rows are 16-byte aligned: N even and the array itself aligned
         for (int n = threadIdx.x; n < N / 2; n += blockDim.x) pd[n] = ps[n];
     } else {
         for (int n = threadIdx.x; n < N; n += blockDim.x) I[cd * N + n] = I[cs * N + n];
@@ -61,11 +67,35 @@ __device__ __forceinline__ double vl_slope(double qm, double q0, double qp) {
     return pr > 0.0 ? 2.0 * pr / (dl + dr) : 0.0;
 }
 
+// PPM (Colella & Woodward 1984) on uniform spacing, no characteristic tracing: the monotonised parabola of the cell with
+// values q[-2..2] around it (p points at the cell, stride st); returns its value at the upper (upper = true) or lower face.
+// CW84 Eq.1.6-1.8 (interface values from van Leer-limited average slopes), Eq.1.10 (monotonisation).
+__device__ __forceinline__ double ppm_dq(double qm, double q0, double qp) {
+    const double dl = q0 - qm, dr = qp - q0;
+    if (dl * dr <= 0.0) return 0.0;
+    const double d = 0.5 * (qp - qm), lim = fmin(2.0 * fabs(dl), 2.0 * fabs(dr));
+    return (d > 0.0 ? 1.0 : -1.0) * fmin(fabs(d), lim);
+}
+__device__ __forceinline__ double ppm_face(const double *__restrict__ p, long long st, bool upper) {
+    const double q0 = p[-2 * st], q1 = p[-st], q2 = p[0], q3 = p[st], q4 = p[2 * st];
+    const double dqm = ppm_dq(q0, q1, q2), dq0 = ppm_dq(q1, q2, q3), dqp = ppm_dq(q2, q3, q4);
+    double qm = q1 + 0.5 * (q2 - q1) - (dq0 - dqm) / 6.0;
+    double qp = q2 + 0.5 * (q3 - q2) - (dqp - dq0) / 6.0;
+    if ((qp - q2) * (q2 - qm) <= 0.0) { qm = q2; qp = q2; }
+    else {
+        const double dq = qp - qm, q6 = 6.0 * (q2 - 0.5 * (qm + qp));
+        if (dq * q6 > dq * dq) qm = 3.0 * q2 - 2.0 * qp;
+        else if (-dq * dq > dq * q6) qp = 3.0 * q2 - 2.0 * qm;
+    }
+    return upper ? qp : qm;
+}
+
 // flux through the face whose record is `f`, between cells L (lower) and R (upper) along a stride `st`.
+// RECON: 0 donor cell, 1 PLM (van Leer, R7), 2 PPM.
 // TAU: the optical-depth-aware flux of Eq.26-29 (readings R15-R18, G1 in DESIGN.md): vL, vR = {u^alphahat (4),
 // alpha_E} of the two cells, tau = tau_dt (alpha_E,L + alpha_E,R)/2 / ((u^0hat_L + u^0hat_R)/2), f = -expm1(-tau^2),
 // g_L/R = -f (1 + 1/n^0bar_L/R), g = (g_L + g_R)/2, the upwind intensity is multiplied by 1 - g_up + g.
-template <bool PLM, bool TAU>
+template <int RECON, bool TAU>
 __device__ __forceinline__ double face_flux(const double *f, double n1, double n2, double n3, const double *__restrict__ pR, long long st,
                                             const double *__restrict__ vL, const double *__restrict__ vR, double tau_dt) {
     const double na = chain4(f, n1, n2, n3), n0 = chain4(f + 4, n1, n2, n3);
@@ -73,11 +103,13 @@ __device__ __forceinline__ double face_flux(const double *f, double n1, double n
     if (na > 0.0) {
         const double qL = pR[-st];
         up = qL;
-        if (PLM) up = qL + 0.5 * vl_slope(pR[-2 * st], qL, pR[0]);
+        if (RECON == 1) up = qL + 0.5 * vl_slope(pR[-2 * st], qL, pR[0]);
+        if (RECON == 2) up = ppm_face(pR - st, st, true);
     } else if (na < 0.0) {
         const double qR = pR[0];
         up = qR;
-        if (PLM) up = qR - 0.5 * vl_slope(pR[-st], qR, pR[st]);
+        if (RECON == 1) up = qR - 0.5 * vl_slope(pR[-st], qR, pR[st]);
+        if (RECON == 2) up = ppm_face(pR, st, false);
     } else {
         return 0.0;
     }
@@ -108,7 +140,7 @@ __global__ void __launch_bounds__(256) k_cell_velocity(DeviceTables t, const dou
     }
 }
 
-template <bool PLM, bool TAU>
+template <int RECON, bool TAU>
 __global__ void __launch_bounds__(256) k_fluxdiv_v1(DeviceTables t, const double *__restrict__ I_in, const double *__restrict__ I0,
                                                    double gam0, double gam1, double beta_dt, double *__restrict__ I_out,
                                                    const double *__restrict__ vel, double tau_dt) {
@@ -153,7 +185,26 @@ __global__ void __launch_bounds__(256) k_fluxdiv_v1(DeviceTables t, const double
         const double ce = -acc;
         const double n0e = chain4(sCell + cl * 36 + 1, __ldg(t.edge_mid + 3 * e), __ldg(t.edge_mid + 3 * e + 1), __ldg(t.edge_mid + 3 * e + 2));
         const int a_up = ce > 0.0 ? __ldg(t.edge_lo + e) : __ldg(t.edge_hi + e);
-        const double Iup = I_in[(c0 + cl) * N + a_up];
+        const double *row = I_in + (c0 + cl) * N;
+        double Iup = row[a_up];
+        if (t.recon_angle == 1 && ce != 0.0) {
+            // R21: van Leer PLM in index space on the latitude-longitude grid; beyond a pole the row of cell (l, m) continues
+            // in cell (l, m + N_psi / 2); periodic in psi.  slot of this edge in the upwind cell: 0 zeta-, 1 zeta+, 2 psi-, 3 psi+
+            int slot = 0;
+            while (__ldg(t.nbr_edge + a_up * RAD_MAXNBR + slot) != e) slot++;
+            const int np = t.npsi, l = a_up / np, m = a_up - l * np;
+            int lo, hi;
+            if (slot < 2) {
+                const int across = l * np + (m + np / 2) % np;
+                lo = l > 0 ? a_up - np : across;
+                hi = l + 1 < t.nzeta ? a_up + np : across;
+            } else {
+                lo = l * np + (m + np - 1) % np;
+                hi = l * np + (m + 1) % np;
+            }
+            const double sl = vl_slope(row[lo], Iup, row[hi]);
+            Iup = (slot & 1) ? Iup + 0.5 * sl : Iup - 0.5 * sl;
+        }
         sFe[cl * E + e] = (ce == 0.0) ? 0.0 : __ldg(t.edge_len + e) * (ce * n0e * Iup);
     }
     __syncthreads();
@@ -170,12 +221,12 @@ __global__ void __launch_bounds__(256) k_fluxdiv_v1(DeviceTables t, const double
         const long long sx = N;
         double div = 0.0;
         const double *vc = TAU ? vel + 5 * c : nullptr;  // this cell's velocity record; the neighbours' are 5 * stride away
-        div += (face_flux<PLM, TAU>(sFx + (cl + 1) * 8, n1, n2, n3, p + sx, sx, vc, vc + 5, tau_dt) -
-                face_flux<PLM, TAU>(sFx + cl * 8, n1, n2, n3, p, sx, vc - 5, vc, tau_dt)) * t.inv_dx[0];
-        div += (face_flux<PLM, TAU>(sFy + CX * 8 + cl * 8, n1, n2, n3, p + sy * N, sy * N, vc, vc + 5 * sy, tau_dt) -
-                face_flux<PLM, TAU>(sFy + cl * 8, n1, n2, n3, p, sy * N, vc - 5 * sy, vc, tau_dt)) * t.inv_dx[1];
-        div += (face_flux<PLM, TAU>(sFz + CX * 8 + cl * 8, n1, n2, n3, p + sz * N, sz * N, vc, vc + 5 * sz, tau_dt) -
-                face_flux<PLM, TAU>(sFz + cl * 8, n1, n2, n3, p, sz * N, vc - 5 * sz, vc, tau_dt)) * t.inv_dx[2];
+        div += (face_flux<RECON, TAU>(sFx + (cl + 1) * 8, n1, n2, n3, p + sx, sx, vc, vc + 5, tau_dt) -
+                face_flux<RECON, TAU>(sFx + cl * 8, n1, n2, n3, p, sx, vc - 5, vc, tau_dt)) * t.inv_dx[0];
+        div += (face_flux<RECON, TAU>(sFy + CX * 8 + cl * 8, n1, n2, n3, p + sy * N, sy * N, vc, vc + 5 * sy, tau_dt) -
+                face_flux<RECON, TAU>(sFy + cl * 8, n1, n2, n3, p, sy * N, vc - 5 * sy, vc, tau_dt)) * t.inv_dx[1];
+        div += (face_flux<RECON, TAU>(sFz + CX * 8 + cl * 8, n1, n2, n3, p + sz * N, sz * N, vc, vc + 5 * sz, tau_dt) -
+                face_flux<RECON, TAU>(sFz + cl * 8, n1, n2, n3, p, sz * N, vc - 5 * sz, vc, tau_dt)) * t.inv_dx[2];
         double adiv = 0.0;
 #pragma unroll
         for (int s = 0; s < RAD_MAXNBR; s++) {
@@ -199,7 +250,8 @@ int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_h
         long long ext[3] = {t.NI, t.NJ, t.NK};
         ext[ax] = 2 * t.ng;
         const long long blocks = ext[0] * ext[1] * ext[2];
-        k_fill_ghosts<<<(unsigned)blocks, 64, 0, s>>>(I, t.N, t.NI, t.NJ, t.NK, t.ng, ax, t.n[ax], bc_lo[ax], bc_hi[ax], (t.N & 1) == 0 && ((uintptr_t)I & 15) == 0);
+        k_fill_ghosts<<<(unsigned)blocks, 64, 0, s>>>(I, t.N, t.NI, t.NJ, t.NK, t.ng, ax, t.n[ax], bc_lo[ax], bc_hi[ax], (t.N & 1) == 0 && ((uintptr_t)I & 15) == 0,
+                                                      t.mirror ? t.mirror + ax * t.N : nullptr);
         if (cudaGetLastError() != cudaSuccess) return -1;
         launches++;
     }
@@ -217,13 +269,14 @@ int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, c
     const int nxb = (t.n[0] + CX - 1) / CX;
     const long long blocks = (long long)nxb * t.n[1] * t.n[2];
     const size_t smem = sizeof(double) * (CX * 36 + (CX + 1) * 8 + 4 * CX * 8 + (size_t)CX * t.E);
-#define RAD_LAUNCH_FD(PLM, TAU)                                                                                     \
-    do {                                                                                                            \
-        cudaFuncSetAttribute(k_fluxdiv_v1<PLM, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
-        k_fluxdiv_v1<PLM, TAU><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out, vel, tau_dt); \
+#define RAD_LAUNCH_FD(RECON, TAU)                                                                                     \
+    do {                                                                                                              \
+        cudaFuncSetAttribute(k_fluxdiv_v1<RECON, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+        k_fluxdiv_v1<RECON, TAU><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out, vel, tau_dt); \
     } while (0)
-    if (p.recon_space == 1) { if (vel) RAD_LAUNCH_FD(true, true); else RAD_LAUNCH_FD(true, false); }
-    else { if (vel) RAD_LAUNCH_FD(false, true); else RAD_LAUNCH_FD(false, false); }
+    if (p.recon_space == 2) { if (vel) RAD_LAUNCH_FD(2, true); else RAD_LAUNCH_FD(2, false); }
+    else if (p.recon_space == 1) { if (vel) RAD_LAUNCH_FD(1, true); else RAD_LAUNCH_FD(1, false); }
+    else { if (vel) RAD_LAUNCH_FD(0, true); else RAD_LAUNCH_FD(0, false); }
 #undef RAD_LAUNCH_FD
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }

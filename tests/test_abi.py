@@ -55,10 +55,19 @@ def test_no_gpu_means_error_not_fallback(so):
     grid = dict(n=(4, 4, 4), x0=(0, 0, 0), dx=(1, 1, 1))
     with pytest.raises(B.RadError) as e:
         B.rad_create(dict(kind=0), dict(grid, ng=1), ("latlon", 2, 4), None, dict(couple=0))
-    assert e.value.status == 1  # RAD_EINVAL: ng must be 2
+    assert e.value.status == 1  # RAD_EINVAL: ng must be 2 or 3
     with pytest.raises(B.RadError) as e:
-        B.rad_create(dict(kind=0), grid, ("latlon", 2, 4), None, dict(couple=0, recon_angle=1))
-    assert e.value.status == 4  # RAD_EUNSUPPORTED
+        B.rad_create(dict(kind=0), grid, ("geodesic", 2), None, dict(couple=0, recon_angle=1))
+    assert e.value.status == 4  # RAD_EUNSUPPORTED: PLM in angle is for lat-lon grids (MAPR is not implemented)
+    with pytest.raises(B.RadError) as e:
+        B.rad_create(dict(kind=0), grid, ("latlon", 2, 5), None, dict(couple=0, recon_angle=1))
+    assert e.value.status == 4  # ... with even npsi (the pole-crossing stencil)
+    with pytest.raises(B.RadError) as e:
+        B.rad_create(dict(kind=0), grid, ("latlon", 2, 4), None, dict(couple=0, recon_space=2))
+    assert e.value.status == 1  # PPM needs ng = 3
+    with pytest.raises(B.RadError) as e:
+        B.rad_create(dict(kind=0), dict(grid, bc_hi=(4, 0, 0)), ("latlon", 2, 4), None, dict(couple=0))
+    assert e.value.status == 1  # bad boundary code
     with pytest.raises(B.RadError) as e:
         B.rad_create(dict(kind=0), grid, ("latlon", 2, 4), None, dict(couple=0, tau_factor=1.0))
     assert e.value.status == 1  # RAD_EINVAL: the optical-depth-aware flux (Eq.26-29) needs opacities

@@ -1,0 +1,329 @@
+"""GPU parity of every path that ships besides the default one: the generic two-kernel path
+(recompute_edge_coeffs, N > 256, odd N), the tile shapes of every angle-count range, the two halves of a stage on their own, the
+moments at every size class, the stage kernel's own upwind decisions, the quartic far from the easy regime, and the round-2
+features (PPM in space, PLM in angle, reflecting walls, velocity estimate, explicit angle tables)."""
+import numpy as np
+import pytest
+import torch
+
+from parity_util import TOL_FLUID, TOL_I, err_dT0, rel_err, rel_err_I
+from test_gpu_parity import B, compare_stage, dev, small_problem  # noqa: F401  (B is the module fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+# ------------------------------------------------------------------------------------------------ every kernel route
+@pytest.mark.parametrize("angles", [("geodesic", 3), ("geodesic", 4), ("latlon", 8, 16), ("latlon", 3, 5)])
+@pytest.mark.parametrize("tau", [0.0, 2.0])
+def test_generic_path_without_stored_coefficients(oracle, B, angles, tau):
+    """recompute_edge_coeffs = 1: no stored coefficients, the stage runs as k_fluxdiv_v1 (+ k_cell_velocity) and the coupling kernel"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (7, 5, 4), angles, recompute_edge_coeffs=1, tau_factor=tau)
+    try:
+        with pytest.raises(B.RadError):   # no tile kernel in this context
+            B.rad_get_table(h, B.TAB_KE, n_interior=7 * 5 * 4)
+        compare_stage(B, A, P, h, I, fluid, opac, 0.03)
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("angles,n", [(("geodesic", 6), (5, 3, 2)), (("latlon", 17, 16), (4, 3, 3)), (("latlon", 7, 9), (4, 3, 3)),
+                                      (("latlon", 8, 16), (9, 6, 5)), (("latlon", 7, 16), (6, 9, 5)), (("geodesic", 5), (5, 4, 6))])
+@pytest.mark.parametrize("tau", [0.0, 1.5])
+def test_every_angle_count_range(oracle, B, angles, n, tau):
+    """N = 362 (geodesic 6) and 272: above the tile kernel's 256, generic kernels incl. k_coupling / k_moments; N = 63: odd, generic;
+    N = 128 (the paper's 8 x 16 grid) and 112: the 96 < N <= 128 tile shape; N = 252: the 2 x 2 tile"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, angles, tau_factor=tau)
+    try:
+        compare_stage(B, A, P, h, I, fluid, opac, 0.03)
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("angles", [("geodesic", 3), ("geodesic", 4), ("geodesic", 6), ("latlon", 7, 9)])
+def test_transport_and_coupling_halves_against_the_oracle(oracle, B, angles):
+    """rad_transport vs orc_transport and rad_couple vs orc_coupling, each on its own (the streaming coupling kernel for even N that
+    fits shared memory, the generic one otherwise)"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (9, 5, 4), angles, bc=(1, 2, 0, 1, 2, 0))
+    try:
+        dI = dev(I); dO = torch.zeros_like(dI)
+        B.rad_transport(h, dI, dO, None, 0.0, 1.0, 0.03)
+        Io = I.copy(); P.fill_ghosts(Io)
+        ref = P.transport(Io, 0.03)
+        assert np.array_equal(dI.cpu().numpy(), Io)
+        assert rel_err_I(P.interior(dO.cpu().numpy()), P.interior(ref)) <= TOL_I
+        # coupling in place on the transported field
+        dC = dev(ref); dT = torch.zeros(P.ncell, dtype=torch.float64, device="cuda"); ddT0 = torch.zeros(4, P.ncell, dtype=torch.float64, device="cuda")
+        nf = B.rad_couple(h, dC, dev(fluid), 0.03, dT, ddT0, count_noroot=True)
+        Ic = ref.copy()
+        T_o, dT0_o, nf_o = P.coupling(Ic, fluid, opac, 0.03)
+        assert nf == nf_o
+        assert rel_err_I(P.interior(dC.cpu().numpy()), P.interior(Ic)) <= TOL_I
+        assert rel_err(P.interior(dT.cpu().numpy()), P.interior(T_o), 0.0) <= TOL_FLUID
+        assert err_dT0(P, ddT0.cpu().numpy(), dT0_o, Ic)[0] <= TOL_FLUID
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("angles", [("latlon", 1, 4), ("geodesic", 2), ("geodesic", 4), ("geodesic", 5), ("geodesic", 6), ("latlon", 7, 9)])
+@pytest.mark.parametrize("frame", [0, 1, 2, 3])
+def test_moments_every_size_class(oracle, B, angles, frame):
+    """N = 4, 42, 162, 252 (streaming kernel), 362 (too large for its shared memory) and 63 (odd): all four frames; odd block
+    length along x (the last pair of a row holds one cell)"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (7, 4, 3), angles)
+    try:
+        ncomp = 10 if frame in (0, 2) else 4
+        out = torch.zeros(ncomp, P.ncell, dtype=torch.float64, device="cuda")
+        B.rad_moments(h, dev(I), frame, dev(fluid), out)
+        ref = P.moments(I, frame, fluid)
+        # an N-term sum in another order: up to ~N eps of the sum of |terms| (N = 362: 4e-14), first moments cancel by up to 1e2
+        for q in range(ncomp):
+            assert rel_err(P.interior(out[q].cpu().numpy()), P.interior(ref[q]), 1e-13 * np.abs(ref).max()) < 4e-12
+    finally:
+        B.rad_destroy(h)
+
+
+def test_stage_kernel_upwind_decisions_bit_exact(oracle, B):
+    """the upwind choices the stage kernel itself takes: the low mantissa bit of its stored edge coefficients (owner is upwind) and the
+    sign of n^a from its own face evaluation on the packed records -- against the oracle's sign tables, bit for bit"""
+    n = (6, 5, 4)
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, ("geodesic", 4))
+    try:
+        fs, es = P.upwind_tables()                               # lower faces of every cell; every unique edge of every cell
+        own = B.rad_get_table(h, B.TAB_OWN_EDGE)
+        ke = B.rad_get_table(h, B.TAB_KE, n_interior=n[0] * n[1] * n[2]).reshape(n[2], n[1], n[0], 3, A.N)
+        es_int = P.interior(es)                                   # [k][j][i][E]
+        bit = (ke.view(np.int64) & 1).astype(bool)
+        checked = 0
+        for q in range(A.N):
+            for j in range(3):
+                e = own[q, j]
+                if e < 0:
+                    assert (ke[..., j, q] == 0).all()
+                    continue
+                sg = es_int[..., e]
+                owner_is_lo = A.edge_lo[e] == q
+                expect_up = (sg > 0) == owner_is_lo                # c_e > 0: the lower angle of the edge is upwind (Eq.25)
+                nz = sg != 0
+                assert np.array_equal(bit[..., j, q][nz], expect_up[nz])
+                assert (ke[..., j, q][~nz] == 0).all() and (ke[..., j, q][nz] != 0).all()
+                checked += int(nz.sum())
+        assert checked > 1000 and set(own[own >= 0]) == set(range(A.E))   # every unique edge is owned exactly once
+        assert len(own[own >= 0]) == A.E
+        # faces: the kernel's table is for the UPPER faces of cell c = the lower faces of the next cell along the axis
+        ks = B.rad_get_table(h, B.TAB_STAGE_FACE_SIGN).reshape(P.shape + (3, A.N))
+        f5 = fs.reshape(P.shape + (3, A.N))
+        assert np.array_equal(ks[:, :, :-1, 0], f5[:, :, 1:, 0])
+        assert np.array_equal(ks[:, :-1, :, 1], f5[:, 1:, :, 1])
+        assert np.array_equal(ks[:-1, :, :, 2], f5[1:, :, :, 2])
+        assert (f5 != 0).all()
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("ratio", [1e6, 1e8, 1e10])
+def test_quartic_far_into_the_gas_dominated_regime(oracle, B, ratio):
+    """cold dense gas, strong scattering: C_v T / Ebar up to 1e10.  Eq.48 multiplies the temperature change by C_v, so the change must
+    be accurate relative to ITSELF; the solver's stopping rule is relative to d (stage_math.cuh).  Fused tile kernel and the
+    streaming coupling kernel both."""
+    A = oracle.Angles("geodesic", 4)
+    n, x0, dx = (6, 4, 4), (3.0, 2.0, 1.0), (0.3, 0.25, 0.2)
+    P = oracle.Problem(A, n, x0, dx, metric_kind=1, M=1.0, a=0.9)
+    rng = np.random.default_rng(9)
+    nc = P.ncell
+    I = np.exp(0.3 * rng.normal(size=(nc, A.N)))             # Ebar ~ 4 pi
+    T = rng.uniform(0.5, 1.5, nc)
+    rho = ratio * 4 * np.pi * (2.0 / 3.0) / T                  # C_v T = rho T / (Gamma - 1) = ratio * Ebar
+    fluid = np.stack([rho, T] + [rng.uniform(-0.2, 0.2, nc) for _ in range(3)])
+    opac = np.stack([rng.uniform(0.5, 2, nc), rng.uniform(0.5, 2, nc), rng.uniform(50, 200, nc)])
+    d_opac = dev(opac)
+    h = B.rad_create(dict(kind=1, M=1.0, a=0.9), dict(n=n, x0=x0, dx=dx), ("geodesic", 4), (d_opac[0], d_opac[1], d_opac[2]), dict())
+    try:
+        compare_stage(B, A, P, h, I, fluid, opac, 0.03)
+        Ic = I.copy(); dC = dev(I)
+        dT = torch.zeros(nc, dtype=torch.float64, device="cuda"); ddT0 = torch.zeros(4, nc, dtype=torch.float64, device="cuda")
+        B.rad_couple(h, dC, dev(fluid), 0.03, dT, ddT0)
+        T_o, dT0_o, _ = P.coupling(Ic, fluid, opac, 0.03)
+        assert rel_err_I(P.interior(dC.cpu().numpy()), P.interior(Ic)) <= TOL_I
+        assert err_dT0(P, ddT0.cpu().numpy(), dT0_o, Ic)[0] <= TOL_FLUID
+        # the temperature change itself, relative to itself (what Eq.48 needs), not to T
+        dTg, dTo = P.interior(dT.cpu().numpy()) - P.interior(fluid[1]), P.interior(T_o) - P.interior(fluid[1])
+        Eb = np.abs(P.interior(P.moments(Ic, 3, fluid)[0]))
+        Cv = P.interior(fluid[0]) * 1.5
+        assert (np.abs(dTg - dTo) * Cv <= 1e-9 * Eb + 4 * 2.0**-53 * Cv * P.interior(fluid[1])).all()
+    finally:
+        B.rad_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ round-2 features
+@pytest.mark.parametrize("angles,n,kind", [(("geodesic", 3), (9, 6, 5), 1), (("latlon", 4, 8), (13, 3, 4), 1), (("geodesic", 2), (5, 5, 5), 0)])
+@pytest.mark.parametrize("bc", [(0, 0, 0, 0, 0, 0), (1, 1, 1, 1, 1, 1), (2, 1, 0, 2, 1, 2)])
+def test_ppm_in_space(oracle, B, angles, n, kind, bc):
+    """recon_space = 2 (PPM) with three ghost cells, every boundary kind"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, angles, kind=kind, a=0.9 if kind else 0.0, bc=bc, ng=3, recon_space=2)
+    try:
+        got, ref = compare_stage(B, A, P, h, I, fluid, opac, 0.03)
+        plm = oracle.Problem(A, n, (3.0, 2.0, 1.0), (0.3, 0.25, 0.2), metric_kind=kind, M=1.0, a=0.9 if kind else 0.0, ng=3, bc_lo=bc[:3], bc_hi=bc[3:])
+        assert np.abs(P.interior(ref) - P.interior(plm.stage(I.copy(), fluid, opac, 0.03)[0])).max() > 1e-4   # PPM is not PLM
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("angles", [("latlon", 4, 8), ("latlon", 6, 12), ("latlon", 1, 4), ("latlon", 5, 2)])
+@pytest.mark.parametrize("recon_space,ng", [(1, 2), (2, 3)])
+def test_plm_in_angle_on_the_latlon_grid(oracle, B, angles, recon_space, ng):
+    """recon_angle = 1 (R21): the pole-crossing stencil in Kerr-Schild, where the angular fluxes are non-zero"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (6, 5, 4), angles, ng=ng, recon_space=recon_space, recon_angle=1)
+    try:
+        got, ref = compare_stage(B, A, P, h, I, fluid, opac, 0.03)
+        if A.N > 8:
+            dc = oracle.Problem(A, (6, 5, 4), (3.0, 2.0, 1.0), (0.3, 0.25, 0.2), metric_kind=1, M=1.0, a=0.9, ng=ng, recon_space=recon_space)
+            assert np.abs(P.interior(ref) - P.interior(dc.stage(I.copy(), fluid, opac, 0.03)[0])).max() > 1e-5
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("angles,bc", [(("latlon", 4, 8), (3, 3, 3, 3, 3, 3)), (("latlon", 4, 8), (2, 0, 1, 3, 3, 1)), (("geodesic", 3), (1, 3, 0, 1, 3, 2)),
+                                      (("geodesic", 4), (0, 0, 0, 0, 3, 0))])
+@pytest.mark.parametrize("n", [(6, 5, 4), (2, 3, 9)])
+def test_reflecting_walls(oracle, B, angles, bc, n):
+    """bc code 3 (R20): mirror cells with mirrored directions, in the ghost fill that precedes the tile kernel; I_in's ghost
+    cells are compared bit for bit inside compare_stage"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, angles, kind=0, a=0.0, bc=bc)
+    try:
+        compare_stage(B, A, P, h, I, fluid, opac, 0.03)
+    finally:
+        B.rad_destroy(h)
+
+
+def test_reflecting_wall_needs_a_symmetric_angle_grid(oracle, B):
+    with pytest.raises(B.RadError) as e:
+        B.rad_create(dict(kind=0), dict(n=(4, 4, 4), x0=(0, 0, 0), dx=(1, 1, 1), bc_hi=(3, 0, 0)), ("geodesic", 2), None, dict(couple=0))
+    assert e.value.status == 4
+    with pytest.raises(B.RadError) as e:
+        B.rad_create(dict(kind=0), dict(n=(4, 4, 4), x0=(0, 0, 0), dx=(1, 1, 1), bc_hi=(3, 0, 0)), ("latlon", 2, 5), None, dict(couple=0))
+    assert e.value.status == 4
+
+
+def rad_dominated_problem(oracle, B, n, angles, seed=7, **params):
+    """cells on both sides of Ebar = rho + u_gas, beamed radiation, moving gas, opacities that give fractions f^a inside (0, 1)"""
+    A = oracle.Angles(*angles)
+    x0, dx = (3.0, 2.0, 1.0), (0.3, 0.25, 0.2)
+    P = oracle.Problem(A, n, x0, dx, metric_kind=1, M=1.0, a=0.5, vel_estimate=params.get("vel_estimate", 1), renorm=params.get("renorm_fluid_weights", 1))
+    rng = np.random.default_rng(seed)
+    nc = P.ncell
+    # faint radiation in the lower half of the block along x, bright in the upper half (transport mixes only across the middle)
+    ii = np.arange(nc) % P.NI
+    scale = (np.where(ii < P.NI // 2, 3e-3, 30.0) * 10.0 ** rng.uniform(-0.3, 0.3, nc))[:, None]
+    lobe = 1.0 + 2.0 * np.maximum(A.nhat @ np.array([0.6, 0.0, 0.8]), 0.0)[None, :] ** 2
+    I = scale * lobe * np.exp(0.2 * rng.normal(size=(nc, A.N)))
+    fluid = np.stack([rng.uniform(0.5, 2, nc), rng.uniform(0.3, 1.5, nc)] + [rng.uniform(-0.3, 0.3, nc) for _ in range(3)])
+    opac = np.stack([10.0 ** rng.uniform(-3, 1, nc), 10.0 ** rng.uniform(-3, 1, nc), 10.0 ** rng.uniform(-3, 1, nc)])
+    d_opac = dev(opac)
+    h = B.rad_create(dict(kind=1, M=1.0, a=0.5), dict(n=n, x0=x0, dx=dx), angles, (d_opac[0], d_opac[1], d_opac[2]), dict(params, vel_estimate=params.get("vel_estimate", 1)))
+    return A, P, h, I, fluid, opac, d_opac   # (the context reads the opacities from d_opac: the caller keeps it alive)
+
+
+@pytest.mark.parametrize("angles,n", [(("geodesic", 4), (7, 5, 4)), (("geodesic", 3), (8, 3, 3)), (("latlon", 5, 16), (5, 4, 3)), (("geodesic", 6), (8, 2, 2))])
+@pytest.mark.parametrize("renorm", [1, 0])
+def test_velocity_estimate(oracle, B, angles, n, renorm):
+    """vel_estimate = 1 (Eq.51-55, reading G8): cells on both sides of the radiation-dominated threshold"""
+    A, P, h, I, fluid, opac, _keep = rad_dominated_problem(oracle, B, n, angles, renorm_fluid_weights=renorm)
+    try:
+        got, ref = compare_stage(B, A, P, h, I, fluid, opac, 0.03)
+        off = oracle.Problem(A, n, (3.0, 2.0, 1.0), (0.3, 0.25, 0.2), metric_kind=1, M=1.0, a=0.5, renorm=renorm).stage(I.copy(), fluid, opac, 0.03)[0]
+        changed = np.abs(P.interior(ref) / P.interior(off) - 1).max(-1) > 1e-6
+        assert 0.05 < changed.mean() < 0.95      # the estimate acted in some cells and not in others
+    finally:
+        B.rad_destroy(h)
+
+
+def test_explicit_angle_tables_reproduce_the_geodesic_grid(oracle, B):
+    """rad_angles kind 2: the library fed its own geodesic tables back gives bit-identical results and tables"""
+    n = (6, 5, 4)
+    A, P, h, I, fluid, opac, d_opac = small_problem(oracle, B, n, ("geodesic", 3))
+    try:
+        nbr, ne = B.rad_get_table(h, B.TAB_NBR), B.rad_get_table(h, B.TAB_NBR_EDGE)
+        elen, emid, enrm = B.rad_get_table(h, B.TAB_EDGE_LEN), B.rad_get_table(h, B.TAB_EDGE_MID), B.rad_get_table(h, B.TAB_EDGE_NRM)
+        elo = B.rad_get_table(h, B.TAB_EDGE_LO)
+        N = A.N
+        tab = dict(nhat=B.rad_get_table(h, B.TAB_NHAT), domega=B.rad_get_table(h, B.TAB_DOMEGA), nnbr=B.rad_get_table(h, B.TAB_NNBR), nbr=nbr,
+                   edge_len=np.zeros((N, 6)), edge_mid=np.zeros((N, 6, 3)), edge_nrm=np.zeros((N, 6, 3)))
+        for q in range(N):
+            for s in range(6):
+                e = ne[q, s]
+                if e >= 0:
+                    tab["edge_len"][q, s] = elen[e]; tab["edge_mid"][q, s] = emid[e]
+                    tab["edge_nrm"][q, s] = enrm[e] if elo[e] == q else -enrm[e]     # pointing from q to the neighbour
+        dI = dev(I); dO = torch.zeros_like(dI); dT = torch.zeros(P.ncell, dtype=torch.float64, device="cuda"); d4 = torch.zeros(4, P.ncell, dtype=torch.float64, device="cuda")
+        B.rad_stage(h, dI, dO, None, dev(fluid), 0.0, 1.0, 0.03, dT, d4)
+    finally:
+        B.rad_destroy(h)
+    A2, P2, h2, I2, fluid2, opac2, _ = small_problem(oracle, B, n, ("geodesic", 3), explicit=tab)
+    try:
+        for t_ in (B.TAB_NBR_EDGE, B.TAB_EDGE_LO, B.TAB_EDGE_HI, B.TAB_EDGE_LEN, B.TAB_EDGE_MID, B.TAB_EDGE_NRM, B.TAB_OWN_EDGE):
+            ref_h = small_problem(oracle, B, (1, 1, 1), ("geodesic", 3), couple=0)[2]
+            try:
+                assert np.array_equal(B.rad_get_table(h2, t_), B.rad_get_table(ref_h, t_))
+            finally:
+                B.rad_destroy(ref_h)
+        dO2 = torch.zeros_like(dO); dT2 = torch.zeros_like(dT); d42 = torch.zeros_like(d4)
+        B.rad_stage(h2, dev(I2), dO2, None, dev(fluid2), 0.0, 1.0, 0.03, dT2, d42)
+        assert torch.equal(dO, dO2) and torch.equal(dT, dT2) and torch.equal(d4, d42)
+        compare_stage(B, A2, P2, h2, I2, fluid2, opac2, 0.03)
+    finally:
+        B.rad_destroy(h2)
+    bad = dict(tab, nhat=tab["nhat"] * 2.0)
+    with pytest.raises(B.RadError) as e:
+        small_problem(oracle, B, (2, 2, 2), ("geodesic", 3), explicit=bad)
+    assert e.value.status == 1
+    asym = dict(tab, nbr=tab["nbr"].copy()); asym["nbr"][0, 0] = 5 if tab["nbr"][0, 0] != 5 else 6
+    with pytest.raises(B.RadError) as e:
+        small_problem(oracle, B, (2, 2, 2), ("geodesic", 3), explicit=asym)
+    assert e.value.status == 1
+
+
+def test_velocity_estimate_full_size_c4(oracle, B):
+    """C4 (96^3 x 162, P_rad / P_gas over five decades: Ebar > rho + u_gas in many cells) at full size with vel_estimate = 1, in the
+    launch configuration bench.py times (tile kernel for the transport + streaming coupling kernel), on sampled sub-blocks"""
+    from paper_2302_04283_b200 import workloads as W
+    from parity_util import make_rad
+    cfg, m = "C4", 6
+    c = W.CONFIGS[cfg]
+    nn, ng, x0, dx = W.grid(cfg)
+    N = W.n_angles(cfg)
+    h0 = B.rad_create(dict(kind=0), dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1)), c["angles"], None, dict(couple=0))
+    nhat = B.rad_get_table(h0, B.TAB_NHAT)
+    B.rad_destroy(h0)
+    inp = W.make_inputs(cfg, nhat, device="cuda")
+    shape = (nn[2] + 2 * ng, nn[1] + 2 * ng, nn[0] + 2 * ng)
+    I = inp["I"].reshape(-1, N).contiguous(); fluid = inp["fluid"].reshape(5, -1).contiguous(); opac = inp["opac"].reshape(3, -1).contiguous()
+    del inp
+    h = make_rad(B, cfg, opac, vel_estimate=1)
+    try:
+        dt = W.CFL * min(dx) / float(B.rad_get_table(h, B.TAB_MAXSPEED).max())
+        O = torch.full_like(I, -7.0)
+        T = torch.zeros(I.shape[0], dtype=torch.float64, device="cuda"); dT0 = torch.zeros(4, I.shape[0], dtype=torch.float64, device="cuda")
+        B.rad_stage(h, I, O, None, fluid, 0.0, 1.0, dt, T, dT0)
+        torch.cuda.synchronize()
+        A = oracle.Angles(*c["angles"])
+        I5 = I.reshape(shape + (N,)); O5 = O.reshape(shape + (N,))
+        f4 = fluid.reshape((5,) + shape); o4 = opac.reshape((3,) + shape); T3 = T.reshape(shape); d4 = dT0.reshape((4,) + shape)
+        acted = 0
+        for (ai, aj, ak) in [(0, 0, 0), (45, 46, 47), (90, 90, 90), (2, 88, 31)]:
+            sl = (slice(ak, ak + m + 2 * ng), slice(aj, aj + m + 2 * ng), slice(ai, ai + m + 2 * ng))
+            kw = dict(metric_kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg), gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT)
+            org = (x0[0] + ai * dx[0], x0[1] + aj * dx[1], x0[2] + ak * dx[2])
+            P = oracle.Problem(A, (m, m, m), org, dx, vel_estimate=1, **kw)
+            Is = I5[sl].cpu().numpy().reshape(-1, N).copy()
+            fs = f4[(slice(None),) + sl].cpu().numpy().reshape(5, -1).copy(); os_ = o4[(slice(None),) + sl].cpu().numpy().reshape(3, -1).copy()
+            out_o, T_o, dT0_o, _ = P.stage(Is, fs, os_, dt)
+            got = O5[sl].cpu().numpy().reshape(-1, N)
+            eI = rel_err_I(P.interior(got), P.interior(out_o))
+            eT = rel_err(P.interior(T3[sl].cpu().numpy().reshape(-1)), P.interior(T_o), 0.0)
+            eD, _ = err_dT0(P, np.stack([d4[(q,) + sl].cpu().numpy().reshape(-1) for q in range(4)]), dT0_o, out_o)
+            assert eI <= TOL_I and eT <= TOL_FLUID and eD <= TOL_FLUID, ((ai, aj, ak), eI, eT, eD)
+            off = oracle.Problem(A, (m, m, m), org, dx, **kw).stage(Is.copy(), fs, os_, dt)[0]
+            acted += int((np.abs(P.interior(out_o) / P.interior(off) - 1).max(-1) > 1e-9).sum())
+        assert acted > 20     # the estimate changed the result in a good number of the sampled cells
+    finally:
+        B.rad_destroy(h)
