@@ -399,168 +399,226 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_couple_stream(const DeviceTa
 
 // ---------------------------------------------------------------------------------------------------------------------------------
 // moments: by linearity every frame's moments follow from the ten tetrad-frame sums M^{ab} = sum_n I dOmega ntil^a ntil^b,
-// ntil = (1, n^1hat, n^2hat, n^3hat); the per-cell transform (tetrad e^mu_ahat for frame 0, n_alpha rows for frame 1, boost
-// Eq.13-14 with G2 for frame 3) is done once per cell after the warp reduction, by lanes 0 and 16 (one cell each).
+// ntil = (1, n^1hat, n^2hat, n^3hat) -- a dense contraction [cells x N] . [N x 10] (Eq.45 in the tetrad frame).  It runs on the
+// FP64 matrix instruction DMMA m8n8k4 (same FP64 pipe as DFMA on B200, measured; 256 multiply-adds per issue slot and no
+// cross-lane reduction): a warp takes 8 cells that are neighbours along x; per step of 4 angles lane l holds
+// A[cell l/4][angle l%4] = I (from the ring slot the bulk copies filled) and B[angle l%4][column l/4] = the table entry for the
+// first eight sums; sums 9 and 10 are two ordinary FMAs per step on the same A value, reduced over the four lanes of a cell at
+// the end.  The per-cell transform (tetrad e^mu_ahat for frame 0, n_alpha rows for frame 1, boost Eq.13-14 with G2 for frame 3)
+// is done once per cell afterwards, one lane per output component.
+// Shared memory rows are padded to Np = 4 (mod 16) doubles so that the eight cells' rows fall into different banks.
 // ---------------------------------------------------------------------------------------------------------------------------------
-constexpr int kMomDepth = 4;
+constexpr int kMomCells = 8;
 constexpr int kMomCellF = 24;  // per-cell scalars of the epilogue: cell record [0..4], [35..49], fluid u^1', u^2', u^3', pad
 
-__global__ void __launch_bounds__(kWarps * 32) k_moments_stream(const DeviceTables t, const double *__restrict__ I, int frame,
-                                                                const double *__restrict__ fluid, double *__restrict__ out) {
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+__host__ __device__ inline int mom_row_stride(int N) { return ((N + 3) / 4 * 4 + 11) / 16 * 16 + 4; }  // >= 4 ceil(N/4), = 4 (mod 16)
+
+__global__ void __launch_bounds__(384) k_moments_mma(const DeviceTables t, const double *__restrict__ I, int frame, const double *__restrict__ fluid,
+                                                     double *__restrict__ out, int depth) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = t.N, L2 = 2 * N;
+    const int N = t.N, nk = (N + 3) >> 2, Np = mom_row_stride(N);
     double *sm = reinterpret_cast<double *>(smem_raw);
-    double4 *sAng = reinterpret_cast<double4 *>(sm);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int perWarp = kMomDepth * L2 + 20 * 33 + 20 + 2 * kMomCellF + 2 * kMomDepth;
-    double *slots = sm + 4 * N + (size_t)w * perWarp, *red = slots + kMomDepth * L2, *tot = red + 20 * 33, *scell = tot + 20;
-    const uint32_t bar0 = smem_u32(scell + 2 * kMomCellF);
-    for (int q = threadIdx.x; q < N; q += blockDim.x) sAng[q] = make_double4(t.domega[q], t.nhat[3 * q], t.nhat[3 * q + 1], t.nhat[3 * q + 2]);
+    double *sB = sm;                                              // [nk][32]: fragment order, columns 0..7
+    double2 *sX = reinterpret_cast<double2 *>(sm + nk * 32);      // [nk][4]: columns 8, 9
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int perWarp = depth * kMomCells * Np + kMomCells * 10 + kMomCells * kMomCellF + 2 * depth;
+    double *slots = sm + nk * 40 + (size_t)w * perWarp, *tot = slots + depth * kMomCells * Np, *scell = tot + kMomCells * 10;
+    const uint32_t bar0 = smem_u32(scell + kMomCells * kMomCellF);
+    // the table: for angle n and column q = (a, b) of (00,01,02,03,11,12,13,22,23,33): dOmega_n ntil^a ntil^b
+    for (int q = threadIdx.x; q < nk * 32; q += blockDim.x) {
+        const int j = q >> 5, l = q & 31, n = 4 * j + (l & 3), col = l >> 2;
+        double v = 0.0;
+        if (n < N) {
+            const double nt[4] = {1.0, t.nhat[3 * n], t.nhat[3 * n + 1], t.nhat[3 * n + 2]};
+            const int ca[8] = {0, 0, 0, 0, 1, 1, 1, 2}, cb[8] = {0, 1, 2, 3, 1, 2, 3, 2};
+            v = t.domega[n] * nt[ca[col]] * nt[cb[col]];
+        }
+        sB[q] = v;
+    }
+    for (int q = threadIdx.x; q < nk * 4; q += blockDim.x) {
+        double2 v = make_double2(0.0, 0.0);
+        if (q < N) { const double w0 = t.domega[q], n2 = t.nhat[3 * q + 1], n3 = t.nhat[3 * q + 2]; v = make_double2(w0 * n2 * n3, w0 * n3 * n3); }
+        sX[q] = v;
+    }
+    for (int q = lane; q < depth * kMomCells * Np; q += 32) slots[q] = 0.0;  // the pad of every row stays zero
     if (lane == 0) {
-        for (int d = 0; d < kMomDepth; d++) mbar_init(bar0 + 16u * d, 1);
+        for (int d = 0; d < depth; d++) mbar_init(bar0 + 16u * d, 1);
         fence_mbar_init();
     }
+    fence_proxy_async();
     __syncthreads();
-    const int ppr = (t.n[0] + 1) >> 1;
-    const long long npairs = (long long)ppr * t.n[1] * t.n[2];
-    const long long nwarp = (long long)gridDim.x * kWarps, wid = (long long)blockIdx.x * kWarps + w;
-    const long long chunk = (npairs + nwarp - 1) / nwarp, pbeg = wid * chunk, pend = min(npairs, pbeg + chunk);
-    if (pbeg >= pend) return;
-    PairIt cur = pair_at(pbeg, ppr, t.n[1], 0), ahead = cur;  // the pair worked on, and the next pair to be copied
-    long long pahead = pbeg;
-    auto issue = [&]() {  // lane 0: the rows of pair `ahead` into its ring slot
-        int cnt;
-        const long long c = pair_cell(t, ahead, cnt);
-        const int sl = (int)((pahead - pbeg) % kMomDepth);
-        const uint32_t bar = bar0 + 16u * sl, bytes = (uint32_t)(cnt * N * 8);
-        if (lane == 0) {
-            mbar_expect_tx(bar, bytes);
-            bulk_g2s(smem_u32(slots + sl * L2), I + c * N, bytes, bar);
-        }
-        pair_next(ahead, ppr, t.n[1]);
-        pahead++;
+    const int gpr = (t.n[0] + kMomCells - 1) / kMomCells;  // groups per row
+    const long long ngroups = (long long)gpr * t.n[1] * t.n[2];
+    const long long nwarp = (long long)gridDim.x * nwarps, wid = (long long)blockIdx.x * nwarps + w;
+    const long long chunk = (ngroups + nwarp - 1) / nwarp, gbeg = wid * chunk, gend = min(ngroups, gbeg + chunk);
+    if (gbeg >= gend) return;
+    // position of a group in the block, advanced by integer adds only: (group along x, row j, plane k) and the flat index of its first cell
+    struct GroupIt { int ig, j, k; long long c; };
+    auto group_at = [&](long long g) {
+        const long long row = g / gpr;
+        GroupIt it;
+        it.ig = (int)(g - row * gpr); it.j = (int)(row % t.n[1]); it.k = (int)(row / t.n[1]);
+        it.c = ((long long)(it.k + t.ng) * t.NJ + (it.j + t.ng)) * t.NI + (kMomCells * it.ig + t.ng);
+        return it;
     };
-    for (int d = 0; d < kMomDepth - 1 && pahead < pend; d++) issue();
-    const int s0 = N >> 5, s1 = (N + 31) >> 5, npass = (L2 + 31) >> 5;
-    const int mycell = lane >> 4, li = lane & 15;
-    for (long long pid = pbeg; pid < pend; pid++) {
-        const int rel = (int)(pid - pbeg), sl = rel % kMomDepth;
-        int cnt;
-        const long long c0 = pair_cell(t, cur, cnt);
-        pair_next(cur, ppr, t.n[1]);
-        if (pahead < pend) issue();  // into the slot read in the previous iteration
-        // the epilogue's per-cell scalars, on their way while the sums are formed: lanes 0..15 cell 0, lanes 16..31 cell 1
-        double cv0 = 0.0, cv1 = 0.0;
-        if (mycell < cnt && frame != 2) {
-            const double *cg = t.cell + (c0 + mycell) * RAD_NCELL;
-            if (li < 5) cv0 = __ldg(cg + li);              // n^0, E_alphahat
-            else cv0 = __ldg(cg + 35 + (li - 5));          // beta^i (3), triad (6), co-triad [44], [45]
-            if (li < 4) cv1 = __ldg(cg + 46 + li);         // co-triad [46..49]
-            else if (li < 7 && frame == 3) cv1 = __ldg(fluid + (long long)(li - 2) * t.ncell + c0 + mycell);  // u^1', u^2', u^3'
+    auto group_next = [&](GroupIt &it) {
+        it.c += kMomCells;
+        if (++it.ig == gpr) {
+            it.ig = 0; it.c += t.NI - (long long)kMomCells * gpr;
+            if (++it.j == t.n[1]) { it.j = 0; ++it.k; it.c += (long long)t.NI * (t.NJ - t.n[1]); }
         }
-        mbar_wait(bar0 + 16u * sl, (uint32_t)((rel / kMomDepth) & 1));
-        const uint32_t aSl = smem_u32(slots + sl * L2);
-        double m[20];  // ten sums of cell 0, ten of cell 1
+    };
+    GroupIt cur = group_at(gbeg), ahead = cur;
+    long long gahead = gbeg;
+    int sl_ahead = 0;
+    auto issue = [&]() {  // the rows of group `ahead` into its ring slot, one bulk copy per cell
+        const int cnt = min(kMomCells, t.n[0] - kMomCells * ahead.ig);
+        const uint32_t bar = bar0 + 16u * sl_ahead;
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(cnt * N * 8));
+        __syncwarp();
+        if (lane < cnt) bulk_g2s(smem_u32(slots + (sl_ahead * kMomCells + lane) * Np), I + (ahead.c + lane) * N, (uint32_t)(N * 8), bar);
+        group_next(ahead);
+        gahead++;
+        if (++sl_ahead == depth) sl_ahead = 0;
+    };
+    for (int d = 0; d < depth - 1 && gahead < gend; d++) issue();
+    const int r = lane >> 2, kk = lane & 3;
+    const int ncomp = (frame == 0 || frame == 2) ? 10 : 4;
+    // the epilogue's per-cell scalars: item q = lane + 32 m = cell * 24 + field; offset relative to the group's first cell
+    // (cell table: doubles past t.cell + c0 * RAD_NCELL; fluid: field * ncell + cell), kind 0 nothing, 1 cell table, 2 fluid
+    int cvoff[6], cvkind[6];
 #pragma unroll
-        for (int q = 0; q < 20; q++) m[q] = 0.0;
-        auto pass = [&](int it, double (&mm)[20], int off, bool valid, int n) {
-            const double4 an = sAng[n];
-            const double w0 = valid ? lds(aSl + 8u * (uint32_t)(it * 32 + lane)) * an.x : 0.0;
-            const double w1 = w0 * an.y, w2 = w0 * an.z, w3 = w0 * an.w;
-            mm[off] += w0; mm[off + 1] += w1; mm[off + 2] += w2; mm[off + 3] += w3;
-            mm[off + 4] = fma(w1, an.y, mm[off + 4]); mm[off + 5] = fma(w1, an.z, mm[off + 5]); mm[off + 6] = fma(w1, an.w, mm[off + 6]);
-            mm[off + 7] = fma(w2, an.z, mm[off + 7]); mm[off + 8] = fma(w2, an.w, mm[off + 8]); mm[off + 9] = fma(w3, an.w, mm[off + 9]);
-        };
-#pragma unroll 2
-        for (int it = 0; it < s0; it++) pass(it, m, 0, true, it * 32 + lane);
-        if (s1 > s0) {  // the pass that straddles the two cells: each lane adds to its own cell's sums
-            const int f = s0 * 32 + lane;
-            const bool second = f >= N, valid = f < cnt * N;
-            double tmp[20];
-#pragma unroll
-            for (int q = 0; q < 10; q++) tmp[q] = 0.0;
-            pass(s0, tmp, 0, valid, valid ? (second ? f - N : f) : 0);
-#pragma unroll
-            for (int q = 0; q < 10; q++) { m[q] += second ? 0.0 : tmp[q]; m[10 + q] += second ? tmp[q] : 0.0; }
+    for (int m = 0; m < 6; m++) {
+        const int q = lane + 32 * m, cl = q / kMomCellF, f = q - cl * kMomCellF;
+        cvkind[m] = 0; cvoff[m] = cl;
+        if (frame != 2) {
+            if (f < 5) { cvkind[m] = 1; cvoff[m] = cl * RAD_NCELL + f; }                  // n^0, E_alphahat
+            else if (f < 20) { cvkind[m] = 1; cvoff[m] = cl * RAD_NCELL + 30 + f; }       // beta^i (3), triad (6), co-triad (6)
+            else if (f < 23 && frame == 3) { cvkind[m] = 2 + (f - 20); }                  // u^1', u^2', u^3' of cell cl
         }
-        if (cnt > 1) {
-#pragma unroll 2
-            for (int it = s1; it < npass; it++) {
-                const int f = it * 32 + lane;
-                const bool valid = f < L2;
-                pass(it, m, 10, valid, valid ? f - N : 0);
+    }
+    int sl = 0, par = 0;
+    for (long long g = gbeg; g < gend; g++) {
+        const int cnt = min(kMomCells, t.n[0] - kMomCells * cur.ig);
+        const long long c0 = cur.c;
+        group_next(cur);
+        if (gahead < gend) issue();  // into the slot read in the previous iteration
+        double cv[6];
+#pragma unroll
+        for (int m = 0; m < 6; m++) {
+            cv[m] = 0.0;
+            const int cl = (lane + 32 * m) / kMomCellF;
+            if (cl < cnt) {
+                if (cvkind[m] == 1) cv[m] = __ldg(t.cell + c0 * RAD_NCELL + cvoff[m]);
+                else if (cvkind[m] >= 2) cv[m] = __ldg(fluid + (long long)cvkind[m] * t.ncell + c0 + cl);
             }
         }
-        __syncwarp();                           // the previous pair's epilogue has read scell and tot
-        scell[lane] = cv0;                      // [cell][16]
-        if (li < 8) scell[32 + mycell * 8 + li] = cv1;  // [cell][8]
-        warp_sums_smem<20>(m, lane, red, tot);  // (its barriers also order the slot reads before the next copy into the slot)
-        if (li >= 10 || mycell >= cnt) continue;
-        // ---- epilogue: lane li of a cell's half produces output component li
-        const long long c = c0 + mycell;
-        const double *M10 = tot + mycell * 10, *ca = scell + mycell * 16, *cb = scell + 32 + mycell * 8;
-        const double M[4][4] = {{M10[0], M10[1], M10[2], M10[3]}, {M10[1], M10[4], M10[5], M10[6]}, {M10[2], M10[5], M10[7], M10[8]}, {M10[3], M10[6], M10[8], M10[9]}};
-        // ca: [0] n^0, [1..4] E_alphahat, [5..7] beta^i, [8..13] triad (x1,x2,x3,y2,y3,z3), [14] theta 1x, [15] theta 1y; cb: [0] theta 1z, [1] 2y, [2] 2z, [3] 3z, [4..6] u^i'
-        if (frame == 2) {
-            out[li * t.ncell + c] = M10[li];
-        } else if (frame == 1) {  // R^0_alpha = n^0 sum n_alpha I dOmega; n_0 = E_ahat ntil^ahat, n_i = theta^a_i n^a
-            if (li < 4) {
-                const double nup0 = ca[0];
-                double v;
+        mbar_wait(bar0 + 16u * sl, (uint32_t)par);
+        const uint32_t aRow = smem_u32(slots + (sl * kMomCells + r) * Np) + 8u * kk;
+        const uint32_t aB = smem_u32(sB) + 8u * lane, aX = smem_u32(sX) + 16u * kk;
+        double d0 = 0.0, d1 = 0.0, e0 = 0.0, e1 = 0.0, x8 = 0.0, x9 = 0.0, y8 = 0.0, y9 = 0.0;
+        int j = 0;
+#pragma unroll 4
+        for (; j + 1 < nk; j += 2) {
+            const double a0 = lds(aRow + 32u * j), a1 = lds(aRow + 32u * j + 32u);
+            const double b0 = lds(aB + 256u * j), b1 = lds(aB + 256u * j + 256u);
+            const double2 p0 = lds2(aX + 64u * j), p1 = lds2(aX + 64u * j + 64u);
+            dmma884(d0, d1, a0, b0);
+            dmma884(e0, e1, a1, b1);
+            x8 = fma(a0, p0.x, x8); x9 = fma(a0, p0.y, x9);
+            y8 = fma(a1, p1.x, y8); y9 = fma(a1, p1.y, y9);
+        }
+        if (j < nk) {
+            const double a0 = lds(aRow + 32u * j), b0 = lds(aB + 256u * j);
+            const double2 p0 = lds2(aX + 64u * j);
+            dmma884(d0, d1, a0, b0);
+            x8 = fma(a0, p0.x, x8); x9 = fma(a0, p0.y, x9);
+        }
+        d0 += e0; d1 += e1; x8 += y8; x9 += y9;
+        x8 += __shfl_xor_sync(0xffffffffu, x8, 1); x9 += __shfl_xor_sync(0xffffffffu, x9, 1);
+        x8 += __shfl_xor_sync(0xffffffffu, x8, 2); x9 += __shfl_xor_sync(0xffffffffu, x9, 2);
+        __syncwarp();  // the previous group's epilogue has read tot and scell; every lane is done with the slot
+        tot[r * 10 + 2 * kk] = d0; tot[r * 10 + 2 * kk + 1] = d1;
+        if (kk == 0) { tot[r * 10 + 8] = x8; tot[r * 10 + 9] = x9; }
+#pragma unroll
+        for (int m = 0; m < 6; m++) scell[lane + 32 * m] = cv[m];
+        __syncwarp();
+        // ---- epilogue.  Frame 0: lane = (cell, nu) forms W^a = M^{ab} e^nu_b and the outputs R^{mu nu} = e^mu_a W^a for mu <= nu
+        // (R^{mu nu} = e^mu_a e^nu_b M^{ab}; e^0_0 = n^0, e^i_0 = -beta^i n^0, e^i_a = triad, upper triangular, R2)
+        if (frame == 0) {
+            const int cl = lane & 7, nu = lane >> 3;
+            if (cl < cnt) {
+                const double *M10 = tot + cl * 10, *ca = scell + cl * kMomCellF;
+                const double nup0 = ca[0], b1 = -ca[5] * nup0, b2 = -ca[6] * nup0, b3 = -ca[7] * nup0;
+                const double t11 = ca[8], t12 = ca[9], t13 = ca[10], t22 = ca[11], t23 = ca[12], t33 = ca[13];
+                const double E0 = nu == 0 ? nup0 : (nu == 1 ? b1 : (nu == 2 ? b2 : b3));
+                const double E1 = nu == 1 ? t11 : 0.0, E2 = nu == 1 ? t12 : (nu == 2 ? t22 : 0.0), E3 = nu == 1 ? t13 : (nu == 2 ? t23 : (nu == 3 ? t33 : 0.0));
+                const double W0 = M10[0] * E0 + M10[1] * E1 + M10[2] * E2 + M10[3] * E3;
+                const double W1 = M10[1] * E0 + M10[4] * E1 + M10[5] * E2 + M10[6] * E3;
+                const double W2 = M10[2] * E0 + M10[5] * E1 + M10[7] * E2 + M10[8] * E3;
+                const double W3 = M10[3] * E0 + M10[6] * E1 + M10[8] * E2 + M10[9] * E3;
+                const long long c = c0 + cl;
+                out[nu * t.ncell + c] = nup0 * W0;                                                                   // (0, nu)
+                if (nu >= 1) out[(3 + nu) * t.ncell + c] = b1 * W0 + t11 * W1 + t12 * W2 + t13 * W3;                 // (1, nu)
+                if (nu >= 2) out[(5 + nu) * t.ncell + c] = b2 * W0 + t22 * W2 + t23 * W3;                            // (2, nu)
+                if (nu == 3) out[9 * t.ncell + c] = b3 * W0 + t33 * W3;                                              // (3, 3)
+            }
+        } else
+        for (int o = lane; o < ncomp * kMomCells; o += 32) {
+            const int li = o >> 3, cl = o & 7;
+            if (cl >= cnt) continue;
+            const long long c = c0 + cl;
+            const double *M10 = tot + cl * 10, *ca = scell + cl * kMomCellF, *cb = ca + 16;
+            // ca: [0] n^0, [1..4] E_alphahat, [5..7] beta^i, [8..13] triad (x1,x2,x3,y2,y3,z3), [14] theta 1x, [15] theta 1y; cb: [0] theta 1z, [1] 2y, [2] 2z, [3] 3z, [4..6] u^i'
+            double v;
+            if (frame == 2) {
+                v = M10[li];
+            } else if (frame == 1) {  // R^0_alpha = n^0 sum n_alpha I dOmega; n_0 = E_ahat ntil^ahat, n_i = theta^a_i n^a
                 if (li == 0) v = ca[1] * M10[0] + ca[2] * M10[1] + ca[3] * M10[2] + ca[4] * M10[3];
                 else if (li == 1) v = ca[14] * M10[1];
                 else if (li == 2) v = ca[15] * M10[1] + cb[1] * M10[2];
                 else v = cb[0] * M10[1] + cb[2] * M10[2] + cb[3] * M10[3];
-                out[li * t.ncell + c] = nup0 * v;
-            }
-        } else if (frame == 0) {  // R^{mu nu} = e^mu_a e^nu_b M^{ab}; e^0_0 = n^0, e^i_0 = -beta^i n^0, e^i_a = triad (upper triangular, R2)
-            const double nup0 = ca[0];
-            const double E[4][4] = {{nup0, 0.0, 0.0, 0.0}, {-ca[5] * nup0, ca[8], ca[9], ca[10]}, {-ca[6] * nup0, 0.0, ca[11], ca[12]}, {-ca[7] * nup0, 0.0, 0.0, ca[13]}};
-            double EM[4][4];
+                v *= ca[0];
+            } else {
+                const double M[4][4] = {{M10[0], M10[1], M10[2], M10[3]}, {M10[1], M10[4], M10[5], M10[6]}, {M10[2], M10[5], M10[7], M10[8]}, {M10[3], M10[6], M10[8], M10[9]}};
+                {  // fluid frame (Eq.13-14 with G2): nbar^0 = u^0 - u_a n^a, nbar^a = n^a + u^a (u_b n^b / (1 + u^0) - 1)
+                    const double th[6] = {ca[14], ca[15], cb[0], cb[1], cb[2], cb[3]};
+                    double uh[4];
+                    tetrad_velocity(th, cb[4], cb[5], cb[6], uh);
+                    const double rr = 1.0 / (1.0 + uh[0]);
+                    double Lm[4][4];
+                    Lm[0][0] = uh[0]; Lm[0][1] = -uh[1]; Lm[0][2] = -uh[2]; Lm[0][3] = -uh[3];
 #pragma unroll
-            for (int mu = 0; mu < 4; mu++)
+                    for (int a2 = 1; a2 < 4; a2++) {
+                        Lm[a2][0] = -uh[a2];
 #pragma unroll
-                for (int b = 0; b < 4; b++) EM[mu][b] = E[mu][0] * M[0][b] + E[mu][1] * M[1][b] + E[mu][2] * M[2][b] + E[mu][3] * M[3][b];
-            int q = 0;
-            double v = 0.0;
+                        for (int b = 1; b < 4; b++) Lm[a2][b] = (a2 == b ? 1.0 : 0.0) + uh[a2] * uh[b] * rr;
+                    }
+                    double LM[4];  // Lambda^0_a M^{ab}
 #pragma unroll
-            for (int mu = 0; mu < 4; mu++)
+                    for (int b = 0; b < 4; b++) LM[b] = Lm[0][0] * M[0][b] + Lm[0][1] * M[1][b] + Lm[0][2] * M[2][b] + Lm[0][3] * M[3][b];
+                    v = 0.0;
 #pragma unroll
-                for (int nu = mu; nu < 4; nu++) {
-                    const double x = EM[mu][0] * E[nu][0] + EM[mu][1] * E[nu][1] + EM[mu][2] * E[nu][2] + EM[mu][3] * E[nu][3];
-                    if (q == li) v = x;
-                    q++;
+                    for (int q = 0; q < 4; q++) {
+                        const double x = LM[0] * Lm[q][0] + LM[1] * Lm[q][1] + LM[2] * Lm[q][2] + LM[3] * Lm[q][3];
+                        if (q == li) v = x;
+                    }
                 }
-            out[li * t.ncell + c] = v;
-        } else if (li < 4) {  // fluid frame (Eq.13-14 with G2): nbar^0 = u^0 - u_a n^a, nbar^a = n^a + u^a (u_b n^b / (1 + u^0) - 1)
-            const double th[6] = {ca[14], ca[15], cb[0], cb[1], cb[2], cb[3]};
-            double uh[4];
-            tetrad_velocity(th, cb[4], cb[5], cb[6], uh);
-            const double r = 1.0 / (1.0 + uh[0]);
-            double Lm[4][4];
-            Lm[0][0] = uh[0]; Lm[0][1] = -uh[1]; Lm[0][2] = -uh[2]; Lm[0][3] = -uh[3];
-#pragma unroll
-            for (int a2 = 1; a2 < 4; a2++) {
-                Lm[a2][0] = -uh[a2];
-#pragma unroll
-                for (int b = 1; b < 4; b++) Lm[a2][b] = (a2 == b ? 1.0 : 0.0) + uh[a2] * uh[b] * r;
-            }
-            double LM[4];  // Lambda^0_a M^{ab}
-#pragma unroll
-            for (int b = 0; b < 4; b++) LM[b] = Lm[0][0] * M[0][b] + Lm[0][1] * M[1][b] + Lm[0][2] * M[2][b] + Lm[0][3] * M[3][b];
-            double v = 0.0;
-#pragma unroll
-            for (int q = 0; q < 4; q++) {
-                const double x = LM[0] * Lm[q][0] + LM[1] * Lm[q][1] + LM[2] * Lm[q][2] + LM[3] * Lm[q][3];
-                if (q == li) v = x;
             }
             out[li * t.ncell + c] = v;
         }
+        if (++sl == depth) { sl = 0; par ^= 1; }
     }
 }
 
 size_t couple_smem(int N) { return sizeof(double) * (4 * (size_t)N + (size_t)kWarps * ((kDepth + 2) * 2 * N + 2 * kCellF + 12 * 33 + 24 + 2 * kDepth)); }
-size_t moments_smem(int N) { return sizeof(double) * (4 * (size_t)N + (size_t)kWarps * (kMomDepth * 2 * N + 20 * 33 + 20 + 2 * kMomCellF + 2 * kMomDepth)); }
+size_t moments_smem(int N, int warps, int depth) {
+    const int nk = (N + 3) / 4;
+    return sizeof(double) * ((size_t)nk * 40 + (size_t)warps * (depth * kMomCells * mom_row_stride(N) + kMomCells * 10 + kMomCells * kMomCellF + 2 * depth));
+}
 
 }  // namespace
 
@@ -589,11 +647,16 @@ int launch_couple_stream(const DeviceTables &t, const Params &p, double *I, cons
 }
 
 int launch_moments_stream(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out, cudaStream_t s) {
-    const size_t smem = moments_smem(t.N);
-    if ((t.N & 1) || ((uintptr_t)I & 15) || smem > (size_t)t.smem_optin) return 0;
-    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (size_t)t.smem_optin / (smem + 1024)));
-    if (cudaFuncSetAttribute(k_moments_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
-    k_moments_stream<<<t.sms * per_sm, kWarps * 32, smem, s>>>(t, I, frame, fluid, out);
+    if ((t.N & 1) || ((uintptr_t)I & 15)) return 0;
+    // ring depth 3 and as many warps as shared memory holds (<= 8); deeper rings do not pay once ~100 KB are in flight per SM
+    int depth = 2, warps = 12;
+    while (warps > 2 && moments_smem(t.N, warps, depth) > (size_t)t.smem_optin) warps--;
+    if (moments_smem(t.N, warps, depth) > (size_t)t.smem_optin) depth = 2;
+    const size_t smem = moments_smem(t.N, warps, depth);
+    if (smem > (size_t)t.smem_optin) return 0;
+    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(4, (size_t)t.smem_optin / (smem + 1024)));
+    if (cudaFuncSetAttribute(k_moments_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
+    k_moments_mma<<<t.sms * per_sm, warps * 32, smem, s>>>(t, I, frame, fluid, out, depth);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
