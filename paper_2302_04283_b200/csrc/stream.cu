@@ -2,19 +2,18 @@
 // the radiation-dominated velocity estimate of Eq.51-55), the ergosphere mask, the fluid increment, and the
 // angular moments (Eq.45, Eq.38).
 //
-// Both kernels read every intensity once and are bound by HBM, so they are built around the memory system:
-//   * a warp owns a ring of shared-memory slots; one bulk asynchronous copy (TMA, 1-D cp.async.bulk, mbarrier completion) brings
-//     the rows of TWO cells that are neighbours along x (2 N contiguous doubles) into a slot, kDepth - 1 pairs ahead of the one
-//     being worked on, so that the copies of all resident warps keep the memory system busy while the arithmetic runs;
-//   * the 2 N intensities of a pair are one flat run: lane l takes the items f = l, l + 32, ... (for N = 162: 11 passes for 324
-//     items, 92 % of the lanes busy, against 84 % with one cell per warp pass).  Passes that lie in one cell use that cell's
-//     scalars from registers; the one pass that straddles the two cells selects per lane;
-//   * angle sums: every lane accumulates the sums of both cells; the lanes' partial sums are transposed through shared memory
-//     (lane q adds up row q), ~24 stores + 32 loads for all sums of both cells instead of a five-level shuffle butterfly each;
-//   * per-cell scalar work (tetrad-frame fluid velocity, velocity estimate, quartic Eq.49) runs in the two half-warps, one cell each.
-// The coupling makes two sweeps over the slot: sweep 1 forms the sums and leaves g1 I and g2 / n0bar^4 of Eq.40 in shared memory,
-// sweep 2 is one fused multiply-add per intensity and the coalesced store.  The fluid increment needs no second reduction: with
-// I_+ - I* = (g1 - 1) I* + src g2', its moments are P + src Q, and P, Q are sums of sweep 1.
+// Both kernels read every intensity once, so they are built around the memory system and around the issue slots (one warp
+// instruction per clock and scheduler is the bound that bites first on B200 for FP64 work like this):
+//   * a warp owns a ring of shared-memory slots; bulk asynchronous copies (TMA, 1-D cp.async.bulk, mbarrier completion) bring the
+//     rows of a GROUP of cells that are neighbours along x into a slot, one group ahead of the one being worked on;
+//   * coupling: a group is 4 cells, a warp pass is 4 cells x 8 angles (lane = cell * 8 + angle slot), so every lane works for ONE
+//     cell: that cell's scalars stay in its registers, the twelve angle sums are accumulated per lane and reduced over the 8
+//     lanes of the cell by three shuffle steps, and the per-cell scalar work (tetrad-frame velocity, velocity estimate, quartic
+//     Eq.49) is shared by 4 cells per warp pass.  Rows are padded to Np = 8 (mod 16) doubles: conflict-free;
+//   * moments: a group is 8 cells and the sums are a DMMA contraction (below).
+// The coupling makes two sweeps over the slot: sweep 1 forms the sums and leaves g1 I (in place) and g2 / n0bar^4 of Eq.40 in
+// shared memory, sweep 2 is one fused multiply-add per intensity and the store.  The fluid increment needs no second reduction:
+// with I_+ - I* = (g1 - 1) I* + src g2', its moments are P + src Q, and P, Q are sums of sweep 1.
 #include <stdint.h>
 
 #include <algorithm>
@@ -25,73 +24,55 @@
 namespace rad {
 namespace {
 
-constexpr int kWarps = 4;   // warps per CTA
-constexpr int kDepth = 3;   // ring slots per warp
+constexpr int kCG = 4;      // cells per group (coupling)
+constexpr int kCA = 8;      // angle slots per cell in a warp pass
+constexpr int kDepth = 2;   // ring slots per warp
 constexpr int kCellF = 20;  // per-cell scalars fetched for the coupling: fluid (5), opacities (3), n^0, E_alphahat (4), co-triad (6), excised
 
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// pairs of cells along x: position of a pair in the block and the flat index of its first cell; advancing is integer adds only
-struct PairIt {
-    int ip, j, k;  // pair number along x, interior row (j, k)
+__host__ __device__ inline int couple_row_stride(int N) { return ((N + 7) / 8 * 8 + 7) / 16 * 16 + 8; }  // >= 8 ceil(N/8), = 8 (mod 16)
+
+// position of a group of G cells along x in the block, advanced by integer adds only
+struct GroupIt {
+    int ig, j, k;  // group number along x, interior row (j, k)
+    long long c;   // flat index of the group's first cell
 };
-__device__ __forceinline__ PairIt pair_at(long long pid, int ppr, int n1, int kzb) {
-    const long long row = pid / ppr;
-    PairIt it;
-    it.ip = (int)(pid - row * ppr);
-    it.j = (int)(row % n1);
-    it.k = (int)(row / n1) + kzb;
+__device__ __forceinline__ GroupIt group_at(const DeviceTables &t, long long g, int gpr, int G, int kzb) {
+    const long long row = g / gpr;
+    GroupIt it;
+    it.ig = (int)(g - row * gpr); it.j = (int)(row % t.n[1]); it.k = (int)(row / t.n[1]) + kzb;
+    it.c = ((long long)(it.k + t.ng) * t.NJ + (it.j + t.ng)) * t.NI + (G * it.ig + t.ng);
     return it;
 }
-__device__ __forceinline__ void pair_next(PairIt &it, int ppr, int n1) {
-    if (++it.ip == ppr) { it.ip = 0; if (++it.j == n1) { it.j = 0; ++it.k; } }
-}
-__device__ __forceinline__ long long pair_cell(const DeviceTables &t, const PairIt &it, int &cnt) {
-    cnt = min(2, t.n[0] - 2 * it.ip);
-    return ((long long)(it.k + t.ng) * t.NJ + (it.j + t.ng)) * t.NI + (2 * it.ip + t.ng);
-}
-
-// sums over the warp of NS values per lane through shared memory: lane l writes its NS partial sums to red[q * 33 + l], lane q < NS
-// adds up row q (odd row stride: the column reads of the NS lanes fall into different banks) and leaves the total in tot[q].
-// red: NS * 33 doubles, tot: NS doubles, both private to the warp.  ~NS stores + 32 loads + 32 adds instead of a 5-level butterfly.
-template <int NS>
-__device__ __forceinline__ void warp_sums_smem(const double (&v)[NS], int lane, double *red, double *tot) {
-    __syncwarp();
-#pragma unroll
-    for (int q = 0; q < NS; q++) red[q * 33 + lane] = v[q];
-    __syncwarp();
-    if (lane < NS) {
-        const double *r = red + lane * 33;
-        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-#pragma unroll
-        for (int i = 0; i < 32; i += 4) { s0 += r[i]; s1 += r[i + 1]; s2 += r[i + 2]; s3 += r[i + 3]; }
-        tot[lane] = (s0 + s1) + (s2 + s3);
+__device__ __forceinline__ void group_next(const DeviceTables &t, GroupIt &it, int gpr, int G) {
+    it.c += G;
+    if (++it.ig == gpr) {
+        it.ig = 0; it.c += t.NI - (long long)G * gpr;
+        if (++it.j == t.n[1]) { it.j = 0; ++it.k; it.c += (long long)t.NI * (t.NJ - t.n[1]); }
     }
-    __syncwarp();
 }
 
-// per-cell scalars of the coupling, in registers
+// sum over the 8 lanes of a cell (lanes that differ in bits 0..2)
+__device__ __forceinline__ double cell_sum8(double v) {
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    return v;
+}
+
+// per-cell scalars of the coupling, in the registers of the cell's lanes
 struct CellK {
     double uh0, uh1, uh2, uh3;  // tetrad-frame fluid four-velocity used in the coupling (R10; Eq.55 when the estimate applies)
     double aEdt, nup0;          // alpha_E beta dt (Eq.33b), n^0
     double E0, E1, E2, E3;      // E_alphahat: n_0 = E_0 + E_a n^a (mask)
-    double live;                // 1: the cell takes part (not excised)
 };
-__device__ __forceinline__ CellK select(const CellK &a, const CellK &b, bool second) {
-    CellK r;
-    r.uh0 = second ? b.uh0 : a.uh0; r.uh1 = second ? b.uh1 : a.uh1; r.uh2 = second ? b.uh2 : a.uh2; r.uh3 = second ? b.uh3 : a.uh3;
-    r.aEdt = second ? b.aEdt : a.aEdt; r.nup0 = second ? b.nup0 : a.nup0;
-    r.E0 = second ? b.E0 : a.E0; r.E1 = second ? b.E1 : a.E1; r.E2 = second ? b.E2 : a.E2; r.E3 = second ? b.E3 : a.E3;
-    r.live = second ? b.live : a.live;
-    return r;
-}
 
 // sweep 1 for one intensity: fluid-frame factors (R11), the twelve summands, and the two numbers sweep 2 needs.
 // With dd = n^0 + n^0bar alpha_E dt, rp = 1/(n^0bar dd):  dOmega_bar = dOmega / n^0bar^2, Ibar dOmega_bar = n^0bar^2 Ihat dOmega,
 // A_1 = sum (n^0/dd) Ibar dOmega_bar, A_2 = dt/4pi sum dOmega rp (Eq.42), and Eq.40 back in the tetrad frame is
 // Ihat_+ = g1 Ihat_- + src g2',  g1 = n^0 / dd,  g2' = 1 / (dd n^0bar^3).
-__device__ __forceinline__ void sweep1_item(const CellK &c, double n0crit, const double4 an, double I, double (&acc)[12], double &a_out, double &b_out,
-                                            bool &masked) {
+__device__ __forceinline__ void sweep1_item(const CellK &c, const double4 an, double I, double (&acc)[12], double &a_out, double &b_out) {
     const double nbar = c.uh0 - fma(c.uh3, an.w, fma(c.uh2, an.z, c.uh1 * an.y));  // n^0bar = -u_alpha n^alpha
     const double dd = fma(nbar, c.aEdt, c.nup0);
     const double rp = rcp3(nbar * dd);
@@ -107,15 +88,14 @@ __device__ __forceinline__ void sweep1_item(const CellK &c, double n0crit, const
     acc[4] += pI; acc[5] = fma(pI, an.y, acc[5]); acc[6] = fma(pI, an.z, acc[6]); acc[7] = fma(pI, an.w, acc[7]);
     const double qI = an.x * g2;
     acc[8] += qI; acc[9] = fma(qI, an.y, acc[9]); acc[10] = fma(qI, an.z, acc[10]); acc[11] = fma(qI, an.w, acc[11]);
-    masked = n0crit > 0.0 && fabs(chain4(c.E0, c.E1, c.E2, c.E3, an.y, an.z, an.w)) < n0crit;  // |n_0| < n_0^crit (pinned chain)
     a_out = g1 * I;
     b_out = g2;
 }
 
 // ---------------------------------------------------------------------------------------------------------------------------------
 // coupling.  VEST: the radiation-dominated velocity estimate of Eq.51-55 (NEXT-2; reading G8 in DESIGN.md).
-// smem per warp: kDepth slots of 2 N doubles (intensities; sweep 1 leaves the masked intensities there), one buffer a[2 N], one
-// buffer b[2 N], 2 x kCellF cell scalars, 8 doubles of per-cell results; per CTA: the angle table {dOmega, n^1, n^2, n^3}[N].
+// smem per CTA: the angle table {dOmega, n^1, n^2, n^3}[8 ceil(N/8)] (zero past N); per warp: kDepth slots of 4 rows of Np doubles
+// (intensities; sweep 1 leaves g1 I there), one buffer b[4][Np], 4 x kCellF cell scalars, the mbarriers.
 // ---------------------------------------------------------------------------------------------------------------------------------
 struct CoupleArgs {
     double *I;
@@ -127,56 +107,64 @@ struct CoupleArgs {
 };
 
 template <bool VEST>
-__global__ void __launch_bounds__(kWarps * 32, 3) k_couple_stream(const DeviceTables t, const Params p, const CoupleArgs a) {
+__global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, const Params p, const CoupleArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = t.N, L2 = 2 * N;
+    const int N = t.N, npass = (N + kCA - 1) / kCA, Np = couple_row_stride(N);
     double *sm = reinterpret_cast<double *>(smem_raw);
-    double4 *sAng = reinterpret_cast<double4 *>(sm);  // [N]
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int perWarp = (kDepth + 2) * L2 + 2 * kCellF + 12 * 33 + 24 + 2 * kDepth;  // doubles (the last 2 kDepth: mbarriers, 8 B each, 16 B apart)
-    double *wbase = sm + 4 * N + (size_t)w * perWarp;
-    double *slots = wbase, *abuf = wbase + kDepth * L2, *bbuf = abuf + L2, *scell = bbuf + L2, *red = scell + 2 * kCellF, *tot = red + 12 * 33;
-    const uint32_t bar0 = smem_u32(tot + 24);
-    for (int q = threadIdx.x; q < N; q += blockDim.x) sAng[q] = make_double4(t.domega[q], t.nhat[3 * q], t.nhat[3 * q + 1], t.nhat[3 * q + 2]);
+    double2 *sA01 = reinterpret_cast<double2 *>(sm), *sA23 = sA01 + npass * kCA;  // {dOmega, n^1}[npass * 8], {n^2, n^3}[npass * 8]
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int perWarp = (kDepth + 1) * kCG * Np + kCG * kCellF + 2 * kDepth;  // doubles (the last 2 kDepth: mbarriers, 8 B each, 16 B apart)
+    double *wbase = sm + 4 * npass * kCA + (size_t)w * perWarp;
+    double *slots = wbase, *bbuf = wbase + kDepth * kCG * Np, *scell = bbuf + kCG * Np;
+    const uint32_t bar0 = smem_u32(scell + kCG * kCellF);
+    for (int q = threadIdx.x; q < npass * kCA; q += blockDim.x) {
+        sA01[q] = q < N ? make_double2(t.domega[q], t.nhat[3 * q]) : make_double2(0.0, 0.0);
+        sA23[q] = q < N ? make_double2(t.nhat[3 * q + 1], t.nhat[3 * q + 2]) : make_double2(0.0, 0.0);
+    }
+    for (int q = lane; q < (kDepth + 1) * kCG * Np; q += 32) wbase[q] = 0.0;  // the pad of every row (and rows never loaded) stay finite
     if (lane == 0) {
         for (int d = 0; d < kDepth; d++) mbar_init(bar0 + 16u * d, 1);
         fence_mbar_init();
     }
+    fence_proxy_async();
     __syncthreads();
 
-    // pairs of cells along x: pairs per row ppr = ceil(n0 / 2); pair id -> (row, first cell)
-    const int n0 = t.n[0], ppr = (n0 + 1) >> 1;
+    const int gpr = (t.n[0] + kCG - 1) / kCG;  // groups per row
     const int kzb = a.kz1 > a.kz0 ? a.kz0 : 0, kze = a.kz1 > a.kz0 ? a.kz1 : t.n[2];
-    const long long npairs = (long long)ppr * t.n[1] * (kze - kzb);
-    const long long nwarp = (long long)gridDim.x * kWarps, wid = (long long)blockIdx.x * kWarps + w;
-    // a warp takes a contiguous chunk of pairs (consecutive pairs are consecutive in memory)
-    const long long chunk = (npairs + nwarp - 1) / nwarp, pbeg = wid * chunk, pend = min(npairs, pbeg + chunk);
-    if (pbeg >= pend) return;
-    PairIt cur = pair_at(pbeg, ppr, t.n[1], kzb), ahead = cur, nxt = cur;  // the pair worked on, the next pair to be copied, the next pair's scalars
-    long long pahead = pbeg;
-    auto issue = [&]() {  // the rows of pair `ahead` into its ring slot
-        int cnt;
-        const long long c = pair_cell(t, ahead, cnt);
-        const int sl = (int)((pahead - pbeg) % kDepth);
-        const uint32_t bar = bar0 + 16u * sl, bytes = (uint32_t)(cnt * N * 8);
+    const long long ngroups = (long long)gpr * t.n[1] * (kze - kzb);
+    const long long nwarp = (long long)gridDim.x * nwarps, wid = (long long)blockIdx.x * nwarps + w;
+    // a warp takes a contiguous chunk of groups (consecutive groups are consecutive in memory)
+    const long long chunk = (ngroups + nwarp - 1) / nwarp, gbeg = wid * chunk, gend = min(ngroups, gbeg + chunk);
+    if (gbeg >= gend) return;
+    GroupIt cur = group_at(t, gbeg, gpr, kCG, kzb), ahead = cur, nxt = cur;  // the group worked on, the next to be copied, the next group's scalars
+    long long gahead = gbeg;
+    int sl_ahead = 0;
+    auto issue = [&]() {  // the rows of group `ahead` into its ring slot, one bulk copy per cell
+        const int cnt = min(kCG, t.n[0] - kCG * ahead.ig);
+        const uint32_t bar = bar0 + 16u * sl_ahead;
         if (lane == 0) {
             fence_proxy_async();  // sweep 1 wrote into this slot through the generic proxy
-            mbar_expect_tx(bar, bytes);
-            bulk_g2s(smem_u32(slots + sl * L2), a.I + c * N, bytes, bar);
+            mbar_expect_tx(bar, (uint32_t)(cnt * N * 8));
         }
-        pair_next(ahead, ppr, t.n[1]);
-        pahead++;
+        __syncwarp();
+        if (lane < cnt) bulk_g2s(smem_u32(slots + (sl_ahead * kCG + lane) * Np), a.I + (ahead.c + lane) * N, (uint32_t)(N * 8), bar);
+        group_next(t, ahead, gpr, kCG);
+        gahead++;
+        if (++sl_ahead == kDepth) sl_ahead = 0;
     };
-    // the 20 per-cell scalars of a pair, fetched by the lanes one pair ahead: item q = cell * 20 + field -> lane q % 32, round q / 32
-    auto fetch_cell = [&](double (&v)[2]) {  // of pair `nxt`
-        int cnt;
-        const long long c0 = pair_cell(t, nxt, cnt);
-        pair_next(nxt, ppr, t.n[1]);
+    // the 20 per-cell scalars of a group (80 values), fetched by the lanes one group ahead: item q = lane + 32 m = cell * 20 + field
+    int pfcell[3], pffield[3];
 #pragma unroll
-        for (int r = 0; r < 2; r++) {
-            const int q = r * 32 + lane, cl = q / kCellF, f = q - cl * kCellF;
+    for (int m = 0; m < 3; m++) { const int q = lane + 32 * m; pfcell[m] = q / kCellF; pffield[m] = q - pfcell[m] * kCellF; }
+    auto fetch_cell = [&](double (&v)[3]) {  // of group `nxt`
+        const int cnt = min(kCG, t.n[0] - kCG * nxt.ig);
+        const long long c0 = nxt.c;
+        group_next(t, nxt, gpr, kCG);
+#pragma unroll
+        for (int m = 0; m < 3; m++) {
+            const int cl = pfcell[m], f = pffield[m];
             double x = 0.0;
-            if (q < 2 * kCellF && cl < cnt) {
+            if (cl < cnt) {
                 const long long c = c0 + cl;
                 if (f < 5) x = __ldg(a.fluid + (long long)f * t.ncell + c);
                 else if (f == 5) x = p.couple ? __ldg(a.aP + c) : 0.0;
@@ -185,32 +173,30 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_couple_stream(const DeviceTa
                 else if (f < 13) x = __ldg(t.cell + c * RAD_NCELL + (f - 8));  // n^0, E_0..3
                 else if (f < 19) x = __ldg(t.cell + c * RAD_NCELL + 44 + (f - 13));  // co-triad
                 else x = __ldg(t.cell + c * RAD_NCELL + 50);  // excised
-            } else if (f == 19 || f == 8) x = 1.0;  // a missing second cell counts as excised (n^0 = 1 keeps its idle lanes finite)
-            v[r] = x;
+            } else if (f == 19 || f == 8) x = 1.0;  // a missing cell counts as excised (n^0 = 1 keeps its idle lanes finite)
+            v[m] = x;
         }
     };
-    for (int d = 0; d < kDepth - 1 && pahead < pend; d++) issue();
-    double cellv[2];
+    for (int d = 0; d < kDepth - 1 && gahead < gend; d++) issue();
+    double cellv[3];
     fetch_cell(cellv);
-    const int s0 = N >> 5;                 // passes 0 .. s0-1 lie in cell 0
-    const int s1 = (N + 31) >> 5;          // passes s1 .. lie in cell 1 (s0 == s1 when N is a multiple of 32)
-    const int npass = (L2 + 31) >> 5;
-    const uint32_t aS_ = smem_u32(slots), aA = smem_u32(abuf), aB = smem_u32(bbuf);
+    const int mycell = lane >> 3, kk = lane & 7;
+    const uint32_t aA01 = smem_u32(sA01) + 16u * kk, aA23 = smem_u32(sA23) + 16u * kk, aB = smem_u32(bbuf) + 8u * (uint32_t)(mycell * Np + kk);
+    const double n0crit = p.n0_crit;
+    int sl = 0, par = 0;
 
-    for (long long pid = pbeg; pid < pend; pid++) {
-        const int rel = (int)(pid - pbeg), sl = rel % kDepth;
-        int cnt;
-        const long long c0 = pair_cell(t, cur, cnt);
-        pair_next(cur, ppr, t.n[1]);
-        // cell scalars of this pair to shared memory, next pair's on their way
+    for (long long g = gbeg; g < gend; g++) {
+        const int cnt = min(kCG, t.n[0] - kCG * cur.ig);
+        const long long c0 = cur.c;
+        group_next(t, cur, gpr, kCG);
+        // cell scalars of this group to shared memory, next group's on their way
         __syncwarp();
 #pragma unroll
-        for (int r = 0; r < 2; r++) if (r * 32 + lane < 2 * kCellF) scell[r * 32 + lane] = cellv[r];
-        if (pid + 1 < pend) fetch_cell(cellv);
-        if (pahead < pend) issue();  // its slot was released at the end of the previous iteration
+        for (int m = 0; m < 3; m++) if (lane + 32 * m < kCG * kCellF) scell[lane + 32 * m] = cellv[m];
+        if (g + 1 < gend) fetch_cell(cellv);
+        if (gahead < gend) issue();  // its slot was released at the end of the previous iteration
         __syncwarp();
-        // ---- per-cell preparation: lanes 0..15 cell 0, lanes 16..31 cell 1 (all lanes of a half compute the same values)
-        const int mycell = lane >> 4;
+        // ---- per-cell preparation: every lane for its own cell (the 8 lanes of a cell compute the same values)
         const double *sc = scell + mycell * kCellF;
         const double rho = sc[0], Tm = sc[1], aPc = sc[5], aEc = sc[6], aSc = sc[7], nup0 = sc[8];
         const bool excised = sc[19] != 0.0, docouple = p.couple && !excised;
@@ -218,43 +204,33 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_couple_stream(const DeviceTa
         ck.uh0 = 1.0; ck.uh1 = ck.uh2 = ck.uh3 = 0.0;
         ck.aEdt = docouple ? (aEc + aSc) * a.dt : 0.0;  // Eq.33b
         ck.nup0 = nup0; ck.E0 = sc[9]; ck.E1 = sc[10]; ck.E2 = sc[11]; ck.E3 = sc[12];
-        ck.live = excised ? 0.0 : 1.0;
         if (docouple) {
             const double u1 = sc[2], u2 = sc[3], u3 = sc[4];
             ck.uh1 = sc[13] * u1 + sc[14] * u2 + sc[15] * u3; ck.uh2 = sc[16] * u2 + sc[17] * u3; ck.uh3 = sc[18] * u3;  // u^ahat = theta^ahat_j u^j' (R10)
-            ck.uh0 = sqrt(1.0 + (ck.uh1 * ck.uh1 + ck.uh2 * ck.uh2 + ck.uh3 * ck.uh3));
+            ck.uh0 = sqrt_ge1(1.0 + (ck.uh1 * ck.uh1 + ck.uh2 * ck.uh2 + ck.uh3 * ck.uh3));
         }
-        mbar_wait(bar0 + 16u * sl, (uint32_t)((rel / kDepth) & 1));
-        const uint32_t aSl = aS_ + (uint32_t)(sl * L2) * 8u;
+        // |n_0| = |E_0 + E_a n^a| >= |E_0| - |E|: only cells with |E_0| - |E| < n_0^crit can have a masked angle (1e-9: rounding of the bound)
+        const bool mymask = n0crit > 0.0 && !excised && fabs(ck.E0) - sqrt(ck.E1 * ck.E1 + ck.E2 * ck.E2 + ck.E3 * ck.E3) < n0crit * (1.0 + 1e-9);
+        const bool anymask = __any_sync(0xffffffffu, mymask);
+        mbar_wait(bar0 + 16u * sl, (uint32_t)par);
+        const uint32_t aI = smem_u32(slots + (sl * kCG + mycell) * Np) + 8u * kk;  // this lane's item of pass j: + 64 j
 
         if (VEST) {
             // ---- Eq.51-55: tetrad-frame moments of I*, radiation velocity, force, clamped fractions, blended velocity
-            double m[2][10];
-#pragma unroll
-            for (int q = 0; q < 10; q++) { m[0][q] = 0.0; m[1][q] = 0.0; }
-            for (int it = 0; it < npass; it++) {
-                const int f = it * 32 + lane;
-                const bool second = f >= N, valid = f < cnt * N;
-                const double4 an = sAng[valid ? (second ? f - N : f) : 0];
-                const double w0 = valid ? lds(aSl + 8u * f) * an.x : 0.0;
-                const double w1 = w0 * an.y, w2 = w0 * an.z, w3 = w0 * an.w;
-                const double v10[10] = {w0, w1, w2, w3, w1 * an.y, w1 * an.z, w1 * an.w, w2 * an.z, w2 * an.w, w3 * an.w};
-                if (it < s0) {
-#pragma unroll
-                    for (int q = 0; q < 10; q++) m[0][q] += v10[q];
-                } else if (it >= s1) {
-#pragma unroll
-                    for (int q = 0; q < 10; q++) m[1][q] += v10[q];
-                } else {
-#pragma unroll
-                    for (int q = 0; q < 10; q++) { m[0][q] += second ? 0.0 : v10[q]; m[1][q] += second ? v10[q] : 0.0; }
-                }
-            }
-            warp_sums_smem<10>(m[0], lane, red, tot);
-            warp_sums_smem<10>(m[1], lane, red, tot + 10);
             double M[10];
 #pragma unroll
-            for (int q = 0; q < 10; q++) M[q] = tot[mycell * 10 + q];
+            for (int q = 0; q < 10; q++) M[q] = 0.0;
+#pragma unroll 2
+            for (int j = 0; j < npass; j++) {
+                const double2 a01 = lds2(aA01 + 128u * j), a23 = lds2(aA23 + 128u * j);
+                const double w0 = lds(aI + 64u * j) * a01.x;
+                const double w1 = w0 * a01.y, w2 = w0 * a23.x, w3 = w0 * a23.y;
+                M[0] += w0; M[1] += w1; M[2] += w2; M[3] += w3;
+                M[4] = fma(w1, a01.y, M[4]); M[5] = fma(w1, a23.x, M[5]); M[6] = fma(w1, a23.y, M[6]);
+                M[7] = fma(w2, a23.x, M[7]); M[8] = fma(w2, a23.y, M[8]); M[9] = fma(w3, a23.y, M[9]);
+            }
+#pragma unroll
+            for (int q = 0; q < 10; q++) M[q] = cell_sum8(M[q]);
             if (docouple) {
                 // R^{ahat bhat} = M: (00,01,02,03,11,12,13,22,23,33).  Ebar = u_a u_b R^{ab} with u_0 = -u^0 (Eq.38 in covariant form)
                 const double R[4][4] = {{M[0], M[1], M[2], M[3]}, {M[1], M[4], M[5], M[6]}, {M[2], M[5], M[7], M[8]}, {M[3], M[6], M[8], M[9]}};
@@ -290,60 +266,25 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_couple_stream(const DeviceTa
                 }
             }
         }
-        // the two cells' scalars for the sweeps: cell 0's from lane 0, cell 1's from lane 16
-        CellK k0, k1;
-        {
-            const unsigned full = 0xffffffffu;
-#define RAD_BC(field) k0.field = __shfl_sync(full, ck.field, 0); k1.field = __shfl_sync(full, ck.field, 16)
-            RAD_BC(uh0); RAD_BC(uh1); RAD_BC(uh2); RAD_BC(uh3); RAD_BC(aEdt); RAD_BC(nup0); RAD_BC(E0); RAD_BC(E1); RAD_BC(E2); RAD_BC(E3); RAD_BC(live);
-#undef RAD_BC
-        }
-        // ---- sweep 1
-        double acc[2][12];
-#pragma unroll
-        for (int q = 0; q < 12; q++) { acc[0][q] = 0.0; acc[1][q] = 0.0; }
-        const double n0crit = p.n0_crit;
-        auto pass1 = [&](int it, const CellK &c, double (&ac)[12], bool valid, int n) {
-            const int f = it * 32 + lane;
-            double4 an = sAng[n];
-            double I = lds(aSl + 8u * f);
-            if (!valid) { an.x = 0.0; I = 0.0; }  // an idle lane adds zeros
-            double a_o, b_o;
-            bool masked;
-            sweep1_item(c, n0crit, an, I, ac, a_o, b_o, masked);
-            if (valid) {
-                if (masked && c.live != 0.0) { a_o = 0.0; b_o = 0.0; sts(aSl + 8u * f, 0.0); }
-                sts(aA + 8u * f, a_o); sts(aB + 8u * f, b_o);
-            }
-        };
-#pragma unroll 2
-        for (int it = 0; it < s0; it++) pass1(it, k0, acc[0], true, it * 32 + lane);
-        if (s1 > s0) {  // the straddling pass
-            const int f = s0 * 32 + lane;
-            const bool second = f >= N;
-            const CellK ks = select(k0, k1, second);
-            const bool valid = f < cnt * N;
-            double tmpa[12];
-#pragma unroll
-            for (int q = 0; q < 12; q++) tmpa[q] = 0.0;
-            pass1(s0, ks, tmpa, valid, valid ? (second ? f - N : f) : 0);
-#pragma unroll
-            for (int q = 0; q < 12; q++) { acc[0][q] += second ? 0.0 : tmpa[q]; acc[1][q] += second ? tmpa[q] : 0.0; }
-        }
-        if (cnt > 1) {
-#pragma unroll 2
-            for (int it = s1; it < npass; it++) {
-                const int f = it * 32 + lane;
-                const bool valid = f < L2;
-                pass1(it, k1, acc[1], valid, valid ? f - N : 0);
-            }
-        }
-        // ---- reduce: 24 sums -> lane l holds sum l (cell l / 16, sum l % 16)
-        warp_sums_smem<12>(acc[0], lane, red, tot);
-        warp_sums_smem<12>(acc[1], lane, red, tot + 12);
+        // ---- sweep 1: the lane's items of its cell, angle n = 8 j + kk
         double S[12];
 #pragma unroll
-        for (int q = 0; q < 12; q++) S[q] = tot[mycell * 12 + q];
+        for (int q = 0; q < 12; q++) S[q] = 0.0;
+#pragma unroll 3
+        for (int j = 0; j < npass; j++) {
+            const double2 a01 = lds2(aA01 + 128u * j), a23 = lds2(aA23 + 128u * j);
+            const double4 an = make_double4(a01.x, a01.y, a23.x, a23.y);  // zeros past N: such an item adds zeros
+            const double I = lds(aI + 64u * j);
+            double a_o, b_o;
+            sweep1_item(ck, an, I, S, a_o, b_o);
+            if (anymask) {  // warp-uniform: some cell of the group lies where |n_0| can drop below n_0^crit
+                const bool masked = mymask && fabs(chain4(ck.E0, ck.E1, ck.E2, ck.E3, an.y, an.z, an.w)) < n0crit;  // pinned chain
+                a_o = masked ? 0.0 : a_o; b_o = masked ? 0.0 : b_o;
+            }
+            sts(aI + 64u * j, a_o); sts(aB + 64u * j, b_o);
+        }
+#pragma unroll
+        for (int q = 0; q < 12; q++) S[q] = cell_sum8(S[q]);
         // ---- per cell: quartic Eq.49 (R13), T_+, source, fluid increment
         double Tp = Tm, src = 0.0;
         bool coupled = false, noroot = false;
@@ -363,7 +304,7 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_couple_stream(const DeviceTa
                 src = (aPc * p.a_rad * T2 * T2 + aSc * Ep) * (a.dt * kInvFourPi);
             }
         }
-        if ((lane & 15) == 0 && mycell < cnt) {
+        if (kk == 0 && mycell < cnt) {
             const long long c = c0 + mycell;
             if (noroot && a.noroot) atomicAdd(a.noroot, 1ull);
             if (a.T_out) a.T_out[c] = Tp;
@@ -376,24 +317,21 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_couple_stream(const DeviceTa
                 a.dT0[3 * t.ncell + c] = -(nup0 * (sc[15] * M1 + sc[17] * M2 + sc[18] * M3));
             }
         }
-        // (src, coupled) of both cells to every lane
-        const double src0 = __shfl_sync(0xffffffffu, coupled ? src : 0.0, 0), src1 = __shfl_sync(0xffffffffu, coupled ? src : 0.0, 16);
-        const bool cp0 = __shfl_sync(0xffffffffu, (int)coupled, 0) != 0, cp1 = __shfl_sync(0xffffffffu, (int)coupled, 16) != 0;
-        const bool ex0 = k0.live == 0.0, ex1 = k1.live == 0.0;
-        // ---- sweep 2: Eq.40 in the tetrad frame, store
+        // ---- sweep 2: Eq.40 in the tetrad frame, store.  A cell that is not coupled keeps what the transport wrote, except for
+        // its masked intensities (b = 0 marks them: g2' is positive otherwise); excised cells keep their zeros.
         __syncwarp();
-        double *out = a.I + c0 * N;
-        for (int it = 0; it < npass; it++) {
-            const int f = it * 32 + lane;
-            if (f >= cnt * N) break;
-            const bool second = f >= N;
-            if (second ? ex1 : ex0) continue;  // excised cells keep what the transport wrote (0)
-            const double Iold = lds(aSl + 8u * f);
-            double Inew = Iold;
-            if (second ? cp1 : cp0) Inew = fma(second ? src1 : src0, lds(aB + 8u * f), lds(aA + 8u * f));
-            out[f] = Inew;
+        {
+            double *out = a.I + (c0 + mycell) * N + kk;
+            const int myn = (mycell < cnt && !excised) ? (N - kk + kCA - 1) / kCA : 0;  // this lane's items
+            const double srcc = coupled ? src : 0.0;
+#pragma unroll 4
+            for (int j = 0; j < myn; j++) {
+                const double b_ = lds(aB + 64u * j), v = fma(srcc, b_, lds(aI + 64u * j));
+                if (coupled || b_ == 0.0) out[kCA * j] = coupled ? v : 0.0;
+            }
         }
         __syncwarp();  // the slot is free for the copy issued at the top of the next iteration
+        if (++sl == kDepth) { sl = 0; par ^= 1; }
     }
 }
 
@@ -455,23 +393,7 @@ __global__ void __launch_bounds__(384) k_moments_mma(const DeviceTables t, const
     const long long nwarp = (long long)gridDim.x * nwarps, wid = (long long)blockIdx.x * nwarps + w;
     const long long chunk = (ngroups + nwarp - 1) / nwarp, gbeg = wid * chunk, gend = min(ngroups, gbeg + chunk);
     if (gbeg >= gend) return;
-    // position of a group in the block, advanced by integer adds only: (group along x, row j, plane k) and the flat index of its first cell
-    struct GroupIt { int ig, j, k; long long c; };
-    auto group_at = [&](long long g) {
-        const long long row = g / gpr;
-        GroupIt it;
-        it.ig = (int)(g - row * gpr); it.j = (int)(row % t.n[1]); it.k = (int)(row / t.n[1]);
-        it.c = ((long long)(it.k + t.ng) * t.NJ + (it.j + t.ng)) * t.NI + (kMomCells * it.ig + t.ng);
-        return it;
-    };
-    auto group_next = [&](GroupIt &it) {
-        it.c += kMomCells;
-        if (++it.ig == gpr) {
-            it.ig = 0; it.c += t.NI - (long long)kMomCells * gpr;
-            if (++it.j == t.n[1]) { it.j = 0; ++it.k; it.c += (long long)t.NI * (t.NJ - t.n[1]); }
-        }
-    };
-    GroupIt cur = group_at(gbeg), ahead = cur;
+    GroupIt cur = group_at(t, gbeg, gpr, kMomCells, 0), ahead = cur;
     long long gahead = gbeg;
     int sl_ahead = 0;
     auto issue = [&]() {  // the rows of group `ahead` into its ring slot, one bulk copy per cell
@@ -480,7 +402,7 @@ __global__ void __launch_bounds__(384) k_moments_mma(const DeviceTables t, const
         if (lane == 0) mbar_expect_tx(bar, (uint32_t)(cnt * N * 8));
         __syncwarp();
         if (lane < cnt) bulk_g2s(smem_u32(slots + (sl_ahead * kMomCells + lane) * Np), I + (ahead.c + lane) * N, (uint32_t)(N * 8), bar);
-        group_next(ahead);
+        group_next(t, ahead, gpr, kMomCells);
         gahead++;
         if (++sl_ahead == depth) sl_ahead = 0;
     };
@@ -504,7 +426,7 @@ __global__ void __launch_bounds__(384) k_moments_mma(const DeviceTables t, const
     for (long long g = gbeg; g < gend; g++) {
         const int cnt = min(kMomCells, t.n[0] - kMomCells * cur.ig);
         const long long c0 = cur.c;
-        group_next(cur);
+        group_next(t, cur, gpr, kMomCells);
         if (gahead < gend) issue();  // into the slot read in the previous iteration
         double cv[6];
 #pragma unroll
@@ -614,7 +536,10 @@ __global__ void __launch_bounds__(384) k_moments_mma(const DeviceTables t, const
     }
 }
 
-size_t couple_smem(int N) { return sizeof(double) * (4 * (size_t)N + (size_t)kWarps * ((kDepth + 2) * 2 * N + 2 * kCellF + 12 * 33 + 24 + 2 * kDepth)); }
+size_t couple_smem(int N, int warps) {
+    const int npass = (N + kCA - 1) / kCA;
+    return sizeof(double) * (4 * (size_t)npass * kCA + (size_t)warps * ((kDepth + 1) * kCG * couple_row_stride(N) + kCG * kCellF + 2 * kDepth));
+}
 size_t moments_smem(int N, int warps, int depth) {
     const int nk = (N + 3) / 4;
     return sizeof(double) * ((size_t)nk * 40 + (size_t)warps * (depth * kMomCells * mom_row_stride(N) + kMomCells * 10 + kMomCells * kMomCellF + 2 * depth));
@@ -625,23 +550,25 @@ size_t moments_smem(int N, int warps, int depth) {
 // 1 if the streaming kernels serve this angle grid and these arrays: rows must be multiples of 16 bytes (bulk copies).
 // I == nullptr asks about the angle grid alone.
 int stream_serves(const DeviceTables &t, const void *I) {
-    return (t.N & 1) == 0 && ((uintptr_t)I & 15) == 0 && couple_smem(t.N) <= (size_t)t.smem_optin;
+    return (t.N & 1) == 0 && ((uintptr_t)I & 15) == 0 && couple_smem(t.N, 2) <= (size_t)t.smem_optin;
 }
 
 // returns 1 (launched), 0 (not served), -1 (CUDA error)
 int launch_couple_stream(const DeviceTables &t, const Params &p, double *I, const double *fluid, const double *aP, const double *aE, const double *aS,
                          double dt, double *T_out, double *dT0, unsigned long long *noroot, cudaStream_t s, int kz0, int kz1) {
     if (!stream_serves(t, I)) return 0;
-    const size_t smem = couple_smem(t.N);
+    int warps = 12;  // as many as shared memory holds
+    while (warps > 2 && couple_smem(t.N, warps) > (size_t)t.smem_optin) warps--;
+    const size_t smem = couple_smem(t.N, warps);
     CoupleArgs a{I, fluid, aP, aE, aS, dt, T_out, dT0, noroot, kz0, kz1};
-    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (size_t)t.smem_optin / (smem + 1024)));
+    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(4, (size_t)t.smem_optin / (smem + 1024)));
     const int grid = t.sms * per_sm;
     if (p.vel_estimate && p.couple) {
         if (cudaFuncSetAttribute(k_couple_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
-        k_couple_stream<true><<<grid, kWarps * 32, smem, s>>>(t, p, a);
+        k_couple_stream<true><<<grid, warps * 32, smem, s>>>(t, p, a);
     } else {
         if (cudaFuncSetAttribute(k_couple_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
-        k_couple_stream<false><<<grid, kWarps * 32, smem, s>>>(t, p, a);
+        k_couple_stream<false><<<grid, warps * 32, smem, s>>>(t, p, a);
     }
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
