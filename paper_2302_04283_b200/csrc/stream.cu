@@ -152,29 +152,31 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
         gahead++;
         if (++sl_ahead == kDepth) sl_ahead = 0;
     };
-    // the 20 per-cell scalars of a group (80 values), fetched by the lanes one group ahead: item q = lane + 32 m = cell * 20 + field
-    int pfcell[3], pffield[3];
+    // the 20 per-cell scalars of a group (80 values), fetched by the lanes one group ahead: item q = lane + 32 m = cell * 20 + field;
+    // its address is pfbase + (first cell of the group + cell) * pfstride (a field array: stride 1, the cell table: stride RAD_NCELL)
+    const double *pfbase[3];
+    int pfcell[3], pfstride[3];
+    double pfdefault[3];  // value of a missing item: a missing cell counts as excised (n^0 = 1 keeps its idle lanes finite)
 #pragma unroll
-    for (int m = 0; m < 3; m++) { const int q = lane + 32 * m; pfcell[m] = q / kCellF; pffield[m] = q - pfcell[m] * kCellF; }
+    for (int m = 0; m < 3; m++) {
+        const int q = lane + 32 * m, cl = q / kCellF, f = q - cl * kCellF;
+        pfcell[m] = q < kCG * kCellF ? cl : kCG;  // items past the table are never fetched
+        pfstride[m] = f < 8 ? 1 : RAD_NCELL;
+        pfdefault[m] = (f == 19 || f == 8) ? 1.0 : 0.0;
+        if (f < 5) pfbase[m] = a.fluid + (long long)f * t.ncell;
+        else if (f < 8) { pfbase[m] = p.couple ? (f == 5 ? a.aP : (f == 6 ? a.aE : a.aS)) : nullptr; if (!p.couple) pfcell[m] = kCG; pfdefault[m] = 0.0; }
+        else if (f < 13) pfbase[m] = t.cell + (f - 8);        // n^0, E_0..3
+        else if (f < 19) pfbase[m] = t.cell + 44 + (f - 13);  // co-triad
+        else pfbase[m] = t.cell + 50;                         // excised
+    }
     auto fetch_cell = [&](double (&v)[3]) {  // of group `nxt`
         const int cnt = min(kCG, t.n[0] - kCG * nxt.ig);
         const long long c0 = nxt.c;
         group_next(t, nxt, gpr, kCG);
 #pragma unroll
         for (int m = 0; m < 3; m++) {
-            const int cl = pfcell[m], f = pffield[m];
-            double x = 0.0;
-            if (cl < cnt) {
-                const long long c = c0 + cl;
-                if (f < 5) x = __ldg(a.fluid + (long long)f * t.ncell + c);
-                else if (f == 5) x = p.couple ? __ldg(a.aP + c) : 0.0;
-                else if (f == 6) x = p.couple ? __ldg(a.aE + c) : 0.0;
-                else if (f == 7) x = p.couple ? __ldg(a.aS + c) : 0.0;
-                else if (f < 13) x = __ldg(t.cell + c * RAD_NCELL + (f - 8));  // n^0, E_0..3
-                else if (f < 19) x = __ldg(t.cell + c * RAD_NCELL + 44 + (f - 13));  // co-triad
-                else x = __ldg(t.cell + c * RAD_NCELL + 50);  // excised
-            } else if (f == 19 || f == 8) x = 1.0;  // a missing cell counts as excised (n^0 = 1 keeps its idle lanes finite)
-            v[m] = x;
+            v[m] = pfdefault[m];
+            if (pfcell[m] < cnt) v[m] = __ldg(pfbase[m] + (c0 + pfcell[m]) * pfstride[m]);
         }
     };
     for (int d = 0; d < kDepth - 1 && gahead < gend; d++) issue();
@@ -323,11 +325,15 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
         {
             double *out = a.I + (c0 + mycell) * N + kk;
             const int myn = (mycell < cnt && !excised) ? (N - kk + kCA - 1) / kCA : 0;  // this lane's items
-            const double srcc = coupled ? src : 0.0;
+            if (__all_sync(0xffffffffu, coupled || myn == 0)) {  // the usual case: every cell of the group has a root
 #pragma unroll 4
-            for (int j = 0; j < myn; j++) {
-                const double b_ = lds(aB + 64u * j), v = fma(srcc, b_, lds(aI + 64u * j));
-                if (coupled || b_ == 0.0) out[kCA * j] = coupled ? v : 0.0;
+                for (int j = 0; j < myn; j++) out[kCA * j] = fma(src, lds(aB + 64u * j), lds(aI + 64u * j));
+            } else {
+                for (int j = 0; j < myn; j++) {
+                    const double b_ = lds(aB + 64u * j);
+                    if (coupled) out[kCA * j] = fma(src, b_, lds(aI + 64u * j));
+                    else if (b_ == 0.0) out[kCA * j] = 0.0;
+                }
             }
         }
         __syncwarp();  // the slot is free for the copy issued at the top of the next iteration
