@@ -169,8 +169,6 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
             const int e = h.nbr_edge[n * RAD_MAXNBR + s];
             if (e >= 0) nbr_w[n * RAD_MAXNBR + s] = (h.edge_lo[e] == n ? 1.0 : -1.0) / h.domega[n];
         }
-    const double *d_edge_nrm_unused = nullptr;
-    (void)d_edge_nrm_unused;
     ok = upload(c, h.nhat, &t.nhat) && upload(c, h.domega, &t.domega) && upload(c, h.nnbr, &t.nnbr) && upload(c, h.nbr_edge, &t.nbr_edge) &&
          upload(c, h.edge_lo, &t.edge_lo) && upload(c, h.edge_hi, &t.edge_hi) && upload(c, h.edge_len, &t.edge_len) &&
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
@@ -292,12 +290,8 @@ rad_status rad_fill_ghosts(rad_ctx *c, double *I, void *stream) {
 // The two halves of a stage on one stream (no argument checks: the callers did them).
 // transport: ghost fill, then the tile kernel (stage5.cu) where it serves the context, else the generic flux-divergence kernel
 // (transport.cu).  `fluid` != nullptr with tau_factor != 0 selects the optical-depth-aware flux (Eq.26-29).
-// With `T_out`/`dT0`/`count` given through `fuse` (rad_stage), the tile kernel does the coupling half in the same launch where that is
-// the faster route (no velocity estimate); the function then returns kFusedDone instead of RAD_OK.
-constexpr int kFusedDone = 1000;
-static int run_transport(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
-                         double beta_dt, cudaStream_t s, int kz0 = 0, int kz1 = 0, bool fill = true, double *T_out = nullptr, double *dT0 = nullptr,
-                         bool count = false, bool fuse = false) {
+static rad_status run_transport(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
+                                double beta_dt, cudaStream_t s, int kz0 = 0, int kz1 = 0, bool fill = true) {
     if (fill) {
         rad_status st = rad_fill_ghosts(c, I_in, s);
         if (st != RAD_OK) return st;
@@ -316,13 +310,9 @@ static int run_transport(rad_ctx *c, double *I_in, double *I_out, const double *
             c->launches += nt;
             a.vel8 = c->vel8;
         }
-        if (fuse) {
-            a.fluid = fluid; a.aP = c->opac.alpha_a_planck; a.aE = c->opac.alpha_a_energy; a.aS = c->opac.alpha_s;
-            a.T_out = T_out; a.dT0 = dT0; a.noroot = count ? c->d_noroot : nullptr;
-        }
-        const int nl = rad::launch_stage_angle(c->dev, c->kp, a, fuse, s);
+        const int nl = rad::launch_stage_angle(c->dev, c->kp, a, s);
         if (nl < 0) return cuda_fail(c, "rad_stage (tile kernel)");
-        if (nl > 0) { c->launches += nl; return fuse ? kFusedDone : (int)RAD_OK; }
+        if (nl > 0) { c->launches += nl; return RAD_OK; }
     }
     if (kz1 > kz0) return fail(c, RAD_EUNSUPPORTED, "slab-wise transport needs the tile kernel");
     const double *vel = nullptr;
@@ -362,7 +352,7 @@ rad_status rad_transport(rad_ctx *c, double *I_in, double *I_out, const double *
     if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_transport: non-finite weights");
     if (c->kp.tau_factor != 0.0) return fail(c, RAD_ESTATE, "rad_transport: with tau_factor != 0 the spatial flux needs the fluid state (Eq.26-29): use rad_stage");
     DeviceGuard guard(c->device);
-    return (rad_status)run_transport(c, I_in, I_out, I0, nullptr, gam0, gam1, beta_dt, (cudaStream_t)stream);
+    return run_transport(c, I_in, I_out, I0, nullptr, gam0, gam1, beta_dt, (cudaStream_t)stream);
 }
 
 rad_status rad_couple(rad_ctx *c, double *I, const double *fluid, double dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
@@ -387,11 +377,10 @@ rad_status rad_stage(rad_ctx *c, double *I_in, double *I_out, const double *I0, 
     DeviceGuard guard(c->device);
     cudaStream_t s = (cudaStream_t)stream;
     if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage: memset");
-    int st = run_transport(c, I_in, I_out, I0, fluid, gam0, gam1, beta_dt, s, 0, 0, true, T_out, dT0, n_noroot != nullptr, !c->kp.vel_estimate);
-    if (st == kFusedDone) return read_noroot(c, n_noroot, s, "rad_stage: readback");
-    if (st != RAD_OK) return (rad_status)st;
+    rad_status st = run_transport(c, I_in, I_out, I0, fluid, gam0, gam1, beta_dt, s);
+    if (st != RAD_OK) return st;
     st = run_coupling(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot != nullptr, s);
-    if (st != RAD_OK) return (rad_status)st;
+    if (st != RAD_OK) return st;
     return read_noroot(c, n_noroot, s, "rad_stage: readback");
 }
 
@@ -449,10 +438,9 @@ static rad_status stage_host_pipelined(rad_ctx *c, const double *I_in_host, doub
         const int ob = (j == 0) ? 0 : kb + ng, oe = (j == nslab - 1) ? t.NK : ke + ng;
         ok = ok && cudaMemcpyAsync(dO + (size_t)ob * plane * t.N, dI + (size_t)ob * plane * t.N, pbytes * (oe - ob), cudaMemcpyDeviceToDevice, st[1]) == cudaSuccess;
         if (!ok) break;
-        {   // the slab's stage: fused in the tile kernel, or transport + streaming coupling (velocity estimate)
-            const int rt = run_transport(c, dI, dO, nullptr, dfl, gam0, gam1, beta_dt, st[1], kb, ke, false, dT, ddT0, n_noroot != nullptr, !c->kp.vel_estimate);
-            if (rt != kFusedDone && (rt != RAD_OK || run_coupling(c, dO, dfl, beta_dt, dT, ddT0, n_noroot != nullptr, st[1], kb, ke) != RAD_OK)) { launch_failed = true; break; }
-        }
+        // the slab's stage: flux divergence in the tile kernel, then the streaming coupling
+        if (run_transport(c, dI, dO, nullptr, dfl, gam0, gam1, beta_dt, st[1], kb, ke, false) != RAD_OK ||
+            run_coupling(c, dO, dfl, beta_dt, dT, ddT0, n_noroot != nullptr, st[1], kb, ke) != RAD_OK) { launch_failed = true; break; }
         ok = cudaEventRecord(evK[j], st[1]) == cudaSuccess && cudaStreamWaitEvent(st[2], evK[j], 0) == cudaSuccess;
         ok = ok && cudaMemcpyAsync(I_out_host + (size_t)ob * plane * t.N, dO + (size_t)ob * plane * t.N, pbytes * (oe - ob), cudaMemcpyDeviceToHost, st[2]) == cudaSuccess;
         const size_t cb = sizeof(double) * plane * (oe - ob), co = (size_t)ob * plane;

@@ -77,9 +77,6 @@ struct StageArgs {
     const double *I_in, *I0;
     double *I_out;
     double gam0, gam1, beta_dt;
-    const double *fluid, *aP, *aE, *aS;  // coupling only
-    double *T_out, *dT0;
-    unsigned long long *noroot;
     const double *vel8; // optical-depth-aware flux (Eq.26-29): per cell {u^alphahat (4), f/2 of the upper x, y, z faces, pad}, or nullptr (Eq.24)
     int kz0, kz1;  // stage5 only: update the interior planes kz0 <= k < kz1 (0-based, without ghosts); kz1 <= kz0 = the whole block
 };
@@ -110,10 +107,9 @@ int stream_serves(const DeviceTables &t, const void *I);
 int launch_couple_stream(const DeviceTables &t, const Params &p, double *I, const double *fluid, const double *aP, const double *aE, const double *aS,
                          double dt, double *T_out, double *dT0, unsigned long long *noroot, cudaStream_t s, int kz0 = 0, int kz1 = 0);
 int launch_moments_stream(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out, cudaStream_t s);
-// angle-resident fused stage kernel (stage5.cu): flux divergence (+ coupling and mask when couple != 0) in one launch:
-// 1 launched, 0 this configuration is not served (caller falls back to launch_fluxdiv + launch_coupling), -1 CUDA error;
-// and its record builder
-int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s);
+// angle-resident fused flux-divergence kernel (stage5.cu): 1 launched, 0 this configuration is not served (caller falls back to
+// launch_fluxdiv), -1 CUDA error; and its record builder
+int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, cudaStream_t s);
 // 1 if launch_stage_angle serves this context (so that a stage can be run slab by slab along z)
 int stage_angle_serves(const DeviceTables &t);
 // TAU table of the angle-resident kernel: vel8[ncell][8], see k_tau_table (stage5.cu)

@@ -1,6 +1,6 @@
-// stage5.cu -- the fused stage kernel, angle-resident version: spatial + angular flux divergence (Eq.22, 24, 25),
-// cons -> prim, locally implicit coupling (section 2.5), ergosphere mask, fluid increment
-// in ONE launch.
+// stage5.cu -- the fused flux-divergence kernel (north_star subsystem 2), angle-resident version: spatial + angular flux
+// divergence (Eq.22, 24, 25) and cons -> prim in ONE launch; the implicit coupling follows in its own streaming kernel
+// (stream.cu; the two-kernel stage measured faster than the single launch that also held the coupling).
 //
 // Mapping:
 //   * a CTA owns a TY x TZ tile of cell columns in the y-z plane and marches along x through KX cells.  A cell is served
@@ -14,9 +14,6 @@
 //     tile's own rows (ring of 4 planes), the 2-deep halo rows of the current plane (2 buffers), the stored angular-edge
 //     coefficients of each cell (2 buffers; the owner of an edge overwrites the coefficient with the edge flux, the
 //     partner angle pulls it from there), and a packed per-cell geometry record (4 buffers).  One __syncthreads per step.
-//   * the coupling's angle sums are warp butterflies followed by a WPC-way exchange through shared memory under a
-//     named barrier private to the cell; the cell's first warp solves the quartic while its last warp writes the previous
-//     step's outputs and prepares the next cell's fluid velocity.
 //   * TAU (template): the optical-depth-aware spatial flux of Eq.26-29 -- a per-cell table (k_tau_table) of u^alphahat and f/2
 //     of the upper faces comes in with the other copies for the tile's cells and the halo cells at distance 1.
 #include "async_copy.cuh"
@@ -26,8 +23,7 @@ namespace rad {
 namespace {
 
 constexpr int RECN = RAD_STAGE_RECN;  // packed per-cell record, see k_pack_rec
-constexpr int USTR = 64;              // a cell's record slot in shared memory: [0..35] record, [36..43] lower y face,
-                                      // [44..51] lower z face, [52..59] rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s
+constexpr int USTR = 52;              // a cell's record slot in shared memory: [0..35] record, [36..43] lower y face, [44..51] lower z face
 
 template <int TY_, int TZ_, int WPC_, bool TAU_ = false>
 struct Tile {
@@ -39,7 +35,7 @@ struct Tile {
 };
 
 struct Layout5 {
-    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oFx, oU, oRed, oRole, oV, oVh, oBar, total;  // offsets in doubles
+    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oFx, oU, oRole, oV, oVh, oBar, total;  // offsets in doubles
 };
 template <class T>
 __host__ __device__ inline Layout5 make_layout5(int N) {
@@ -53,8 +49,7 @@ __host__ __device__ inline Layout5 make_layout5(int N) {
     L.oFz = L.oFy + 2 * T::NFY * L.Np;
     L.oFx = L.oFz + 2 * T::NFZ * L.Np;  // the lower z face of cell (0,0), computed by cell (1,1) (load balance)
     L.oU = L.oFx + 2 * L.Np;
-    L.oRed = L.oU + 4 * T::NC * USTR;
-    L.oRole = L.oRed + T::NC * (2 * T::WPC * 4 + 8);  // per cell: two sets of WPC partial sums, then (T_+, source, flag)
+    L.oRole = L.oU + 4 * T::NC * USTR;
     L.oV = L.oRole + T::NR * 4;                       // TAU: velocity records (8 doubles) of the own cells, 4 buffers
     L.oVh = L.oV + (T::TAU ? 4 * T::NC * 8 : 0);      // ... and of the halo cells at distance 1, 2 buffers
     L.oBar = L.oVh + (T::TAU ? 2 * T::NVH * 8 : 0);
@@ -143,7 +138,7 @@ __device__ __forceinline__ FaceRec lds_face(uint32_t addr) {  // warp-uniform ad
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-template <int NITER, int WPC, int TY, int TZ, int MINB, bool PLM, bool COUPLE, bool TAU>
+template <int NITER, int WPC, int TY, int TZ, int MINB, bool PLM, bool TAU>
 __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     k_stage5(const DeviceTables t, const Params p, const StageArgs a, const Layout5 L, const int KX) {
     using T = Tile<TY, TZ, WPC, TAU>;
@@ -266,13 +261,12 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     const uint32_t lane8 = (uint32_t)nbase * 8u;                                      // byte offset of angle it: lane8 + it * ITB ...
     const uint32_t last8 = last_valid ? lane8 + (NITER - 1) * ITB : 0u;              // ... except the last
     unsigned rx[NITER], ry[NITER], rz[NITER];
-    double n1[NITER], n2[NITER], n3[NITER], dom[NITER], winv[NITER];
+    double n1[NITER], n2[NITER], n3[NITER], winv[NITER];
 #pragma unroll
     for (int it = 0; it < NITER; it++) {
         const bool v = it < NITER - 1 || last_valid;
         const int n = v ? nbase + it * WPC * 32 : 0;
         n1[it] = t.nhat[3 * n]; n2[it] = t.nhat[3 * n + 1]; n3[it] = t.nhat[3 * n + 2];
-        dom[it] = v ? t.domega[n] : 0.0;
         winv[it] = v ? t.winv[n] : 0.0;
         const uint4 rec = reinterpret_cast<const uint4 *>(t.ang_rec)[n];
         const unsigned z = 3u * (unsigned)N;
@@ -284,13 +278,6 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     double xm1[NITER], x0[NITER], xp1[NITER], carry[NITER];
 #pragma unroll
     for (int it = 0; it < NITER; it++) { xm1[it] = 0.0; x0[it] = 0.0; xp1[it] = 0.0; carry[it] = 0.0; }
-    // lanes 0..7 of a cell's first warp prefetch rho, T, u1', u2', u3', alpha_P, alpha_E, alpha_s of the next cell
-    constexpr int WH = WPC - 1;  // the warp of a cell that does the per-cell chores (fluid prefetch, tetrad velocity, outputs); warp 0 solves the quartic
-    const bool pf_lane = COUPLE && active && wc == WH && (lane < 5 || (lane < 8 && p.couple));
-    auto fluid_ptr = [&](int step) -> const double * {
-        const double *base = lane < 5 ? a.fluid + (long long)lane * t.ncell : (lane == 5 ? a.aP : (lane == 6 ? a.aE : a.aS));
-        return base + c_first + step;
-    };
     if (active) {
         const double *Ic = a.I_in + c_first * N;
         const double *fr = t.rec + (c_first - 1) * RECN;
@@ -309,7 +296,6 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             }
             carry[it] = face_flux<PLM, TAU>(f, n1[it], n2[it], n3[it], xm2, xm1[it], x0[it], xp1[it], GL, GR, fhx);
         }
-        if (COUPLE && wc == WH && lane < 8) sts(smb + 8u * (uint32_t)(L.oU + cs * USTR + 52 + lane), pf_lane ? __ldg(fluid_ptr(0)) : 0.0);
     }
     const int barid = 1 + cs;
     // per-warp byte offsets of the eight stencil neighbours inside a ring plane / a halo buffer (bit q of nbHalo: halo)
@@ -338,56 +324,9 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     // takes over the lower z face of cell (0,0)
     const bool helped = TY >= 2 && TZ >= 2 && j0 + 1 < t.n[1] + ng && k0 + 1 < kze + ng;
     const bool is_helper = helped && cs == TY + 1, is_helpee = helped && cs == 0;
-    const uint32_t aRed = smb + 8u * (uint32_t)(L.oRed + cs * (2 * WPC * 4 + 8));
     const uint32_t N8 = (uint32_t)N * 8u;
     double *outp = a.I_out + c_first * N;
     const double *I0p = a.I0 ? a.I0 + c_first * N : nullptr;
-
-    // tetrad-frame four-velocity of the fluid in the cell of step u (R10), by the cell's last warp: u^ahat = theta^ahat_j u^j',
-    // u^0hat = sqrt(1 + |u|^2); needs the record and the fluid values of that cell in shared memory
-    auto tetrad = [&](int u) {
-        const uint32_t aUu = aU0 + (uint32_t)(u & 3) * (NC * USTR * 8u);
-        double uh0 = 1.0, uh1 = 0.0, uh2 = 0.0, uh3 = 0.0;
-        if (p.couple) {
-            const double2 t0 = lds2(aUu + 8 * 30), t1 = lds2(aUu + 8 * 32), t2 = lds2(aUu + 8 * 34);
-            const double2 f1 = lds2(aUu + 8 * 54);
-            const double u3 = lds(aUu + 8 * 56);
-            uh1 = t0.x * f1.x + t0.y * f1.y + t1.x * u3;
-            uh2 = t1.y * f1.y + t2.x * u3;
-            uh3 = t2.y * u3;
-            uh0 = sqrt_ge1(1.0 + (uh1 * uh1 + uh2 * uh2 + uh3 * uh3));
-        }
-        if (lane == 0) { sts2(aUu + 8 * 60, uh0, uh1); sts2(aUu + 8 * 62, uh2, uh3); }
-    };
-    if (COUPLE && active && wc == WH) {  // step 0: its record arrives with the first group of copies
-        mbar_wait(bar0, 0);
-        __syncwarp();
-        tetrad(0);
-    }
-    // T_+, the count of cells without a root and the fluid increment of step sp, by lane 0 of the cell's last warp, one
-    // cell barrier after the partial sums were written
-    auto emit = [&](int sp) {
-        const uint32_t aUp = aU0 + (uint32_t)(sp & 3) * (NC * USTR * 8u);
-        double M0 = 0.0, M1 = 0.0, M2 = 0.0, M3 = 0.0;
-#pragma unroll
-        for (int q = 0; q < WPC; q++) {
-            const double2 v0 = lds2(aRed + (WPC + q) * 32), v1 = lds2(aRed + (WPC + q) * 32 + 16);
-            M0 += v0.x; M1 += v0.y; M2 += v1.x; M3 += v1.y;
-        }
-        const double Tp = lds(aRed + WPC * 64 + (sp & 1) * 32), flag = lds(aRed + WPC * 64 + (sp & 1) * 32 + 16);
-        const long long c = c_first + sp;
-        if (flag < 0.0 && a.noroot) atomicAdd(a.noroot, 1ull);
-        if (a.T_out) a.T_out[c] = Tp;
-        if (a.dT0) {  // R^0_alpha = sum n^0 n_alpha I dOmega; n^0 n_0 = W_ahat n^ahat, n_i = theta^a_i n^a
-            const double nup0 = lds(aUp + 8 * 24);
-            const double2 w01 = lds2(aUp + 8 * 26), w23 = lds2(aUp + 8 * 28);
-            const double2 t0 = lds2(aUp + 8 * 30), t1 = lds2(aUp + 8 * 32), t2 = lds2(aUp + 8 * 34);
-            a.dT0[c] = -(w01.x * M0 + w01.y * M1 + w23.x * M2 + w23.y * M3);
-            a.dT0[t.ncell + c] = -(nup0 * (t0.x * M1));
-            a.dT0[2 * t.ncell + c] = -(nup0 * (t0.y * M1 + t1.y * M2));
-            a.dT0[3 * t.ncell + c] = -(nup0 * (t1.x * M1 + t2.x * M2 + t2.y * M3));
-        }
-    };
 
 #pragma unroll 1
     for (int s = 0; s < nsteps; s++) {
@@ -399,12 +338,11 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         const uint32_t haloS = aHalo + (uint32_t)b * ((uint32_t)(NH * Np) * 8u);  // halo rows of plane s
         const uint32_t aEb = aE0 + (uint32_t)b * ((uint32_t)(NC * Kp) * 8u);
         const uint32_t aUb = aU0 + (uint32_t)(s & 3) * (NC * USTR * 8u);
-        double d[NITER], xp2[NITER], fnext = 0.0;
+        double d[NITER], xp2[NITER];
 #pragma unroll
         for (int it = 0; it < NITER; it++) asm volatile("" : "+r"(rx[it]), "+r"(ry[it]), "+r"(rz[it]));  // unpack per step: the unpacked offsets would be spilled
 
         if (active) {
-            if (pf_lane && s + 1 < nsteps) fnext = __ldg(fluid_ptr(s + 1));
             const uint32_t ownrow = ringS + ownOff;
             const uint32_t newrow = aRing + (uint32_t)((s + 2) & 3) * planeB + ownOff;
 #pragma unroll
@@ -562,108 +500,19 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         }
         // ---- flux-divergence update of C = n^0 n_0 I (Eq.22, stage form R8), cons -> prim
         const double2 c01 = lds2(aUb + 8 * 24);
-        const double nup0 = c01.x;
         const bool excised = c01.y != 0.0;
         const double2 w01 = lds2(aUb + 8 * 26), w23 = lds2(aUb + 8 * 28);  // n^0 E_alphahat
-        const double mbdt = -a.beta_dt, thr = p.n0_crit * nup0;  // |n_0| < n0_crit  <=>  |n^0 n_0| < n0_crit n^0
+        const double mbdt = -a.beta_dt;
         double Is[NITER];
-        unsigned maskbits = 0;
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
             const double wgt = chain4(w01.x, w01.y, w23.x, w23.y, n1[it], n2[it], n3[it]);  // n^0 n_0 at the cell centre
-            if (fabs(wgt) < thr) maskbits |= 1u << it;
             double v = a.gam1 * x0[it];
             if (I0p != nullptr) v = fma(a.gam0, __ldg(I0p + (OFF8(it) >> 3)), v);
             v = fma(mbdt * d[it], rcp3(wgt), v);
             Is[it] = (excised || !(it < NITER - 1 || last_valid)) ? 0.0 : v;
         }
 
-        if (COUPLE) {
-            // ---- locally implicit coupling (section 2.5, Eq.31-50), fluid increment, mask
-            const bool enable = !excised, docouple = p.couple && enable;
-            const double2 u01 = lds2(aUb + 8 * 60), u23 = lds2(aUb + 8 * 62);
-            const double uh0 = docouple ? u01.x : 1.0, uh1 = docouple ? u01.y : 0.0, uh2 = docouple ? u23.x : 0.0, uh3 = docouple ? u23.y : 0.0;
-            const double2 f3 = lds2(aUb + 8 * 58);              // alpha_E (absorption part), alpha_s
-            const double aEdt = (f3.x + f3.y) * a.beta_dt;      // Eq.33b
-            // sweep 1.  With dd = n^0 + n^0bar alpha_E dt, rp = 1/(n^0bar dd):  dOmega_bar = dOmega / n^0bar^2 (R11),
-            // Ibar dOmega_bar = n^0bar^2 Ihat dOmega,  A_1 = sum (n^0/dd) Ibar dOmega_bar, A_2 = dt/4pi sum dOmega rp (Eq.42),
-            // and Eq.40 back in the tetrad frame is  Ihat_+ = g1 Ihat_- + src / (dd n^0bar^3),  g1 = n^0 / dd.
-            double g1[NITER], g2r4[NITER];
-            double Wsum = 0.0, A1 = 0.0, A2 = 0.0, Em = 0.0;
-#pragma unroll
-            for (int it = 0; it < NITER; it++) {
-                const double nbar = uh0 - fma(uh3, n3[it], fma(uh2, n2[it], uh1 * n1[it]));  // n^0bar = -u_alpha n^alpha
-                const double dd = fma(nbar, aEdt, nup0);
-                const double rp = rcp3(nbar * dd);
-                const double rd = nbar * rp, rn = dd * rp, rn2 = rn * rn;
-                const double x = (nbar * nbar) * (Is[it] * dom[it]);                        // Ibar dOmega_bar (Eq.38 summand)
-                g1[it] = nup0 * rd;
-                g2r4[it] = rn2 * rp;
-                Em += x;
-                A1 = fma(g1[it], x, A1);                                                    // Eq.42a
-                A2 = fma(dom[it], rp, A2);                                                  // Eq.42b
-                Wsum = fma(dom[it], rn2, Wsum);
-            }
-            // the cell's first warp sums the partial sums, solves the quartic and hands (T_+, source, coupled) to the others
-            warp_sum4_to(Wsum, A1, A2, Em, lane, aRed + (uint32_t)wc * 32u);
-            if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
-            if (wc == 0) {
-                Wsum = A1 = A2 = Em = 0.0;
-#pragma unroll
-                for (int q = 0; q < WPC; q++) {
-                    const double2 v0 = lds2(aRed + q * 32), v1 = lds2(aRed + q * 32 + 16);
-                    Wsum += v0.x; A1 += v0.y; A2 += v1.x; Em += v1.y;
-                }
-                const double2 f0 = lds2(aUb + 8 * 52);          // rho, T_-
-                const double aP = lds(aUb + 8 * 57), aS = f3.y;
-                const double Tm = f0.y;
-                double Tp = Tm, src = 0.0, flag = 0.0;            // flag: 1 coupled, -1 no root
-                if (docouple) {
-                    const double scale = p.renorm ? kFourPi * rcp3(Wsum) : 1.0;             // R12
-                    A1 *= scale; Em *= scale; A2 *= scale * (a.beta_dt * kInvFourPi);
-                    const double Cv = f0.x * p.rgm1;
-                    const double B4 = A2 * aP * p.a_rad, om = 1.0 - A2 * aS;               // Eq.50
-                    const double B1 = Cv * om, Bp = A1 - om * Em;
-                    double dTemp = 0.0;
-                    if (!quartic_delta(B4, B1, Bp, Tm, dTemp)) {
-                        flag = -1.0;
-                    } else {
-                        flag = 1.0;
-                        Tp = Tm + dTemp;
-                        const double Ep = Em - Cv * dTemp;                                  // Eq.48
-                        const double T2 = Tp * Tp;
-                        src = (aP * p.a_rad * T2 * T2 + aS * Ep) * (a.beta_dt * kInvFourPi);
-                    }
-                }
-                if (lane == 0) { sts2(aRed + WPC * 64 + b * 32, Tp, src); sts(aRed + WPC * 64 + b * 32 + 16, flag); }
-            }
-            if (wc == WH) {  // meanwhile the cell's last warp writes the outputs of the previous step and prepares the next one
-                if (lane == 0 && s > 0) emit(s - 1);
-                if (s + 1 < nsteps) {
-                    if (lane < 8) sts(aU0 + (uint32_t)((s + 1) & 3) * (NC * USTR * 8u) + 8u * (52 + lane), fnext);
-                    mbar_wait(bar0 + 8u * (b ^ 1), ((s + 1) >> 1) & 1);  // the record of the next cell (copied two steps ahead)
-                    __syncwarp();
-                    tetrad(s + 1);
-                }
-            }
-            if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
-            const double2 bc = lds2(aRed + WPC * 64 + b * 32);
-            const double flag = lds(aRed + WPC * 64 + b * 32 + 16);
-            const double src = bc.y;
-            const bool coupled = flag > 0.0;
-            // sweep 2: Eq.40, fluid increment through the tetrad-frame first moments of the change, mask
-            double M0 = 0.0, M1 = 0.0, M2 = 0.0, M3 = 0.0;
-#pragma unroll
-            for (int it = 0; it < NITER; it++) {
-                const double Iold = Is[it];
-                double Inew = coupled ? fma(src, g2r4[it], g1[it] * Iold) : Iold;
-                const double wI = dom[it] * (Inew - Iold);
-                M0 += wI; M1 = fma(wI, n1[it], M1); M2 = fma(wI, n2[it], M2); M3 = fma(wI, n3[it], M3);
-                if (thr > 0.0 && enable && ((maskbits >> it) & 1u)) Inew = 0.0;
-                Is[it] = Inew;
-            }
-            warp_sum4_to(M0, M1, M2, M3, lane, aRed + (uint32_t)(WPC + wc) * 32u);
-        }
 #pragma unroll
         for (int it = 0; it < NITER; it++) {
             if (it < NITER - 1 || last_valid) outp[OFF8(it) >> 3] = Is[it];
@@ -671,10 +520,6 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         }
         outp += N;
         if (I0p != nullptr) I0p += N;
-    }
-    if (COUPLE && active) {
-        if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
-        if (wc == WH && lane == 0) emit(nsteps - 1);
     }
 #undef OFF8
 }
@@ -726,7 +571,7 @@ __global__ void __launch_bounds__(256) k_stage_face_signs(const DeviceTables t, 
 }
 
 template <int NITER, int WPC, int TY, int TZ, int MINB, bool TAU>
-int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
+int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, cudaStream_t s) {
     using T = Tile<TY, TZ, WPC, TAU>;
     const Layout5 L = make_layout5<T>(t.N);
     const size_t smem = sizeof(double) * (size_t)L.total;
@@ -745,21 +590,20 @@ int launch5t(const DeviceTables &t, const Params &p, const StageArgs &a, bool co
     }
     dim3 grid((t.n[0] + KX - 1) / KX, (t.n[1] + TY - 1) / TY, (nz + TZ - 1) / TZ);
     if (grid.y > 65535 || grid.z > 65535) return 0;
-#define RAD_LAUNCH5(PLM, CPL)                                                                                          \
+#define RAD_LAUNCH5(PLM)                                                                                               \
     do {                                                                                                               \
-        if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
-        k_stage5<NITER, WPC, TY, TZ, MINB, PLM, CPL, TAU><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                                  \
+        if (cudaFuncSetAttribute(k_stage5<NITER, WPC, TY, TZ, MINB, PLM, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
+        k_stage5<NITER, WPC, TY, TZ, MINB, PLM, TAU><<<grid, T::NT, smem, s>>>(t, p, a, L, KX);                         \
     } while (0)
-    if (p.recon_space == 1) { if (couple) RAD_LAUNCH5(true, true); else RAD_LAUNCH5(true, false); }
-    else { if (couple) RAD_LAUNCH5(false, true); else RAD_LAUNCH5(false, false); }
+    if (p.recon_space == 1) RAD_LAUNCH5(true); else RAD_LAUNCH5(false);
 #undef RAD_LAUNCH5
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
 template <int NITER, int WPC, int TY, int TZ, int MINB = 1>
-int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
-    if (a.vel8 != nullptr) return launch5t<NITER, WPC, TY, TZ, MINB, true>(t, p, a, couple, s);
-    return launch5t<NITER, WPC, TY, TZ, MINB, false>(t, p, a, couple, s);
+int launch5(const DeviceTables &t, const Params &p, const StageArgs &a, cudaStream_t s) {
+    if (a.vel8 != nullptr) return launch5t<NITER, WPC, TY, TZ, MINB, true>(t, p, a, s);
+    return launch5t<NITER, WPC, TY, TZ, MINB, false>(t, p, a, s);
 }
 
 // TAU: per-cell record of the optical-depth-aware flux for EVERY cell (ghosts included), 8 doubles: tetrad-frame fluid velocity
@@ -808,10 +652,10 @@ __global__ void __launch_bounds__(256) k_tau_table(const DeviceTables t, const d
     } while (0)
 
 // returns 1 (launched), 0 (this configuration is not served by this kernel), -1 (CUDA error)
-int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, bool couple, cudaStream_t s) {
+int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, cudaStream_t s) {
     if (!stage_angle_serves(t)) return 0;
     if (((uintptr_t)a.I_in & 15) || ((uintptr_t)a.vel8 & 15)) return 0;  // rows are brought in by 16-byte bulk copies
-#define RAD_S5_CALL(NITER, WPC, TY, TZ) return launch5<NITER, WPC, TY, TZ>(t, p, a, couple, s)
+#define RAD_S5_CALL(NITER, WPC, TY, TZ) return launch5<NITER, WPC, TY, TZ>(t, p, a, s)
     RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
 #undef RAD_S5_CALL
     return 0;

@@ -6,7 +6,7 @@ import pytest
 import torch
 
 from paper_2302_04283_b200 import workloads as W
-from parity_util import DT0_FLOOR, TOL_FLUID, TOL_I, err_dT0, make_oracle, make_rad, oracle_tables_to_rad, rel_err, rel_err_I
+from parity_util import TOL_FLUID, TOL_I, err_dT0, make_oracle, make_rad, oracle_tables_to_rad, rel_err, rel_err_I
 
 pytestmark = pytest.mark.gpu
 
