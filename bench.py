@@ -1,17 +1,22 @@
-"""bench.py -- one radiation stage (ghost fill + fused flux divergence + implicit coupling + mask) per "step".
+"""bench.py -- one radiation stage (ghost fill + fused flux-divergence kernel + streaming implicit-coupling kernel) per "step".
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--n CELLS] [--impl reference]
+    python bench.py --ncu-raw FILE.csv --ncu-cmd "..."     # fold an `ncu --page raw --csv` export into profiles/r2_kernels.csv
 
 Metric (BASELINE.json): intensity-cell updates per second per radiation stage, FP64; one update = one
 (cell, angle) pair advanced one stage.  Default workload: config C3, the 128^3 x 162-angle Kerr-Schild block the
 north_star target is quoted on.  Inputs are seeded synthetic (paper_2302_04283_b200.workloads), resident in HBM
 before the timed region; the intensity arrays (2 x 2.98 GB) exceed L2 (126 MB), so no flush is needed.
 
-One JSON line on stdout (rank 0).  `value` is device-timed (CUDA events on the launching stream, max over ranks);
-`e2e` is the same stage through rad_stage_host with pinned HOST buffers, copies inside the timed region;
-`roofline` is for the fused stage kernel k_stage5 (the only kernel of a step), from the CUDA-event time of the timed region; `cpu_baseline` is the oracle
-timed on the host cores on a bounded sub-block of the same workload.  With --gpus N > 1 (torchrun) every rank
-runs an independent replica of the block ("replicas only": the path has no collective), scaling = weak.
+One JSON line on stdout (rank 0).  `value` is device-timed (CUDA events on the launching stream, max over ranks) over K calls
+of rad_stage; `e2e` is the same stage through rad_stage_host with pinned HOST buffers, copies inside the timed region;
+`roofline` is for the dominant kernel, the fused flux-divergence kernel k_stage5 (north_star's target row), whose average
+launch duration is measured live with CUDA events over K launches through rad_transport on the same inputs;
+`roofline_coupling` likewise for the coupling kernel (rad_couple); `cpu_baseline` is the oracle timed on the host cores on a
+bounded sub-block of the same workload.  Figures that come from ncu (DRAM traffic, FP64 instruction counts) are read from the
+committed profiles/r2_kernels.csv, keyed by the kernel instance names the library reports (rad_stage_kernels); a kernel that is
+not in the file gets null.  With --gpus N > 1 (torchrun) every rank runs an independent replica of the block ("replicas
+only": the path has no collective), scaling = weak.
 """
 import argparse
 import json
@@ -35,21 +40,84 @@ def algorithmic_bytes_per_update(N):
     return 16.0 + 640.0 / N
 
 
+def fluxdiv_bytes_per_update(N):
+    """flux-divergence kernel = read I (8) + write I* (8) + 536 B of compact geometry per cell (43 cell + 24 face doubles)"""
+    return 16.0 + 536.0 / N
+
+
+def coupling_bytes_per_update(N):
+    """coupling kernel = read I* (8) + write I_+ (8) + 104 B per cell (5 fluid, 3 opacity in; 5 out)"""
+    return 16.0 + 104.0 / N
+
+
 def design_bytes_per_update(N):
-    """what the kernel as built must move: read I (8) + write I_+ (8) + the stored angular-edge coefficients (3 doubles per
-    update) + per cell 288 B packed record, ~48 B lower-face records of the tile edge,
-    64 B fluid and opacities, 40 B T_+ and fluid increment"""
-    return 16.0 + 24.0 + 440.0 / N
+    """what the flux-divergence kernel as built must move: read I (8) + write I* (8) + the stored angular-edge coefficients
+    (3 doubles per update) + per cell 288 B packed record and ~48 B lower-face records of the tile edge"""
+    return 16.0 + 24.0 + 336.0 / N
 
 
-# DRAM bytes per launch of the stage kernel from the committed ncu --set full capture (dram__bytes_read.sum +
-# dram__bytes_write.sum; profiles/r1_k_stage5_ncu_full.md), for the workload it was taken on: (config, cells per axis, recon)
-NCU_TRAFFIC_BYTES = {("C3", None, 1): 15.86e9}
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_kernels.csv")
+PROFILE_FIELDS = ["kernel", "workload", "ms", "dram_read_bytes", "dram_write_bytes", "inst_warp", "fp64_inst_warp", "fp64_pipe_pct", "issue_pct",
+                  "smem_wavefronts", "smem_bank_conflicts", "registers", "grid", "block"]
 
-# FP64-pipe instruction slots per update of the stage kernel (DESIGN.md 'rooflines'): FP64 warp instructions x 32 lanes /
-# updates, from the ncu instruction counts under profiles/ (idle lanes of the last angle group included); one slot = one
-# DFMA-equivalent issue = 2 flop of the measured DFMA peak
-FP64_SLOTS_PER_UPDATE = {True: 177.0, False: 118.0}  # with / without coupling
+
+def norm_kernel(name):
+    """'void rad::<unnamed>::k_stage5<(int)3, (int)2, ..., (bool)0>(rad::DeviceTables, ...)' -> 'k_stage5<3,2,...,0>'"""
+    import re
+    m = re.search(r"(k_[A-Za-z0-9_]+)(<[^>]*>)?", name)
+    if not m:
+        return name
+    return m.group(1) + re.sub(r"\((int|bool)\)|\s", "", m.group(2) or "")
+
+
+def profile_row(kernel, workload):
+    """the committed ncu figures of a kernel instance on a workload, or None (no figure is printed for a kernel that is not there)"""
+    import csv
+    try:
+        with open(PROFILE_CSV) as f:
+            for r in csv.DictReader(f):
+                if r["kernel"] == kernel and r["workload"] == workload:
+                    return r
+    except OSError:
+        pass
+    return None
+
+
+def ingest_ncu(raw_csv, cmd, workload):
+    """fold `ncu -i X.ncu-rep --page raw --csv` into profiles/r2_kernels.csv (one row per kernel instance and workload)"""
+    import csv
+    rows = list(csv.reader(open(raw_csv)))
+    h = rows[0]
+    want = {"ms": ("gpu__time_duration.sum", 1e-6), "dram_read_bytes": ("dram__bytes_read.sum", 1.0), "dram_write_bytes": ("dram__bytes_write.sum", 1.0),
+            "inst_warp": ("smsp__inst_executed.sum", 1.0), "fp64_inst_warp": ("smsp__inst_executed_pipe_fp64.sum", 1.0),
+            "fp64_pipe_pct": ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", 1.0), "issue_pct": ("smsp__issue_active.avg.pct_of_peak_sustained_active", 1.0),
+            "smem_wavefronts": ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", 1.0), "smem_bank_conflicts": ("l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum", 1.0),
+            "registers": ("launch__registers_per_thread", 1.0), "grid": ("launch__grid_size", 1.0), "block": ("launch__block_size", 1.0)}
+    unit_scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "ms": 1e6, "us": 1e3, "ns": 1.0, "s": 1e9}
+    old = []
+    try:
+        with open(PROFILE_CSV) as f:
+            old = list(csv.DictReader(f))
+    except OSError:
+        pass
+    for v in rows[2:]:
+        d = dict(zip(h, v))
+        r = {"kernel": norm_kernel(d["Kernel Name"]), "workload": workload}
+        for k, (m, sc) in want.items():
+            if m not in d or d[m] == "":
+                r[k] = ""
+                continue
+            x = float(d[m].replace(",", "")) * unit_scale.get(rows[1][h.index(m)], 1.0) * (sc if k == "ms" else 1.0)
+            r[k] = repr(x)
+        old = [o for o in old if not (o["kernel"] == r["kernel"] and o["workload"] == r["workload"])] + [r]
+    with open(PROFILE_CSV, "w", newline="") as f:
+        w = csv.DictWriter(f, fieldnames=PROFILE_FIELDS)
+        w.writeheader()
+        for o in old:
+            w.writerow({k: o.get(k, "") for k in PROFILE_FIELDS})
+    with open(PROFILE_CSV[:-4] + ".md", "a") as f:
+        f.write(f"* rows for workload `{workload}` from `{os.path.basename(raw_csv)}`: `{cmd}`\n")
+    print(f"{PROFILE_CSV}: {len(old)} rows")
 
 
 class ClockSampler:
@@ -69,10 +137,16 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
+    def wait_first(self, timeout=5.0):
+        """nvidia-smi takes a moment to start: the timed region begins only once samples arrive"""
+        t0 = time.time()
+        while self.proc and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.01)
+
     def summary(self, t0, t1):
         if self.proc:
             self.proc.terminate()
-        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.05] or [r for _, r in self.rows[-3:]]
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.02]
         sm, mx, reasons = [], 0, set()
         for r in rows:
             f = [x.strip() for x in r.split(",")]
@@ -161,20 +235,35 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def omp_threads(n):
+    """threads the oracle's OpenMP regions use from now on (libgomp's global setting; the oracle itself is not touched)"""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C3")
     ap.add_argument("--n", type=int, default=None, help="override cells per axis (same box)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-n", type=int, default=None, help="sub-block size of the oracle sample (default: 64 for --impl reference, 96 for the cpu_baseline leg)")
     ap.add_argument("--recon", type=int, default=1, help="spatial reconstruction: 1 PLM (the workload's), 0 donor cell (diagnostic)")
-    ap.add_argument("--tau-factor", type=float, default=0.0, help="constant of Eq.26: > 0 times the stage with the optical-depth-aware flux (NEXT-1; separate kernels)")
+    ap.add_argument("--tau-factor", type=float, default=0.0, help="constant of Eq.26: > 0 times the stage with the optical-depth-aware flux (NEXT-1)")
+    ap.add_argument("--vel-estimate", type=int, default=0, help="1: radiation-dominated velocity estimate Eq.51-55 in the coupling (NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ncu-raw", default=None, help="fold this `ncu --page raw --csv` export into profiles/r2_kernels.csv and exit")
+    ap.add_argument("--ncu-cmd", default="", help="the ncu command that produced --ncu-raw (recorded beside the csv)")
     args = ap.parse_args()
+    if args.ncu_raw:
+        return ingest_ncu(args.ncu_raw, args.ncu_cmd, args.config if args.n is None else f"{args.config}/n={args.n}")
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
@@ -200,12 +289,14 @@ def main():
     if world > 1:
         dist.barrier()
     B.lib()
+    sampler = ClockSampler(local) if rank == 0 else None  # started early: nvidia-smi needs a moment before its first sample
 
     cfg = args.config
     c = W.CONFIGS[cfg]
     nn, ng, x0, dx = W.grid(cfg, args.n)
     N = W.n_angles(cfg)
     updates = nn[0] * nn[1] * nn[2] * N
+    workload = cfg if args.n is None else f"{cfg}/n={args.n}"
 
     # angle directions from the library itself (a context without geometry cost: 1 cell)
     h0 = B.rad_create(dict(kind=0), dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1)), c["angles"], None, dict(couple=0), local)
@@ -219,10 +310,12 @@ def main():
     T_out = torch.zeros(ncell, dtype=torch.float64, device="cuda"); dT0 = torch.zeros(4, ncell, dtype=torch.float64, device="cuda")
     h = B.rad_create(dict(kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg)),
                      dict(n=nn, x0=x0, dx=dx, bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3), c["angles"], (opac[0], opac[1], opac[2]),
-                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=args.recon, renorm_fluid_weights=1, couple=1, tau_factor=args.tau_factor), local)
+                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=args.recon, renorm_fluid_weights=1, couple=1,
+                          tau_factor=args.tau_factor, vel_estimate=args.vel_estimate), local)
     vmax = float(B.rad_get_table(h, B.TAB_MAXSPEED).max())
     dt = W.CFL * min(dx) / vmax
     stream = torch.cuda.current_stream()
+    k_flux, k_cpl = B.rad_stage_kernels(h)
 
     def stage():
         # every step advances the same seeded state I_a -> I_b (fixed work per step; I_b is fully rewritten)
@@ -237,7 +330,8 @@ def main():
     for _ in range(args.warmup):
         stage()
     sync_all()
-    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.wait_first()
     l0 = B.rad_launch_count(h)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.time()
@@ -250,9 +344,8 @@ def main():
     launches = B.rad_launch_count(h) - l0
     ms = ev0.elapsed_time(ev1) / args.steps
     ms = max_over_ranks(ms, world, "cuda")
-    clocks = sampler.summary(t0, t1) if sampler else None
 
-    # the stage kernel without its coupling half, and the stand-alone coupling kernel, for the record
+    # the step's kernels one by one, live: K launches each on the same inputs, CUDA events on the launching stream
     def time_call(fn, reps):
         for _ in range(2):
             fn()
@@ -267,34 +360,58 @@ def main():
 
     reps = max(3, args.steps)
     ms_flux = None
-    if args.tau_factor == 0.0:  # (with the optical-depth-aware flux the transport half alone has no fluid state)
+    if args.tau_factor == 0.0:  # (with the optical-depth-aware flux the transport half needs the fluid state: timed through the stage only)
         ms_flux = time_call(lambda: B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream), reps)
         B.rad_transport(h, I_a, I_b, None, 0.0, 1.0, dt, stream=stream)
     ms_cpl = time_call(lambda: B.rad_couple(h, I_b, fluid, dt, T_out, dT0, stream=stream), reps)
-    # roofline of the dominant kernel = the fused stage kernel k_stage (flux divergence + coupling in one launch): with
-    # caller-filled ghosts it is the only kernel of a step, so its average launch duration is the CUDA-event time of the
-    # timed region / launches
+    mom = torch.zeros(10, ncell, dtype=torch.float64, device="cuda")
+    ms_mom = time_call(lambda: B.rad_moments(h, I_a, 0, fluid, mom, stream=stream), reps)
+    clocks = sampler.summary(t0, time.time()) if sampler else None  # the timed region and the per-kernel loops that follow it
+    del mom
+
     kernels_per_step = max(1, launches // max(1, args.steps))
     peak, peak_src = measured_peak()
-    bpu = algorithmic_bytes_per_update(N)
-    achieved = bpu * updates / (ms * 1e-3) / 1e9
-    kname = "k_stage5 (fused flux divergence + implicit coupling + mask, one launch per step)" if args.tau_factor == 0.0 else \
-        "k_tau_table + k_stage5<TAU> (tile kernel with the Eq.28 factor): the step's two kernels together"
-    roofline = {"kernel": kname, "bound": "hbm",
-                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg, args.n, args.recon)),
-                "traffic_source": "ncu --set full capture, profiles/r1_k_stage5_ncu_full.md (bytes per launch)" if (cfg, args.n, args.recon) in NCU_TRAFFIC_BYTES else None,
-                "peak_source": peak_src,
-                "algorithmic_bytes_per_update": bpu, "design_bytes_per_update": design_bytes_per_update(N),
-                "design_frac": design_bytes_per_update(N) * updates / (ms * 1e-3) / 1e9 / peak,
-                "ms_per_launch": ms / kernels_per_step, "kernels_per_step": kernels_per_step,
-                "flux_divergence_only_ms": ms_flux, "standalone_coupling_kernel_ms": ms_cpl}
     dfma = B.rad_probe_fp64(h)
-    slots = FP64_SLOTS_PER_UPDATE[True]
-    roofline_alu = {"kernel": kname, "bound": "alu", "unit": "TFLOP/s", "peak": 2.0 * dfma / 1e12,
-                    "peak_source": "measured live: rad_probe_fp64 (register-only DFMA kernel, CUDA events)",
-                    "achieved": 2.0 * slots * updates / (ms * 1e-3) / 1e12, "fp64_slots_per_update": slots,
-                    "note": "one FP64-pipe instruction slot per lane = 2 flop (DFMA-equivalent)"}
-    roofline_alu["frac"] = roofline_alu["achieved"] / roofline_alu["peak"]
+
+    def hbm_block(kernel, what, bpu, ms_k, extra=None):
+        """roofline of one kernel: algorithmic bytes per launch / its average launch duration, against the measured copy bandwidth"""
+        if ms_k is None:
+            return None
+        achieved = bpu * updates / (ms_k * 1e-3) / 1e9
+        prof = profile_row(kernel, workload)
+        traffic = (float(prof["dram_read_bytes"]) + float(prof["dram_write_bytes"])) if prof and prof["dram_read_bytes"] else None
+        blk = {"kernel": f"{kernel} ({what})", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+               "traffic": traffic, "traffic_source": "profiles/r2_kernels.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch)" if traffic else None,
+               "traffic_frac": (traffic / (ms_k * 1e-3) / 1e9 / peak) if traffic else None,
+               "peak_source": peak_src, "algorithmic_bytes_per_update": bpu, "ms_per_launch": ms_k,
+               "how_timed": "CUDA events over %d launches of this kernel alone on the step's inputs, same process, right after the timed region" % reps}
+        if prof and prof["fp64_inst_warp"]:
+            slots = 32.0 * float(prof["fp64_inst_warp"]) / updates  # issued FP64 lane slots per update (idle lanes included)
+            blk["alu"] = {"bound": "alu", "unit": "TFLOP/s", "peak": 2.0 * dfma / 1e12, "peak_source": "measured live: rad_probe_fp64 (register-only DFMA kernel, CUDA events)",
+                          "fp64_slots_per_update_issued": slots, "achieved": 2.0 * slots * updates / (ms_k * 1e-3) / 1e12,
+                          "frac": 2.0 * slots * updates / (ms_k * 1e-3) / (2.0 * dfma),
+                          "fp64_pipe_pct_ncu": float(prof["fp64_pipe_pct"]), "issue_pct_ncu": float(prof["issue_pct"]),
+                          "note": "one FP64-pipe instruction slot per lane = 2 flop (DFMA-equivalent); slots counted by ncu (profiles/r2_kernels.csv)"}
+        if extra:
+            blk.update(extra)
+        return blk
+
+    if args.tau_factor == 0.0:
+        roofline = hbm_block(k_flux, "fused spatial + angular flux divergence, cons -> prim: the dominant kernel of the step", fluxdiv_bytes_per_update(N), ms_flux,
+                             {"design_bytes_per_update": design_bytes_per_update(N),
+                              "design_frac": design_bytes_per_update(N) * updates / (ms_flux * 1e-3) / 1e9 / peak,
+                              "share_of_step": ms_flux / ms, "kernels_per_step": kernels_per_step})
+    else:  # k_tau_table + k_stage5<TAU> + coupling: the step as a whole on the stage's bytes
+        roofline = hbm_block(k_flux, "flux divergence with the Eq.28 factor; timed through the whole step", 32.0 + 640.0 / N, ms, {"kernels_per_step": kernels_per_step})
+    roofline_coupling = hbm_block(k_cpl, "implicit coupling, mask, fluid increment", coupling_bytes_per_update(N), ms_cpl, {"share_of_step": ms_cpl / ms})
+    stage_bpu = fluxdiv_bytes_per_update(N) + coupling_bytes_per_update(N)
+    roofline_stage = {"kernel": "whole step (all kernels of one rad_stage)", "bound": "hbm", "unit": "GB/s", "peak": peak,
+                      "algorithmic_bytes_per_update": stage_bpu, "achieved": stage_bpu * updates / (ms * 1e-3) / 1e9,
+                      "frac": stage_bpu * updates / (ms * 1e-3) / 1e9 / peak,
+                      "single_pass_bytes_per_update": algorithmic_bytes_per_update(N),
+                      "single_pass_frac": algorithmic_bytes_per_update(N) * updates / (ms * 1e-3) / 1e9 / peak}
+    moments = {"kernel": "k_moments_mma (rad_moments, frame 0)", "ms_per_call": ms_mom, "achieved": 8.0 * updates / (ms_mom * 1e-3) / 1e9, "unit": "GB/s",
+               "frac": 8.0 * updates / (ms_mom * 1e-3) / 1e9 / peak, "algorithmic_bytes_per_update": 8.0}
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -303,7 +420,7 @@ def main():
         hO = torch.empty(I_a.shape, dtype=torch.float64, pin_memory=True)
         hfl = fluid.cpu().pin_memory(); hop = opac.cpu().pin_memory()
         hT = torch.empty(ncell, dtype=torch.float64, pin_memory=True); hdT = torch.empty(4, ncell, dtype=torch.float64, pin_memory=True)
-        nrep = max(1, min(args.steps, 3))
+        nrep = max(1, min(args.steps, 10))
         B.rad_stage_host(h, hI, hO, hfl, hop, 0.0, 1.0, dt, hT, hdT)
         sync_all()
         w0 = time.perf_counter()
@@ -313,7 +430,7 @@ def main():
         w = (time.perf_counter() - w0) / nrep
         w = max_over_ranks(w, world, "cuda")
         e2e = {"value": world * updates / w, "unit": UNIT, "h2d_bytes_per_step": int(hI.numel() * 8 + hfl.numel() * 8 + hop.numel() * 8),
-               "d2h_bytes_per_step": int(hO.numel() * 8 + hT.numel() * 8 + hdT.numel() * 8), "ms_per_step": w * 1e3}
+               "d2h_bytes_per_step": int(hO.numel() * 8 + hT.numel() * 8 + hdT.numel() * 8), "ms_per_step": w * 1e3, "repetitions": nrep}
         del hI, hO
     B.rad_destroy(h)
 
@@ -331,13 +448,20 @@ def main():
         ups = 2 * smp.updates / sec
         cpu = {"value": ups, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
                "sample": f"{nsub}^3-cell sub-block (low corner, own ghosts) of {cfg}, {N} angles, 2 timed stages after 1 warm-up, {sec:.1f} s"}
+        if omp_threads(1):  # the same oracle on one thread, on a smaller sample of the same block
+            n1 = min(nsub, 32)
+            smp1 = OracleSample(cfg, n1, args.tau_factor)
+            s1 = smp1.run()
+            cpu["one_thread"] = {"value": smp1.updates / s1, "unit": UNIT, "cores": 1, "sample": f"{n1}^3-cell sub-block, one stage, {s1:.1f} s"}
+            omp_threads(os.cpu_count())
     line = {"metric": METRIC, "value": whole_job_value(updates, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{cfg}: {c['angles']} angles={N}, {nn[0]}^3 cells + 2 ghosts, metric kind {c['metric']} a={c['a']}, box {c['box']}",
-                       "updates_per_step": updates, "tau_factor": args.tau_factor, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "updates_per_step": updates, "tau_factor": args.tau_factor, "vel_estimate": args.vel_estimate,
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs (2 x %.2f GB) exceed L2; no flush" % (I_a.numel() * 8 / 1e9)},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_alu": roofline_alu,
-            "cpu_baseline": cpu}
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_fluxdiv": roofline,
+            "roofline_coupling": roofline_coupling, "roofline_stage": roofline_stage, "moments": moments, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -206,6 +206,12 @@ long long rad_ncells_total(const rad_ctx *);
 /* kernels launched by this context so far (bench.py's gpu_launches) */
 long long rad_launch_count(const rad_ctx *);
 
+/* Names of the kernels one rad_stage launches on this context after the ghost fill, "flux-divergence kernel;coupling kernel", each
+ * written as ncu prints the instance without casts and blanks, e.g. "k_stage5<3,2,4,2,1,1,0>;k_couple_stream<0>".  bench.py keys
+ * the committed ncu summaries (the .csv files under profiles/) with them and prints no profile figure for a kernel whose name it does not find.
+ * buf: HOST, nbytes >= 128.  RAD_EINVAL if the buffer is too small. */
+rad_status rad_stage_kernels(rad_ctx *, char *buf /* HOST */, size_t nbytes);
+
 /* Measurement helper (not part of the stage): the device's FP64 fused-multiply-add rate, in lane-level DFMA
  * operations per second (x2 = flop/s), from a register-only kernel timed with CUDA events; synchronises.
  * bench.py uses it as the denominator of the FP64 ("alu") roofline of the stage kernel. */

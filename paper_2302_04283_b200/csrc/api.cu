@@ -511,6 +511,16 @@ rad_status rad_moments(rad_ctx *c, const double *I, int frame, const double *flu
     return RAD_OK;
 }
 
+rad_status rad_stage_kernels(rad_ctx *c, char *buf, size_t nbytes) {
+    if (!c || !buf || nbytes == 0) return fail(c, RAD_EINVAL, "rad_stage_kernels: NULL argument");
+    char a[96];
+    rad::stage_angle_kernel_name(c->dev, c->kp, c->kp.tau_factor != 0.0, a, sizeof a);
+    const bool stream = rad::stream_serves(c->dev, nullptr) != 0;
+    const int w = snprintf(buf, nbytes, "%s;%s", a, stream ? (c->kp.vel_estimate && c->kp.couple ? "k_couple_stream<1>" : "k_couple_stream<0>") : "k_coupling");
+    if (w < 0 || (size_t)w >= nbytes) return fail(c, RAD_EINVAL, "rad_stage_kernels: buffer too small");
+    return RAD_OK;
+}
+
 rad_status rad_probe_fp64(rad_ctx *c, double *dfma_per_sec) {
     if (!c || !dfma_per_sec) return fail(c, RAD_EINVAL, "rad_probe_fp64: NULL argument");
     DeviceGuard guard(c->device);

@@ -110,6 +110,7 @@ int launch_moments_stream(const DeviceTables &t, const double *I, int frame, con
 // angle-resident fused flux-divergence kernel (stage5.cu): 1 launched, 0 this configuration is not served (caller falls back to
 // launch_fluxdiv), -1 CUDA error; and its record builder
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, cudaStream_t s);
+int stage_angle_kernel_name(const DeviceTables &t, const Params &p, bool tau, char *buf, size_t n);
 // 1 if launch_stage_angle serves this context (so that a stage can be run slab by slab along z)
 int stage_angle_serves(const DeviceTables &t);
 // TAU table of the angle-resident kernel: vel8[ncell][8], see k_tau_table (stage5.cu)

@@ -16,6 +16,8 @@
 //     partner angle pulls it from there), and a packed per-cell geometry record (4 buffers).  One __syncthreads per step.
 //   * TAU (template): the optical-depth-aware spatial flux of Eq.26-29 -- a per-cell table (k_tau_table) of u^alphahat and f/2
 //     of the upper faces comes in with the other copies for the tile's cells and the halo cells at distance 1.
+#include <cstdio>
+
 #include "async_copy.cuh"
 #include "stage_math.cuh"
 
@@ -656,6 +658,15 @@ int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &
     if (!stage_angle_serves(t)) return 0;
     if (((uintptr_t)a.I_in & 15) || ((uintptr_t)a.vel8 & 15)) return 0;  // rows are brought in by 16-byte bulk copies
 #define RAD_S5_CALL(NITER, WPC, TY, TZ) return launch5<NITER, WPC, TY, TZ>(t, p, a, s)
+    RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
+#undef RAD_S5_CALL
+    return 0;
+}
+
+// the instance launch_stage_angle runs for this context, written as ncu prints it without casts and blanks (profiles/*.csv key)
+int stage_angle_kernel_name(const DeviceTables &t, const Params &p, bool tau, char *buf, size_t n) {
+    if (!stage_angle_serves(t)) return snprintf(buf, n, "k_fluxdiv");
+#define RAD_S5_CALL(NITER, WPC, TY, TZ) return snprintf(buf, n, "k_stage5<%d,%d,%d,%d,1,%d,%d>", NITER, WPC, TY, TZ, p.recon_space == 1 ? 1 : 0, tau ? 1 : 0)
     RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
 #undef RAD_S5_CALL
     return 0;

@@ -327,3 +327,62 @@ def test_velocity_estimate_full_size_c4(oracle, B):
         assert acted > 20     # the estimate changed the result in a good number of the sampled cells
     finally:
         B.rad_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ memory and ordering hygiene
+# compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md), so the two classes of defect it would find are hunted with
+# checks of our own: a data race on the shared-memory tiles shows up as results that change from run to run, an out-of-bounds access
+# as a guard band around the caller's arrays that is no longer intact (or as a canary value that leaked into the results).
+@pytest.mark.parametrize("n,angles,tau", [((9, 6, 5), ("geodesic", 4), 0.0), ((7, 5, 3), ("geodesic", 3), 1.5), ((5, 9, 37), ("latlon", 4, 8), 0.0),
+                                          ((13, 3, 2), ("geodesic", 5), 0.0), ((4, 4, 4), ("geodesic", 6), 0.0)])
+def test_stage_and_moments_are_bitwise_reproducible(oracle, B, n, angles, tau):
+    """ten runs of the stage (tile kernel with its mbarrier-ordered shared-memory ring, named barriers and in-place coefficient/flux
+    exchange; streaming coupling kernel with its per-warp ring) and of the moments on the same inputs give the same bits"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, angles, tau_factor=tau)
+    try:
+        dI = dev(I); dfl = dev(fluid)
+        ref = None
+        for rep in range(10):
+            dO = torch.full_like(dI, float(rep)); dT = torch.zeros(P.ncell, dtype=torch.float64, device="cuda")
+            ddT0 = torch.zeros(4, P.ncell, dtype=torch.float64, device="cuda"); mom = torch.zeros(10, P.ncell, dtype=torch.float64, device="cuda")
+            B.rad_stage(h, dI, dO, None, dfl, 0.0, 1.0, 0.03, dT, ddT0)
+            B.rad_moments(h, dO, 0, dfl, mom)
+            got = [P.interior(x.cpu().numpy()) for x in (dO, dT)] + [P.interior(ddT0[m].cpu().numpy()) for m in range(4)] + [P.interior(mom[m].cpu().numpy()) for m in range(10)]
+            if ref is None:
+                ref = got
+            else:
+                assert all(np.array_equal(a, b) for a, b in zip(got, ref)), f"run {rep} differs from run 0"
+    finally:
+        B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("n,angles", [((9, 6, 5), ("geodesic", 4)), ((3, 5, 9), ("geodesic", 3)), ((1, 1, 1), ("latlon", 4, 8)), ((6, 5, 4), ("geodesic", 6))])
+def test_guard_bands_around_caller_arrays_stay_intact(oracle, B, n, angles):
+    """every caller array sits between two guard bands of NaN in one allocation: after a stage and a moments call the bands are
+    untouched (no out-of-bounds write) and no NaN reached an interior result (no out-of-bounds read that matters)"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, angles)
+    G = 4096  # doubles per guard band
+
+    def guarded(x):
+        buf = torch.full((x.size + 2 * G,), float("nan"), dtype=torch.float64, device="cuda")
+        view = buf[G:G + x.size].view(*x.shape)
+        view.copy_(torch.as_tensor(x))
+        return buf, view
+
+    try:
+        bufs = {}
+        for name, arr in (("I", I), ("O", np.zeros_like(I)), ("fluid", fluid), ("T", np.zeros(P.ncell)), ("dT0", np.zeros((4, P.ncell))), ("mom", np.zeros((10, P.ncell)))):
+            bufs[name] = guarded(arr)
+        B.rad_stage(h, bufs["I"][1], bufs["O"][1], None, bufs["fluid"][1], 0.0, 1.0, 0.03, bufs["T"][1], bufs["dT0"][1])
+        B.rad_moments(h, bufs["O"][1], 0, bufs["fluid"][1], bufs["mom"][1])
+        torch.cuda.synchronize()
+        for name, (buf, view) in bufs.items():
+            assert bool(torch.isnan(buf[:G]).all()) and bool(torch.isnan(buf[-G:]).all()), f"guard band of {name} was written"
+        out = bufs["O"][1].cpu().numpy()
+        assert np.isfinite(P.interior(out)).all() and np.isfinite(P.interior(bufs["T"][1].cpu().numpy())).all()
+        assert all(np.isfinite(P.interior(bufs["dT0"][1][m].cpu().numpy())).all() for m in range(4))
+        assert all(np.isfinite(P.interior(bufs["mom"][1][m].cpu().numpy())).all() for m in range(10))
+        out_o, _, _, _ = P.stage(I.copy(), fluid, opac, 0.03)
+        assert rel_err_I(P.interior(out), P.interior(out_o)) <= TOL_I
+    finally:
+        B.rad_destroy(h)
