@@ -93,6 +93,8 @@ def ingest_ncu(raw_csv, cmd, workload):
             "fp64_pipe_pct": ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", 1.0), "issue_pct": ("smsp__issue_active.avg.pct_of_peak_sustained_active", 1.0),
             "smem_wavefronts": ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", 1.0), "smem_bank_conflicts": ("l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum", 1.0),
             "registers": ("launch__registers_per_thread", 1.0), "grid": ("launch__grid_size", 1.0), "block": ("launch__block_size", 1.0)}
+    # FP64 warp instructions are not exported as a count: pipe-active fraction x active cycles x SMs x 2 issues per cycle and SM (64 lanes)
+    derive = ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", "sm__cycles_active.avg", "device__attribute_multiprocessor_count")
     unit_scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "ms": 1e6, "us": 1e3, "ns": 1.0, "s": 1e9}
     old = []
     try:
@@ -109,6 +111,9 @@ def ingest_ncu(raw_csv, cmd, workload):
                 continue
             x = float(d[m].replace(",", "")) * unit_scale.get(rows[1][h.index(m)], 1.0) * (sc if k == "ms" else 1.0)
             r[k] = repr(x)
+        if all(m in d and d[m] != "" for m in derive):
+            pct, cyc, sms = (float(d[m].replace(",", "")) for m in derive)
+            r["fp64_inst_warp"] = repr(pct / 100.0 * cyc * sms * 2.0)
         old = [o for o in old if not (o["kernel"] == r["kernel"] and o["workload"] == r["workload"])] + [r]
     with open(PROFILE_CSV, "w", newline="") as f:
         w = csv.DictWriter(f, fieldnames=PROFILE_FIELDS)
@@ -259,11 +264,22 @@ def main():
     ap.add_argument("--vel-estimate", type=int, default=0, help="1: radiation-dominated velocity estimate Eq.51-55 in the coupling (NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--probe-pipes", action="store_true", help="print the FP64 pipe probe (DMMA vs DFMA, alone and mixed) and exit")
     ap.add_argument("--ncu-raw", default=None, help="fold this `ncu --page raw --csv` export into profiles/r2_kernels.csv and exit")
     ap.add_argument("--ncu-cmd", default="", help="the ncu command that produced --ncu-raw (recorded beside the csv)")
     args = ap.parse_args()
     if args.ncu_raw:
         return ingest_ncu(args.ncu_raw, args.ncu_cmd, args.config if args.n is None else f"{args.config}/n={args.n}")
+    if args.probe_pipes:
+        from paper_2302_04283_b200 import binding as B
+        from paper_2302_04283_b200 import build
+        build.build()
+        h = B.rad_create(dict(kind=0), dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1)), ("geodesic", 1), None, dict(couple=0), 0)
+        v = B.rad_probe_fp64_pipes(h)
+        B.rad_destroy(h)
+        names = ["dmma_alone", "dfma_alone", "dmma_in_mix_4_8", "dfma_in_mix_4_8", "dmma_in_mix_1_8", "dfma_in_mix_1_8"]
+        print(json.dumps({"fp64_pipe_probe_multiply_adds_per_sec": dict(zip(names, v)), "sum_mix_4_8": v[2] + v[3], "sum_mix_1_8": v[4] + v[5]}))
+        return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
