@@ -6,7 +6,8 @@
 // trip count per thread the ownership is balanced: an orientation of the edge graph in which every angle owns
 // at most ceil(deg/2) <= 3 of its <= 6 edges (and therefore receives at most 3).  Such an orientation always
 // exists (pair up odd-degree vertices and follow Euler circuits); it is found here by reversing paths from
-// overloaded to underloaded vertices, in a fixed deterministic order.
+// overloaded to underloaded vertices, in a fixed deterministic order.  The owned edges of an angle then get SLOTS 0..2 by an
+// edge colouring (below) under which the received edges of every angle have different slots as well.
 #include <algorithm>
 #include <queue>
 
@@ -63,26 +64,51 @@ bool build_edge_ownership(const AngleTables &a, EdgeOwnership &o, std::string &e
         if (out[v] > hi(v) || out[v] < lo(v)) {  // a later reversal never unbalances a settled vertex, but check
             err = "edge ownership is not balanced"; return false;
         }
+    // Slots.  The slot of an edge at its owner is a COLOUR in {0, 1, 2} chosen so that the edges an angle owns have different colours
+    // (one slot each) and the edges it receives have different colours too: then the k-th flux an angle pulls always sits in slot k
+    // of its owner, and a kernel needs only the owner's angle index per pulled edge.  Such a colouring is a proper edge colouring of
+    // the bipartite graph (owner side, partner side) of maximum degree 3, which exists by Koenig's theorem; it is found by the
+    // alternating-path argument of its proof, in a fixed deterministic order (increasing edge id).
+    std::vector<int> colour(E, -1);
+    std::vector<int> atX((size_t)N * kMaxOwn, -1), atY((size_t)N * kMaxOwn, -1);  // edge of colour c at owner side x / partner side y
+    auto partner = [&](int e) { const int v = owner[e]; return (a.edge_lo[e] == v) ? a.edge_hi[e] : a.edge_lo[e]; };
+    for (int e = 0; e < E; e++) {
+        const int x = owner[e], y = partner(e);
+        int ca = -1, cb = -1;
+        for (int c = kMaxOwn - 1; c >= 0; c--) { if (atX[(size_t)x * kMaxOwn + c] < 0) ca = c; if (atY[(size_t)y * kMaxOwn + c] < 0) cb = c; }
+        if (ca < 0 || cb < 0) { err = "edge colouring: a vertex has more than 3 edges on one side"; return false; }
+        if (atY[(size_t)y * kMaxOwn + ca] >= 0) {
+            // colour ca is taken at y: swap ca <-> cb along the maximal path that leaves y on colour ca (it cannot reach x, where ca is free)
+            std::vector<int> path;
+            int side = 1, v = y, want = ca;  // side 1: at a partner-side vertex, follow `want`
+            while (true) {
+                const int f = side ? atY[(size_t)v * kMaxOwn + want] : atX[(size_t)v * kMaxOwn + want];
+                if (f < 0) break;
+                path.push_back(f);
+                v = side ? owner[f] : partner(f);
+                side ^= 1;
+                want = (want == ca) ? cb : ca;
+            }
+            for (int f : path) { atX[(size_t)owner[f] * kMaxOwn + colour[f]] = -1; atY[(size_t)partner(f) * kMaxOwn + colour[f]] = -1; }
+            for (int f : path) {
+                colour[f] = (colour[f] == ca) ? cb : ca;
+                atX[(size_t)owner[f] * kMaxOwn + colour[f]] = f; atY[(size_t)partner(f) * kMaxOwn + colour[f]] = f;
+            }
+        }
+        colour[e] = ca;
+        atX[(size_t)x * kMaxOwn + ca] = e; atY[(size_t)y * kMaxOwn + ca] = e;
+    }
     o.own_edge.assign((size_t)N * kMaxOwn, -1);
     o.own_partner.assign((size_t)N * kMaxOwn, -1);
     o.pull_pos.assign((size_t)N * kMaxOwn, -1);
-    std::vector<int> nown(N, 0), npull(N, 0), slot_of_edge(E, -1);
-    for (int e = 0; e < E; e++) {  // increasing edge id => slots in increasing edge id per owner
-        const int v = owner[e];
-        if (nown[v] >= kMaxOwn) { err = "owner overflow"; return false; }
-        const int p = (a.edge_lo[e] == v) ? a.edge_hi[e] : a.edge_lo[e];
-        slot_of_edge[e] = nown[v];
-        o.own_edge[(size_t)v * kMaxOwn + nown[v]] = e;
-        o.own_partner[(size_t)v * kMaxOwn + nown[v]] = p;
-        nown[v]++;
-    }
     for (int e = 0; e < E; e++) {
-        const int v = owner[e];
-        const int p = (a.edge_lo[e] == v) ? a.edge_hi[e] : a.edge_lo[e];
+        const int v = owner[e], p = partner(e), c = colour[e];
+        if (o.own_edge[(size_t)v * kMaxOwn + c] >= 0) { err = "edge colouring: owner slot used twice"; return false; }
+        o.own_edge[(size_t)v * kMaxOwn + c] = e;
+        o.own_partner[(size_t)v * kMaxOwn + c] = p;
         if (p == v) continue;  // degenerate self edge (npsi = 1): carries no net flux
-        if (npull[p] >= kMaxOwn) { err = "partner overflow"; return false; }
-        o.pull_pos[(size_t)p * kMaxOwn + npull[p]] = slot_of_edge[e] * N + v;
-        npull[p]++;
+        if (o.pull_pos[(size_t)p * kMaxOwn + c] >= 0) { err = "edge colouring: partner slot used twice"; return false; }
+        o.pull_pos[(size_t)p * kMaxOwn + c] = c * N + v;  // the k-th pull of an angle comes from slot k of its owner
     }
     return true;
 }

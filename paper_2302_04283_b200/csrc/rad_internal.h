@@ -28,7 +28,7 @@ constexpr int kMaxOwn = 3;
 struct EdgeOwnership {
     std::vector<int> own_edge;     // [N][3] unique edge id owned in slot j, or -1
     std::vector<int> own_partner;  // [N][3] angle at the far end of that edge, or -1
-    std::vector<int> pull_pos;     // [N][3] position j*N + owner of a flux this angle receives, or -1
+    std::vector<int> pull_pos;     // [N][3] entry k: position k*N + owner of the flux this angle receives from slot k of its owner, or -1
 };
 bool build_edge_ownership(const AngleTables &a, EdgeOwnership &out, std::string &err);
 
