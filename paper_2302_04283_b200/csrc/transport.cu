@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(256) k_cell_velocity(DeviceTables t, const dou
 }
 
 template <int RECON, bool TAU>
-__global__ void __launch_bounds__(256) k_fluxdiv_v1(DeviceTables t, const double *__restrict__ I_in, const double *__restrict__ I0,
+__global__ void __launch_bounds__(256) k_fluxdiv(DeviceTables t, const double *__restrict__ I_in, const double *__restrict__ I0,
                                                    double gam0, double gam1, double beta_dt, double *__restrict__ I_out,
                                                    const double *__restrict__ vel, double tau_dt) {
     extern __shared__ double smem[];
@@ -271,8 +271,8 @@ int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, c
     const size_t smem = sizeof(double) * (CX * 36 + (CX + 1) * 8 + 4 * CX * 8 + (size_t)CX * t.E);
 #define RAD_LAUNCH_FD(RECON, TAU)                                                                                     \
     do {                                                                                                              \
-        cudaFuncSetAttribute(k_fluxdiv_v1<RECON, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
-        k_fluxdiv_v1<RECON, TAU><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out, vel, tau_dt); \
+        cudaFuncSetAttribute(k_fluxdiv<RECON, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+        k_fluxdiv<RECON, TAU><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out, vel, tau_dt); \
     } while (0)
     if (p.recon_space == 2) { if (vel) RAD_LAUNCH_FD(2, true); else RAD_LAUNCH_FD(2, false); }
     else if (p.recon_space == 1) { if (vel) RAD_LAUNCH_FD(1, true); else RAD_LAUNCH_FD(1, false); }

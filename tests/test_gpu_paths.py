@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 @pytest.mark.parametrize("angles", [("geodesic", 3), ("geodesic", 4), ("latlon", 8, 16), ("latlon", 3, 5)])
 @pytest.mark.parametrize("tau", [0.0, 2.0])
 def test_generic_path_without_stored_coefficients(oracle, B, angles, tau):
-    """recompute_edge_coeffs = 1: no stored coefficients, the stage runs as k_fluxdiv_v1 (+ k_cell_velocity) and the coupling kernel"""
+    """recompute_edge_coeffs = 1: no stored coefficients, the stage runs as k_fluxdiv (+ k_cell_velocity) and the coupling kernel"""
     A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (7, 5, 4), angles, recompute_edge_coeffs=1, tau_factor=tau)
     try:
         with pytest.raises(B.RadError):   # no tile kernel in this context
@@ -386,3 +386,25 @@ def test_guard_bands_around_caller_arrays_stay_intact(oracle, B, n, angles):
         assert rel_err_I(P.interior(out), P.interior(out_o)) <= TOL_I
     finally:
         B.rad_destroy(h)
+
+
+def test_measurement_helpers(oracle, B):
+    """rad_stage_kernels names the instances a stage launches (the key of profiles/r2_kernels.csv); the FP64 probes run, and the
+    matrix instruction adds nothing to the scalar FP64 rate (same pipe: DESIGN.md 'stored versus recomputed')"""
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (4, 4, 4), ("geodesic", 4))
+    try:
+        kf, kc = B.rad_stage_kernels(h)
+        assert kf == "k_stage5<3,2,4,2,1,1,0>" and kc == "k_couple_stream<0>"
+        dfma = B.rad_probe_fp64(h)
+        v = B.rad_probe_fp64_pipes(h)
+        assert dfma > 1e12 and all(x > 1e12 for x in v)
+        assert v[2] + v[3] < 1.15 * max(v[0], v[1]) and v[4] + v[5] < 1.15 * max(v[0], v[1])
+    finally:
+        B.rad_destroy(h)
+    for angles, want in ((("geodesic", 6), ("k_fluxdiv", "k_couple_stream<0>")),   # N = 362: generic flux divergence, streaming coupling
+                         (("latlon", 7, 9), ("k_fluxdiv", "k_coupling"))):          # N = 63, odd: generic kernels
+        A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (4, 4, 4), angles)
+        try:
+            assert B.rad_stage_kernels(h) == want
+        finally:
+            B.rad_destroy(h)
