@@ -185,8 +185,8 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
             for (int n = 0; n < h.N; n++) {
                 for (int q = 0; q < 3; q++) {  // unused slots: partner 0 (its q_e is 0) and the always-zero flux slot 3N
                     const int pa = c->own.own_partner[(size_t)n * 3 + q], pu = c->own.pull_pos[(size_t)n * 3 + q];
-                    rec[(size_t)n * 8 + q] = (short)(unsigned short)(pa >= 0 ? pa : 0);
-                    rec[(size_t)n * 8 + 3 + q] = (short)(unsigned short)(pu >= 0 ? pu : 3 * h.N);
+                    rec[(size_t)n * 8 + q] = (short)(unsigned short)(8 * (pa >= 0 ? pa : 0));          // byte offsets in a row of doubles
+                    rec[(size_t)n * 8 + 3 + q] = (short)(unsigned short)(8 * (pu >= 0 ? pu : 3 * h.N));
                 }
                 winv[n] = 1.0 / h.domega[n];
             }

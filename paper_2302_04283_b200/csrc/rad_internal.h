@@ -58,7 +58,7 @@ struct DeviceTables {
     // geometry
     const double *cell;  // [ncell][RAD_NCELL]
     const double *face;  // [ncell][3][RAD_NFACE]
-    // fused stage kernel (stage5.cu): per-angle record {own_partner[3], pull_pos[3], 0, 0} as 8 x int16 (16 B),
+    // fused stage kernel (stage5.cu): per-angle record {8 own_partner[3], 8 pull_pos[3], 0, 0} (byte offsets) as 8 x uint16 (16 B),
     // 1/dOmega, the owned edge ids, and the stored edge coefficients
     const short *ang_rec;    // [N][8]
     const double *winv;      // [N]

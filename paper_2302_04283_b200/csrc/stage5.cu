@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         n1[it] = t.nhat[3 * n]; n2[it] = t.nhat[3 * n + 1]; n3[it] = t.nhat[3 * n + 2];
         winv[it] = v ? t.winv[n] : 0.0;
         const uint4 rec = reinterpret_cast<const uint4 *>(t.ang_rec)[n];
-        const unsigned z = 3u * (unsigned)N;
+        const unsigned z = 24u * (unsigned)N;  // byte offset of the always-zero slot 3 N
         rx[it] = v ? rec.x : 0u; ry[it] = v ? rec.y : (z << 16); rz[it] = v ? rec.z : (z | (z << 16));
     }
 #define OFF8(it) ((it) < NITER - 1 ? lane8 + (uint32_t)(it) * ITB : last8)
@@ -311,7 +311,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
 #pragma unroll
                 for (int jj = 0; jj < 3; jj++) {
                     const bool owner_up = (__double2loint(q[jj]) & 1) != 0;
-                    G[jj] = lds_unless(ownrow + pj[jj] * 8u, owner_up, x0[it]);  // the upwind intensity: the thread's own (in a register) or the partner's
+                    G[jj] = lds_unless(ownrow + pj[jj], owner_up, x0[it]);  // the upwind intensity: the thread's own (in a register) or the partner's
                 }
 #pragma unroll
                 for (int jj = 0; jj < 3; jj++) G[jj] *= q[jj];
@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             if (WPC > 1) named_bar_sync(barid, WPC * 32); else __syncwarp();
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
-                const double pulled = (lds(aEb + (ry[it] >> 16) * 8u) + lds(aEb + (rz[it] & 0xffffu) * 8u)) + lds(aEb + (rz[it] >> 16) * 8u);  // unused -> slot 3N = 0
+                const double pulled = (lds(aEb + (ry[it] >> 16)) + lds(aEb + (rz[it] & 0xffffu))) + lds(aEb + (rz[it] >> 16));  // unused -> slot 3N = 0
                 d[it] = (d[it] - pulled) * winv[it];
             }
             // ---- spatial fluxes (Eq.24).  x: the upper face; the lower one is carried
