@@ -206,6 +206,15 @@ long long rad_ncells_total(const rad_ctx *);
 /* kernels launched by this context so far (bench.py's gpu_launches) */
 long long rad_launch_count(const rad_ctx *);
 
+/* Halo exchange between two blocks on the same device that touch along `axis` (0 x, 1 y, 2 z), block `hi` above block `lo`: the
+ * communication task of a stage for a domain cut into blocks, one context per block.  The upper ghost layers of I_lo
+ * receive the first ng interior layers of I_hi and the lower ghost layers of I_hi the last ng interior layers of I_lo, over the
+ * full extent (ghosts included) of the other two axes.  Both contexts must agree in angle grid size, ghost depth and the extents
+ * across the axis (RAD_EINVAL otherwise); the touching boundaries should carry boundary code 0 (caller-filled) so that rad_stage
+ * leaves the exchanged layers alone.  Call it for x, then y, then z before rad_stage, like the ghost fill, so that edges and corners
+ * are consistent.  I_lo, I_hi: DEVICE, each laid out for its own context.  Enqueued on `stream` (2 launches); no sync. */
+rad_status rad_exchange_halo(rad_ctx *lo, double *I_lo, rad_ctx *hi, double *I_hi, int axis, void *cuda_stream);
+
 /* Names of the kernels one rad_stage launches on this context after the ghost fill, "flux-divergence kernel;coupling kernel", each
  * written as ncu prints the instance without casts and blanks, e.g. "k_stage5<3,2,4,2,1,1,0>;k_couple_stream<0>".  bench.py keys
  * the committed ncu summaries (the .csv files under profiles/) with them and prints no profile figure for a kernel whose name it does not find.

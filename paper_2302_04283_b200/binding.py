@@ -20,7 +20,7 @@ NCELL, NFACE, MAXNBR = 52, 8, 6
  TAB_STAGE_FACE_SIGN) = range(20)
 
 EXPORTS = ["rad_create", "rad_stage", "rad_stage_host", "rad_fill_ghosts", "rad_transport", "rad_couple", "rad_moments",
-           "rad_get_table", "rad_stage_kernels", "rad_probe_fp64", "rad_probe_fp64_pipes", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
+           "rad_get_table", "rad_exchange_halo", "rad_stage_kernels", "rad_probe_fp64", "rad_probe_fp64_pipes", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
 
 
 class RadError(RuntimeError):
@@ -76,6 +76,7 @@ def lib():
         L.rad_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
         L.rad_probe_fp64.argtypes = [vp, C.POINTER(C.c_double)]
         L.rad_probe_fp64_pipes.argtypes = [vp, C.POINTER(C.c_double)]
+        L.rad_exchange_halo.argtypes = [vp, vp, vp, vp, C.c_int, vp]
         L.rad_stage_kernels.argtypes = [vp, C.c_char_p, C.c_size_t]
         L.rad_ncells_total.argtypes = [vp]; L.rad_ncells_total.restype = C.c_longlong
         L.rad_launch_count.argtypes = [vp]; L.rad_launch_count.restype = C.c_longlong
@@ -173,6 +174,11 @@ def rad_stage_host(ctx, I_in, I_out, fluid, opac, gam0, gam1, beta_dt, T_out=Non
 
 def rad_fill_ghosts(ctx, I, stream=None):
     _check(ctx, lib().rad_fill_ghosts(ctx, _dp(I), _stream(stream)))
+
+
+def rad_exchange_halo(ctx_lo, I_lo, ctx_hi, I_hi, axis, stream=None):
+    """halo exchange between block lo and its neighbour hi above it along `axis` (same device)"""
+    _check(ctx_lo, lib().rad_exchange_halo(ctx_lo, _dp(I_lo), ctx_hi, _dp(I_hi), int(axis), _stream(stream)))
 
 
 def rad_transport(ctx, I_in, I_out, I0, gam0, gam1, beta_dt, stream=None):

@@ -287,6 +287,22 @@ rad_status rad_fill_ghosts(rad_ctx *c, double *I, void *stream) {
     return RAD_OK;
 }
 
+rad_status rad_exchange_halo(rad_ctx *lo, double *I_lo, rad_ctx *hi, double *I_hi, int axis, void *stream) {
+    if (!lo || !hi || !I_lo || !I_hi) return fail(lo ? lo : hi, RAD_EINVAL, "rad_exchange_halo: NULL argument");
+    if (axis < 0 || axis > 2) return fail(lo, RAD_EINVAL, "rad_exchange_halo: axis must be 0, 1 or 2");
+    const rad::DeviceTables &a = lo->dev, &b = hi->dev;
+    if (lo->device != hi->device || a.N != b.N || a.ng != b.ng) return fail(lo, RAD_EINVAL, "rad_exchange_halo: the blocks differ in device, angle count or ghost depth");
+    for (int d = 0; d < 3; d++)
+        if (d != axis && a.n[d] != b.n[d]) return fail(lo, RAD_EINVAL, "rad_exchange_halo: the blocks differ in an extent across the axis");
+    if (a.n[axis] < a.ng || b.n[axis] < b.ng) return fail(lo, RAD_EINVAL, "rad_exchange_halo: a block is thinner than the ghost depth");
+    if (I_lo == I_hi) return fail(lo, RAD_EINVAL, "rad_exchange_halo: the two blocks share an array");
+    DeviceGuard guard(lo->device);
+    const int nl = rad::launch_exchange_halo(a, I_lo, b, I_hi, axis, (cudaStream_t)stream);
+    if (nl < 0) return cuda_fail(lo, "rad_exchange_halo");
+    lo->launches += nl;
+    return RAD_OK;
+}
+
 // The two halves of a stage on one stream (no argument checks: the callers did them).
 // transport: ghost fill, then the tile kernel (stage5.cu) where it serves the context, else the generic flux-divergence kernel
 // (transport.cu).  `fluid` != nullptr with tau_factor != 0 selects the optical-depth-aware flux (Eq.26-29).

@@ -92,6 +92,7 @@ struct Params {
 // kernel launchers (each returns the number of kernels it launched, or -1 after setting a CUDA error)
 int launch_geometry(const rad_metric &m, const rad_grid &g, double *cell, double *face, long long ncell,
                     cudaStream_t s);
+int launch_exchange_halo(const DeviceTables &lo, double *I_lo, const DeviceTables &hi, double *I_hi, int axis, cudaStream_t s);
 int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_hi[3], double *I, cudaStream_t s);
 int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, const double *I0, double gam0,
                    double gam1, double beta_dt, double *I_out, cudaStream_t s, const double *vel = nullptr, double tau_dt = 0.0);

@@ -52,6 +52,31 @@ __global__ void k_fill_ghosts(double *__restrict__ I, int N, int NI, int NJ, int
 }
 
 // ------------------------------------------------------------------------------------------------
+// halo copy between two blocks that touch along `axis` (the communication task of a stage, on one device): nlayers
+// layers of `src` starting at index src_first along the axis go to the layers of `dst` starting at dst_first; the other two
+// extents (ghosts included) are the same in both blocks.  One CTA per cell, threads over angles.
+// ------------------------------------------------------------------------------------------------
+__global__ void k_copy_halo(const double *__restrict__ src, double *__restrict__ dst, int N, int e0, int e1, int e2, int axis, int src_first, int dst_first,
+                            int src_ext, int dst_ext, int vec2) {
+    int d[3];
+    long long b = blockIdx.x;
+    d[0] = (int)(b % e0); b /= e0;
+    d[1] = (int)(b % e1); b /= e1;
+    d[2] = (int)b;
+    int sdim[3] = {e0, e1, e2}, ddim[3] = {e0, e1, e2}, sidx[3] = {d[0], d[1], d[2]}, didx[3] = {d[0], d[1], d[2]};
+    sdim[axis] = src_ext; ddim[axis] = dst_ext;
+    sidx[axis] = src_first + d[axis]; didx[axis] = dst_first + d[axis];
+    const long long cs = ((long long)sidx[2] * sdim[1] + sidx[1]) * sdim[0] + sidx[0], cd = ((long long)didx[2] * ddim[1] + didx[1]) * ddim[0] + didx[0];
+    if (vec2) {
+        const double2 *ps = reinterpret_cast<const double2 *>(src + cs * N);
+        double2 *pd = reinterpret_cast<double2 *>(dst + cd * N);
+        for (int n = threadIdx.x; n < N / 2; n += blockDim.x) pd[n] = ps[n];
+    } else {
+        for (int n = threadIdx.x; n < N; n += blockDim.x) dst[cd * N + n] = src[cs * N + n];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // fused flux divergence, version 1: one CTA per run of CX cells along x
 // ------------------------------------------------------------------------------------------------
 constexpr int CX = 8;
@@ -256,6 +281,20 @@ int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_h
         launches++;
     }
     return launches;
+}
+
+// both directions of the exchange between block `lo` and block `hi` = its neighbour above along `axis`: 2 launches, -1 on a CUDA error
+int launch_exchange_halo(const DeviceTables &lo, double *I_lo, const DeviceTables &hi, double *I_hi, int axis, cudaStream_t s) {
+    const int ng = lo.ng, N = lo.N;
+    int e[3] = {lo.NI, lo.NJ, lo.NK};
+    const int lo_ext = e[axis], hi_ext = axis == 0 ? hi.NI : (axis == 1 ? hi.NJ : hi.NK);
+    e[axis] = ng;
+    const long long blocks = (long long)e[0] * e[1] * e[2];
+    const int vec2 = (N & 1) == 0 && ((uintptr_t)I_lo & 15) == 0 && ((uintptr_t)I_hi & 15) == 0;
+    // the upper ghost layers of lo <- the first interior layers of hi; the lower ghost layers of hi <- the last interior layers of lo
+    k_copy_halo<<<(unsigned)blocks, 64, 0, s>>>(I_hi, I_lo, N, e[0], e[1], e[2], axis, ng, lo_ext - ng, hi_ext, lo_ext, vec2);
+    k_copy_halo<<<(unsigned)blocks, 64, 0, s>>>(I_lo, I_hi, N, e[0], e[1], e[2], axis, lo_ext - 2 * ng, 0, lo_ext, hi_ext, vec2);
+    return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
 
 int launch_cell_velocity(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double *vel, cudaStream_t s) {

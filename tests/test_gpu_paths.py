@@ -408,3 +408,68 @@ def test_measurement_helpers(oracle, B):
             assert B.rad_stage_kernels(h) == want
         finally:
             B.rad_destroy(h)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_two_blocks_with_halo_exchange_equal_one_block(oracle, B, axis):
+    """NEXT-4: a block cut in two along `axis`, one context per half, outflow on the outer boundaries and caller-filled on the
+    cut with rad_exchange_halo before every stage, reproduces the undivided block over two stages (bit for bit for a cut in x, to rounding for y and z, where the
+    tile edges move) -- and the undivided block matches the oracle"""
+    n = [7, 5, 6]; n[axis] = 12
+    ang, dx, x0, ng, dt = ("geodesic", 3), (0.25, 0.5, 0.125), [3.0, 2.0, 1.0], 2, 0.02   # binary fractions: both cuts see the same coordinates
+    bc = (2,) * 6
+    A, P, h, I, fluid, opac, _ = small_problem(oracle, B, tuple(n), ang, bc=bc, x0=tuple(x0), dx=dx)
+    N = A.N
+    shape = (n[2] + 4, n[1] + 4, n[0] + 4)
+    ax_np = 2 - axis                      # numpy axis of the cut
+    half = n[axis] // 2
+    def part(arr, lo):                    # [..., k, j, i, (n)] -> the half block incl. its ghosts
+        sl = [slice(None)] * 3
+        sl[ax_np] = slice(0, half + 4) if lo else slice(half, n[axis] + 4)
+        return sl
+    try:
+        # the undivided block: two stages, ping-pong
+        dA = dev(I); dB = torch.zeros_like(dA); dfl = dev(fluid)
+        B.rad_stage(h, dA, dB, None, dfl, 0.0, 1.0, dt)
+        out1 = dB.cpu().numpy().copy()
+        dB2 = dB.clone(); dA2 = torch.zeros_like(dA)
+        B.rad_stage(h, dB2, dA2, None, dfl, 0.0, 1.0, dt)
+        big = dA2.cpu().numpy().reshape(shape + (N,))
+        o1, _, _, _ = P.stage(I.copy(), fluid, opac, dt)
+        assert rel_err_I(P.interior(out1), P.interior(o1)) <= TOL_I
+        # the two halves
+        ctx, Iin, Iout, fl = [], [], [], []
+        I4 = I.reshape(shape + (N,)); f4 = fluid.reshape((5,) + shape); op4 = opac.reshape((3,) + shape)
+        for lo in (True, False):
+            nn = list(n); nn[axis] = half
+            xx = list(x0); xx[axis] = x0[axis] + (0 if lo else half * dx[axis])
+            bl = [2, 2, 2]; bh = [2, 2, 2]
+            (bh if lo else bl)[axis] = 0
+            sl = part(None, lo)
+            dop = dev(np.ascontiguousarray(op4[(slice(None),) + tuple(sl)]).reshape(3, -1))
+            ctx.append(B.rad_create(dict(kind=1, M=1.0, a=0.9), dict(n=tuple(nn), ng=ng, x0=tuple(xx), dx=dx, bc_lo=tuple(bl), bc_hi=tuple(bh)), ang,
+                                    (dop[0], dop[1], dop[2]), dict()))
+            Iin.append(dev(np.ascontiguousarray(I4[tuple(sl)]).reshape(-1, N))); Iout.append(torch.zeros_like(Iin[-1]))
+            fl.append(dev(np.ascontiguousarray(f4[(slice(None),) + tuple(sl)]).reshape(5, -1)))
+        try:
+            for _ in range(2):
+                B.rad_exchange_halo(ctx[0], Iin[0], ctx[1], Iin[1], axis)
+                for q in range(2):
+                    B.rad_stage(ctx[q], Iin[q], Iout[q], None, fl[q], 0.0, 1.0, dt)
+                Iin, Iout = Iout, Iin
+            for q, lo in enumerate((True, False)):
+                nn = list(n); nn[axis] = half
+                got = Iin[q].cpu().numpy().reshape((nn[2] + 4, nn[1] + 4, nn[0] + 4, N))[2:-2, 2:-2, 2:-2]
+                sl = [slice(2, -2)] * 3
+                sl[ax_np] = slice(2, 2 + half) if lo else slice(2 + half, 2 + n[axis])
+                if axis == 0:   # a cut across the march direction changes no operation order: same bits
+                    assert np.array_equal(got, big[tuple(sl)]), f"half {q} differs from the undivided block"
+                else:           # a cut in y or z moves the tile edges: a face flux enters the sum of a cell at another position (rounding only)
+                    assert rel_err_I(got, big[tuple(sl)]) <= 1e-13, f"half {q} differs from the undivided block"
+            with pytest.raises(B.RadError):
+                B.rad_exchange_halo(ctx[0], Iin[0], ctx[1], Iin[1], 5)
+        finally:
+            for c in ctx:
+                B.rad_destroy(c)
+    finally:
+        B.rad_destroy(h)
