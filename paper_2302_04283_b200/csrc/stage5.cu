@@ -33,29 +33,35 @@ struct Tile {
     static constexpr int TY = TY_, TZ = TZ_, WPC = WPC_;
     static constexpr bool TAU = TAU_;  // optical-depth-aware flux (Eq.26-29): per-cell velocity records of the tile and its 1-deep halo
     static constexpr int NVH = 2 * TZ + 2 * TY;  // halo cells at distance 1 (no corners)
-    static constexpr int NC = TY * TZ, NH = 4 * TZ + 4 * TY, NR0 = 3 * NC + NH + TY + TZ, NR = NR0 + (TAU ? NC + NVH : 0), NT = NC * WPC * 32;
+    static constexpr int NC = TY * TZ, NH = 4 * TZ + 4 * TY, NR0 = 4 * NC + NH + TY + TZ, NR = NR0 + (TAU ? NC + NVH : 0), NT = NC * WPC * 32;
     static constexpr int NFY = (TY - 1) * TZ, NFZ = TY * (TZ - 1);
 };
 
+// Shared memory: two PAGES (step parity), each holding everything that changes with the step and is dead after the step's CTA
+// barrier -- the tile's own rows of plane s, the halo rows of plane s, the own rows of plane s + 2 (the x stencil's new value), the
+// edge coefficients, the published face fluxes (TAU: the velocity records of the halo cells) -- so that every address of a step is
+// (page base + thread offset) + a loop-invariant offset; then the packed records (4 buffers: read after the barrier too).
 struct Layout5 {
-    int Np, Kp, oRing, oHalo, oE, oFy, oFz, oFx, oU, oRole, oV, oVh, oBar, total;  // offsets in doubles
+    int Np, Kp, pHalo, pAhead, pE, pFy, pFz, pFx, pVh, PG, oPage, oU, oRole, oV, oBar, total;  // offsets in doubles (p*: inside a page)
 };
 template <class T>
 __host__ __device__ inline Layout5 make_layout5(int N) {
     Layout5 L;
     L.Np = (N + 1) & ~1;
     L.Kp = (3 * N + 3) & ~1;  // 3 N coefficients / fluxes + the always-zero slot 3N
-    L.oRing = 0;
-    L.oHalo = L.oRing + 4 * T::NC * L.Np;
-    L.oE = L.oHalo + 2 * T::NH * L.Np;
-    L.oFy = L.oE + 2 * T::NC * L.Kp;
-    L.oFz = L.oFy + 2 * T::NFY * L.Np;
-    L.oFx = L.oFz + 2 * T::NFZ * L.Np;  // the lower z face of cell (0,0), computed by cell (1,1) (load balance)
-    L.oU = L.oFx + 2 * L.Np;
+    L.pHalo = T::NC * L.Np;
+    L.pAhead = L.pHalo + T::NH * L.Np;
+    L.pE = L.pAhead + T::NC * L.Np;
+    L.pFy = L.pE + T::NC * L.Kp;
+    L.pFz = L.pFy + T::NFY * L.Np;
+    L.pFx = L.pFz + T::NFZ * L.Np;  // the lower z face of cell (0,0), computed by cell (1,1) (load balance)
+    L.pVh = L.pFx + L.Np;           // TAU: velocity records (8 doubles) of the halo cells at distance 1
+    L.PG = L.pVh + (T::TAU ? T::NVH * 8 : 0);
+    L.oPage = 0;
+    L.oU = L.oPage + 2 * L.PG;
     L.oRole = L.oU + 4 * T::NC * USTR;
-    L.oV = L.oRole + T::NR * 4;                       // TAU: velocity records (8 doubles) of the own cells, 4 buffers
-    L.oVh = L.oV + (T::TAU ? 4 * T::NC * 8 : 0);      // ... and of the halo cells at distance 1, 2 buffers
-    L.oBar = L.oVh + (T::TAU ? 2 * T::NVH * 8 : 0);
+    L.oV = L.oRole + T::NR * 4;     // TAU: velocity records of the own cells, 4 buffers
+    L.oBar = L.oV + (T::TAU ? 4 * T::NC * 8 : 0);
     L.total = L.oBar + 3;  // two mbarriers, then the bytes of one step's copies
     return L;
 }
@@ -133,8 +139,8 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             if (jj < t.NJ && kk < t.NK) {
                 const long long c0 = ((long long)kk * t.NJ + jj) * t.NI + i_begin;
                 r.stride = N; r.bytes = row_bytes;
-                if (tid < NC) { r.src0 = a.I_in + (c0 + 2) * N; r.dst0 = L.oRing + tid * Np; r.dstride = NC * Np; r.nbufm1 = 3; r.boff = 2; }
-                else { r.src0 = a.I_in + c0 * N; r.dst0 = L.oHalo + (tid - NC) * Np; r.dstride = NH * Np; r.nbufm1 = 1; }
+                r.src0 = a.I_in + c0 * N; r.dstride = L.PG; r.nbufm1 = 1;
+                r.dst0 = L.oPage + (tid < NC ? tid * Np : L.pHalo + (tid - NC) * Np);
             }
         } else if (TAU && tid >= T::NR0) {
             // velocity records (8 doubles: u^alphahat, f/2 of the three upper faces, pad) of plane u: the own cells (4 buffers) and
@@ -146,24 +152,27 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 const int h = q - NC;
                 if (h < 2 * TZ) { kk = k0 + (h >> 1); jj = (h & 1) ? j0 + TY : j0 - 1; }
                 else { jj = j0 + ((h - 2 * TZ) >> 1); kk = ((h - 2 * TZ) & 1) ? k0 + TZ : k0 - 1; }
-                r.dst0 = L.oVh + h * 8; r.dstride = T::NVH * 8; r.nbufm1 = 1;
+                r.dst0 = L.oPage + L.pVh + h * 8; r.dstride = L.PG; r.nbufm1 = 1;
             }
             if (jj < t.NJ && kk < t.NK) {
                 r.src0 = a.vel8 + (((long long)kk * t.NJ + jj) * t.NI + i_begin) * 8; r.stride = 8; r.bytes = 64;
             }
         } else {
             const int q = tid - NC - NH;
-            int kind, ccs;  // 0 edge coefficients, 1 cell record, 2 lower y face, 3 lower z face
+            int kind, ccs;  // 0 edge coefficients, 1 cell record, 2 lower y face, 3 lower z face, 4 own row of plane u + 2
             if (q < NC) { kind = 0; ccs = q; }
             else if (q < 2 * NC) { kind = 1; ccs = q - NC; }
             else if (q < 2 * NC + TZ) { kind = 2; ccs = (q - 2 * NC) * TY; }
-            else { kind = 3; ccs = q - 2 * NC - TZ; }
+            else if (q < 2 * NC + TZ + TY) { kind = 3; ccs = q - 2 * NC - TZ; }
+            else { kind = 4; ccs = q - 2 * NC - TZ - TY; }
             const int jj = j0 + ccs % TY, kk = k0 + ccs / TY;
             if (jj < t.n[1] + ng && kk < kze + ng) {
                 const long long c0 = ((long long)kk * t.NJ + jj) * t.NI + i_begin;
-                if (kind == 0) {
+                if (kind == 4) {
+                    r.src0 = a.I_in + (c0 + 2) * N; r.stride = N; r.dst0 = L.oPage + L.pAhead + ccs * Np; r.dstride = L.PG; r.nbufm1 = 1; r.bytes = row_bytes;
+                } else if (kind == 0) {
                     const long long ci = ((long long)(kk - ng) * t.n[1] + (jj - ng)) * t.n[0] + (i_begin - ng);
-                    r.src0 = t.ke + ci * 3 * N; r.stride = 3 * N; r.dst0 = L.oE + ccs * Kp; r.dstride = NC * Kp; r.nbufm1 = 1; r.bytes = 3 * row_bytes;
+                    r.src0 = t.ke + ci * 3 * N; r.stride = 3 * N; r.dst0 = L.oPage + L.pE + ccs * Kp; r.dstride = L.PG; r.nbufm1 = 1; r.bytes = 3 * row_bytes;
                 } else {
                     r.stride = RECN; r.dstride = NC * USTR; r.nbufm1 = 3;
                     if (kind == 1) { r.src0 = t.rec + c0 * RECN; r.dst0 = L.oU + ccs * USTR; r.bytes = RECN * 8; }
@@ -175,8 +184,8 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         roles[tid] = r;
     }
     if (wc == 0 && lane < 2) {  // the always-zero flux slot of both coefficient buffers
-        sm[L.oE + (lane * NC + cs) * Kp + 3 * N] = 0.0;
-        if (3 * N + 1 < Kp) sm[L.oE + (lane * NC + cs) * Kp + 3 * N + 1] = 0.0;
+        sm[L.oPage + lane * L.PG + L.pE + cs * Kp + 3 * N] = 0.0;
+        if (3 * N + 1 < Kp) sm[L.oPage + lane * L.PG + L.pE + cs * Kp + 3 * N + 1] = 0.0;
     }
     if (tid == 0) {
         mbar_init(bar0, 1); mbar_init(bar0 + 8u, 1);
@@ -184,15 +193,15 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     }
     __syncthreads();
     if (tid == 0) {
-        uint32_t own_bytes = 0, step_bytes = 0;
-        for (int r = 0; r < NR; r++) { step_bytes += (uint32_t)roles[r].bytes; if (r < NC) own_bytes += (uint32_t)roles[r].bytes; }
-        mbar_expect_tx(bar0, step_bytes + own_bytes);
-        if (nsteps > 1) mbar_expect_tx(bar0 + 8u, step_bytes + own_bytes);
+        uint32_t step_bytes = 0;
+        for (int r = 0; r < NR; r++) step_bytes += (uint32_t)roles[r].bytes;
+        mbar_expect_tx(bar0, step_bytes);
+        if (nsteps > 1) mbar_expect_tx(bar0 + 8u, step_bytes);
         *reinterpret_cast<uint32_t *>(sm + L.oBar + 2) = step_bytes;
     }
     __syncthreads();
-    // everything step u needs that is not yet resident, signalled on full[u & 1]: own rows of plane u+2 (ring slot
-    // (u+2) & 3), halo rows of plane u, coefficients and records of the cells of plane u
+    // everything step u needs, signalled on full[u & 1]: own and halo rows of plane u, own rows of plane u + 2, coefficients and
+    // records of the cells of plane u
     const int myrole = (tid >> 5) + (T::NT / 32) * lane;  // the copies of a step are spread over all warps (a warp issues its lanes' copies one by one)
     auto issue = [&](int u) {
         const Role r = roles[myrole];
@@ -204,7 +213,6 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     if (myrole < NR) {
         issue(0);
         if (nsteps > 1) issue(1);
-        if (myrole < NC) { issue(-2); if (nsteps > 1) issue(-1); }  // own rows of planes 0 and 1
     }
 
     // ---- the thread's angles: n = lane + 32 wc + 32 WPC it.  Only the last one can fall past N; such a slot is idle:
@@ -251,9 +259,9 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         }
     }
     const int barid = 1 + cs;
-    // per-warp byte offsets of the eight stencil neighbours inside a ring plane / a halo buffer (bit q of nbHalo: halo)
+    // loop-invariant byte offsets inside a page (warp-uniform): the eight stencil neighbours' rows, the cell's own row, its row two
+    // planes ahead, its coefficients, where it publishes and takes face fluxes
     uint32_t nbOff[8];
-    unsigned nbHalo = 0;
 #pragma unroll
     for (int q = 0; q < 8; q++) {
         const int dq = (q & 3) < 2 ? (q & 3) - 2 : (q & 3) - 1;  // -2, -1, +1, +2
@@ -261,18 +269,18 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         if (q < 4) {
             const int yy = wy + dq;
             if (yy >= 0 && yy < TY) row = wz * TY + yy;
-            else { row = wz * 4 + (yy < 0 ? yy + 2 : yy - TY + 2); nbHalo |= 1u << q; }
+            else row = NC + wz * 4 + (yy < 0 ? yy + 2 : yy - TY + 2);
         } else {
             const int zz = wz + dq;
             if (zz >= 0 && zz < TZ) row = zz * TY + wy;
-            else { row = 4 * TZ + wy * 4 + (zz < 0 ? zz + 2 : zz - TZ + 2); nbHalo |= 1u << q; }
+            else row = NC + 4 * TZ + wy * 4 + (zz < 0 ? zz + 2 : zz - TZ + 2);
         }
-        nbOff[q] = (uint32_t)(row * Np) * 8u;
+        nbOff[q] = (uint32_t)(row * Np) * 8u;  // (the halo rows follow the NC own rows)
     }
-    const uint32_t ownOff = (uint32_t)(cs * Np) * 8u;
-    const uint32_t aRing = smb + 8u * L.oRing, aHalo = smb + 8u * L.oHalo, planeB = (uint32_t)(NC * Np) * 8u;
-    const uint32_t aE0 = smb + 8u * (uint32_t)(L.oE + cs * Kp), aU0 = smb + 8u * (uint32_t)(L.oU + cs * USTR);
-    const uint32_t aFy = smb + 8u * L.oFy, aFz = smb + 8u * L.oFz, aFx = smb + 8u * L.oFx;
+    const uint32_t ownOff = (uint32_t)(cs * Np) * 8u, aheadOff = 8u * (uint32_t)(L.pAhead + cs * Np), eOff = 8u * (uint32_t)(L.pE + cs * Kp);
+    const uint32_t pubY = 8u * (uint32_t)(L.pFy + (wz * (TY - 1) + wy) * Np), pubZ = 8u * (uint32_t)(L.pFz + (wz * TY + wy) * Np), fxOff = 8u * (uint32_t)L.pFx;
+    const uint32_t aPage = smb + 8u * L.oPage, pageB = 8u * (uint32_t)L.PG, N8p = 8u * (uint32_t)Np;
+    const uint32_t aU0 = smb + 8u * (uint32_t)(L.oU + cs * USTR);
     // load balance: cell (0,0) would compute five faces (x, upper y and z, lower y and z), cell (1,1) three; cell (1,1)
     // takes over the lower z face of cell (0,0)
     const bool helped = TY >= 2 && TZ >= 2 && j0 + 1 < t.n[1] + ng && k0 + 1 < kze + ng;
@@ -287,24 +295,25 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
         mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
         if (TAU && s + 1 < nsteps) mbar_wait(bar0 + 8u * (b ^ 1), ((s + 1) >> 1) & 1);  // the velocity records of plane s+1 (x face above)
         if (tid == 0 && s + 2 < nsteps) mbar_expect_tx(bar0 + 8u * b, *reinterpret_cast<volatile uint32_t *>(sm + L.oBar + 2));  // re-armed for step s+2 (copies start after the barrier below)
-        const uint32_t ringS = aRing + (uint32_t)(s & 3) * planeB;          // own rows of plane s
-        const uint32_t haloS = aHalo + (uint32_t)b * ((uint32_t)(NH * Np) * 8u);  // halo rows of plane s
-        const uint32_t aEb = aE0 + (uint32_t)b * ((uint32_t)(NC * Kp) * 8u);
+        const uint32_t pg = aPage + (uint32_t)b * pageB;   // this step's page
+        const uint32_t aEb = pg + eOff;
+        uint32_t tb[NITER];                                // page base + the thread's angle offset
+#pragma unroll
+        for (int it = 0; it < NITER; it++) tb[it] = pg + OFF8(it);
         const uint32_t aUb = aU0 + (uint32_t)(s & 3) * (NC * USTR * 8u);
         double d[NITER], xp2[NITER];
 #pragma unroll
         for (int it = 0; it < NITER; it++) asm volatile("" : "+r"(rx[it]), "+r"(ry[it]), "+r"(rz[it]));  // unpack per step: the unpacked offsets would be spilled
 
         if (active) {
-            const uint32_t ownrow = ringS + ownOff;
-            const uint32_t newrow = aRing + (uint32_t)((s + 2) & 3) * planeB + ownOff;
+            const uint32_t ownrow = pg + ownOff;
 #pragma unroll
-            for (int it = 0; it < NITER; it++) xp2[it] = lds(newrow + OFF8(it));
+            for (int it = 0; it < NITER; it++) xp2[it] = lds(tb[it] + aheadOff);
             // ---- angular fluxes (Eq.25, donor cell in angle): owners turn q_e into the edge flux in place
 #pragma unroll
             for (int it = 0; it < NITER; it++) {  // loads first, stores last: the volatile accesses keep their order
                 const unsigned pj[3] = {rx[it] & 0xffffu, rx[it] >> 16, ry[it] & 0xffffu};
-                const uint32_t qa = aEb + OFF8(it);
+                const uint32_t qa = tb[it] + eOff;
                 double q[3], G[3];
 #pragma unroll
                 for (int jj = 0; jj < 3; jj++) q[jj] = lds(qa + (uint32_t)jj * N8);  // unused slots have q = 0
@@ -329,7 +338,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             }
             // ---- spatial fluxes (Eq.24).  x: the upper face; the lower one is carried
             double G0[NITER];  // TAU: G of this cell per angle
-            const uint32_t vOwn = smb + 8u * (uint32_t)(L.oV + ((s & 3) * NC + cs) * 8), vHal = smb + 8u * (uint32_t)(L.oVh + b * T::NVH * 8);
+            const uint32_t vOwn = smb + 8u * (uint32_t)(L.oV + ((s & 3) * NC + cs) * 8), vHal = pg + 8u * (uint32_t)L.pVh;
             double2 own46 = make_double2(0.0, 0.0);  // f/2 of the upper x and y faces
             double own6 = 0.0;                       // ... and of the upper z face
             if (TAU) {
@@ -357,10 +366,9 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
 #pragma unroll
             for (int ax = 1; ax <= 2; ax++) {
                 const int q0 = ax == 1 ? 0 : 4;
-                const uint32_t rm2 = ((nbHalo >> q0) & 1u ? haloS : ringS) + nbOff[q0], rm1 = ((nbHalo >> (q0 + 1)) & 1u ? haloS : ringS) + nbOff[q0 + 1],
-                               rp1 = ((nbHalo >> (q0 + 2)) & 1u ? haloS : ringS) + nbOff[q0 + 2], rp2 = ((nbHalo >> (q0 + 3)) & 1u ? haloS : ringS) + nbOff[q0 + 3];
+                const uint32_t rm2 = nbOff[q0], rm1 = nbOff[q0 + 1], rp1 = nbOff[q0 + 2], rp2 = nbOff[q0 + 3];  // (offsets: added to tb[it])
                 const bool low_edge = (ax == 1 ? wy : wz) == 0, publish = ax == 1 ? wy < TY - 1 : wz < TZ - 1;
-                const uint32_t pub = ax == 1 ? aFy + (uint32_t)((b * T::NFY + wz * (TY - 1) + wy) * Np) * 8u : aFz + (uint32_t)((b * T::NFZ + wz * TY + wy) * Np) * 8u;
+                const uint32_t pub = ax == 1 ? pubY : pubZ;
                 const FaceRec fh = lds_face(aUb + 64 * ax);
                 double2 q01 = make_double2(1.0, 0.0), q23 = make_double2(0.0, 0.0);  // TAU: velocity of the cell above along this axis
                 if (TAU) {
@@ -376,8 +384,8 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
                     gu[it] = face_geom(fh, n1[it], n2[it], n3[it]);
-                    p1[it] = lds(rp1 + OFF8(it));
-                    far[it] = PLM ? lds((gu[it].neg ? rp2 : rm1) + OFF8(it)) : 0.0;
+                    p1[it] = lds(tb[it] + rp1);
+                    far[it] = PLM ? lds(tb[it] + (gu[it].neg ? rp2 : rm1)) : 0.0;
                 }
 #pragma unroll
                 for (int it = 0; it < NITER; it++) {
@@ -388,7 +396,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
                 if (publish) {
 #pragma unroll
                     for (int it = 0; it < NITER; it++)
-                        if (it < NITER - 1 || last_valid) sts(pub + OFF8(it), F[it]);
+                        if (it < NITER - 1 || last_valid) sts(tb[it] + pub, F[it]);
                 }
                 if (low_edge && !(ax == 2 && is_helpee)) {
                     const FaceRec fl = lds_face(aUb + (ax == 1 ? 8 * 36 : 8 * 44));
@@ -401,8 +409,8 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
 #pragma unroll
                     for (int it = 0; it < NITER; it++) {  // the lower face: between the cell below (m1) and this one
                         const FaceGeom gl = face_geom(fl, n1[it], n2[it], n3[it]);
-                        const double m1 = lds(rm1 + OFF8(it));
-                        const double farl = PLM ? (gl.neg ? p1[it] : lds_unless(rm2 + OFF8(it), gl.neg, 0.0)) : 0.0;
+                        const double m1 = lds(tb[it] + rm1);
+                        const double farl = PLM ? (gl.neg ? p1[it] : lds_unless(tb[it] + rm2, gl.neg, 0.0)) : 0.0;
                         d[it] -= face_value<PLM, TAU>(gl, gl.neg ? x0[it] : m1, farl, x0[it] - m1,
                                                       TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0, TAU ? G0[it] : 0.0, fhl);
                     }
@@ -410,27 +418,27 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             }
         }
         if (is_helper) {  // lower z face of cell (0,0): rows z-2, z-1 of column 0 are halo rows, z and z+1 ring rows
-            const uint32_t r_m2 = haloS + (uint32_t)((4 * TZ) * Np) * 8u, r_m1 = haloS + (uint32_t)((4 * TZ + 1) * Np) * 8u, r_0 = ringS,
-                           r_p1 = ringS + (uint32_t)(TY * Np) * 8u;
+            // (page offsets) rows z-2, z-1 of column 0: the first two z halo rows; z: own row 0; z+1: own row TY
+            const uint32_t r_m2 = (uint32_t)((NC + 4 * TZ) * Np) * 8u, r_m1 = (uint32_t)((NC + 4 * TZ + 1) * Np) * 8u, r_0 = 0u, r_p1 = (uint32_t)(TY * Np) * 8u;
             const FaceRec fl = lds_face(aUb - (uint32_t)cs * (USTR * 8u) + 8 * 44);
             double2 l01 = make_double2(1.0, 0.0), l23 = make_double2(0.0, 0.0), r01 = l01, r23 = l23;
             double fhl = 0.0;
             if (TAU) {  // cell (0,0) and the halo cell below it in z
-                const uint32_t vl = smb + 8u * (uint32_t)(L.oVh + (b * T::NVH + 2 * TZ) * 8), vr = smb + 8u * (uint32_t)(L.oV + ((s & 3) * NC) * 8);
+                const uint32_t vl = pg + 8u * (uint32_t)(L.pVh + 2 * TZ * 8), vr = smb + 8u * (uint32_t)(L.oV + ((s & 3) * NC) * 8);
                 l01 = lds2(vl); l23 = lds2(vl + 16); fhl = lds(vl + 48); r01 = lds2(vr); r23 = lds2(vr + 16);
             }
             double q0[NITER];
 #pragma unroll
             for (int it = 0; it < NITER; it++) {
                 const FaceGeom gl = face_geom(fl, n1[it], n2[it], n3[it]);
-                const double q1 = lds(r_m1 + OFF8(it)), q2 = lds(r_0 + OFF8(it));
-                const double farl = PLM ? lds((gl.neg ? r_p1 : r_m2) + OFF8(it)) : 0.0;
+                const double q1 = lds(tb[it] + r_m1), q2 = lds(tb[it] + r_0);
+                const double farl = PLM ? lds(tb[it] + (gl.neg ? r_p1 : r_m2)) : 0.0;
                 q0[it] = face_value<PLM, TAU>(gl, gl.neg ? q2 : q1, farl, q2 - q1, TAU ? tau_G(l01.x, l01.y, l23.x, l23.y, n1[it], n2[it], n3[it]) : 0.0,
                                               TAU ? tau_G(r01.x, r01.y, r23.x, r23.y, n1[it], n2[it], n3[it]) : 0.0, fhl);
             }
 #pragma unroll
             for (int it = 0; it < NITER; it++)
-                if (it < NITER - 1 || last_valid) sts(aFx + (uint32_t)(b * Np) * 8u + OFF8(it), q0[it]);
+                if (it < NITER - 1 || last_valid) sts(tb[it] + fxOff, q0[it]);
         }
         __syncthreads();  // the fluxes of this plane are published; nobody reads the rows, halo and coefficients of plane s any more
         if (s + 2 < nsteps && myrole < NR) issue(s + 2);
@@ -438,18 +446,16 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
 
         if (is_helpee) {
 #pragma unroll
-            for (int it = 0; it < NITER; it++) d[it] -= lds(aFx + (uint32_t)(b * Np) * 8u + OFF8(it));
+            for (int it = 0; it < NITER; it++) d[it] -= lds(tb[it] + fxOff);
         }
 
         if (wy > 0) {
-            const uint32_t src = aFy + (uint32_t)((b * T::NFY + wz * (TY - 1) + wy - 1) * Np) * 8u;
 #pragma unroll
-            for (int it = 0; it < NITER; it++) d[it] -= lds(src + OFF8(it));
+            for (int it = 0; it < NITER; it++) d[it] -= lds(tb[it] + (pubY - N8p));  // what the cell below in y published
         }
         if (wz > 0) {
-            const uint32_t src = aFz + (uint32_t)((b * T::NFZ + (wz - 1) * TY + wy) * Np) * 8u;
 #pragma unroll
-            for (int it = 0; it < NITER; it++) d[it] -= lds(src + OFF8(it));
+            for (int it = 0; it < NITER; it++) d[it] -= lds(tb[it] + (pubZ - (uint32_t)TY * N8p));  // ... in z
         }
         // ---- flux-divergence update of C = n^0 n_0 I (Eq.22, stage form R8), cons -> prim
         const double2 c01 = lds2(aUb + 8 * 24);
