@@ -212,7 +212,9 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
             ck.uh0 = sqrt_ge1(1.0 + (ck.uh1 * ck.uh1 + ck.uh2 * ck.uh2 + ck.uh3 * ck.uh3));
         }
         // |n_0| = |E_0 + E_a n^a| >= |E_0| - |E|: only cells with |E_0| - |E| < n_0^crit can have a masked angle (1e-9: rounding of the bound)
-        const bool mymask = n0crit > 0.0 && !excised && fabs(ck.E0) - sqrt(ck.E1 * ck.E1 + ck.E2 * ck.E2 + ck.E3 * ck.E3) < n0crit * (1.0 + 1e-9);
+        // (compared in squares: |E_0| - n_0^crit (1 + 1e-9) < |E|  <=>  that difference is negative or its square is below |E|^2)
+        const double mgap = fabs(ck.E0) - n0crit * (1.0 + 1e-9);
+        const bool mymask = n0crit > 0.0 && !excised && (mgap < 0.0 || mgap * mgap < ck.E1 * ck.E1 + ck.E2 * ck.E2 + ck.E3 * ck.E3);
         const bool anymask = __any_sync(0xffffffffu, mymask);
         mbar_wait(bar0 + 16u * sl, (uint32_t)par);
         const uint32_t aI = smem_u32(slots + (sl * kCG + mycell) * Np) + 8u * kk;  // this lane's item of pass j: + 64 j
@@ -326,8 +328,11 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
             double *out = a.I + (c0 + mycell) * N + kk;
             const int myn = (mycell < cnt && !excised) ? (N - kk + kCA - 1) / kCA : 0;  // this lane's items
             if (__all_sync(0xffffffffu, coupled || myn == 0)) {  // the usual case: every cell of the group has a root
+                const int nall = N / kCA;  // items every lane has; lanes kk < N % 8 have one more
 #pragma unroll 4
-                for (int j = 0; j < myn; j++) out[kCA * j] = fma(src, lds(aB + 64u * j), lds(aI + 64u * j));
+                for (int j = 0; j < nall; j++)
+                    if (myn) out[kCA * j] = fma(src, lds(aB + 64u * j), lds(aI + 64u * j));
+                if (myn > nall) out[kCA * nall] = fma(src, lds(aB + 64u * nall), lds(aI + 64u * nall));
             } else {
                 for (int j = 0; j < myn; j++) {
                     const double b_ = lds(aB + 64u * j);
