@@ -216,7 +216,7 @@ long long rad_launch_count(const rad_ctx *);
 rad_status rad_exchange_halo(rad_ctx *lo, double *I_lo, rad_ctx *hi, double *I_hi, int axis, void *cuda_stream);
 
 /* Names of the kernels one rad_stage launches on this context after the ghost fill, "flux-divergence kernel;coupling kernel", each
- * written as ncu prints the instance without casts and blanks, e.g. "k_stage5<3,2,4,2,1,1,0>;k_couple_stream<0>".  bench.py keys
+ * written as ncu prints the instance without casts and blanks, e.g. "k_stage5<3,2,4,2,1,1,0>;k_couple_stream<0,21>".  bench.py keys
  * the committed ncu summaries (the .csv files under profiles/) with them and prints no profile figure for a kernel whose name it does not find.
  * buf: HOST, nbytes >= 128.  RAD_EINVAL if the buffer is too small. */
 rad_status rad_stage_kernels(rad_ctx *, char *buf /* HOST */, size_t nbytes);

@@ -106,10 +106,11 @@ struct CoupleArgs {
     int kz0, kz1;  // interior planes kz0 <= k < kz1 (0-based, without ghosts); kz1 <= kz0 = the whole block
 };
 
-template <bool VEST>
+// NPASS: the number of passes ceil(N / 8) as a compile-time constant (the sweeps are then straight-line code), or 0 = taken from N
+template <bool VEST, int NPASS>
 __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, const Params p, const CoupleArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int N = t.N, npass = (N + kCA - 1) / kCA, Np = couple_row_stride(N);
+    const int N = t.N, npass = NPASS ? NPASS : (N + kCA - 1) / kCA, Np = couple_row_stride(N);
     double *sm = reinterpret_cast<double *>(smem_raw);
     double2 *sA01 = reinterpret_cast<double2 *>(sm), *sA23 = sA01 + npass * kCA;  // {dOmega, n^1}[npass * 8], {n^2, n^3}[npass * 8]
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
@@ -274,7 +275,7 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
         double S[12];
 #pragma unroll
         for (int q = 0; q < 12; q++) S[q] = 0.0;
-#pragma unroll 3
+#pragma unroll(NPASS ? NPASS : 3)
         for (int j = 0; j < npass; j++) {
             const double2 a01 = lds2(aA01 + 128u * j), a23 = lds2(aA23 + 128u * j);
             const double4 an = make_double4(a01.x, a01.y, a23.x, a23.y);  // zeros past N: such an item adds zeros
@@ -328,11 +329,11 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
             double *out = a.I + (c0 + mycell) * N + kk;
             const int myn = (mycell < cnt && !excised) ? (N - kk + kCA - 1) / kCA : 0;  // this lane's items
             if (__all_sync(0xffffffffu, coupled || myn == 0)) {  // the usual case: every cell of the group has a root
-                const int nall = N / kCA;  // items every lane has; lanes kk < N % 8 have one more
-#pragma unroll 4
+                const int nall = NPASS ? (NPASS - 1) : N / kCA;  // items every lane has; the last pass may be partial
+#pragma unroll(NPASS ? NPASS : 4)
                 for (int j = 0; j < nall; j++)
                     if (myn) out[kCA * j] = fma(src, lds(aB + 64u * j), lds(aI + 64u * j));
-                if (myn > nall) out[kCA * nall] = fma(src, lds(aB + 64u * nall), lds(aI + 64u * nall));
+                for (int j = nall; j < myn; j++) out[kCA * j] = fma(src, lds(aB + 64u * j), lds(aI + 64u * j));
             } else {
                 for (int j = 0; j < myn; j++) {
                     const double b_ = lds(aB + 64u * j);
@@ -574,13 +575,17 @@ int launch_couple_stream(const DeviceTables &t, const Params &p, double *I, cons
     CoupleArgs a{I, fluid, aP, aE, aS, dt, T_out, dT0, noroot, kz0, kz1};
     const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(4, (size_t)t.smem_optin / (smem + 1024)));
     const int grid = t.sms * per_sm;
-    if (p.vel_estimate && p.couple) {
-        if (cudaFuncSetAttribute(k_couple_stream<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
-        k_couple_stream<true><<<grid, warps * 32, smem, s>>>(t, p, a);
-    } else {
-        if (cudaFuncSetAttribute(k_couple_stream<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
-        k_couple_stream<false><<<grid, warps * 32, smem, s>>>(t, p, a);
-    }
+    const int npass = (t.N + kCA - 1) / kCA;
+#define RAD_COUPLE_LAUNCH(VEST, NP)                                                                                                                  \
+    do {                                                                                                                                             \
+        if (cudaFuncSetAttribute(k_couple_stream<VEST, NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;       \
+        k_couple_stream<VEST, NP><<<grid, warps * 32, smem, s>>>(t, p, a);                                                                            \
+    } while (0)
+    if (p.vel_estimate && p.couple) RAD_COUPLE_LAUNCH(true, 0);
+    else if (npass == 21) RAD_COUPLE_LAUNCH(false, 21);  // N = 161..168 (geodesic level 4)
+    else if (npass == 12) RAD_COUPLE_LAUNCH(false, 12);  // N = 89..96 (geodesic level 3)
+    else RAD_COUPLE_LAUNCH(false, 0);
+#undef RAD_COUPLE_LAUNCH
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
