@@ -289,7 +289,7 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
     double *outp = a.I_out + c_first * N;
     const double *I0p = a.I0 ? a.I0 + c_first * N : nullptr;
 
-#pragma unroll 1
+#pragma unroll 2  // (with the pages, a step's parity becomes a compile-time constant: C3 5.07 -> 4.80 ms; unrolling by 4: 4.88)
     for (int s = 0; s < nsteps; s++) {
         const int b = s & 1;
         mbar_wait(bar0 + 8u * b, (s >> 1) & 1);
