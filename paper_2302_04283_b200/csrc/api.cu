@@ -174,7 +174,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
     t.mirror = nullptr;
     if (ok && any_wall) ok = upload(c, mirror, &t.mirror);
-    // fused stage kernel: balanced edge ownership, per-angle records, 1/dOmega
+    // tile kernel (stage5.cu): balanced and coloured edge ownership, per-angle records, 1/dOmega
     t.fused_ok = 0; t.ang_rec = nullptr; t.winv = nullptr; t.own_edge = nullptr; t.ke = nullptr; t.rec = nullptr;
     const bool tile_cfg = g->ng == 2 && p->recon_space <= 1 && p->recon_angle == 0;  // what the tile kernel (stage5.cu) implements
     if (ok && h.N <= 256 && tile_cfg) {

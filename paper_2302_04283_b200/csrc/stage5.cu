@@ -10,10 +10,12 @@
 //   * every face flux is computed ONCE: a cell computes the flux through its upper y and z faces and publishes it in
 //     shared memory; the neighbour above takes it as its lower-face flux after the CTA barrier of the step (only the
 //     cells on the low edges of the tile compute their lower faces themselves).
-//   * shared memory is filled by bulk asynchronous copies (TMA, 1-D) two steps ahead, completion on two mbarriers: the
-//     tile's own rows (ring of 4 planes), the 2-deep halo rows of the current plane (2 buffers), the stored angular-edge
-//     coefficients of each cell (2 buffers; the owner of an edge overwrites the coefficient with the edge flux, the
-//     partner angle pulls it from there), and a packed per-cell geometry record (4 buffers).  One __syncthreads per step.
+//   * shared memory is filled by bulk asynchronous copies (TMA, 1-D) two steps ahead, completion on two mbarriers, into one
+//     of two PAGES (step parity): the tile's own rows and the 2-deep halo rows of the current plane, the own rows two planes
+//     ahead (the x stencil's new value), the stored angular-edge coefficients of each cell (the owner of an edge overwrites
+//     the coefficient with the edge flux, the partner angle pulls it from there) and the published face fluxes; the packed
+//     per-cell geometry records have 4 buffers of their own.  Every address of a step is page base + a loop-invariant offset,
+//     and the step loop is unrolled by two, so the page is a compile-time choice.  One __syncthreads per step.
 //   * TAU (template): the optical-depth-aware spatial flux of Eq.26-29 -- a per-cell table (k_tau_table) of u^alphahat and f/2
 //     of the upper faces comes in with the other copies for the tile's cells and the halo cells at distance 1.
 #include <cstdio>
