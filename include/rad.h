@@ -206,6 +206,16 @@ long long rad_ncells_total(const rad_ctx *);
 /* kernels launched by this context so far (bench.py's gpu_launches) */
 long long rad_launch_count(const rad_ctx *);
 
+/* Host-only helper (needs no device): the angle grid's unique edges and the ownership tables the tile kernel works with (edges.cpp).
+ * Every unique edge e = (edge_lo[e], edge_hi[e]) is owned by one of its two angles, at most three per angle, in a slot 0..2
+ * (own_edge[n][slot] = e or -1, own_partner[n][slot] = the angle at the other end); the slots are a colouring under which the edges an
+ * angle RECEIVES have different slots too: pull_pos[n][k] = k * nang + owner of the edge angle n receives from slot k, or -1.
+ * nang, nedge: HOST out.  The arrays are HOST, int, optional (NULL = not wanted), each with room for `capacity` entries: edge_lo / edge_hi
+ * need nedge, the others 3 * nang; with all five NULL only the sizes are returned.  RAD_EUNSUPPORTED if the grid has an angle with
+ * more than six edges. */
+rad_status rad_edge_ownership(const rad_angles *, int *nang, int *nedge, int *edge_lo, int *edge_hi, int *own_edge, int *own_partner, int *pull_pos,
+                              size_t capacity);
+
 /* Halo exchange between two blocks on the same device that touch along `axis` (0 x, 1 y, 2 z), block `hi` above block `lo`: the
  * communication task of a stage for a domain cut into blocks, one context per block.  The upper ghost layers of I_lo
  * receive the first ng interior layers of I_hi and the lower ghost layers of I_hi the last ng interior layers of I_lo, over the

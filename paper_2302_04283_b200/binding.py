@@ -20,7 +20,7 @@ NCELL, NFACE, MAXNBR = 52, 8, 6
  TAB_STAGE_FACE_SIGN) = range(20)
 
 EXPORTS = ["rad_create", "rad_stage", "rad_stage_host", "rad_fill_ghosts", "rad_transport", "rad_couple", "rad_moments",
-           "rad_get_table", "rad_exchange_halo", "rad_stage_kernels", "rad_probe_fp64", "rad_probe_fp64_pipes", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
+           "rad_get_table", "rad_edge_ownership", "rad_exchange_halo", "rad_stage_kernels", "rad_probe_fp64", "rad_probe_fp64_pipes", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
 
 
 class RadError(RuntimeError):
@@ -76,6 +76,7 @@ def lib():
         L.rad_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
         L.rad_probe_fp64.argtypes = [vp, C.POINTER(C.c_double)]
         L.rad_probe_fp64_pipes.argtypes = [vp, C.POINTER(C.c_double)]
+        L.rad_edge_ownership.argtypes = [C.POINTER(_Angles), C.POINTER(C.c_int), C.POINTER(C.c_int), vp, vp, vp, vp, vp, C.c_size_t]
         L.rad_exchange_halo.argtypes = [vp, vp, vp, vp, C.c_int, vp]
         L.rad_stage_kernels.argtypes = [vp, C.c_char_p, C.c_size_t]
         L.rad_ncells_total.argtypes = [vp]; L.rad_ncells_total.restype = C.c_longlong
@@ -174,6 +175,25 @@ def rad_stage_host(ctx, I_in, I_out, fluid, opac, gam0, gam1, beta_dt, T_out=Non
 
 def rad_fill_ghosts(ctx, I, stream=None):
     _check(ctx, lib().rad_fill_ghosts(ctx, _dp(I), _stream(stream)))
+
+
+def rad_edge_ownership(angles):
+    """host only (no device needed): dict(N, E, edge_lo, edge_hi, own_edge[N][3], own_partner[N][3], pull_pos[N][3]) of an angle grid
+    given as ("latlon", nzeta, npsi) or ("geodesic", nlev)"""
+    a = _Angles(0, int(angles[1]), int(angles[2]), 0) if angles[0] == "latlon" else _Angles(1, 0, 0, int(angles[1]))
+    n, e = C.c_int(0), C.c_int(0)
+    L = lib()
+    st = L.rad_edge_ownership(C.byref(a), C.byref(n), C.byref(e), None, None, None, None, None, 0)
+    if st != 0:
+        raise RadError(st, L.rad_last_error(None).decode())
+    N, E = n.value, e.value
+    cap = max(E, 3 * N)
+    arr = [np.full(cap, -9, np.int32) for _ in range(5)]
+    st = L.rad_edge_ownership(C.byref(a), C.byref(n), C.byref(e), *[C.c_void_p(x.ctypes.data) for x in arr], cap)
+    if st != 0:
+        raise RadError(st, L.rad_last_error(None).decode())
+    return dict(N=N, E=E, edge_lo=arr[0][:E].copy(), edge_hi=arr[1][:E].copy(), own_edge=arr[2][:3 * N].reshape(N, 3).copy(),
+                own_partner=arr[3][:3 * N].reshape(N, 3).copy(), pull_pos=arr[4][:3 * N].reshape(N, 3).copy())
 
 
 def rad_exchange_halo(ctx_lo, I_lo, ctx_hi, I_hi, axis, stream=None):

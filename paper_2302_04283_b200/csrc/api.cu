@@ -287,6 +287,29 @@ rad_status rad_fill_ghosts(rad_ctx *c, double *I, void *stream) {
     return RAD_OK;
 }
 
+rad_status rad_edge_ownership(const rad_angles *a, int *nang, int *nedge, int *edge_lo, int *edge_hi, int *own_edge, int *own_partner, int *pull_pos,
+                              size_t capacity) {
+    if (!a || !nang || !nedge) return fail(nullptr, RAD_EINVAL, "rad_edge_ownership: NULL argument");
+    rad::AngleTables h;
+    rad::EdgeOwnership o;
+    std::string err;
+    const bool ok = (a->kind == 0) ? rad::build_latlon(a->nzeta, a->npsi, h, err)
+                  : (a->kind == 1) ? rad::build_geodesic(a->nlev, h, err)
+                  : (a->kind == 2) ? rad::build_explicit(a->nang, a->nhat, a->domega, a->nnbr, a->nbr, a->edge_len, a->edge_mid, a->edge_nrm, h, err)
+                                   : (err = "bad angle grid kind", false);
+    if (!ok) return fail(nullptr, RAD_EINVAL, "rad_edge_ownership: " + err);
+    *nang = h.N; *nedge = h.E;
+    if (!rad::build_edge_ownership(h, o, err)) return fail(nullptr, RAD_EUNSUPPORTED, "rad_edge_ownership: " + err);
+    if (!edge_lo && !edge_hi && !own_edge && !own_partner && !pull_pos) return RAD_OK;  // sizes only
+    if ((size_t)h.E > capacity || (size_t)3 * h.N > capacity) return fail(nullptr, RAD_EINVAL, "rad_edge_ownership: capacity too small");
+    if (edge_lo) memcpy(edge_lo, h.edge_lo.data(), sizeof(int) * h.E);
+    if (edge_hi) memcpy(edge_hi, h.edge_hi.data(), sizeof(int) * h.E);
+    if (own_edge) memcpy(own_edge, o.own_edge.data(), sizeof(int) * 3 * h.N);
+    if (own_partner) memcpy(own_partner, o.own_partner.data(), sizeof(int) * 3 * h.N);
+    if (pull_pos) memcpy(pull_pos, o.pull_pos.data(), sizeof(int) * 3 * h.N);
+    return RAD_OK;
+}
+
 rad_status rad_exchange_halo(rad_ctx *lo, double *I_lo, rad_ctx *hi, double *I_hi, int axis, void *stream) {
     if (!lo || !hi || !I_lo || !I_hi) return fail(lo ? lo : hi, RAD_EINVAL, "rad_exchange_halo: NULL argument");
     if (axis < 0 || axis > 2) return fail(lo, RAD_EINVAL, "rad_exchange_halo: axis must be 0, 1 or 2");
