@@ -473,6 +473,7 @@ struct orc_problem {
     int kind; double M, a, excise_r;
     int n[3], ng, NI, NJ, NK;
     double x0[3], dx[3];
+    double *xf[3];   /* R22: face coordinates of a stretched grid, [n + 2 ng + 1] per axis, or NULL (uniform: x0 + (i - ng) dx) */
     int bc_lo[3], bc_hi[3];
     const orc_angles *ang;
     double gamma_gas, a_rad, n0_crit;
@@ -524,10 +525,31 @@ static void pack_face(const double *pt, int axis, double *f) {
     }
 }
 
-orc_problem *orc_create(int kind, double M, double a, double excise_r, const int n[3], int ng, const double x0[3],
-                        const double dx[3], const int bc_lo[3], const int bc_hi[3], const orc_angles *ang,
-                        double gamma_gas, double a_rad, double n0_crit, int recon_space, int renorm, int couple) {
+/* coordinate of the lower face of cell `i` along axis d, and the cell's centre and width (Eq.20b,c with sqrt(-g) = 1 on a Cartesian
+ * tensor-product grid: Delta A_a / Delta V = 1 / Delta x^a of the cell) */
+static double face_coord(const orc_problem *P, int d, int i) { return P->xf[d] ? P->xf[d][i] : P->x0[d] + (i - P->ng) * P->dx[d]; }
+static double centre_coord(const orc_problem *P, int d, int i) {
+    return P->xf[d] ? 0.5 * (P->xf[d][i] + P->xf[d][i + 1]) : P->x0[d] + (i - P->ng + 0.5) * P->dx[d];
+}
+static double cell_width(const orc_problem *P, int d, int i) { return P->xf[d] ? P->xf[d][i + 1] - P->xf[d][i] : P->dx[d]; }
+
+/* xf0, xf1, xf2: face coordinates of a stretched Cartesian grid along x, y, z (NEXT-4, Eq.20b,c; reading R22), each with
+ * n + 2 ng + 1 entries (ghost cells included), or NULL for the uniform spacing dx from x0 */
+orc_problem *orc_create_stretched(int kind, double M, double a, double excise_r, const int n[3], int ng, const double x0[3],
+                                  const double dx[3], const int bc_lo[3], const int bc_hi[3], const orc_angles *ang,
+                                  double gamma_gas, double a_rad, double n0_crit, int recon_space, int renorm, int couple,
+                                  const double *xf0, const double *xf1, const double *xf2) {
     orc_problem *P = calloc(1, sizeof(*P));
+    {
+        const double *src[3] = {xf0, xf1, xf2};
+        for (int d = 0; d < 3; d++) {
+            P->xf[d] = NULL;
+            if (src[d]) {
+                P->xf[d] = malloc(sizeof(double) * (n[d] + 2 * ng + 1));
+                memcpy(P->xf[d], src[d], sizeof(double) * (n[d] + 2 * ng + 1));
+            }
+        }
+    }
     P->kind = kind; P->M = M; P->a = a; P->excise_r = excise_r; P->ng = ng; P->ang = ang;
     for (int d = 0; d < 3; d++) { P->n[d] = n[d]; P->x0[d] = x0[d]; P->dx[d] = dx[d]; P->bc_lo[d] = bc_lo[d]; P->bc_hi[d] = bc_hi[d]; }
     P->NI = n[0] + 2 * ng; P->NJ = n[1] + 2 * ng; P->NK = n[2] + 2 * ng;
@@ -558,7 +580,7 @@ orc_problem *orc_create(int kind, double M, double a, double excise_r, const int
                 long long c = cidx(P, k, j, i);
                 int id[3] = {i, j, k};
                 double xc[3], pt[ORC_NPOINT];
-                for (int d = 0; d < 3; d++) xc[d] = x0[d] + (id[d] - ng + 0.5) * dx[d];
+                for (int d = 0; d < 3; d++) xc[d] = centre_coord(P, d, id[d]);
                 orc_geometry_point(kind, M, a, xc, pt);
                 pack_cell(pt, &P->cell[c * ORC_NCELL]);
                 if (kind == 1 && excise_r > 0) { /* Kerr-Schild radius of the cell centre */
@@ -568,14 +590,25 @@ orc_problem *orc_create(int kind, double M, double a, double excise_r, const int
                 }
                 for (int ax = 0; ax < 3; ax++) { /* R6: face quantities at the face centre */
                     double xf[3] = {xc[0], xc[1], xc[2]};
-                    xf[ax] = x0[ax] + (id[ax] - ng) * dx[ax];
+                    xf[ax] = face_coord(P, ax, id[ax]);
                     orc_geometry_point(kind, M, a, xf, pt);
                     pack_face(pt, ax, &P->face[(c * 3 + ax) * ORC_NFACE]);
                 }
             }
     return P;
 }
-void orc_destroy(orc_problem *P) { if (!P) return; free(P->cell); free(P->face); free(P->excised); free(P->mirror); free(P); }
+orc_problem *orc_create(int kind, double M, double a, double excise_r, const int n[3], int ng, const double x0[3],
+                        const double dx[3], const int bc_lo[3], const int bc_hi[3], const orc_angles *ang,
+                        double gamma_gas, double a_rad, double n0_crit, int recon_space, int renorm, int couple) {
+    return orc_create_stretched(kind, M, a, excise_r, n, ng, x0, dx, bc_lo, bc_hi, ang, gamma_gas, a_rad, n0_crit, recon_space, renorm, couple,
+                                NULL, NULL, NULL);
+}
+void orc_destroy(orc_problem *P) {
+    if (!P) return;
+    free(P->cell); free(P->face); free(P->excised); free(P->mirror);
+    for (int d = 0; d < 3; d++) free(P->xf[d]);
+    free(P);
+}
 long long orc_ncells_total(const orc_problem *P) { return P->ncell; }
 void orc_get_geometry(const orc_problem *P, double *cell, double *face, int *excised) {
     if (cell) memcpy(cell, P->cell, sizeof(double) * P->ncell * ORC_NCELL);
@@ -758,9 +791,9 @@ static void transport_impl(const orc_problem *P, const double *I_in, const doubl
                         double nlo0 = contract4(cg + 17, nh); /* n_0 */
                         /* Eq.22: spatial flux divergence; uniform Cartesian grid with sqrt(-g)=1 => dA/dV = 1/dx */
                         double div = 0.0;
-                        div += (face_flux(P, I_in, 0, i + 1, j, k, n, vel, tau_dt) - face_flux(P, I_in, 0, i, j, k, n, vel, tau_dt)) / P->dx[0];
-                        div += (face_flux(P, I_in, 1, i, j + 1, k, n, vel, tau_dt) - face_flux(P, I_in, 1, i, j, k, n, vel, tau_dt)) / P->dx[1];
-                        div += (face_flux(P, I_in, 2, i, j, k + 1, n, vel, tau_dt) - face_flux(P, I_in, 2, i, j, k, n, vel, tau_dt)) / P->dx[2];
+                        div += (face_flux(P, I_in, 0, i + 1, j, k, n, vel, tau_dt) - face_flux(P, I_in, 0, i, j, k, n, vel, tau_dt)) / cell_width(P, 0, i);
+                        div += (face_flux(P, I_in, 1, i, j + 1, k, n, vel, tau_dt) - face_flux(P, I_in, 1, i, j, k, n, vel, tau_dt)) / cell_width(P, 1, j);
+                        div += (face_flux(P, I_in, 2, i, j, k + 1, n, vel, tau_dt) - face_flux(P, I_in, 2, i, j, k, n, vel, tau_dt)) / cell_width(P, 2, k);
                         /* angular flux divergence: (1/dOmega) sum_e +-dlambda_e F_e, + where the edge normal points out of n */
                         double adiv = 0.0;
                         for (int s = 0; s < A->nnbr[n]; s++) {

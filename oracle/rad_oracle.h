@@ -49,6 +49,12 @@ orc_problem *orc_create(int metric_kind, double M, double a, double excise_r, co
                         const double x0[3], const double dx[3], const int bc_lo[3],
                         const int bc_hi[3], const orc_angles *ang, double gamma_gas, double a_rad,
                         double n0_crit, int recon_space, int renorm, int couple);
+/* the same on a stretched Cartesian grid (NEXT-4; Eq.20b,c with sqrt(-g) = 1: Delta A_a / Delta V = 1 / Delta x^a of the cell; reading R22:
+ * reconstruction in index space): xf0, xf1, xf2 = face coordinates along x, y, z incl. ghost cells (n + 2 ng + 1 entries), or NULL = uniform */
+orc_problem *orc_create_stretched(int kind, double M, double a, double excise_r, const int n[3], int ng, const double x0[3],
+                                  const double dx[3], const int bc_lo[3], const int bc_hi[3], const orc_angles *ang,
+                                  double gamma_gas, double a_rad, double n0_crit, int recon_space, int renorm, int couple,
+                                  const double *xf0, const double *xf1, const double *xf2);
 void orc_destroy(orc_problem *);
 long long orc_ncells_total(const orc_problem *);
 /* geometry tables built at create: cell[ncells_total][ORC_NCELL], face[ncells_total][3][ORC_NFACE],

@@ -49,6 +49,8 @@ def lib():
         L.orc_create.restype = vp
         L.orc_create.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, ip, C.c_int, dp, dp, ip, ip, vp,
                                  C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int]
+        L.orc_create_stretched.restype = vp
+        L.orc_create_stretched.argtypes = L.orc_create.argtypes + [vp, vp, vp]
         L.orc_destroy.argtypes = [vp]
         L.orc_ncells_total.restype = C.c_longlong
         L.orc_ncells_total.argtypes = [vp]
@@ -131,7 +133,7 @@ class Problem:
 
     def __init__(self, angles, n, x0, dx, metric_kind=0, M=1.0, a=0.0, excise_r=0.0, ng=2, bc_lo=(0, 0, 0), bc_hi=(0, 0, 0),
                  gamma_gas=5.0 / 3.0, a_rad=1.0, n0_crit=0.1, recon_space=1, renorm=1, couple=1, tau_factor=0.0, recon_angle=0,
-                 vel_estimate=0, dt0_literal=0):
+                 vel_estimate=0, dt0_literal=0, xf=None):
         L = lib()
         self.angles = angles
         self.n = tuple(int(v) for v in n); self.ng = ng
@@ -139,8 +141,14 @@ class Problem:
         self.shape = (self.NK, self.NJ, self.NI)
         self.N = angles.N
         i3 = (C.c_int * 3); d3 = (C.c_double * 3)
-        self.h = L.orc_create(metric_kind, M, a, excise_r, i3(*self.n), ng, d3(*x0), d3(*dx), i3(*bc_lo), i3(*bc_hi), angles.h,
-                              gamma_gas, a_rad, n0_crit, recon_space, renorm, couple)
+        # xf: face coordinates of a stretched Cartesian grid, per axis an array of n + 2 ng + 1 values or None (uniform spacing dx from x0)
+        self.xf = [None if (xf is None or xf[d] is None) else np.ascontiguousarray(xf[d], dtype=np.float64) for d in range(3)]
+        for d in range(3):
+            if self.xf[d] is not None and self.xf[d].shape != (self.n[d] + 2 * ng + 1,):
+                raise ValueError("xf[%d] needs n + 2 ng + 1 entries" % d)
+        fp = [None if v is None else C.c_void_p(v.ctypes.data) for v in self.xf]
+        self.h = L.orc_create_stretched(metric_kind, M, a, excise_r, i3(*self.n), ng, d3(*x0), d3(*dx), i3(*bc_lo), i3(*bc_hi), angles.h,
+                                        gamma_gas, a_rad, n0_crit, recon_space, renorm, couple, *fp)
         self.ncell = L.orc_ncells_total(self.h)
         self.tau_factor = float(tau_factor)
         L.orc_set_tau_factor(self.h, self.tau_factor)   # constant of Eq.26; 0 = free-streaming flux Eq.24
