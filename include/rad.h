@@ -72,6 +72,12 @@ typedef struct {
                                the direction whose wall-normal tetrad component is flipped (reading R20); needs an angle
                                grid that is symmetric under that flip (every lat-lon grid with even npsi; the geodesic
                                grid for the y axis only), else rad_create returns RAD_EUNSUPPORTED */
+    const double *xf[3];    /* stretched Cartesian grid (NEXT-4; Eq.20b,c): per axis NULL (uniform: faces at x0 + i dx) or
+                               HOST array of the n + 2 ng + 1 face coordinates of that axis, ghost cells included, strictly
+                               increasing; copied at create.  With sqrt(-g) = 1 the area-to-volume ratio of a cell is
+                               Delta A_a / Delta V = 1 / (its width along a); geometry is evaluated at the true cell and face
+                               centres; reconstruction works in index space (reading R22).  A stretched axis sends the stage
+                               through the generic flux-divergence kernel (the tile kernel shares face fluxes divided by one dx) */
 } rad_grid;
 
 typedef struct {

@@ -36,7 +36,7 @@ class _Metric(C.Structure):
 
 class _Grid(C.Structure):
     _fields_ = [("n", C.c_int * 3), ("ng", C.c_int), ("x0", C.c_double * 3), ("dx", C.c_double * 3),
-                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3)]
+                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3), ("xf", C.c_void_p * 3)]
 
 
 class _Angles(C.Structure):
@@ -125,13 +125,18 @@ def _check(ctx, st):
 
 
 def rad_create(metric, grid, angles, opac, params, device=0):
-    """metric: dict(kind, M, a, excise_r, cell_tab, face_tab); grid: dict(n, x0, dx, bc_lo, bc_hi[, ng]);
+    """metric: dict(kind, M, a, excise_r, cell_tab, face_tab); grid: dict(n, x0, dx, bc_lo, bc_hi[, ng][, xf = per axis None or face coordinates]);
     angles: ("latlon", nzeta, npsi), ("geodesic", nlev) or ("explicit", dict(nhat, domega, nnbr, nbr, edge_len, edge_mid, edge_nrm)); opac: (alpha_a_planck, alpha_a_energy, alpha_s) CUDA
     tensors or None; params: dict of rad_params fields.  Returns an opaque handle."""
     m = _Metric(int(metric.get("kind", 0)), float(metric.get("M", 1.0)), float(metric.get("a", 0.0)), float(metric.get("excise_r", 0.0)),
                 _dp(metric.get("cell_tab")), _dp(metric.get("face_tab")))
     i3, d3 = C.c_int * 3, C.c_double * 3
-    g = _Grid(i3(*grid["n"]), int(grid.get("ng", 2)), d3(*grid["x0"]), d3(*grid["dx"]), i3(*grid.get("bc_lo", (0, 0, 0))), i3(*grid.get("bc_hi", (0, 0, 0))))
+    xfa = [None if (grid.get("xf") is None or grid["xf"][d] is None) else np.ascontiguousarray(grid["xf"][d], dtype=np.float64) for d in range(3)]
+    for d in range(3):
+        if xfa[d] is not None and xfa[d].shape != (int(grid["n"][d]) + 2 * int(grid.get("ng", 2)) + 1,):
+            raise ValueError("grid xf[%d] needs n + 2 ng + 1 face coordinates" % d)
+    g = _Grid(i3(*grid["n"]), int(grid.get("ng", 2)), d3(*grid["x0"]), d3(*grid["dx"]), i3(*grid.get("bc_lo", (0, 0, 0))), i3(*grid.get("bc_hi", (0, 0, 0))),
+              (C.c_void_p * 3)(*[None if v is None else v.ctypes.data for v in xfa]))
     keep = []
     if angles[0] == "latlon":
         a = _Angles(0, int(angles[1]), int(angles[2]), 0)

@@ -89,6 +89,15 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
         if (g->bc_lo[d] < 0 || g->bc_lo[d] > 3 || g->bc_hi[d] < 0 || g->bc_hi[d] > 3) return fail(nullptr, RAD_EINVAL, "rad_create: bad boundary code");
         if ((g->bc_lo[d] == 3 || g->bc_hi[d] == 3) && g->n[d] < g->ng) return fail(nullptr, RAD_EINVAL, "rad_create: a reflecting wall needs n[d] >= ng");
     }
+    bool stretched = false;
+    for (int d = 0; d < 3; d++) {
+        if (!g->xf[d]) continue;
+        stretched = true;
+        for (int i = 0; i < g->n[d] + 2 * g->ng; i++)
+            if (!std::isfinite(g->xf[d][i]) || !std::isfinite(g->xf[d][i + 1]) || !(g->xf[d][i + 1] > g->xf[d][i]))
+                return fail(nullptr, RAD_EINVAL, "rad_create: xf must be finite and strictly increasing");
+    }
+    if (stretched && m->kind == 2) return fail(nullptr, RAD_EINVAL, "rad_create: a tabulated metric carries its own positions: xf must be NULL");
     if (m->kind < 0 || m->kind > 2) return fail(nullptr, RAD_EINVAL, "rad_create: bad metric kind");
     if (m->kind == 1 && (!finite_pos(m->M) || !std::isfinite(m->a) || std::fabs(m->a) > m->M)) return fail(nullptr, RAD_EINVAL, "rad_create: bad M or a");
     if (m->kind == 2 && (!m->cell_tab || !m->face_tab)) return fail(nullptr, RAD_EINVAL, "rad_create: tabulated metric needs cell_tab and face_tab");
@@ -147,7 +156,15 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
             mirror[(size_t)d * h.N + n] = found;
         }
     }
-    for (int d = 0; d < 3; d++) { t.n[d] = g->n[d]; t.inv_dx[d] = 1.0 / g->dx[d]; }
+    for (int d = 0; d < 3; d++) { t.n[d] = g->n[d]; t.inv_dx[d] = 1.0 / g->dx[d]; t.xf[d] = nullptr; t.inv_w[d] = nullptr; }
+    c->grid.xf[0] = c->grid.xf[1] = c->grid.xf[2] = nullptr;  // the caller's arrays are not kept
+    for (int d = 0; d < 3 && ok; d++) {
+        if (!g->xf[d]) continue;
+        const int m = g->n[d] + 2 * g->ng;
+        std::vector<double> f(g->xf[d], g->xf[d] + m + 1), iw(m);
+        for (int i = 0; i < m; i++) iw[i] = 1.0 / (f[i + 1] - f[i]);
+        ok = upload(c, f, &t.xf[d]) && upload(c, iw, &t.inv_w[d]);
+    }
     t.NI = g->n[0] + 2 * g->ng; t.NJ = g->n[1] + 2 * g->ng; t.NK = g->n[2] + 2 * g->ng;
     if (cudaDeviceGetAttribute(&t.sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
         cudaDeviceGetAttribute(&t.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) != cudaSuccess) {
@@ -169,14 +186,14 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
             const int e = h.nbr_edge[n * RAD_MAXNBR + s];
             if (e >= 0) nbr_w[n * RAD_MAXNBR + s] = (h.edge_lo[e] == n ? 1.0 : -1.0) / h.domega[n];
         }
-    ok = upload(c, h.nhat, &t.nhat) && upload(c, h.domega, &t.domega) && upload(c, h.nnbr, &t.nnbr) && upload(c, h.nbr_edge, &t.nbr_edge) &&
+    ok = ok && upload(c, h.nhat, &t.nhat) && upload(c, h.domega, &t.domega) && upload(c, h.nnbr, &t.nnbr) && upload(c, h.nbr_edge, &t.nbr_edge) &&
          upload(c, h.edge_lo, &t.edge_lo) && upload(c, h.edge_hi, &t.edge_hi) && upload(c, h.edge_len, &t.edge_len) &&
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);
     t.mirror = nullptr;
     if (ok && any_wall) ok = upload(c, mirror, &t.mirror);
     // tile kernel (stage5.cu): balanced and coloured edge ownership, per-angle records, 1/dOmega
     t.fused_ok = 0; t.ang_rec = nullptr; t.winv = nullptr; t.own_edge = nullptr; t.ke = nullptr; t.rec = nullptr;
-    const bool tile_cfg = g->ng == 2 && p->recon_space <= 1 && p->recon_angle == 0;  // what the tile kernel (stage5.cu) implements
+    const bool tile_cfg = g->ng == 2 && p->recon_space <= 1 && p->recon_angle == 0 && !stretched;  // what the tile kernel (stage5.cu) implements
     if (ok && h.N <= 256 && tile_cfg) {
         std::string oerr;
         if (rad::build_edge_ownership(h, c->own, oerr)) {
@@ -212,7 +229,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
         ok = cudaMemcpy(cell, m->cell_tab, sizeof(double) * t.ncell * RAD_NCELL, cudaMemcpyDeviceToDevice) == cudaSuccess &&
              cudaMemcpy(face, m->face_tab, sizeof(double) * t.ncell * 3 * RAD_NFACE, cudaMemcpyDeviceToDevice) == cudaSuccess;
     } else {
-        int nl = rad::launch_geometry(*m, *g, cell, face, t.ncell, 0);
+        int nl = rad::launch_geometry(*m, *g, t.xf, cell, face, t.ncell, 0);
         ok = nl > 0 && cudaDeviceSynchronize() == cudaSuccess;
         if (ok) c->launches += nl;
     }

@@ -150,18 +150,21 @@ __device__ void point_geometry(int kind, double M, double a, double px, double p
             }
 }
 
+// xfx, xfy, xfz: face coordinates of a stretched axis (device), or nullptr = uniform spacing from (x0, y0, z0)
 __global__ void k_geometry(int kind, double M, double a, double excise_r, int NI, int NJ, int NK, int ng, double x0, double y0,
-                           double z0, double dx, double dy, double dz, double *__restrict__ cell, double *__restrict__ face) {
+                           double z0, double dx, double dy, double dz, const double *__restrict__ xfx, const double *__restrict__ xfy,
+                           const double *__restrict__ xfz, double *__restrict__ cell, double *__restrict__ face) {
     const long long ncell = (long long)NI * NJ * NK;
     const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t >= 4 * ncell) return;
     const long long c = t >> 2;
     const int pt = (int)(t & 3);  // 0 centre, 1..3 lower face along axis pt-1
     const int i = (int)(c % NI), j = (int)((c / NI) % NJ), k = (int)(c / ((long long)NI * NJ));
-    double px = x0 + (i - ng + 0.5) * dx, py = y0 + (j - ng + 0.5) * dy, pz = z0 + (k - ng + 0.5) * dz;
-    if (pt == 1) px = x0 + (i - ng) * dx;
-    if (pt == 2) py = y0 + (j - ng) * dy;
-    if (pt == 3) pz = z0 + (k - ng) * dz;
+    double px = xfx ? 0.5 * (xfx[i] + xfx[i + 1]) : x0 + (i - ng + 0.5) * dx, py = xfy ? 0.5 * (xfy[j] + xfy[j + 1]) : y0 + (j - ng + 0.5) * dy,
+           pz = xfz ? 0.5 * (xfz[k] + xfz[k + 1]) : z0 + (k - ng + 0.5) * dz;
+    if (pt == 1) px = xfx ? xfx[i] : x0 + (i - ng) * dx;
+    if (pt == 2) py = xfy ? xfy[j] : y0 + (j - ng) * dy;
+    if (pt == 3) pz = xfz ? xfz[k] : z0 + (k - ng) * dz;
     PointGeom G;
     point_geometry(kind, M, a, px, py, pz, pt == 0, G);
     if (pt == 0) {
@@ -199,12 +202,12 @@ __global__ void k_geometry(int kind, double M, double a, double excise_r, int NI
 
 }  // namespace
 
-int launch_geometry(const rad_metric &m, const rad_grid &g, double *cell, double *face, long long ncell, cudaStream_t s) {
+int launch_geometry(const rad_metric &m, const rad_grid &g, const double *const xf_dev[3], double *cell, double *face, long long ncell, cudaStream_t s) {
     const int NI = g.n[0] + 2 * g.ng, NJ = g.n[1] + 2 * g.ng, NK = g.n[2] + 2 * g.ng;
     const int threads = 128;
     const long long blocks = (4 * ncell + threads - 1) / threads;
     k_geometry<<<(unsigned)blocks, threads, 0, s>>>(m.kind, m.M, m.a, m.excise_r, NI, NJ, NK, g.ng, g.x0[0], g.x0[1], g.x0[2],
-                                                    g.dx[0], g.dx[1], g.dx[2], cell, face);
+                                                    g.dx[0], g.dx[1], g.dx[2], xf_dev[0], xf_dev[1], xf_dev[2], cell, face);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

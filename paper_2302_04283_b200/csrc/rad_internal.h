@@ -44,6 +44,8 @@ struct DeviceTables {
     long long ncell;
     int sms, smem_optin;  // device: SM count and the opt-in shared memory per CTA (bytes), queried once in rad_create
     double inv_dx[3];
+    const double *xf[3];     // stretched grid: face coordinates of axis d (n + 2 ng + 1), or nullptr (uniform)
+    const double *inv_w[3];  // ... and 1 / width of every cell of that axis (n + 2 ng), or nullptr
     // angle tables
     const double *nhat;      // [N][3]
     const double *domega;    // [N]
@@ -90,7 +92,7 @@ struct Params {
 };
 
 // kernel launchers (each returns the number of kernels it launched, or -1 after setting a CUDA error)
-int launch_geometry(const rad_metric &m, const rad_grid &g, double *cell, double *face, long long ncell,
+int launch_geometry(const rad_metric &m, const rad_grid &g, const double *const xf_dev[3], double *cell, double *face, long long ncell,
                     cudaStream_t s);
 int launch_exchange_halo(const DeviceTables &lo, double *I_lo, const DeviceTables &hi, double *I_hi, int axis, cudaStream_t s);
 int launch_fill_ghosts(const DeviceTables &t, const int bc_lo[3], const int bc_hi[3], double *I, cudaStream_t s);

@@ -81,23 +81,6 @@ __device__ __forceinline__ double tau_G(double u0, double u1, double u2, double 
     return -(1.0 + rcp3(u0 - (u1 * n1 + u2 * n2 + u3 * n3)));
 }
 
-// sums of four values over the warp, written to shared memory at `dst` (32 bytes) by the lanes that hold them after the
-// butterfly: the first two steps halve the number of values a lane carries instead of adding four values each
-__device__ __forceinline__ void warp_sum4_to(double a, double b, double c, double d, int lane, uint32_t dst) {
-    const unsigned full = 0xffffffffu;
-    const bool u16 = (lane & 16) != 0;
-    double k0 = u16 ? c : a, k1 = u16 ? d : b;
-    k0 += __shfl_xor_sync(full, u16 ? a : c, 16);
-    k1 += __shfl_xor_sync(full, u16 ? b : d, 16);
-    const bool u8 = (lane & 8) != 0;
-    double k = u8 ? k1 : k0;
-    k += __shfl_xor_sync(full, u8 ? k0 : k1, 8);
-    k += __shfl_xor_sync(full, k, 4);
-    k += __shfl_xor_sync(full, k, 2);
-    k += __shfl_xor_sync(full, k, 1);
-    if ((lane & 7) == 0) asm volatile("st.shared.f64 [%0], %1;" ::"r"(dst + (uint32_t)lane), "d"(k) : "memory");  // lanes 0, 8, 16, 24 hold a, b, c, d
-}
-
 // ------------------------------------------------------------------------------------------------------------------
 template <int NITER, int WPC, int TY, int TZ, int MINB, bool PLM, bool TAU>
 __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)

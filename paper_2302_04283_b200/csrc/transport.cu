@@ -233,6 +233,8 @@ __global__ void __launch_bounds__(256) k_fluxdiv(DeviceTables t, const double *_
         sFe[cl * E + e] = (ce == 0.0) ? 0.0 : __ldg(t.edge_len + e) * (ce * n0e * Iup);
     }
     __syncthreads();
+    // Delta A_a / Delta V of the cells of this run (Eq.20b,c with sqrt(-g) = 1): 1 / dx, or 1 / (the cell's width) on a stretched axis
+    const double idy = t.inv_w[1] ? t.inv_w[1][j] : t.inv_dx[1], idz = t.inv_w[2] ? t.inv_w[2][k] : t.inv_dx[2];
 
     // phase B: spatial fluxes and the update, per (cell, angle)
     for (int q = threadIdx.x; q < ncx * N; q += blockDim.x) {
@@ -247,11 +249,11 @@ __global__ void __launch_bounds__(256) k_fluxdiv(DeviceTables t, const double *_
         double div = 0.0;
         const double *vc = TAU ? vel + 5 * c : nullptr;  // this cell's velocity record; the neighbours' are 5 * stride away
         div += (face_flux<RECON, TAU>(sFx + (cl + 1) * 8, n1, n2, n3, p + sx, sx, vc, vc + 5, tau_dt) -
-                face_flux<RECON, TAU>(sFx + cl * 8, n1, n2, n3, p, sx, vc - 5, vc, tau_dt)) * t.inv_dx[0];
+                face_flux<RECON, TAU>(sFx + cl * 8, n1, n2, n3, p, sx, vc - 5, vc, tau_dt)) * (t.inv_w[0] ? t.inv_w[0][i0 + cl] : t.inv_dx[0]);
         div += (face_flux<RECON, TAU>(sFy + CX * 8 + cl * 8, n1, n2, n3, p + sy * N, sy * N, vc, vc + 5 * sy, tau_dt) -
-                face_flux<RECON, TAU>(sFy + cl * 8, n1, n2, n3, p, sy * N, vc - 5 * sy, vc, tau_dt)) * t.inv_dx[1];
+                face_flux<RECON, TAU>(sFy + cl * 8, n1, n2, n3, p, sy * N, vc - 5 * sy, vc, tau_dt)) * idy;
         div += (face_flux<RECON, TAU>(sFz + CX * 8 + cl * 8, n1, n2, n3, p + sz * N, sz * N, vc, vc + 5 * sz, tau_dt) -
-                face_flux<RECON, TAU>(sFz + cl * 8, n1, n2, n3, p, sz * N, vc - 5 * sz, vc, tau_dt)) * t.inv_dx[2];
+                face_flux<RECON, TAU>(sFz + cl * 8, n1, n2, n3, p, sz * N, vc - 5 * sz, vc, tau_dt)) * idz;
         double adiv = 0.0;
 #pragma unroll
         for (int s = 0; s < RAD_MAXNBR; s++) {

@@ -473,3 +473,36 @@ def test_two_blocks_with_halo_exchange_equal_one_block(oracle, B, axis):
                 B.rad_destroy(c)
     finally:
         B.rad_destroy(h)
+
+
+# ------------------------------------------------------------------------------------------------ NEXT-4: stretched Cartesian grid
+@pytest.mark.parametrize("angles,recon,tau", [(("geodesic", 3), 1, 0.0), (("geodesic", 4), 0, 0.0), (("latlon", 4, 8), 1, 1.5), (("geodesic", 2), 2, 0.0)])
+def test_stretched_grid_parity(oracle, B, angles, recon, tau):
+    """face coordinates handed to rad_create (rad_grid.xf): geometry at the true cell and face centres, Delta A / Delta V = 1 / cell width
+    (Eq.20b,c with sqrt(-g) = 1), the generic flux-divergence kernel; against the oracle's stretched grid (tests/test_oracle_stretched.py)"""
+    from test_oracle_stretched import stretched_faces
+    n, x0, dx, ng = (7, 5, 4), (3.0, 2.0, 1.0), (0.3, 0.25, 0.2), (3 if recon == 2 else 2)
+    xf = [stretched_faces(n[0], ng, x0[0], dx[0], 1.7, 51), None, stretched_faces(n[2], ng, x0[2], dx[2], 1.5, 53)]   # x and z stretched, y uniform
+    A = oracle.Angles(*angles)
+    bc = (1, 2, 0, 1, 2, 0)
+    P = oracle.Problem(A, n, x0, dx, metric_kind=1, M=1.0, a=0.9, ng=ng, bc_lo=bc[:3], bc_hi=bc[3:], recon_space=recon, tau_factor=tau, xf=xf)
+    rng = np.random.default_rng(7)
+    nc = P.ncell
+    I = np.exp(rng.normal(size=(nc, A.N)))
+    fluid = np.stack([rng.uniform(0.5, 2, nc), rng.uniform(0.3, 1.5, nc)] + [rng.uniform(-0.4, 0.4, nc) for _ in range(3)])
+    opac = np.stack([rng.uniform(0.1, 30, nc) for _ in range(3)])
+    d_opac = dev(opac)
+    h = B.rad_create(dict(kind=1, M=1.0, a=0.9), dict(n=n, ng=ng, x0=x0, dx=dx, bc_lo=bc[:3], bc_hi=bc[3:], xf=xf), angles, (d_opac[0], d_opac[1], d_opac[2]),
+                     dict(recon_space=recon, tau_factor=tau))
+    try:
+        assert B.rad_stage_kernels(h)[0] == "k_fluxdiv"
+        gc, gf = B.rad_get_table(h, B.TAB_CELL), B.rad_get_table(h, B.TAB_FACE)
+        from parity_util import oracle_tables_to_rad
+        rc, rf = oracle_tables_to_rad(*P.geometry())
+        assert np.abs(gc - rc).max() < 1e-13 and np.abs(gf - rf).max() < 1e-13
+        compare_stage(B, A, P, h, I, fluid, opac, 0.02)
+        with pytest.raises(B.RadError):   # faces must increase
+            bad = [xf[0][::-1].copy(), None, None]
+            B.rad_create(dict(kind=1, M=1.0, a=0.9), dict(n=n, ng=ng, x0=x0, dx=dx, xf=bad), angles, (d_opac[0], d_opac[1], d_opac[2]), dict())
+    finally:
+        B.rad_destroy(h)
