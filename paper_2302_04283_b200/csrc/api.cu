@@ -575,7 +575,7 @@ rad_status rad_stage_kernels(rad_ctx *c, char *buf, size_t nbytes) {
     char b[64];
     const int npass = (c->dev.N + 7) / 8;  // the pass counts the streaming kernel is instantiated for (stream.cu: launch_couple_stream)
     if (!stream) snprintf(b, sizeof b, "k_coupling");
-    else if (c->kp.vel_estimate && c->kp.couple) snprintf(b, sizeof b, "k_couple_stream<1,0>");
+    else if (c->kp.vel_estimate && c->kp.couple) snprintf(b, sizeof b, "k_couple_stream<1,%d>", npass == 21 ? 21 : 0);
     else snprintf(b, sizeof b, "k_couple_stream<0,%d>", (npass == 21 || npass == 12) ? npass : 0);
     const int w = snprintf(buf, nbytes, "%s;%s", a, b);
     if (w < 0 || (size_t)w >= nbytes) return fail(c, RAD_EINVAL, "rad_stage_kernels: buffer too small");

@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
             double M[10];
 #pragma unroll
             for (int q = 0; q < 10; q++) M[q] = 0.0;
-#pragma unroll 2
+#pragma unroll(NPASS ? NPASS : 2)
             for (int j = 0; j < npass; j++) {
                 const double2 a01 = lds2(aA01 + 128u * j), a23 = lds2(aA23 + 128u * j);
                 const double w0 = lds(aI + 64u * j) * a01.x;
@@ -581,7 +581,7 @@ int launch_couple_stream(const DeviceTables &t, const Params &p, double *I, cons
         if (cudaFuncSetAttribute(k_couple_stream<VEST, NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;       \
         k_couple_stream<VEST, NP><<<grid, warps * 32, smem, s>>>(t, p, a);                                                                            \
     } while (0)
-    if (p.vel_estimate && p.couple) RAD_COUPLE_LAUNCH(true, 0);
+    if (p.vel_estimate && p.couple) { if (npass == 21) RAD_COUPLE_LAUNCH(true, 21); else RAD_COUPLE_LAUNCH(true, 0); }
     else if (npass == 21) RAD_COUPLE_LAUNCH(false, 21);  // N = 161..168 (geodesic level 4)
     else if (npass == 12) RAD_COUPLE_LAUNCH(false, 12);  // N = 89..96 (geodesic level 3)
     else RAD_COUPLE_LAUNCH(false, 0);
