@@ -27,11 +27,13 @@ def test_generic_path_without_stored_coefficients(oracle, B, angles, tau):
 
 
 @pytest.mark.parametrize("angles,n", [(("geodesic", 6), (5, 3, 2)), (("latlon", 17, 16), (4, 3, 3)), (("latlon", 7, 9), (4, 3, 3)),
-                                      (("latlon", 8, 16), (9, 6, 5)), (("latlon", 7, 16), (6, 9, 5)), (("geodesic", 5), (5, 4, 6))])
+                                      (("latlon", 8, 16), (9, 6, 5)), (("latlon", 7, 16), (6, 9, 5)), (("geodesic", 5), (5, 4, 6)),
+                                      (("latlon", 4, 41), (5, 4, 3)), (("latlon", 6, 16), (6, 4, 5)), (("latlon", 2, 84), (5, 3, 3))])
 @pytest.mark.parametrize("tau", [0.0, 1.5])
 def test_every_angle_count_range(oracle, B, angles, n, tau):
     """N = 362 (geodesic 6) and 272: above the tile kernel's 256, generic kernels incl. k_coupling / k_moments; N = 63: odd, generic;
-    N = 128 (the paper's 8 x 16 grid) and 112: the 96 < N <= 128 tile shape; N = 252: the 2 x 2 tile"""
+    N = 128 (the paper's 8 x 16 grid) and 112: the 96 < N <= 128 tile shape; N = 252: the 2 x 2 tile; N = 164 and 168: the 21-pass coupling
+    instance away from N = 162; N = 96: every lane of the warp-per-cell tile busy"""
     A, P, h, I, fluid, opac, _ = small_problem(oracle, B, n, angles, tau_factor=tau)
     try:
         compare_stage(B, A, P, h, I, fluid, opac, 0.03)
