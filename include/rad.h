@@ -152,6 +152,38 @@ rad_status rad_stage(rad_ctx *, double *I_in, double *I_out, const double *I0, c
                      double gam0, double gam1, double beta_dt, double *T_out, double *dT0,
                      long long *n_noroot, void *cuda_stream);
 
+/* rad_stage for callers that cannot ask the CUDA allocator for memory once their run is under way.
+ *
+ * Who that is: a time integrator that calls the stage thousands of times from inside its step loop, after it has
+ *   (a) handed all remaining device memory to a pool of its own (a torch caching allocator sized to the card, an AMR framework's
+ *       arena), so that a late cudaMalloc inside the library fails or evicts the pool, or
+ *   (b) put the fluid solver, the halo copies and the radiation stage on different streams: cudaMalloc and cudaFree wait for the
+ *       whole device, so one allocation in the middle of a step stalls every stream of the application, or
+ *   (c) promised its users a device-memory footprint that is fixed once set-up is over.
+ * rad_stage itself allocates in one situation: with the optical-depth-aware flux (tau_factor > 0, Eq.26-29) its first call on a
+ * context takes a per-cell table (8 doubles per cell) from cudaMalloc, which the table kernel writes and the flux-divergence
+ * kernel reads.  rad_stage_static computes the same stage -- same kernels, same arguments, same results bit for bit -- with that
+ * table in an array that is part of librad.so's device image instead: RAD_STATIC_MAX_CELLS x 8 doubles = 4 MiB, resident on every
+ * GPU that loads the library from the load until the process exits, whether or not this entry point is ever called.
+ * It calls no cudaMalloc, cudaFree or other allocating routine, on any call, for any tau_factor (with tau_factor = 0 the array is
+ * not touched and the call is rad_stage under another name).
+ *
+ *  - Limit: the block, ghost layers included, may have at most RAD_STATIC_MAX_CELLS cells (65 536: e.g. 36 x 36 x 36 interior
+ *    cells with ng = 2, which covers the paper's 32^3 blocks).  A larger context gets RAD_EUNSUPPORTED and a message
+ *    that names both numbers; nothing is launched.  Use rad_stage for those.
+ *  - First call on a device: looks up where the array sits in that device's memory (one cudaGetSymbolAddress, result cached per
+ *    device ordinal).  The look-up is not a stream operation: make this first call during set-up, before any stream capture.
+ *  - One array for everybody: all contexts, streams and host threads of the process share it on a given device.  Two calls
+ *    whose kernels can overlap on the GPU (different streams without an event between them, or two host threads) overwrite
+ *    each other's table and both results are garbage.  Calls on one stream, or ordered by events, are safe.
+ *  - Nothing needs clearing between calls: every call rewrites the table entries of all its cells before reading any, and
+ *    reads no others; the rest of the array keeps stale values of earlier, larger blocks.
+ * Arguments, outputs, aliasing rules and the other status codes are those of rad_stage. */
+#define RAD_STATIC_MAX_CELLS 65536
+rad_status rad_stage_static(rad_ctx *, double *I_in, double *I_out, const double *I0, const double *fluid,
+                            double gam0, double gam1, double beta_dt, double *T_out, double *dT0,
+                            long long *n_noroot, void *cuda_stream);
+
 /* Same stage with HOST buffers (same shapes): copies I_in, fluid and the three opacity arrays
  * host->device into library-owned scratch, runs the stage, copies I_out, T_out, dT0 back, and
  * synchronises.  With caller-filled boundaries and an angle grid the tile kernel serves, the block is

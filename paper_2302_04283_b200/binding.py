@@ -19,7 +19,7 @@ NCELL, NFACE, MAXNBR = 52, 8, 6
  TAB_EDGE_MID, TAB_EDGE_NRM, TAB_CELL, TAB_FACE, TAB_FACE_SIGN, TAB_EDGE_SIGN, TAB_MAXSPEED, TAB_OWN_EDGE, TAB_KE,
  TAB_STAGE_FACE_SIGN) = range(20)
 
-EXPORTS = ["rad_create", "rad_stage", "rad_stage_host", "rad_fill_ghosts", "rad_transport", "rad_couple", "rad_moments",
+EXPORTS = ["rad_create", "rad_stage", "rad_stage_static", "rad_stage_host", "rad_fill_ghosts", "rad_transport", "rad_couple", "rad_moments",
            "rad_get_table", "rad_edge_ownership", "rad_exchange_halo", "rad_stage_kernels", "rad_probe_fp64", "rad_probe_fp64_pipes", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
 
 
@@ -68,6 +68,7 @@ def lib():
         vp, d, ll = C.c_void_p, C.c_double, C.POINTER(C.c_longlong)
         L.rad_create.argtypes = [C.POINTER(_Metric), C.POINTER(_Grid), C.POINTER(_Angles), C.POINTER(_Opac), C.POINTER(_Params), C.c_int, C.POINTER(vp)]
         L.rad_stage.argtypes = [vp, vp, vp, vp, vp, d, d, d, vp, vp, ll, vp]
+        L.rad_stage_static.argtypes = [vp, vp, vp, vp, vp, d, d, d, vp, vp, ll, vp]
         L.rad_stage_host.argtypes = [vp, vp, vp, vp, vp, d, d, d, vp, vp, ll]
         L.rad_fill_ghosts.argtypes = [vp, vp, vp]
         L.rad_transport.argtypes = [vp, vp, vp, vp, d, d, d, vp]
@@ -166,6 +167,21 @@ def rad_stage(ctx, I_in, I_out, I0, fluid, gam0, gam1, beta_dt, T_out=None, dT0=
     n = C.c_longlong(0)
     st = lib().rad_stage(ctx, _dp(I_in), _dp(I_out), _dp(I0), _dp(fluid), gam0, gam1, beta_dt, _dp(T_out), _dp(dT0),
                          C.byref(n) if count_noroot else None, _stream(stream))
+    _check(ctx, st)
+    return n.value if count_noroot else None
+
+
+STATIC_MAX_CELLS = 65536  # RAD_STATIC_MAX_CELLS
+
+
+def rad_stage_static(ctx, I_in, I_out, I0, fluid, gam0, gam1, beta_dt, T_out=None, dT0=None, count_noroot=False, stream=None):
+    """rad_stage without any device allocation, for step loops that run after the application has given the rest of the card to its own
+    memory pool or that cannot afford the device-wide stall of a cudaMalloc: the optical-depth-aware flux's per-cell table sits in a
+    4 MiB array inside librad.so instead.  Blocks of at most STATIC_MAX_CELLS cells (ghosts included), else RadError status 4;
+    calls that may overlap on the GPU share that array and must be ordered by the caller (see rad.h)."""
+    n = C.c_longlong(0)
+    st = lib().rad_stage_static(ctx, _dp(I_in), _dp(I_out), _dp(I0), _dp(fluid), gam0, gam1, beta_dt, _dp(T_out), _dp(dT0),
+                                C.byref(n) if count_noroot else None, _stream(stream))
     _check(ctx, st)
     return n.value if count_noroot else None
 

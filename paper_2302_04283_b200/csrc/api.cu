@@ -2,6 +2,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -656,6 +657,91 @@ rad_status rad_get_table(rad_ctx *c, int which, void *host_out, size_t nbytes) {
     if (!ok) return cuda_fail(c, "rad_get_table");
     c->launches += nl;
     return RAD_OK;
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// rad_stage_static: the stage of rad_stage for callers that must not allocate (see include/rad.h).
+//
+// With the optical-depth-aware flux (tau_factor > 0, Eq.26-29) a stage needs a per-cell table between its first kernel (which
+// writes it from the fluid state) and the flux-divergence kernel (which reads it): scratch, neither input nor output.  rad_stage
+// takes that table from cudaMalloc on its first call.  Here it lives in the array below, which is part of the library image:
+// the driver places it when the library is loaded on a device and nothing is requested from the allocator afterwards.
+// ------------------------------------------------------------------------------------------------
+#define RAD_STATIC_DOUBLES_PER_CELL 8
+static __device__ __align__(256) double g_static_table[(size_t)RAD_STATIC_MAX_CELLS * RAD_STATIC_DOUBLES_PER_CELL];  // 4 MiB on every device that loads librad.so
+
+namespace {
+constexpr int kMaxStaticDevices = 64;
+double *g_static_addr[kMaxStaticDevices];  // per device ordinal: where g_static_table sits in that device's memory (nullptr = not asked yet)
+std::mutex g_static_mutex;
+
+// In host code `g_static_table` names a host-side shadow of the symbol, not device memory: handing it to a kernel would make the
+// kernel touch the wrong address.  The device address has to be asked for, once per device and with that device current.
+cudaError_t static_table_address(int device, double **out) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_table);
+        if (e != cudaSuccess) return e;
+        g_static_addr[device] = static_cast<double *>(p);
+    }
+    *out = g_static_addr[device];
+    return cudaSuccess;
+}
+}  // namespace
+
+rad_status rad_stage_static(rad_ctx *c, double *I_in, double *I_out, const double *I0, const double *fluid, double gam0, double gam1,
+                            double beta_dt, double *T_out, double *dT0, long long *n_noroot, void *stream) {
+    if (!c || !fluid || !I_in || !I_out) return fail(c, RAD_EINVAL, "rad_stage_static: NULL argument");
+    if (I_in == I_out || I0 == I_out) return fail(c, RAD_EINVAL, "rad_stage_static: I_out must not alias I_in or I0 (the stencil reads old values)");
+    if (!std::isfinite(gam0) || !std::isfinite(gam1) || !std::isfinite(beta_dt)) return fail(c, RAD_EINVAL, "rad_stage_static: non-finite weights");
+    if ((c->kp.couple || c->kp.tau_factor != 0.0) && (!c->opac.alpha_a_planck || !c->opac.alpha_a_energy || !c->opac.alpha_s))
+        return fail(c, RAD_ESTATE, "rad_stage_static: context has no opacities");
+    if (c->dev.ncell > (long long)RAD_STATIC_MAX_CELLS) {
+        char buf[192];
+        snprintf(buf, sizeof buf, "rad_stage_static: the block has %lld cells with its ghost layers, the built-in table holds RAD_STATIC_MAX_CELLS = %d; use rad_stage",
+                 c->dev.ncell, (int)RAD_STATIC_MAX_CELLS);
+        return fail(c, RAD_EUNSUPPORTED, buf);
+    }
+    if (c->device < 0 || c->device >= kMaxStaticDevices) return fail(c, RAD_EUNSUPPORTED, "rad_stage_static: device ordinal beyond the per-device address table");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return cuda_fail(c, "rad_stage_static: cudaSetDevice");
+    double *table = nullptr;
+    if (static_table_address(c->device, &table) != cudaSuccess) return cuda_fail(c, "rad_stage_static: cudaGetSymbolAddress");
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n_noroot && cudaMemsetAsync(c->d_noroot, 0, sizeof(unsigned long long), s) != cudaSuccess) return cuda_fail(c, "rad_stage_static: memset");
+    rad_status st = rad_fill_ghosts(c, I_in, s);
+    if (st != RAD_OK) return st;
+    // flux divergence.  Both table builders write every one of the block's cells, so nothing of an earlier call is read and
+    // nothing has to be cleared; the array's tail beyond this block keeps whatever the last larger block left there.
+    const bool tau = c->kp.tau_factor != 0.0;
+    rad::StageArgs a{};
+    a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
+    int nl = 0;
+    if (rad::stage_angle_serves(c->dev)) {  // tile kernel: {u^alphahat, f/2 of the upper faces}, 8 doubles per cell
+        if (tau) {
+            const int nt = rad::launch_tau_table(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->kp.tau_factor * beta_dt, table, s);
+            if (nt < 0) return cuda_fail(c, "rad_stage_static (velocity table)");
+            c->launches += nt;
+            a.vel8 = table;
+        }
+        nl = rad::launch_stage_angle(c->dev, c->kp, a, s);
+        if (nl < 0) return cuda_fail(c, "rad_stage_static (tile kernel)");
+    }
+    if (nl == 0) {  // generic kernel: {u^alphahat, alpha_E}, 5 doubles per cell
+        if (tau) {
+            const int nv = rad::launch_cell_velocity(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, table, s);
+            if (nv < 0) return cuda_fail(c, "rad_stage_static (velocity table)");
+            c->launches += nv;
+        }
+        nl = rad::launch_fluxdiv(c->dev, c->kp, I_in, I0, gam0, gam1, beta_dt, I_out, s, tau ? table : nullptr, c->kp.tau_factor * beta_dt);
+        if (nl < 0) return cuda_fail(c, "rad_stage_static (flux divergence)");
+    }
+    c->launches += nl;
+    st = run_coupling(c, I_out, fluid, beta_dt, T_out, dT0, n_noroot != nullptr, s);
+    if (st != RAD_OK) return st;
+    return read_noroot(c, n_noroot, s, "rad_stage_static: readback");
 }
 
 }  // extern "C"
