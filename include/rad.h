@@ -89,7 +89,9 @@ typedef struct {
      * angles of an edge must list each other); per (angle, slot): the edge's arc length edge_len[nang][RAD_MAXNBR]
      * (Delta lambda, Eq.20f), unit vector to its midpoint edge_mid[nang][RAD_MAXNBR][3] and in-sphere unit normal
      * edge_nrm[nang][RAD_MAXNBR][3] pointing from the angle to that neighbour.  An edge's data are read from the entry of
-     * its lower-numbered angle.  Errors: RAD_EINVAL (NULL, non-unit nhat, non-positive domega, asymmetric lists). */
+     * its lower-numbered angle.  Errors: RAD_EINVAL (NULL, non-unit nhat, non-positive domega, asymmetric lists, negative or
+     * non-finite edge_len, edge_mid that is not a finite unit vector, edge_nrm that is not finite or is zero; edge_nrm need
+     * not be unit: it carries the metric factor of its coordinate, 1 / sin zeta on the psi edges of a lat-lon grid, Eq.16c). */
     int nang;
     const double *nhat, *domega, *edge_len, *edge_mid, *edge_nrm;
     const int *nnbr, *nbr;
@@ -124,7 +126,10 @@ typedef struct {
     int vel_estimate;          /* radiation-dominated velocity estimate (Eq.51-55; reading G8 in DESIGN.md):
                                   1 = in cells where Ebar exceeds rho + u_gas the coupling uses the fluid velocity of Eq.55
                                       (blend of the gas velocity and the radiation velocity of Eq.51 with the clamped
-                                      fractions of Eq.54) instead of the pre-coupling velocity; 0 = always the pre-coupling velocity */
+                                      fractions of Eq.54) instead of the pre-coupling velocity; 0 = always the pre-coupling velocity.
+                                  Restrictions (the estimate lives in the streaming coupling kernel only): with couple = 1, rad_create returns
+                                  RAD_EUNSUPPORTED for an odd number of angles or one whose rows do not fit that kernel's shared memory, and
+                                  rad_stage / rad_couple return RAD_EUNSUPPORTED at run time for an intensity array that is not 16-byte aligned */
 } rad_params;
 
 /* Build a context: angle tables on the host (section 2.6), geometry tables on the device (section 2.1-2.2,

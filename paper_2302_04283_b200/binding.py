@@ -125,6 +125,22 @@ def _check(ctx, st):
         raise RadError(st, lib().rad_last_error(ctx).decode())
 
 
+def _angles(angles):
+    """rad_angles from ("latlon", nzeta, npsi), ("geodesic", nlev) or ("explicit", dict of host tables: rad_angles kind 2 in rad.h);
+    returns the struct and the host arrays it points into (to be kept alive across the call)"""
+    if angles[0] == "latlon":
+        return _Angles(0, int(angles[1]), int(angles[2]), 0), []
+    if angles[0] == "geodesic":
+        return _Angles(1, 0, 0, int(angles[1])), []
+    if angles[0] != "explicit":
+        raise ValueError("angle grid: ('latlon', nzeta, npsi), ('geodesic', nlev) or ('explicit', tables)")
+    tb = angles[1]
+    f64 = lambda k: np.ascontiguousarray(tb[k], dtype=np.float64)
+    i32 = lambda k: np.ascontiguousarray(tb[k], dtype=np.int32)
+    keep = [f64("nhat"), f64("domega"), f64("edge_len"), f64("edge_mid"), f64("edge_nrm"), i32("nnbr"), i32("nbr")]
+    return _Angles(2, 0, 0, 0, int(keep[1].shape[0]), *[C.c_void_p(x.ctypes.data) for x in keep]), keep
+
+
 def rad_create(metric, grid, angles, opac, params, device=0):
     """metric: dict(kind, M, a, excise_r, cell_tab, face_tab); grid: dict(n, x0, dx, bc_lo, bc_hi[, ng][, xf = per axis None or face coordinates]);
     angles: ("latlon", nzeta, npsi), ("geodesic", nlev) or ("explicit", dict(nhat, domega, nnbr, nbr, edge_len, edge_mid, edge_nrm)); opac: (alpha_a_planck, alpha_a_energy, alpha_s) CUDA
@@ -138,17 +154,7 @@ def rad_create(metric, grid, angles, opac, params, device=0):
             raise ValueError("grid xf[%d] needs n + 2 ng + 1 face coordinates" % d)
     g = _Grid(i3(*grid["n"]), int(grid.get("ng", 2)), d3(*grid["x0"]), d3(*grid["dx"]), i3(*grid.get("bc_lo", (0, 0, 0))), i3(*grid.get("bc_hi", (0, 0, 0))),
               (C.c_void_p * 3)(*[None if v is None else v.ctypes.data for v in xfa]))
-    keep = []
-    if angles[0] == "latlon":
-        a = _Angles(0, int(angles[1]), int(angles[2]), 0)
-    elif angles[0] == "geodesic":
-        a = _Angles(1, 0, 0, int(angles[1]))
-    else:  # ("explicit", dict of host tables): see rad_angles kind 2 in rad.h
-        tb = angles[1]
-        f64 = lambda k: np.ascontiguousarray(tb[k], dtype=np.float64)
-        i32 = lambda k: np.ascontiguousarray(tb[k], dtype=np.int32)
-        keep = [f64("nhat"), f64("domega"), f64("edge_len"), f64("edge_mid"), f64("edge_nrm"), i32("nnbr"), i32("nbr")]
-        a = _Angles(2, 0, 0, 0, int(keep[1].shape[0]), *[C.c_void_p(x.ctypes.data) for x in keep])
+    a, keep = _angles(angles)
     o = _Opac(*(_dp(x) for x in opac)) if opac is not None else None
     p = _Params(float(params.get("gamma_gas", 5.0 / 3.0)), float(params.get("a_rad", 1.0)), float(params.get("n0_crit", 0.1)),
                 int(params.get("recon_space", 1)), int(params.get("recon_angle", 0)), int(params.get("renorm_fluid_weights", 1)),
@@ -200,8 +206,8 @@ def rad_fill_ghosts(ctx, I, stream=None):
 
 def rad_edge_ownership(angles):
     """host only (no device needed): dict(N, E, edge_lo, edge_hi, own_edge[N][3], own_partner[N][3], pull_pos[N][3]) of an angle grid
-    given as ("latlon", nzeta, npsi) or ("geodesic", nlev)"""
-    a = _Angles(0, int(angles[1]), int(angles[2]), 0) if angles[0] == "latlon" else _Angles(1, 0, 0, int(angles[1]))
+    given as ("latlon", nzeta, npsi), ("geodesic", nlev) or ("explicit", tables)"""
+    a, keep = _angles(angles)  # noqa: F841  (keep: the host tables stay alive until the calls below return)
     n, e = C.c_int(0), C.c_int(0)
     L = lib()
     st = L.rad_edge_ownership(C.byref(a), C.byref(n), C.byref(e), None, None, None, None, None, 0)

@@ -274,6 +274,10 @@ bool build_explicit(int N, const double *nhat, const double *domega, const int *
             if (sm < 0) { err = "explicit angle grid: neighbour lists are not symmetric"; return false; }
             const size_t q = (size_t)n * RAD_MAXNBR + s;
             if (!std::isfinite(edge_len[q]) || edge_len[q] < 0.0) { err = "explicit angle grid: bad edge length"; return false; }
+            double m2 = 0.0, k2 = 0.0;  // a NaN here would reach every stored coefficient of every cell without any error
+            for (int c = 0; c < 3; c++) { m2 += edge_mid[3 * q + c] * edge_mid[3 * q + c]; k2 += edge_nrm[3 * q + c] * edge_nrm[3 * q + c]; }
+            // (edge_nrm carries the metric factor of its coordinate: 1 / sin zeta on the psi edges of a latitude-longitude grid, Eq.16c)
+            if (!(std::fabs(m2 - 1.0) < 1e-6) || !std::isfinite(k2) || !(k2 > 0.0)) { err = "explicit angle grid: edge_mid must be finite unit vectors, edge_nrm finite and non-zero"; return false; }
             push_edge(t, n, s, m, sm, edge_len[q], {edge_mid[3 * q], edge_mid[3 * q + 1], edge_mid[3 * q + 2]},
                       {edge_nrm[3 * q], edge_nrm[3 * q + 1], edge_nrm[3 * q + 2]});
         }

@@ -271,7 +271,7 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
             c->launches += nl;
             t.rec = c->rec;
         } else {
-            cudaGetLastError();  // not fatal: the older stage kernel serves the context
+            cudaGetLastError();  // not fatal: without the records the generic flux-divergence kernel (transport.cu) serves the context
         }
     }
     *out = c;
@@ -356,7 +356,7 @@ static rad_status run_transport(rad_ctx *c, double *I_in, double *I_out, const d
     const bool tau = c->kp.tau_factor != 0.0;
     rad::StageArgs a{};
     a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt; a.kz0 = kz0; a.kz1 = kz1;
-    if (rad::stage_angle_serves(c->dev)) {
+    if (rad::stage_angle_serves(c->dev, tau)) {  // decided once: the table below is built for the kernel that will read it
         if (tau) {  // per-cell table {u^alphahat, f/2 of the upper faces}
             if (!c->vel8 && cudaMalloc((void **)&c->vel8, sizeof(double) * 8 * (size_t)c->dev.ncell) != cudaSuccess) {
                 cudaGetLastError();
@@ -719,7 +719,7 @@ rad_status rad_stage_static(rad_ctx *c, double *I_in, double *I_out, const doubl
     rad::StageArgs a{};
     a.I_in = I_in; a.I0 = I0; a.I_out = I_out; a.gam0 = gam0; a.gam1 = gam1; a.beta_dt = beta_dt;
     int nl = 0;
-    if (rad::stage_angle_serves(c->dev)) {  // tile kernel: {u^alphahat, f/2 of the upper faces}, 8 doubles per cell
+    if (rad::stage_angle_serves(c->dev, tau)) {  // tile kernel: {u^alphahat, f/2 of the upper faces}, 8 doubles per cell
         if (tau) {
             const int nt = rad::launch_tau_table(c->dev, fluid, c->opac.alpha_a_energy, c->opac.alpha_s, c->kp.tau_factor * beta_dt, table, s);
             if (nt < 0) return cuda_fail(c, "rad_stage_static (velocity table)");

@@ -32,6 +32,10 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
                  : "memory");
 }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// Orders the calling thread's earlier ordinary (generic-proxy) shared-memory accesses before later asynchronous-proxy accesses
+// (bulk copies) to the same bytes.  To be executed by every thread that WROTE the bytes, before the barrier that hands them to the
+// thread issuing the copy: a barrier alone orders the generic proxy only.
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // barrier among the `nthreads` threads that use the same id (1..15; 0 is __syncthreads)
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }

@@ -114,8 +114,9 @@ int launch_moments_stream(const DeviceTables &t, const double *I, int frame, con
 // launch_fluxdiv), -1 CUDA error; and its record builder
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, cudaStream_t s);
 int stage_angle_kernel_name(const DeviceTables &t, const Params &p, bool tau, char *buf, size_t n);
-// 1 if launch_stage_angle serves this context (so that a stage can be run slab by slab along z)
-int stage_angle_serves(const DeviceTables &t);
+// 1 if launch_stage_angle serves this context (so that a stage can be run slab by slab along z); tau: with the velocity records of
+// the optical-depth-aware flux in shared memory (a larger layout: some angle counts fit without them only)
+int stage_angle_serves(const DeviceTables &t, bool tau = false);
 // TAU table of the angle-resident kernel: vel8[ncell][8], see k_tau_table (stage5.cu)
 int launch_tau_table(const DeviceTables &t, const double *fluid, const double *aE, const double *aS, double tau_dt, double *vel8, cudaStream_t s);
 int launch_pack_rec(const DeviceTables &t, double *rec, cudaStream_t s);

@@ -425,6 +425,9 @@ __global__ void __launch_bounds__(TY *TZ *WPC * 32, MINB)
             for (int it = 0; it < NITER; it++)
                 if (it < NITER - 1 || last_valid) sts(tb[it] + fxOff, q0[it]);
         }
+        // the edge fluxes (written over the coefficients) and the published face fluxes went through the generic proxy; the copies of
+        // step s + 2 overwrite the same bytes through the asynchronous proxy: every writer fences before the barrier
+        fence_proxy_async();
         __syncthreads();  // the fluxes of this plane are published; nobody reads the rows, halo and coefficients of plane s any more
         if (s + 2 < nsteps && myrole < NR) issue(s + 2);
         if (!active) continue;
@@ -597,7 +600,7 @@ __global__ void __launch_bounds__(256) k_tau_table(const DeviceTables t, const d
 
 // returns 1 (launched), 0 (this configuration is not served by this kernel), -1 (CUDA error)
 int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &a, cudaStream_t s) {
-    if (!stage_angle_serves(t)) return 0;
+    if (!stage_angle_serves(t, a.vel8 != nullptr)) return 0;
     if (((uintptr_t)a.I_in & 15) || ((uintptr_t)a.vel8 & 15)) return 0;  // rows are brought in by 16-byte bulk copies
 #define RAD_S5_CALL(NITER, WPC, TY, TZ) return launch5<NITER, WPC, TY, TZ>(t, p, a, s)
     RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
@@ -607,17 +610,20 @@ int launch_stage_angle(const DeviceTables &t, const Params &p, const StageArgs &
 
 // the instance launch_stage_angle runs for this context, written as ncu prints it without casts and blanks (profiles/*.csv key)
 int stage_angle_kernel_name(const DeviceTables &t, const Params &p, bool tau, char *buf, size_t n) {
-    if (!stage_angle_serves(t)) return snprintf(buf, n, "k_fluxdiv");
+    if (!stage_angle_serves(t, tau)) return snprintf(buf, n, "k_fluxdiv");
 #define RAD_S5_CALL(NITER, WPC, TY, TZ) return snprintf(buf, n, "k_stage5<%d,%d,%d,%d,1,%d,%d>", NITER, WPC, TY, TZ, p.recon_space == 1 ? 1 : 0, tau ? 1 : 0)
     RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
 #undef RAD_S5_CALL
     return 0;
 }
 
-int stage_angle_serves(const DeviceTables &t) {
+int stage_angle_serves(const DeviceTables &t, bool tau) {
     if (!t.fused_ok || t.ke == nullptr || t.rec == nullptr || (t.N & 1) || t.N > 256) return 0;  // rows must be multiples of 16 bytes
     if (((uintptr_t)t.ke & 15) || ((uintptr_t)t.rec & 15)) return 0;
-#define RAD_S5_CALL(NITER, WPC, TY, TZ) return sizeof(double) * (size_t)make_layout5<Tile<TY, TZ, WPC, false>>(t.N).total <= (size_t)t.smem_optin
+    // the layout with the velocity records (TAU) is the larger one: N ~ 176..180 fits without them only
+#define RAD_S5_CALL(NITER, WPC, TY, TZ)                                                                                           \
+    return sizeof(double) * (size_t)(tau ? make_layout5<Tile<TY, TZ, WPC, true>>(t.N).total : make_layout5<Tile<TY, TZ, WPC, false>>(t.N).total) <= \
+           (size_t)t.smem_optin
     RAD_S5_DISPATCH(t.N, RAD_S5_CALL);
 #undef RAD_S5_CALL
     return 0;

@@ -29,7 +29,6 @@ constexpr int kCA = 8;      // angle slots per cell in a warp pass
 constexpr int kDepth = 2;   // ring slots per warp
 constexpr int kCellF = 20;  // per-cell scalars fetched for the coupling: fluid (5), opacities (3), n^0, E_alphahat (4), co-triad (6), excised
 
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 __host__ __device__ inline int couple_row_stride(int N) { return ((N + 7) / 8 * 8 + 7) / 16 * 16 + 8; }  // >= 8 ceil(N/8), = 8 (mod 16)
 
@@ -143,10 +142,8 @@ __global__ void __launch_bounds__(384) k_couple_stream(const DeviceTables t, con
     auto issue = [&]() {  // the rows of group `ahead` into its ring slot, one bulk copy per cell
         const int cnt = min(kCG, t.n[0] - kCG * ahead.ig);
         const uint32_t bar = bar0 + 16u * sl_ahead;
-        if (lane == 0) {
-            fence_proxy_async();  // sweep 1 wrote into this slot through the generic proxy
-            mbar_expect_tx(bar, (uint32_t)(cnt * N * 8));
-        }
+        fence_proxy_async();  // every lane: sweep 1 wrote into this slot through the generic proxy, the copies below go through the asynchronous one
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(cnt * N * 8));
         __syncwarp();
         if (lane < cnt) bulk_g2s(smem_u32(slots + (sl_ahead * kCG + lane) * Np), a.I + (ahead.c + lane) * N, (uint32_t)(N * 8), bar);
         group_next(t, ahead, gpr, kCG);
@@ -591,10 +588,10 @@ int launch_couple_stream(const DeviceTables &t, const Params &p, double *I, cons
 
 int launch_moments_stream(const DeviceTables &t, const double *I, int frame, const double *fluid, double *out, cudaStream_t s) {
     if ((t.N & 1) || ((uintptr_t)I & 15)) return 0;
-    // ring depth 3 and as many warps as shared memory holds (<= 8); deeper rings do not pay once ~100 KB are in flight per SM
-    int depth = 2, warps = 12;
+    // ring depth 2 and as many warps as shared memory holds (<= 12); deeper rings do not pay once ~100 KB are in flight per SM
+    const int depth = 2;
+    int warps = 12;
     while (warps > 2 && moments_smem(t.N, warps, depth) > (size_t)t.smem_optin) warps--;
-    if (moments_smem(t.N, warps, depth) > (size_t)t.smem_optin) depth = 2;
     const size_t smem = moments_smem(t.N, warps, depth);
     if (smem > (size_t)t.smem_optin) return 0;
     const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(4, (size_t)t.smem_optin / (smem + 1024)));

@@ -312,7 +312,7 @@ int launch_fluxdiv(const DeviceTables &t, const Params &p, const double *I_in, c
     const size_t smem = sizeof(double) * (CX * 36 + (CX + 1) * 8 + 4 * CX * 8 + (size_t)CX * t.E);
 #define RAD_LAUNCH_FD(RECON, TAU)                                                                                     \
     do {                                                                                                              \
-        cudaFuncSetAttribute(k_fluxdiv<RECON, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+        if (cudaFuncSetAttribute(k_fluxdiv<RECON, TAU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1; \
         k_fluxdiv<RECON, TAU><<<(unsigned)blocks, 256, smem, s>>>(t, I_in, I0, gam0, gam1, beta_dt, I_out, vel, tau_dt); \
     } while (0)
     if (p.recon_space == 2) { if (vel) RAD_LAUNCH_FD(2, true); else RAD_LAUNCH_FD(2, false); }

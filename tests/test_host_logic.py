@@ -54,3 +54,41 @@ def test_edge_ownership_is_a_balanced_orientation_with_a_proper_slot_colouring(l
 def test_edge_ownership_is_deterministic(lib):
     a, b = B.rad_edge_ownership(("geodesic", 4)), B.rad_edge_ownership(("geodesic", 4))
     assert all(np.array_equal(a[k], b[k]) for k in ("own_edge", "own_partner", "pull_pos"))
+
+
+def explicit_tables(A):
+    """rad_angles kind 2 tables (rad.h) of an oracle angle grid: per (angle, slot) edge data, the normal pointing from the angle to its neighbour"""
+    N = A.N
+    tab = dict(nhat=A.nhat.copy(), domega=A.domega.copy(), nnbr=A.nnbr.copy(), nbr=A.nbr.copy(),
+               edge_len=np.zeros((N, 6)), edge_mid=np.zeros((N, 6, 3)), edge_nrm=np.zeros((N, 6, 3)))
+    for q in range(N):
+        for s in range(6):
+            e = A.nbr_edge[q, s]
+            if e >= 0:
+                tab["edge_len"][q, s] = A.edge_len[e]; tab["edge_mid"][q, s] = A.edge_mid[e]
+                tab["edge_nrm"][q, s] = A.edge_nrm[e] if A.edge_lo[e] == q else -A.edge_nrm[e]
+    return tab
+
+
+@pytest.mark.parametrize("angles", [("geodesic", 2), ("latlon", 4, 8)])
+def test_edge_ownership_of_explicit_tables(lib, oracle, angles):
+    """an ("explicit", tables) grid goes through the same marshalling as rad_create's (ADVICE round 2) and gives the named grid's ownership;
+    edge midpoints that are not finite unit vectors and non-finite edge normals are refused instead of poisoning the stored coefficients"""
+    A = oracle.Angles(*angles)
+    tab = explicit_tables(A)
+    a, b = B.rad_edge_ownership(angles), B.rad_edge_ownership(("explicit", tab))
+    assert a["N"] == b["N"] and a["E"] == b["E"]
+    if angles[0] == "geodesic":  # the explicit builder numbers the unique edges in the geodesic grid's own order (first occurrence)
+        assert all(np.array_equal(a[k], b[k]) for k in ("edge_lo", "edge_hi", "own_edge", "own_partner", "pull_pos"))
+    else:                        # latitude-longitude: another numbering of the same edges; every one of them owned once
+        assert sorted(zip(a["edge_lo"].tolist(), a["edge_hi"].tolist())) == sorted(zip(b["edge_lo"].tolist(), b["edge_hi"].tolist()))
+        assert sorted(b["own_edge"][b["own_edge"] >= 0].tolist()) == list(range(b["E"]))
+    e0 = int(np.argmax(A.nbr_edge[0] >= 0))  # a slot of angle 0 that holds an edge whose lower angle is 0
+    for key, val in (("edge_mid", np.nan), ("edge_nrm", np.inf), ("edge_mid", 3.0), ("edge_nrm", np.nan)):
+        bad = dict(tab, **{key: tab[key].copy()})
+        bad[key][0, e0, 1] = val
+        with pytest.raises(B.RadError) as e:
+            B.rad_edge_ownership(("explicit", bad))
+        assert e.value.status == 1 and "edge_mid must be finite unit vectors" in str(e.value)
+    with pytest.raises(ValueError):
+        B.rad_edge_ownership(("icosahedral", 2))
