@@ -447,6 +447,13 @@ def main():
         w = max_over_ranks(w, world, "cuda")
         e2e = {"value": world * updates / w, "unit": UNIT, "h2d_bytes_per_step": int(hI.numel() * 8 + hfl.numel() * 8 + hop.numel() * 8),
                "d2h_bytes_per_step": int(hO.numel() * 8 + hT.numel() * 8 + hdT.numel() * 8), "ms_per_step": w * 1e3, "repetitions": nrep}
+        # outside the timed region: what the host path returned is what rad_stage computes on the device, bit for bit (interior cells)
+        stage()
+        torch.cuda.synchronize()
+        shp = (nn[2] + 2 * ng, nn[1] + 2 * ng, nn[0] + 2 * ng)
+        itr = (slice(ng, -ng),) * 3
+        same = bool(torch.equal(hO.view(shp + (N,))[itr], I_b.cpu().view(shp + (N,))[itr])) and bool(torch.equal(hT.view(shp)[itr], T_out.cpu().view(shp)[itr]))
+        e2e["output_checked"] = "interior I_out and T_out of rad_stage_host equal rad_stage's device results bit for bit" if same else "MISMATCH against rad_stage"
         del hI, hO
     B.rad_destroy(h)
 

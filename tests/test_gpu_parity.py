@@ -129,6 +129,11 @@ def test_stage_parity(oracle, B, cfg, n, level):
     assert r["I"] <= TOL_I, r
     assert r["T"] <= TOL_FLUID and r["dT0"] <= TOL_FLUID, r
     assert r["Tchange"] > 1e-8  # the coupling did something (C2, C5 are gas-dominated: ~5e-7)
+    # the dT0 floor is a noise allowance, not a hiding place: no cell of C1-C4 sits under it.  C5's recipe is gas dominated and close to
+    # equilibrium (increments ~1e-6 |R^0_0|: most of its cells ARE in the floor's regime, where a relative bar of 1e-10 is not
+    # reachable in FP64); that regime is anchored by test_gpu_dt0_anchor.py against a long-double evaluation instead
+    if cfg != "C5":
+        assert r["on_floor"] <= 0.01, r
 
 
 @pytest.mark.parametrize("kw", [dict(recon_space=0), dict(couple=0), dict(renorm_fluid_weights=0), dict(n0_crit=0.0)])
@@ -361,10 +366,25 @@ def test_full_size_sampled(oracle, B, cfg, m, corners):
             got = O5[sl].cpu().numpy().reshape(-1, N)
             eI = rel_err_I(P.interior(got), P.interior(out_o))
             eT = rel_err(P.interior(T3[sl].cpu().numpy().reshape(-1)), P.interior(T_o), 0.0)
-            eD, _ = err_dT0(P, np.stack([d4[(q,) + sl].cpu().numpy().reshape(-1) for q in range(4)]), dT0_o, out_o)
+            eD, on_floor = err_dT0(P, np.stack([d4[(q,) + sl].cpu().numpy().reshape(-1) for q in range(4)]), dT0_o, out_o)
             assert eI <= TOL_I and eT <= TOL_FLUID and eD <= TOL_FLUID, (cfg, (ai, aj, ak), eI, eT, eD)
+            assert cfg == "C5" or on_floor <= 0.01, (cfg, (ai, aj, ak), on_floor)   # (C5: see test_stage_parity)
         # ghost cells of I_out are never written
         assert float(O5[:ng].max()) == -7.0 and float(O5[:, :ng].max()) == -7.0 and float(O5[:, :, -ng:].max()) == -7.0
+        if cfg == "C3":
+            # rad_stage_host at the size bench.py's e2e figure is taken on (128 planes x 162 angles through the three-stream slab
+            # pipeline): interior intensities, temperature and fluid increment equal rad_stage's bit for bit; ghosts of I_out carry I_in
+            itr = (slice(ng, -ng),) * 3
+            hI = I.cpu(); hO = torch.full_like(hI, -5.0); hfl = fluid.cpu(); hop = opac.cpu()
+            hT = torch.zeros(I.shape[0], dtype=torch.float64); hd = torch.zeros(4, I.shape[0], dtype=torch.float64)
+            nfh = B.rad_stage_host(h, hI, hO, hfl, hop, 0.0, 1.0, dt, hT, hd, count_noroot=True)
+            assert nfh == 0
+            hO5 = hO.reshape(shape + (N,)); want = O5.cpu()
+            assert torch.equal(hO5[itr], want[itr])
+            assert torch.equal(hT.reshape(shape)[itr], T3.cpu()[itr])
+            assert torch.equal(hd.reshape((4,) + shape)[(slice(None),) + itr], d4.cpu()[(slice(None),) + itr])
+            hI5 = hI.reshape(shape + (N,))
+            assert torch.equal(hO5[:ng], hI5[:ng]) and torch.equal(hO5[:, :, -ng:], hI5[:, :, -ng:])
     finally:
         B.rad_destroy(h)
 

@@ -115,3 +115,78 @@ def test_stage_weights(oracle):
     heun = P.transport(I, 0.5 * dt, I0=I0, gam0=0.5, gam1=0.5)
     expect = 0.5 * I0 + 0.5 * I + (fe - I)
     assert np.abs(P.interior(heun) - P.interior(expect)).max() < 1e-14
+
+
+# ------------------------------------------------------------------------------------------------ signal speed and upwind tables
+def face_geometry(oracle, P, kind, M, a, x0, dx):
+    """alpha and the tetrad e[mu][ahat] at the centre of every cell's LOWER x, y, z face, straight from geometry_point (pinned in
+    test_oracle_geometry.py), independent of the problem's own face table: arrays [ncell][3] and [ncell][3][4][4]"""
+    ng = P.ng
+    al = np.zeros((P.ncell, 3)); e = np.zeros((P.ncell, 3, 4, 4))
+    for k in range(P.NK):
+        for j in range(P.NJ):
+            for i in range(P.NI):
+                c = P.cell_index(k, j, i)
+                ctr = np.array([x0[0] + (i - ng + 0.5) * dx[0], x0[1] + (j - ng + 0.5) * dx[1], x0[2] + (k - ng + 0.5) * dx[2]])
+                for ax in range(3):
+                    x = ctr.copy(); x[ax] -= 0.5 * dx[ax]
+                    g = oracle.geometry_point(kind, M, a, x)
+                    al[c, ax] = g["alpha"]; e[c, ax] = g["e"]
+    return al, e
+
+
+def test_max_speed_minkowski_is_the_largest_direction_cosine(oracle):
+    """flat space, Cartesian tetrad: n^a / n^0 = nhat^a, so the bound per axis is max_n |nhat^a| exactly (R9)"""
+    for angles in (("geodesic", 2), ("latlon", 3, 8)):
+        A = oracle.Angles(*angles)
+        P = oracle.Problem(A, (3, 2, 2), (0.0, 0.0, 0.0), (0.5, 0.4, 0.3), metric_kind=0)
+        v, vax = P.max_speed()
+        assert tuple(vax) == tuple(np.abs(A.nhat).max(0))
+        assert v == max(vax)
+
+
+def test_max_speed_and_face_signs_kerr_schild_against_geometry_point(oracle):
+    """Kerr-Schild: |n^a / n^0| with n^a = e^a_0hat + e^a_bhat nhat^b and n^0 = e^0_0hat = 1 / alpha (Eq.11, R2) evaluated by numpy from
+    geometry_point at every lower face centre (ghost cells included) reproduces orc_max_speed; the signs of the same n^a reproduce
+    orc_upwind_tables' face table (Eq.24).  A shared misreading of the face record (n^0 taken for alpha, a transposed tetrad row, the
+    cell centre instead of the face centre) fails here."""
+    kind, M, a = 1, 1.0, 0.9
+    x0, dx = (2.5, -1.0, 0.5), (0.4, 0.5, 0.3)
+    A = oracle.Angles("geodesic", 2)
+    P = oracle.Problem(A, (3, 4, 2), x0, dx, metric_kind=kind, M=M, a=a)
+    al, e = face_geometry(oracle, P, kind, M, a, x0, dx)
+    n4 = np.concatenate([np.ones((A.N, 1)), A.nhat], 1)
+    assert np.abs(e[:, :, 0, 1:]).max() == 0.0 and np.abs(e[:, :, 0, 0] * al - 1).max() < 1e-14   # e^0_ahat = (1/alpha, 0, 0, 0)
+    na = np.stack([e[:, ax, ax + 1, :] @ n4.T for ax in range(3)], 1)        # [ncell][3][N]: n^a through the lower face along a
+    speed = np.abs(na) * al[:, :, None]
+    v, vax = P.max_speed()
+    assert np.abs(np.array(vax) - speed.max((0, 2))).max() < 1e-13
+    assert v == max(vax) and 0.5 < v < 3.0          # light in Kerr-Schild coordinates near the hole: of order one, not alpha^2 or 1/alpha^2 off
+    far = oracle.Problem(A, (2, 2, 2), (400.0, 300.0, 200.0), dx, metric_kind=kind, M=M, a=a)
+    assert abs(far.max_speed()[0] - np.abs(A.nhat).max()) < 2e-2      # far from the hole the flat-space value comes back
+    fs, es = P.upwind_tables()
+    sure = np.abs(na) > 1e-12
+    assert np.array_equal(fs[sure], np.sign(na[sure]).astype(np.int8))
+    assert set(np.unique(fs)) <= {-1, 0, 1} and (fs == 1).any() and (fs == -1).any()
+
+
+def test_edge_sign_table_is_the_sign_of_the_edge_coefficient(oracle):
+    """orc_upwind_tables' edge table = sgn c_e cell by cell, with c_e from orc_edge_coeffs (pinned against Eq.16b,c in
+    test_oracle_geometry.py) and, independently, as the numpy contraction -S[c][k] N^c (n^a n^b)_k of the cell record with the edge's
+    midpoint direction and in-sphere normal (Eq.16-17, Eq.25)"""
+    A = oracle.Angles("geodesic", 3)
+    P = oracle.Problem(A, (3, 2, 2), (3.0, 2.0, 1.0), (0.3, 0.25, 0.2), metric_kind=1, M=1.0, a=0.9)
+    _, es = P.upwind_tables(faces=False)
+    cell = P.geometry()[0]
+    n4 = np.concatenate([np.ones((A.E, 1)), A.edge_mid], 1)
+    iu = [(p, q) for p in range(4) for q in range(p, 4)]
+    quad = np.stack([n4[:, p] * n4[:, q] for p, q in iu], 1)                 # [E][10], the order 00,01,02,03,11,12,13,22,23,33
+    for c in range(P.ncell):
+        ce, _ = P.edge_coeffs(c)
+        assert np.array_equal(es[c], np.sign(ce).astype(np.int8))
+        S = cell[c, 33:63].reshape(3, 10)
+        ce_np = -np.einsum("ck,ec,ek->e", S, A.edge_nrm, quad)
+        sure = np.abs(ce_np) > 1e-12 * np.abs(S).max()
+        assert np.abs(ce_np - ce).max() < 1e-13 * max(1.0, np.abs(S).max())
+        assert np.array_equal(es[c][sure], np.sign(ce_np[sure]).astype(np.int8))
+    assert (es == 1).any() and (es == -1).any()
