@@ -1,7 +1,6 @@
 """bench.py -- one radiation stage (ghost fill + fused flux-divergence kernel + streaming implicit-coupling kernel) per "step".
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--n CELLS] [--impl reference]
-    python bench.py --ncu-raw FILE.csv --ncu-cmd "..."     # fold an `ncu --page raw --csv` export into profiles/r2_kernels.csv
 
 Metric (BASELINE.json): intensity-cell updates per second per radiation stage, FP64; one update = one
 (cell, angle) pair advanced one stage.  Default workload: config C3, the 128^3 x 162-angle Kerr-Schild block the
@@ -14,8 +13,8 @@ of rad_stage; `e2e` is the same stage through rad_stage_host with pinned HOST bu
 launch duration is measured live with CUDA events over K launches through rad_transport on the same inputs;
 `roofline_coupling` likewise for the coupling kernel (rad_couple); `cpu_baseline` is the oracle timed on the host cores on a
 bounded sub-block of the same workload.  Figures that come from ncu (DRAM traffic, FP64 instruction counts) are read from the
-committed profiles/r2_kernels.csv, keyed by the kernel instance names the library reports (rad_stage_kernels); a kernel that is
-not in the file gets null.  With --gpus N > 1 (torchrun) every rank runs an independent replica of the block ("replicas
+committed profiles/r3_kernels.csv, keyed by the kernel instance names the library reports (rad_stage_kernels); a kernel that is
+not in the file, or whose sources changed since its row was captured (src_sha16), gets null.  With --gpus N > 1 (torchrun) every rank runs an independent replica of the block ("replicas
 only": the path has no collective), scaling = weak.
 """
 import argparse
@@ -56,9 +55,27 @@ def design_bytes_per_update(N):
     return 16.0 + 24.0 + 336.0 / N
 
 
-PROFILE_CSV = os.path.join(ROOT, "profiles", "r2_kernels.csv")
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r3_kernels.csv")
 PROFILE_FIELDS = ["kernel", "workload", "ms", "dram_read_bytes", "dram_write_bytes", "inst_warp", "fp64_inst_warp", "fp64_pipe_pct", "issue_pct",
-                  "smem_wavefronts", "smem_bank_conflicts", "registers", "grid", "block"]
+                  "smem_wavefronts", "smem_bank_conflicts", "registers", "grid", "block", "src_sha16"]
+KERNEL_SOURCES = {"k_stage5": ["stage5.cu"], "k_couple_stream": ["stream.cu"], "k_moments_mma": ["stream.cu"], "k_fluxdiv": ["transport.cu"],
+                  "k_coupling": ["coupling.cu"]}
+
+
+def kernel_source_hash(kernel):
+    """sha256 (16 hex digits) over the sources a kernel is compiled from: its .cu, every header of csrc/ and the build flags.  A row of
+    the committed ncu table carries the hash of the sources it was captured on; a row whose hash differs from today's describes other
+    code and its figures are not printed (a kernel may change and keep its instance name)."""
+    import glob
+    import hashlib
+    from paper_2302_04283_b200 import build
+    csrc = os.path.join(ROOT, "paper_2302_04283_b200", "csrc")
+    files = [os.path.join(csrc, f) for f in KERNEL_SOURCES.get(kernel.split("<")[0], [])]
+    files += sorted(glob.glob(os.path.join(csrc, "*.cuh")) + glob.glob(os.path.join(csrc, "*.h")))
+    h = hashlib.sha256(" ".join(f for f in build.FLAGS if not f.startswith("/")).encode())
+    for f in files:
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
 
 
 def norm_kernel(name):
@@ -71,58 +88,17 @@ def norm_kernel(name):
 
 
 def profile_row(kernel, workload):
-    """the committed ncu figures of a kernel instance on a workload, or None (no figure is printed for a kernel that is not there)"""
+    """the committed ncu figures of a kernel instance on a workload, or None: no figure is printed for a kernel that is not in the
+    table, nor for one whose sources changed after the row was captured"""
     import csv
     try:
         with open(PROFILE_CSV) as f:
             for r in csv.DictReader(f):
                 if r["kernel"] == kernel and r["workload"] == workload:
-                    return r
+                    return r if r.get("src_sha16") == kernel_source_hash(kernel) else None
     except OSError:
         pass
     return None
-
-
-def ingest_ncu(raw_csv, cmd, workload):
-    """fold `ncu -i X.ncu-rep --page raw --csv` into profiles/r2_kernels.csv (one row per kernel instance and workload)"""
-    import csv
-    rows = list(csv.reader(open(raw_csv)))
-    h = rows[0]
-    want = {"ms": ("gpu__time_duration.sum", 1e-6), "dram_read_bytes": ("dram__bytes_read.sum", 1.0), "dram_write_bytes": ("dram__bytes_write.sum", 1.0),
-            "inst_warp": ("smsp__inst_executed.sum", 1.0), "fp64_inst_warp": ("smsp__inst_executed_pipe_fp64.sum", 1.0),
-            "fp64_pipe_pct": ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", 1.0), "issue_pct": ("smsp__issue_active.avg.pct_of_peak_sustained_active", 1.0),
-            "smem_wavefronts": ("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", 1.0), "smem_bank_conflicts": ("l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum", 1.0),
-            "registers": ("launch__registers_per_thread", 1.0), "grid": ("launch__grid_size", 1.0), "block": ("launch__block_size", 1.0)}
-    # FP64 warp instructions are not exported as a count: pipe-active fraction x active cycles x SMs x 2 issues per cycle and SM (64 lanes)
-    derive = ("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", "sm__cycles_active.avg", "device__attribute_multiprocessor_count")
-    unit_scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "ms": 1e6, "us": 1e3, "ns": 1.0, "s": 1e9}
-    old = []
-    try:
-        with open(PROFILE_CSV) as f:
-            old = list(csv.DictReader(f))
-    except OSError:
-        pass
-    for v in rows[2:]:
-        d = dict(zip(h, v))
-        r = {"kernel": norm_kernel(d["Kernel Name"]), "workload": workload}
-        for k, (m, sc) in want.items():
-            if m not in d or d[m] == "":
-                r[k] = ""
-                continue
-            x = float(d[m].replace(",", "")) * unit_scale.get(rows[1][h.index(m)], 1.0) * (sc if k == "ms" else 1.0)
-            r[k] = repr(x)
-        if all(m in d and d[m] != "" for m in derive):
-            pct, cyc, sms = (float(d[m].replace(",", "")) for m in derive)
-            r["fp64_inst_warp"] = repr(pct / 100.0 * cyc * sms * 2.0)
-        old = [o for o in old if not (o["kernel"] == r["kernel"] and o["workload"] == r["workload"])] + [r]
-    with open(PROFILE_CSV, "w", newline="") as f:
-        w = csv.DictWriter(f, fieldnames=PROFILE_FIELDS)
-        w.writeheader()
-        for o in old:
-            w.writerow({k: o.get(k, "") for k in PROFILE_FIELDS})
-    with open(PROFILE_CSV[:-4] + ".md", "a") as f:
-        f.write(f"* rows for workload `{workload}` from `{os.path.basename(raw_csv)}`: `{cmd}`\n")
-    print(f"{PROFILE_CSV}: {len(old)} rows")
 
 
 class ClockSampler:
@@ -264,22 +240,7 @@ def main():
     ap.add_argument("--vel-estimate", type=int, default=0, help="1: radiation-dominated velocity estimate Eq.51-55 in the coupling (NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--probe-pipes", action="store_true", help="print the FP64 pipe probe (DMMA vs DFMA, alone and mixed) and exit")
-    ap.add_argument("--ncu-raw", default=None, help="fold this `ncu --page raw --csv` export into profiles/r2_kernels.csv and exit")
-    ap.add_argument("--ncu-cmd", default="", help="the ncu command that produced --ncu-raw (recorded beside the csv)")
     args = ap.parse_args()
-    if args.ncu_raw:
-        return ingest_ncu(args.ncu_raw, args.ncu_cmd, args.config if args.n is None else f"{args.config}/n={args.n}")
-    if args.probe_pipes:
-        from paper_2302_04283_b200 import binding as B
-        from paper_2302_04283_b200 import build
-        build.build()
-        h = B.rad_create(dict(kind=0), dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1)), ("geodesic", 1), None, dict(couple=0), 0)
-        v = B.rad_probe_fp64_pipes(h)
-        B.rad_destroy(h)
-        names = ["dmma_alone", "dfma_alone", "dmma_in_mix_4_8", "dfma_in_mix_4_8", "dmma_in_mix_1_8", "dfma_in_mix_1_8"]
-        print(json.dumps({"fp64_pipe_probe_multiply_adds_per_sec": dict(zip(names, v)), "sum_mix_4_8": v[2] + v[3], "sum_mix_1_8": v[4] + v[5]}))
-        return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
@@ -397,7 +358,7 @@ def main():
         prof = profile_row(kernel, workload)
         traffic = (float(prof["dram_read_bytes"]) + float(prof["dram_write_bytes"])) if prof and prof["dram_read_bytes"] else None
         blk = {"kernel": f"{kernel} ({what})", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-               "traffic": traffic, "traffic_source": "profiles/r2_kernels.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch)" if traffic else None,
+               "traffic": traffic, "traffic_source": "profiles/r3_kernels.csv (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per launch)" if traffic else None,
                "traffic_frac": (traffic / (ms_k * 1e-3) / 1e9 / peak) if traffic else None,
                "peak_source": peak_src, "algorithmic_bytes_per_update": bpu, "ms_per_launch": ms_k,
                "how_timed": "CUDA events over %d launches of this kernel alone on the step's inputs, same process, right after the timed region" % reps}
@@ -407,7 +368,7 @@ def main():
                           "fp64_slots_per_update_issued": slots, "achieved": 2.0 * slots * updates / (ms_k * 1e-3) / 1e12,
                           "frac": 2.0 * slots * updates / (ms_k * 1e-3) / (2.0 * dfma),
                           "fp64_pipe_pct_ncu": float(prof["fp64_pipe_pct"]), "issue_pct_ncu": float(prof["issue_pct"]),
-                          "note": "one FP64-pipe instruction slot per lane = 2 flop (DFMA-equivalent); slots counted by ncu (profiles/r2_kernels.csv)"}
+                          "note": "one FP64-pipe instruction slot per lane = 2 flop (DFMA-equivalent); slots counted by ncu (profiles/r3_kernels.csv)"}
         if extra:
             blk.update(extra)
         return blk

@@ -279,12 +279,6 @@ rad_status rad_stage_kernels(rad_ctx *, char *buf /* HOST */, size_t nbytes);
  * bench.py uses it as the denominator of the FP64 ("alu") roofline of the stage kernel. */
 rad_status rad_probe_fp64(rad_ctx *, double *dfma_per_sec /* HOST */);
 
-/* Measurement helper: do the FP64 matrix instruction (DMMA m8n8k4, used by rad_moments) and the scalar DFMA share one pipe on this device?
- * out6 (HOST): multiply-add lane operations per second of {DMMA alone, DFMA alone, DMMA and DFMA with 4 matrix + 8 scalar chains per
- * thread, DMMA and DFMA with 1 matrix + 8 scalar chains}; one DMMA = 256 multiply-adds.  Synchronises.  (DESIGN.md "stored versus
- * recomputed": the answer decides whether the angular coefficients could be recomputed on a second pipe.) */
-rad_status rad_probe_fp64_pipes(rad_ctx *, double *out6 /* HOST */);
-
 /* Text of the last error on this context (or of the last failed rad_create if ctx is NULL).  Never NULL. */
 const char *rad_last_error(const rad_ctx *);
 

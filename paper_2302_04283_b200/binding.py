@@ -20,7 +20,7 @@ NCELL, NFACE, MAXNBR = 52, 8, 6
  TAB_STAGE_FACE_SIGN) = range(20)
 
 EXPORTS = ["rad_create", "rad_stage", "rad_stage_static", "rad_stage_host", "rad_fill_ghosts", "rad_transport", "rad_couple", "rad_moments",
-           "rad_get_table", "rad_edge_ownership", "rad_exchange_halo", "rad_stage_kernels", "rad_probe_fp64", "rad_probe_fp64_pipes", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
+           "rad_get_table", "rad_edge_ownership", "rad_exchange_halo", "rad_stage_kernels", "rad_probe_fp64", "rad_ncells_total", "rad_launch_count", "rad_last_error", "rad_destroy"]
 
 
 class RadError(RuntimeError):
@@ -76,7 +76,6 @@ def lib():
         L.rad_moments.argtypes = [vp, vp, C.c_int, vp, vp, vp]
         L.rad_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
         L.rad_probe_fp64.argtypes = [vp, C.POINTER(C.c_double)]
-        L.rad_probe_fp64_pipes.argtypes = [vp, C.POINTER(C.c_double)]
         L.rad_edge_ownership.argtypes = [C.POINTER(_Angles), C.POINTER(C.c_int), C.POINTER(C.c_int), vp, vp, vp, vp, vp, C.c_size_t]
         L.rad_exchange_halo.argtypes = [vp, vp, vp, vp, C.c_int, vp]
         L.rad_stage_kernels.argtypes = [vp, C.c_char_p, C.c_size_t]
@@ -248,13 +247,6 @@ def rad_probe_fp64(ctx):
     v = C.c_double(0.0)
     _check(ctx, lib().rad_probe_fp64(ctx, C.byref(v)))
     return v.value
-
-
-def rad_probe_fp64_pipes(ctx):
-    """multiply-add lane operations per second: (DMMA alone, DFMA alone, DMMA / DFMA in a 4 + 8 chain mix, DMMA / DFMA in a 1 + 8 mix)"""
-    v = (C.c_double * 6)()
-    _check(ctx, lib().rad_probe_fp64_pipes(ctx, v))
-    return list(v)
 
 
 def rad_stage_kernels(ctx):

@@ -590,13 +590,6 @@ rad_status rad_probe_fp64(rad_ctx *c, double *dfma_per_sec) {
     return RAD_OK;
 }
 
-rad_status rad_probe_fp64_pipes(rad_ctx *c, double *out6) {
-    if (!c || !out6) return fail(c, RAD_EINVAL, "rad_probe_fp64_pipes: NULL argument");
-    DeviceGuard guard(c->device);
-    if (rad::probe_fp64_pipes(out6, &c->launches) != 0) return cuda_fail(c, "rad_probe_fp64_pipes");
-    return RAD_OK;
-}
-
 rad_status rad_get_table(rad_ctx *c, int which, void *host_out, size_t nbytes) {
     if (!c || !host_out) return fail(c, RAD_EINVAL, "rad_get_table: NULL argument");
     DeviceGuard guard(c->device);

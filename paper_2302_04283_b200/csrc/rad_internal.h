@@ -126,6 +126,5 @@ int launch_sign_tables(const DeviceTables &t, signed char *face_sign, signed cha
 int launch_maxspeed(const DeviceTables &t, double *out3, cudaStream_t s);
 // probe.cu: measured FP64 FMA rate of the current device (lane operations per second); 0 on success
 int probe_dfma_rate(double *dfma_per_sec, long long *launches);
-int probe_fp64_pipes(double *out6, long long *launches);
 
 }  // namespace rad

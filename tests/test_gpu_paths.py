@@ -391,16 +391,13 @@ def test_guard_bands_around_caller_arrays_stay_intact(oracle, B, n, angles):
 
 
 def test_measurement_helpers(oracle, B):
-    """rad_stage_kernels names the instances a stage launches (the key of profiles/r2_kernels.csv); the FP64 probes run, and the
-    matrix instruction adds nothing to the scalar FP64 rate (same pipe: DESIGN.md 'stored versus recomputed')"""
+    """rad_stage_kernels names the instances a stage launches (the key of the kernel table under profiles/); the FP64 rate probe runs"""
     A, P, h, I, fluid, opac, _ = small_problem(oracle, B, (4, 4, 4), ("geodesic", 4))
     try:
         kf, kc = B.rad_stage_kernels(h)
         assert kf == "k_stage5<3,2,4,2,1,1,0>" and kc == "k_couple_stream<0,21>"
         dfma = B.rad_probe_fp64(h)
-        v = B.rad_probe_fp64_pipes(h)
-        assert dfma > 1e12 and all(x > 1e12 for x in v)
-        assert v[2] + v[3] < 1.15 * max(v[0], v[1]) and v[4] + v[5] < 1.15 * max(v[0], v[1])
+        assert 1e12 < dfma < 1e14
     finally:
         B.rad_destroy(h)
     for angles, want in ((("geodesic", 6), ("k_fluxdiv", "k_couple_stream<0,0>")),   # N = 362: generic flux divergence, streaming coupling
