@@ -235,7 +235,9 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override cells per axis (same box)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-n", type=int, default=None, help="sub-block size of the oracle sample (default: 64 for --impl reference, 96 for the cpu_baseline leg)")
-    ap.add_argument("--recon", type=int, default=1, help="spatial reconstruction: 1 PLM (the workload's), 0 donor cell (diagnostic)")
+    ap.add_argument("--recon", type=int, default=1, help="spatial reconstruction: 1 PLM (the workload's), 0 donor cell (diagnostic), 2 PPM (NEXT-3: 3 ghost layers, generic flux-divergence kernel)")
+    ap.add_argument("--recon-angle", type=int, default=0, help="1: PLM in angle on a latitude-longitude grid (NEXT-3; config C1's grid, e.g. --config C1 --n 64; generic kernel)")
+    ap.add_argument("--recompute-edge-coeffs", type=int, default=0, help="1: no stored angular coefficients (rad_params.recompute_edge_coeffs): the generic flux-divergence kernel")
     ap.add_argument("--tau-factor", type=float, default=0.0, help="constant of Eq.26: > 0 times the stage with the optical-depth-aware flux (NEXT-1)")
     ap.add_argument("--vel-estimate", type=int, default=0, help="1: radiation-dominated velocity estimate Eq.51-55 in the coupling (NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -270,7 +272,8 @@ def main():
 
     cfg = args.config
     c = W.CONFIGS[cfg]
-    nn, ng, x0, dx = W.grid(cfg, args.n)
+    ng_arg = 3 if args.recon == 2 else None
+    nn, ng, x0, dx = W.grid(cfg, args.n, ng=ng_arg)
     N = W.n_angles(cfg)
     updates = nn[0] * nn[1] * nn[2] * N
     workload = cfg if args.n is None else f"{cfg}/n={args.n}"
@@ -279,16 +282,16 @@ def main():
     h0 = B.rad_create(dict(kind=0), dict(n=(1, 1, 1), x0=(0, 0, 0), dx=(1, 1, 1)), c["angles"], None, dict(couple=0), local)
     nhat = B.rad_get_table(h0, B.TAB_NHAT)
     B.rad_destroy(h0)
-    inp = W.make_inputs(cfg, nhat, n=args.n, device=f"cuda:{local}")
+    inp = W.make_inputs(cfg, nhat, n=args.n, device=f"cuda:{local}", ng=ng_arg)
     I_a = inp["I"].reshape(-1, N).contiguous(); fluid = inp["fluid"].reshape(5, -1).contiguous(); opac = inp["opac"].reshape(3, -1).contiguous()
     del inp
     I_b = I_a.clone()
     ncell = fluid.shape[1]
     T_out = torch.zeros(ncell, dtype=torch.float64, device="cuda"); dT0 = torch.zeros(4, ncell, dtype=torch.float64, device="cuda")
     h = B.rad_create(dict(kind=c["metric"], M=c["M"], a=c["a"], excise_r=W.excise_radius(cfg)),
-                     dict(n=nn, x0=x0, dx=dx, bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3), c["angles"], (opac[0], opac[1], opac[2]),
-                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=args.recon, renorm_fluid_weights=1, couple=1,
-                          tau_factor=args.tau_factor, vel_estimate=args.vel_estimate), local)
+                     dict(n=nn, ng=ng, x0=x0, dx=dx, bc_lo=(c["bc"],) * 3, bc_hi=(c["bc"],) * 3), c["angles"], (opac[0], opac[1], opac[2]),
+                     dict(gamma_gas=W.GAMMA_GAS, a_rad=W.A_RAD, n0_crit=W.N0_CRIT, recon_space=args.recon, recon_angle=args.recon_angle, renorm_fluid_weights=1, couple=1,
+                          tau_factor=args.tau_factor, vel_estimate=args.vel_estimate, recompute_edge_coeffs=args.recompute_edge_coeffs), local)
     vmax = float(B.rad_get_table(h, B.TAB_MAXSPEED).max())
     dt = W.CFL * min(dx) / vmax
     stream = torch.cuda.current_stream()
@@ -375,9 +378,9 @@ def main():
 
     if args.tau_factor == 0.0:
         roofline = hbm_block(k_flux, "fused spatial + angular flux divergence, cons -> prim: the dominant kernel of the step", fluxdiv_bytes_per_update(N), ms_flux,
-                             {"design_bytes_per_update": design_bytes_per_update(N),
-                              "design_frac": design_bytes_per_update(N) * updates / (ms_flux * 1e-3) / 1e9 / peak,
-                              "share_of_step": ms_flux / ms, "kernels_per_step": kernels_per_step})
+                             dict({"share_of_step": ms_flux / ms, "kernels_per_step": kernels_per_step},
+                                  **({"design_bytes_per_update": design_bytes_per_update(N),
+                                      "design_frac": design_bytes_per_update(N) * updates / (ms_flux * 1e-3) / 1e9 / peak} if k_flux.startswith("k_stage5") else {})))
     else:  # k_tau_table + k_stage5<TAU> + coupling: the step as a whole on the stage's bytes
         roofline = hbm_block(k_flux, "flux divergence with the Eq.28 factor; timed through the whole step", 32.0 + 640.0 / N, ms, {"kernels_per_step": kernels_per_step})
     roofline_coupling = hbm_block(k_cpl, "implicit coupling, mask, fluid increment", coupling_bytes_per_update(N), ms_cpl, {"share_of_step": ms_cpl / ms})
@@ -440,10 +443,12 @@ def main():
             omp_threads(os.cpu_count())
     line = {"metric": METRIC, "value": whole_job_value(updates, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{cfg}: {c['angles']} angles={N}, {nn[0]}^3 cells + 2 ghosts, metric kind {c['metric']} a={c['a']}, box {c['box']}",
+            "config": {"workload": f"{cfg}: {c['angles']} angles={N}, {nn[0]}^3 cells + {ng} ghosts, metric kind {c['metric']} a={c['a']}, box {c['box']}",
                        "updates_per_step": updates, "tau_factor": args.tau_factor, "vel_estimate": args.vel_estimate,
+                       "recon_space": args.recon, "recon_angle": args.recon_angle, "recompute_edge_coeffs": args.recompute_edge_coeffs,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": "inputs (2 x %.2f GB) exceed L2; no flush" % (I_a.numel() * 8 / 1e9)},
+                       "l2": ("inputs (2 x %.2f GB) exceed L2; no flush" if I_a.numel() * 8 > 2 * 126e6 else "inputs (2 x %.3f GB) FIT the 126 MB L2 and are not flushed: a warm-L2 figure")
+                             % (I_a.numel() * 8 / 1e9)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_fluxdiv": roofline,
             "roofline_coupling": roofline_coupling, "roofline_stage": roofline_stage, "moments": moments, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)

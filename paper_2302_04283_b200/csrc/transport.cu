@@ -165,8 +165,28 @@ __global__ void __launch_bounds__(256) k_cell_velocity(DeviceTables t, const dou
     }
 }
 
+// R21: van Leer PLM in index space on the latitude-longitude grid for the edge value of the upwind angle a_up; beyond a pole
+// the row of cell (l, m) continues in cell (l, m + N_psi / 2); periodic in psi.  slot of this edge in the upwind cell: 0 zeta-, 1 zeta+,
+// 2 psi-, 3 psi+
+__device__ __noinline__ double plm_angle(const int *__restrict__ nbr_edge, int np, int nzeta, const double *__restrict__ row, int a_up, int e, double Iup) {
+    int slot = 0;
+    while (__ldg(nbr_edge + a_up * RAD_MAXNBR + slot) != e) slot++;
+    const int l = a_up / np, m = a_up - l * np;
+    int lo, hi;
+    if (slot < 2) {
+        const int across = l * np + (m + np / 2) % np;
+        lo = l > 0 ? a_up - np : across;
+        hi = l + 1 < nzeta ? a_up + np : across;
+    } else {
+        lo = l * np + (m + np - 1) % np;
+        hi = l * np + (m + 1) % np;
+    }
+    const double sl = vl_slope(row[lo], Iup, row[hi]);
+    return (slot & 1) ? Iup + 0.5 * sl : Iup - 0.5 * sl;
+}
+
 template <int RECON, bool TAU>
-__global__ void __launch_bounds__(256) k_fluxdiv(DeviceTables t, const double *__restrict__ I_in, const double *__restrict__ I0,
+__global__ void __launch_bounds__(256, 4) k_fluxdiv(DeviceTables t, const double *__restrict__ I_in, const double *__restrict__ I0,
                                                    double gam0, double gam1, double beta_dt, double *__restrict__ I_out,
                                                    const double *__restrict__ vel, double tau_dt) {
     extern __shared__ double smem[];
@@ -199,38 +219,39 @@ __global__ void __launch_bounds__(256) k_fluxdiv(DeviceTables t, const double *_
     }
     __syncthreads();
 
-    // phase A: angular fluxes, once per unique edge (Eq.25, donor cell in angle)
-    for (int q = threadIdx.x; q < ncx * E; q += blockDim.x) {
-        const int cl = q / E, e = q % E;
-        const double *S = sCell + cl * 36 + 5;
-        const double *T = t.edge_T + (long long)e * 30;
-        double acc = 0.0;
+    // phase A: angular fluxes, once per unique edge (Eq.25, donor cell in angle).  A thread takes an edge for all cells of the run:
+    // the edge's 30 products N^c (n^a n^b), its midpoint direction, length and end angles are loaded once and stay in registers
+    // (they were fetched per cell before: 90 loads per intensity update through L1, the kernel's bottleneck); the cell's S comes
+    // from shared memory as a broadcast.  The 30-term chain keeps its order, so the results are the same bit for bit.
+    for (int e = threadIdx.x; e < E; e += blockDim.x) {
+        double acc[CX];  // the chains of the run's cells side by side (each a dependent sequence of 30 FP64 operations)
 #pragma unroll
-        for (int w = 0; w < 30; w++) acc = fma(S[w], __ldg(T + w), acc);  // pinned 30-term chain
-        const double ce = -acc;
-        const double n0e = chain4(sCell + cl * 36 + 1, __ldg(t.edge_mid + 3 * e), __ldg(t.edge_mid + 3 * e + 1), __ldg(t.edge_mid + 3 * e + 2));
-        const int a_up = ce > 0.0 ? __ldg(t.edge_lo + e) : __ldg(t.edge_hi + e);
-        const double *row = I_in + (c0 + cl) * N;
-        double Iup = row[a_up];
-        if (t.recon_angle == 1 && ce != 0.0) {
-            // R21: van Leer PLM in index space on the latitude-longitude grid; beyond a pole the row of cell (l, m) continues
-            // in cell (l, m + N_psi / 2); periodic in psi.  slot of this edge in the upwind cell: 0 zeta-, 1 zeta+, 2 psi-, 3 psi+
-            int slot = 0;
-            while (__ldg(t.nbr_edge + a_up * RAD_MAXNBR + slot) != e) slot++;
-            const int np = t.npsi, l = a_up / np, m = a_up - l * np;
-            int lo, hi;
-            if (slot < 2) {
-                const int across = l * np + (m + np / 2) % np;
-                lo = l > 0 ? a_up - np : across;
-                hi = l + 1 < t.nzeta ? a_up + np : across;
-            } else {
-                lo = l * np + (m + np - 1) % np;
-                hi = l * np + (m + 1) % np;
+        for (int cl = 0; cl < CX; cl++) acc[cl] = 0.0;
+#pragma unroll
+        for (int half = 0; half < 2; half++) {  // the edge's products in two halves of 15: fewer registers, the chain order is kept
+            double T[15];
+#pragma unroll
+            for (int w = 0; w < 15; w++) T[w] = __ldg(t.edge_T + (long long)e * 30 + half * 15 + w);
+#pragma unroll
+            for (int w = 0; w < 15; w++) {
+#pragma unroll
+                for (int cl = 0; cl < CX; cl++) acc[cl] = fma(sCell[min(cl, ncx - 1) * 36 + 5 + half * 15 + w], T[w], acc[cl]);  // pinned 30-term chain
             }
-            const double sl = vl_slope(row[lo], Iup, row[hi]);
-            Iup = (slot & 1) ? Iup + 0.5 * sl : Iup - 0.5 * sl;
         }
-        sFe[cl * E + e] = (ce == 0.0) ? 0.0 : __ldg(t.edge_len + e) * (ce * n0e * Iup);
+        const double m1 = __ldg(t.edge_mid + 3 * e), m2 = __ldg(t.edge_mid + 3 * e + 1), m3 = __ldg(t.edge_mid + 3 * e + 2);
+        const double len = __ldg(t.edge_len + e);
+        const int elo = __ldg(t.edge_lo + e), ehi = __ldg(t.edge_hi + e);
+#pragma unroll
+        for (int cl = 0; cl < CX; cl++) {
+            if (cl >= ncx) break;
+            const double ce = -acc[cl];
+            const double n0e = chain4(sCell + cl * 36 + 1, m1, m2, m3);
+            const int a_up = ce > 0.0 ? elo : ehi;
+            const double *row = I_in + (c0 + cl) * N;
+            double Iup = row[a_up];
+            if (t.recon_angle == 1 && ce != 0.0) Iup = plm_angle(t.nbr_edge, t.npsi, t.nzeta, row, a_up, e, Iup);
+            sFe[cl * E + e] = (ce == 0.0) ? 0.0 : len * (ce * n0e * Iup);
+        }
     }
     __syncthreads();
     // Delta A_a / Delta V of the cells of this run (Eq.20b,c with sqrt(-g) = 1): 1 / dx, or 1 / (the cell's width) on a stretched axis

@@ -36,7 +36,7 @@ def n_angles(cfg):
     return a[1] * a[2] if a[0] == "latlon" else 10 * a[1] * a[1] + 2
 
 
-def grid(cfg, n=None, sub=None):
+def grid(cfg, n=None, sub=None, ng=None):
     """(n, ng, x0, dx) of a config; `n` overrides the cell count (same box: a coarser block); `sub` keeps the
     spacing of the n-cell block but takes only the sub^3 cells at its low corner (a bounded sample)."""
     c = CONFIGS[cfg] if isinstance(cfg, str) else cfg
@@ -44,7 +44,7 @@ def grid(cfg, n=None, sub=None):
     lo, hi = c["box"]
     dx = (hi - lo) / n
     m = n if sub is None else sub
-    return (m, m, m), NG, (lo, lo, lo), (dx, dx, dx)
+    return (m, m, m), (NG if ng is None else ng), (lo, lo, lo), (dx, dx, dx)
 
 
 def excise_radius(cfg):
@@ -136,7 +136,7 @@ def _solenoidal(x, y, z, box, seed, vmax, nmodes=24, kmax=8):
 
 
 # ----------------------------------------------------------------------------- the recipes
-def make_inputs(cfg, nhat, n=None, device="cpu", sub=None):
+def make_inputs(cfg, nhat, n=None, device="cpu", sub=None, ng=None):
     """Inputs of one stage for config `cfg` ("C1".."C5").
 
     nhat: [N,3] unit directions of the angle grid (from the implementation under test).
@@ -150,7 +150,7 @@ def make_inputs(cfg, nhat, n=None, device="cpu", sub=None):
     """
     c = CONFIGS[cfg]
     seed = c["seed"]
-    nn, ng, x0, dx = grid(cfg, n, sub)
+    nn, ng, x0, dx = grid(cfg, n, sub, ng)  # (ng = 3: the ghost depth PPM needs; the default 2 is the workload's)
     nhat = torch.as_tensor(nhat, dtype=torch.float64, device=device)
     N = nhat.shape[0]
     NI, NJ, NK = nn[0] + 2 * ng, nn[1] + 2 * ng, nn[2] + 2 * ng
