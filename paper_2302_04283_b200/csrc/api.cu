@@ -187,6 +187,16 @@ rad_status rad_create(const rad_metric *m, const rad_grid *g, const rad_angles *
             const int e = h.nbr_edge[n * RAD_MAXNBR + s];
             if (e >= 0) nbr_w[n * RAD_MAXNBR + s] = (h.edge_lo[e] == n ? 1.0 : -1.0) / h.domega[n];
         }
+    std::vector<double> nhat_t((size_t)3 * h.N), nbr_w_t((size_t)RAD_MAXNBR * h.N);
+    std::vector<int> nbr_edge_t((size_t)RAD_MAXNBR * h.N);
+    for (int n = 0; n < h.N; n++) {
+        for (int d = 0; d < 3; d++) nhat_t[(size_t)d * h.N + n] = h.nhat[3 * n + d];
+        for (int s = 0; s < RAD_MAXNBR; s++) {
+            nbr_edge_t[(size_t)s * h.N + n] = h.nbr_edge[n * RAD_MAXNBR + s];
+            nbr_w_t[(size_t)s * h.N + n] = nbr_w[n * RAD_MAXNBR + s];
+        }
+    }
+    ok = ok && upload(c, nhat_t, &t.nhat_t) && upload(c, nbr_edge_t, &t.nbr_edge_t) && upload(c, nbr_w_t, &t.nbr_w_t);
     ok = ok && upload(c, h.nhat, &t.nhat) && upload(c, h.domega, &t.domega) && upload(c, h.nnbr, &t.nnbr) && upload(c, h.nbr_edge, &t.nbr_edge) &&
          upload(c, h.edge_lo, &t.edge_lo) && upload(c, h.edge_hi, &t.edge_hi) && upload(c, h.edge_len, &t.edge_len) &&
          upload(c, h.edge_mid, &t.edge_mid) && upload(c, edge_T, &t.edge_T) && upload(c, nbr_w, &t.nbr_w);

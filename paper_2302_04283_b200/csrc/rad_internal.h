@@ -57,6 +57,10 @@ struct DeviceTables {
     const double *edge_T;    // [E][30]  pinned products N^c * (n^a n^b)
     // per angle: signed weights of its edges, sgn * dlambda_e / dOmega_n, [N][6] (0 where no edge)
     const double *nbr_w;
+    // the same per-angle tables angle-innermost, for kernels whose lanes run over angles (coalesced: k_fluxdiv's update phase)
+    const double *nhat_t;    // [3][N]
+    const int *nbr_edge_t;   // [6][N]
+    const double *nbr_w_t;   // [6][N]
     // geometry
     const double *cell;  // [ncell][RAD_NCELL]
     const double *face;  // [ncell][3][RAD_NFACE]

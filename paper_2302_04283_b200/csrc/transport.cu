@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(256, 4) k_fluxdiv(DeviceTables t, const double
         const double *cg = sCell + cl * 36;
         double *out = I_out + c * N + n;
         if (cg[35] != 0.0) { *out = 0.0; continue; }
-        const double n1 = __ldg(t.nhat + 3 * n), n2 = __ldg(t.nhat + 3 * n + 1), n3 = __ldg(t.nhat + 3 * n + 2);
+        const double n1 = __ldg(t.nhat_t + n), n2 = __ldg(t.nhat_t + N + n), n3 = __ldg(t.nhat_t + 2 * N + n);  // (angle-innermost tables: coalesced)
         const double *p = I_in + c * N + n;
         const long long sx = N;
         double div = 0.0;
@@ -278,8 +278,8 @@ __global__ void __launch_bounds__(256, 4) k_fluxdiv(DeviceTables t, const double
         double adiv = 0.0;
 #pragma unroll
         for (int s = 0; s < RAD_MAXNBR; s++) {
-            const int e = __ldg(t.nbr_edge + n * RAD_MAXNBR + s);
-            if (e >= 0) adiv = fma(__ldg(t.nbr_w + n * RAD_MAXNBR + s), sFe[cl * E + e], adiv);
+            const int e = __ldg(t.nbr_edge_t + s * N + n);
+            if (e >= 0) adiv = fma(__ldg(t.nbr_w_t + s * N + n), sFe[cl * E + e], adiv);
         }
         div += adiv;
         const double w = cg[0] * chain4(cg + 1, n1, n2, n3);  // n^0 n_0
