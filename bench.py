@@ -94,7 +94,8 @@ def profile_row(kernel, workload):
     try:
         with open(PROFILE_CSV) as f:
             for r in csv.DictReader(f):
-                if r["kernel"] == kernel and r["workload"] == workload:
+                # (the library reports the generic kernel without its template arguments: "k_fluxdiv" matches the row "k_fluxdiv<1,0>")
+                if (r["kernel"] == kernel or ("<" not in kernel and r["kernel"].split("<")[0] == kernel)) and r["workload"] == workload:
                     return r if r.get("src_sha16") == kernel_source_hash(kernel) else None
     except OSError:
         pass
